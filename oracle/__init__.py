@@ -1,0 +1,28 @@
+"""CPU oracle for the free-space Poisson convolution (arxiv 2405.02603).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only ``tests/``, ``__graft_entry__.smoke()`` and the
+``cpu_baseline`` / ``--impl reference`` legs of ``bench.py`` may import this package.  It shares no
+code with ``paper_2405_02603_b200`` (the CUDA path) and neither imports the other.
+
+The arithmetic lives in ``fsp_oracle.c`` (plain C, fp64, textbook radix-2 FFT / direct DFT); this
+package only builds that file with gcc and marshals numpy arrays into it.
+"""
+from .oracle import (  # noqa: F401
+    HOCKNEY,
+    VICO,
+    VICO_2,
+    G0_DEFAULT,
+    ALPHA_DEFAULT,
+    OraclePlan,
+    build,
+    dct1,
+    direct_sum,
+    fft1d,
+    fft3d,
+    green_spectrum,
+    green_table,
+    num_threads,
+    set_num_threads,
+    solve_with_spectrum,
+    vg_window,
+)

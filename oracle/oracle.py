@@ -1,0 +1,215 @@
+"""ctypes marshalling for ``fsp_oracle.c`` (TEST INFRASTRUCTURE -- see ``oracle/__init__.py``).
+
+No arithmetic of the method is done in this file: every function checks shapes, hands contiguous
+numpy fp64 arrays to the C oracle and returns the result.
+"""
+from __future__ import annotations
+
+import ctypes
+import math
+import os
+import subprocess
+import threading
+
+import numpy as np
+
+HOCKNEY, VICO, VICO_2 = 0, 1, 2  # PAPER.md:199 solver names HOCKNEY / VICO / VICO_2
+G0_DEFAULT = 1.0 / (4.0 * math.pi)  # DESIGN.md reading R5
+ALPHA_DEFAULT = 1.1
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "fsp_oracle.c")
+_LIB = os.path.join(_HERE, "libfsp_oracle.so")
+_lock = threading.Lock()
+_lib = None
+
+_dp = ctypes.POINTER(ctypes.c_double)
+_lp = ctypes.POINTER(ctypes.c_long)
+
+
+def build(force: bool = False) -> str:
+    """Compile fsp_oracle.c with gcc (-O2 -fopenmp).  Returns the path of the shared object."""
+    with _lock:
+        stale = (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC)
+        if force or stale:
+            tmp = _LIB + f".tmp{os.getpid()}"
+            cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-o", tmp, _SRC, "-lm"]
+            subprocess.run(cmd, check=True)
+            os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(_LIB)
+        L, I, D = ctypes.c_long, ctypes.c_int, ctypes.c_double
+        lib.orc_num_threads.restype = I
+        lib.orc_set_num_threads.argtypes = [I]
+        lib.orc_set_num_threads.restype = None
+        lib.orc_fft1d.argtypes = [L, _dp, _dp, I, I]
+        lib.orc_fft3d.argtypes = [L, L, L, _dp, I, I]
+        lib.orc_dct1.argtypes = [L, L, _dp, _dp, I]
+        lib.orc_vg_window.argtypes = [L, L, L, _dp, D]
+        lib.orc_vg_window.restype = D
+        lib.orc_green_table_he.argtypes = [L, L, L, _dp, D, _dp]
+        lib.orc_green_table_vg.argtypes = [L, L, L, _dp, D, I, _dp]
+        lib.orc_green_table_vg2.argtypes = [L, L, L, _dp, D, I, _dp]
+        lib.orc_green_spectrum.argtypes = [L, L, L, _dp, I, _dp]
+        lib.orc_solve.argtypes = [L, L, L, _dp, _dp, I, _dp, _dp]
+        lib.orc_direct_sum.argtypes = [L, L, L, _dp, _dp, _dp, L, _lp, _dp]
+        _lib = lib
+    return _lib
+
+
+def _check(rc: int, what: str) -> None:
+    if rc == -2:
+        raise MemoryError(f"oracle {what}: out of memory")
+    if rc != 0:
+        raise ValueError(f"oracle {what}: invalid argument (rc={rc})")
+
+
+def _d(a: np.ndarray):
+    return a.ctypes.data_as(_dp)
+
+
+def _h3(h) -> np.ndarray:
+    h = np.ascontiguousarray(np.broadcast_to(np.asarray(h, dtype=np.float64), (3,)))
+    return h
+
+
+def num_threads() -> int:
+    return int(_load().orc_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    _load().orc_set_num_threads(int(n))
+
+
+def fft1d(x: np.ndarray, sign: int = -1, method: int = 0) -> np.ndarray:
+    """Unscaled 1-D DFT of a complex vector; method 0 = radix-2 (direct if not 2^k), 1 = direct."""
+    x = np.ascontiguousarray(x, dtype=np.complex128)
+    out = np.empty_like(x)
+    _check(_load().orc_fft1d(x.size, _d(x.view(np.float64)), _d(out.view(np.float64)), sign, method),
+           "fft1d")
+    return out
+
+
+def fft3d(a: np.ndarray, sign: int = -1, method: int = 0) -> np.ndarray:
+    """Unscaled separable 3-D DFT (returns a new array)."""
+    a = np.array(a, dtype=np.complex128, order="C", copy=True)
+    assert a.ndim == 3
+    _check(_load().orc_fft3d(a.shape[0], a.shape[1], a.shape[2], _d(a.view(np.float64)), sign, method),
+           "fft3d")
+    return a
+
+
+def dct1(x: np.ndarray, nout: int | None = None, method: int = 1) -> np.ndarray:
+    """Un-normalised DCT-I (REDFT00 convention) of n+1 reals, first nout outputs."""
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    n = x.size - 1
+    nout = n + 1 if nout is None else nout
+    out = np.empty(nout, dtype=np.float64)
+    _check(_load().orc_dct1(n, nout, _d(x), _d(out), method), "dct1")
+    return out
+
+
+def vg_window(N, h, alpha: float = ALPHA_DEFAULT) -> float:
+    h = _h3(h)
+    return float(_load().orc_vg_window(N[0], N[1], N[2], _d(h), alpha))
+
+
+def green_table(algorithm: int, N, h, g0: float = G0_DEFAULT, alpha: float = ALPHA_DEFAULT,
+                method: int = 0) -> np.ndarray:
+    """Real-space kernel table T of shape (Nx+1, Ny+1, Nz+1) for HOCKNEY / VICO / VICO_2."""
+    Nx, Ny, Nz = (int(v) for v in N)
+    h = _h3(h)
+    T = np.empty((Nx + 1, Ny + 1, Nz + 1), dtype=np.float64)
+    lib = _load()
+    if algorithm == HOCKNEY:
+        rc = lib.orc_green_table_he(Nx, Ny, Nz, _d(h), g0, _d(T))
+    elif algorithm == VICO:
+        rc = lib.orc_green_table_vg(Nx, Ny, Nz, _d(h), alpha, method, _d(T))
+    elif algorithm == VICO_2:
+        rc = lib.orc_green_table_vg2(Nx, Ny, Nz, _d(h), alpha, method, _d(T))
+    else:
+        raise ValueError("unknown algorithm")
+    _check(rc, "green_table")
+    return T
+
+
+def green_spectrum(T: np.ndarray, method: int = 0) -> np.ndarray:
+    """F{G2}: unscaled 3-D DFT of the mirrored table on the doubled grid, complex (2Nx,2Ny,2Nz)."""
+    T = np.ascontiguousarray(T, dtype=np.float64)
+    Nx, Ny, Nz = (s - 1 for s in T.shape)
+    G = np.empty((2 * Nx, 2 * Ny, 2 * Nz), dtype=np.complex128)
+    _check(_load().orc_green_spectrum(Nx, Ny, Nz, _d(T), method, _d(G.view(np.float64))),
+           "green_spectrum")
+    return G
+
+
+def solve_with_spectrum(Ghat: np.ndarray, h, rho: np.ndarray, method: int = 0) -> np.ndarray:
+    """Steps 1-5 of PAPER.md:67-82 with a precomputed F{G2}."""
+    rho = np.ascontiguousarray(rho, dtype=np.float64)
+    Nx, Ny, Nz = rho.shape
+    Ghat = np.ascontiguousarray(Ghat, dtype=np.complex128)
+    assert Ghat.shape == (2 * Nx, 2 * Ny, 2 * Nz)
+    h = _h3(h)
+    phi = np.empty_like(rho)
+    _check(_load().orc_solve(Nx, Ny, Nz, _d(h), _d(Ghat.view(np.float64)), method, _d(rho), _d(phi)),
+           "solve")
+    return phi
+
+
+def direct_sum(T: np.ndarray, h, rho: np.ndarray, idx: np.ndarray | None = None) -> np.ndarray:
+    """Def. O1: the plain O(V^2) discrete convolution, at all points or at flat indices ``idx``."""
+    rho = np.ascontiguousarray(rho, dtype=np.float64)
+    T = np.ascontiguousarray(T, dtype=np.float64)
+    Nx, Ny, Nz = rho.shape
+    assert T.shape == (Nx + 1, Ny + 1, Nz + 1)
+    h = _h3(h)
+    lib = _load()
+    if idx is None:
+        out = np.empty(rho.size, dtype=np.float64)
+        _check(lib.orc_direct_sum(Nx, Ny, Nz, _d(h), _d(T), _d(rho), rho.size, None, _d(out)),
+               "direct_sum")
+        return out.reshape(rho.shape)
+    idx = np.ascontiguousarray(idx, dtype=np.int64)
+    assert ctypes.sizeof(ctypes.c_long) == 8
+    out = np.empty(idx.size, dtype=np.float64)
+    _check(lib.orc_direct_sum(Nx, Ny, Nz, _d(h), _d(T), _d(rho), idx.size, idx.ctypes.data_as(_lp),
+                              _d(out)), "direct_sum")
+    return out
+
+
+class OraclePlan:
+    """plan / precompute_green / solve on host arrays, mirroring the product's four calls.
+
+    PAPER.md:65 (mesh, spacings), :199 (algorithm names), :98 (Green's function computed once and
+    reused every solve).
+    """
+
+    def __init__(self, N, h, algorithm: int, g0: float = G0_DEFAULT, alpha: float = ALPHA_DEFAULT,
+                 method: int = 0):
+        self.N = tuple(int(v) for v in N)
+        self.h = _h3(h).copy()
+        self.algorithm = int(algorithm)
+        self.g0, self.alpha, self.method = float(g0), float(alpha), int(method)
+        self.T = None
+        self.Ghat = None
+
+    def precompute_green(self, keep_spectrum: bool = True):
+        self.T = green_table(self.algorithm, self.N, self.h, self.g0, self.alpha, self.method)
+        self.Ghat = green_spectrum(self.T, self.method) if keep_spectrum else None
+        return self
+
+    def solve(self, rho: np.ndarray) -> np.ndarray:
+        if self.T is None:
+            raise RuntimeError("solve before precompute_green")
+        if self.Ghat is None:
+            self.Ghat = green_spectrum(self.T, self.method)
+        return solve_with_spectrum(self.Ghat, self.h, rho, self.method)
+
+    def direct_sum(self, rho: np.ndarray, idx=None) -> np.ndarray:
+        return direct_sum(self.T, self.h, rho, idx)
