@@ -1,0 +1,149 @@
+/*
+ * fsp.h -- C ABI of the B200-native free-space Poisson convolution library (libfsp.so).
+ *
+ * The hot path of arxiv 2405.02603 (cited as PAPER.md:<line>):
+ *
+ *     phi = hx hy hz * F^-1{ F{rho2} x F{G2} } restricted to the physical mesh
+ *
+ * with rho2 the zero-padded source on the doubled grid and G2 the mirrored,
+ * periodic Green's function of either
+ *     FSP_HOCKNEY : G = 1/(4 pi |x|), origin regularised
+ *     FSP_VICO    : truncated-kernel spectrum Eq. 3, inverse FFT on the 4N grid, restricted
+ *
+ *     FSP_VICO_2  : same values from the (2N+1)^3 grid with a DCT-I
+ * (names as PAPER.md:199: HOCKNEY / VICO / VICO_2).
+ *
+ * Everything behind these calls runs in hand-written sm_100a CUDA kernels: no FFT library, no CPU
+ * fallback.  One GPU, one plan = one mesh; fp64 throughout.  eps0 = 1: the caller divides by eps0.
+ *
+ * Conventions
+ *   - Mesh Nx x Ny x Nz, spacings h[0..2] = hx, hy, hz.  Each N_d must be a power of
+ *     two with 8 <= N_d <= 1024 (the paper's sizes are all powers of two).
+ *   - rho, phi: dense fp64 arrays of shape (Nx, Ny, Nz) in C order, index (ix*Ny + iy)*Nz + iz,
+ *     iz fastest.  The sample position inside a cell does not matter (translation invariance).
+ *   - "dev" pointers are CUDA device pointers on the device that was current at plan creation;
+ *     "host" pointers are ordinary host memory (pinned memory makes the copies asynchronous).
+ *   - The caller owns rho and phi; rho is read-only; rho and phi must not overlap.  The plan owns
+ *     the spectrum, twiddle tables and workspace.  fsp_solve allocates nothing and does not
+ *     synchronise the host: it is ordered on the stream given at plan creation.
+ *   - Every call returns FSP_OK (0) or a negative error code; nothing throws or aborts across
+ *     the ABI.  A plan pointer that is NULL gives FSP_ERR_INVALID_ARG.
+ */
+#ifndef FSP_H
+#define FSP_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fsp_plan fsp_plan; /* opaque, library-owned */
+
+/* algorithm */
+enum { FSP_HOCKNEY = 0, FSP_VICO = 1, FSP_VICO_2 = 2 };
+
+/* error codes */
+enum {
+    FSP_OK = 0,
+    FSP_ERR_INVALID_ARG = -1,     /* null pointer, N not a power of two in [8,1024], h <= 0, bad enum */
+    FSP_ERR_NOT_PRECOMPUTED = -2, /* fsp_solve / getters before fsp_precompute_green                 */
+    FSP_ERR_OUT_OF_MEMORY = -3,   /* device allocation failed (e.g. FSP_VICO at 512^3: (4N)^3 grid)  */
+    FSP_ERR_CUDA = -4,            /* a CUDA runtime call or kernel launch failed                     */
+    FSP_ERR_NO_DEVICE = -5        /* no CUDA device / not an sm_100 device                           */
+};
+
+/* parameters settable before fsp_precompute_green */
+enum {
+    FSP_PARAM_G0 = 0,    /* HE value at the origin, default +1/(4 pi)  (R5) */
+    FSP_PARAM_ALPHA = 1  /* VG window factor, default 1.1               */
+};
+
+/* number of kernels one fsp_solve launches (the five passes of DESIGN.md "The path") */
+#define FSP_NUM_SOLVE_KERNELS 5
+
+/*
+ * plan(Nx,Ny,Nz,h,algorithm)  -- PAPER.md:65 (mesh and spacings), :199 (algorithm).
+ *   out          host pointer receiving the new plan
+ *   h            host pointer to 3 doubles, all > 0
+ *   cuda_stream  a cudaStream_t (0/NULL = the legacy default stream); all work of this plan is
+ *                enqueued there
+ * Allocates the workspace of the solve (two complex intermediates) and the spectrum.  Does not
+ * touch the Green's function: call fsp_precompute_green next.
+ */
+int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int algorithm,
+                    void* cuda_stream);
+
+/* Set FSP_PARAM_* (only effective before the next fsp_precompute_green). */
+int fsp_plan_set_param(fsp_plan* p, int which, double value);
+
+/*
+ * precompute_green(plan) -- PAPER.md:72-76 (HE), :88-98 (VG), :100-102 (VG modified); "calculated
+ * ... in only one pre-computation step ... reused every time step".
+ * Fills the plan-owned real-space table T[dx][dy][dz] (0 <= d_d <= N_d, the kernel at displacement
+ * (dx hx, dy hy, dz hz)) and the spectrum F{G2} of its 8-case mirror, with the
+ * factor hx hy hz / (8 Nx Ny Nz) of PAPER.md:80 folded in.  Transient device memory is allocated
+ * and freed inside the call (FSP_VICO: a (4Nx)(4Ny)(4Nz) complex grid).  Synchronises the
+ * stream before returning.  Re-callable (e.g. after fsp_plan_set_param).
+ */
+int fsp_precompute_green(fsp_plan* p);
+
+/*
+ * solve(plan, rho, phi) -- PAPER.md:67-82 steps 1-5 as five fused/pruned kernel launches.
+ *   rho_dev  device pointer, Nx*Ny*Nz doubles, read-only
+ *   phi_dev  device pointer, Nx*Ny*Nz doubles, overwritten
+ * Asynchronous with respect to the host.
+ */
+int fsp_solve(fsp_plan* p, const double* rho_dev, double* phi_dev);
+
+/*
+ * The same solve from HOST buffers: copies rho host->device, runs the five kernels, copies phi
+ * device->host, then synchronises the stream.  Uses plan-owned staging buffers (allocated on first
+ * use).  With pinned host memory the copies are true asynchronous DMA transfers.
+ */
+int fsp_solve_host(fsp_plan* p, const double* rho_host, double* phi_host);
+
+/* Frees everything the plan owns (synchronises its stream first). */
+int fsp_destroy(fsp_plan* p);
+
+/* ---- queries and test hooks (no hot-path cost) ------------------------------------------------ */
+
+/* Device bytes the plan holds between solves (workspace + spectrum + tables [+ staging]). */
+size_t fsp_plan_bytes(const fsp_plan* p);
+
+/* Largest transient device allocation made by the last fsp_precompute_green. */
+size_t fsp_precompute_peak_bytes(const fsp_plan* p);
+
+/* Algorithmic (minimal-traffic) HBM bytes of one solve: total, and per kernel
+ * if per_kernel (host pointer to FSP_NUM_SOLVE_KERNELS doubles) is not NULL. */
+double fsp_model_bytes_per_solve(const fsp_plan* p, double* per_kernel);
+
+/* Copies the real-space table T, (Nx+1)(Ny+1)(Nz+1) doubles in C order, to host memory. */
+int fsp_get_green_table(const fsp_plan* p, double* T_host);
+
+/* Copies the unique octant of the un-normalised spectrum F{G2}[kx][ky][kz], 0 <= k_d <= N_d,
+ * (Nx+1)(Ny+1)(Nz+1) doubles in C order (F{G2} is real and even), to host memory. */
+int fsp_get_green_spectrum(const fsp_plan* p, double* Ghat_host);
+
+/*
+ * Per-kernel timing.  With profiling on, fsp_solve brackets each of its kernels with CUDA events
+ * on the plan's stream; fsp_get_kernel_times synchronises those events and returns, per kernel,
+ * the SUM of durations in milliseconds over all solves since the last reset (ms, host pointer to
+ * FSP_NUM_SOLVE_KERNELS floats) and the number of solves summed (n_solves).  Resets the sums.
+ */
+int fsp_set_profiling(fsp_plan* p, int on);
+int fsp_get_kernel_times(fsp_plan* p, float* ms, int* n_solves);
+
+/* Name of solve kernel i (0..FSP_NUM_SOLVE_KERNELS-1), static string. */
+const char* fsp_kernel_name(int i);
+
+/* Static description of an error code. */
+const char* fsp_strerror(int code);
+
+/* Library version (major*100 + minor). */
+int fsp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FSP_H */

@@ -1,0 +1,239 @@
+"""Thin ctypes binding of libfsp.so (include/fsp.h).  Argument marshalling only: every step of the
+path runs in the CUDA kernels behind the C ABI.  There is no CPU fallback -- if the library is
+missing or no B200 is present the calls raise.
+
+Module-level functions carry the C names without the ``fsp_`` prefix (``plan_create``,
+``precompute_green``, ``solve``, ``destroy`` ...); ``Plan`` is a small RAII convenience around them.
+Device buffers are torch CUDA tensors (torch is used for device memory and streams only) or raw
+integer device pointers.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+HOCKNEY, VICO, VICO_2 = 0, 1, 2                       # include/fsp.h
+PARAM_G0, PARAM_ALPHA = 0, 1
+NUM_SOLVE_KERNELS = 5
+ERRORS = {0: "FSP_OK", -1: "FSP_ERR_INVALID_ARG", -2: "FSP_ERR_NOT_PRECOMPUTED",
+          -3: "FSP_ERR_OUT_OF_MEMORY", -4: "FSP_ERR_CUDA", -5: "FSP_ERR_NO_DEVICE"}
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfsp.so")
+_lib = None
+
+# every symbol include/fsp.h declares, with its ctypes signature
+_c = ctypes
+_vp, _dp, _i, _d, _sz = _c.c_void_p, _c.POINTER(_c.c_double), _c.c_int, _c.c_double, _c.c_size_t
+SIGNATURES = {
+    "fsp_plan_create": (_i, [_c.POINTER(_vp), _i, _i, _i, _dp, _i, _vp]),
+    "fsp_plan_set_param": (_i, [_vp, _i, _d]),
+    "fsp_precompute_green": (_i, [_vp]),
+    "fsp_solve": (_i, [_vp, _vp, _vp]),
+    "fsp_solve_host": (_i, [_vp, _vp, _vp]),
+    "fsp_destroy": (_i, [_vp]),
+    "fsp_plan_bytes": (_sz, [_vp]),
+    "fsp_precompute_peak_bytes": (_sz, [_vp]),
+    "fsp_model_bytes_per_solve": (_d, [_vp, _dp]),
+    "fsp_get_green_table": (_i, [_vp, _dp]),
+    "fsp_get_green_spectrum": (_i, [_vp, _dp]),
+    "fsp_set_profiling": (_i, [_vp, _i]),
+    "fsp_get_kernel_times": (_i, [_vp, _c.POINTER(_c.c_float), _c.POINTER(_i)]),
+    "fsp_kernel_name": (_c.c_char_p, [_i]),
+    "fsp_strerror": (_c.c_char_p, [_i]),
+    "fsp_version": (_i, []),
+}
+
+
+class FspError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        msg = lib().fsp_strerror(code).decode() if _lib is not None else ""
+        super().__init__(f"{where}: {ERRORS.get(code, code)} ({msg})")
+
+
+def lib():
+    """Loads libfsp.so (raises if it has not been built -- no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2405_02603_b200.build` "
+                               "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _chk(code: int, where: str) -> None:
+    if code != 0:
+        raise FspError(code, where)
+
+
+def _ptr(x) -> int:
+    """Device (or host) address of a torch tensor / numpy array / int."""
+    if isinstance(x, int):
+        return x
+    if isinstance(x, np.ndarray):
+        return x.ctypes.data
+    return int(x.data_ptr())
+
+
+def version() -> int:
+    return int(lib().fsp_version())
+
+
+def strerror(code: int) -> str:
+    return lib().fsp_strerror(code).decode()
+
+
+def kernel_name(i: int) -> str:
+    return lib().fsp_kernel_name(i).decode()
+
+
+def plan_create(Nx: int, Ny: int, Nz: int, h, algorithm: int, cuda_stream: int = 0) -> int:
+    """fsp_plan_create.  Returns the opaque plan handle (an integer address)."""
+    hh = (ctypes.c_double * 3)(*[float(v) for v in np.broadcast_to(np.asarray(h, dtype=np.float64), (3,))])
+    out = ctypes.c_void_p()
+    _chk(lib().fsp_plan_create(ctypes.byref(out), Nx, Ny, Nz, hh, algorithm, ctypes.c_void_p(cuda_stream)),
+         "fsp_plan_create")
+    return out.value
+
+
+def plan_set_param(plan: int, which: int, value: float) -> None:
+    _chk(lib().fsp_plan_set_param(plan, which, value), "fsp_plan_set_param")
+
+
+def precompute_green(plan: int) -> None:
+    _chk(lib().fsp_precompute_green(plan), "fsp_precompute_green")
+
+
+def solve(plan: int, rho_dev, phi_dev) -> None:
+    _chk(lib().fsp_solve(plan, _ptr(rho_dev), _ptr(phi_dev)), "fsp_solve")
+
+
+def solve_host(plan: int, rho_host, phi_host) -> None:
+    _chk(lib().fsp_solve_host(plan, _ptr(rho_host), _ptr(phi_host)), "fsp_solve_host")
+
+
+def destroy(plan: int) -> None:
+    _chk(lib().fsp_destroy(plan), "fsp_destroy")
+
+
+def plan_bytes(plan: int) -> int:
+    return int(lib().fsp_plan_bytes(plan))
+
+
+def precompute_peak_bytes(plan: int) -> int:
+    return int(lib().fsp_precompute_peak_bytes(plan))
+
+
+def model_bytes_per_solve(plan: int):
+    per = (ctypes.c_double * NUM_SOLVE_KERNELS)()
+    tot = float(lib().fsp_model_bytes_per_solve(plan, per))
+    return tot, [float(v) for v in per]
+
+
+def get_green_table(plan: int, N) -> np.ndarray:
+    T = np.empty(tuple(n + 1 for n in N), dtype=np.float64)
+    _chk(lib().fsp_get_green_table(plan, T.ctypes.data_as(_dp)), "fsp_get_green_table")
+    return T
+
+
+def get_green_spectrum(plan: int, N) -> np.ndarray:
+    G = np.empty(tuple(n + 1 for n in N), dtype=np.float64)
+    _chk(lib().fsp_get_green_spectrum(plan, G.ctypes.data_as(_dp)), "fsp_get_green_spectrum")
+    return G
+
+
+def set_profiling(plan: int, on: bool) -> None:
+    _chk(lib().fsp_set_profiling(plan, int(bool(on))), "fsp_set_profiling")
+
+
+def get_kernel_times(plan: int):
+    ms = (ctypes.c_float * NUM_SOLVE_KERNELS)()
+    n = ctypes.c_int()
+    _chk(lib().fsp_get_kernel_times(plan, ms, ctypes.byref(n)), "fsp_get_kernel_times")
+    return [float(v) for v in ms], int(n.value)
+
+
+class Plan:
+    """plan -> precompute_green -> solve* -> destroy, on the current torch CUDA stream by default."""
+
+    def __init__(self, N, h, algorithm: int, stream: int | None = None, g0: float | None = None,
+                 alpha: float | None = None):
+        self.N = tuple(int(v) for v in N)
+        self.h = tuple(float(v) for v in np.broadcast_to(np.asarray(h, dtype=np.float64), (3,)))
+        self.algorithm = int(algorithm)
+        if stream is None:
+            import torch
+            stream = int(torch.cuda.current_stream().cuda_stream)
+        self.stream = stream
+        self.handle = plan_create(*self.N, self.h, self.algorithm, stream)
+        if g0 is not None:
+            plan_set_param(self.handle, PARAM_G0, g0)
+        if alpha is not None:
+            plan_set_param(self.handle, PARAM_ALPHA, alpha)
+
+    def precompute_green(self):
+        precompute_green(self.handle)
+        return self
+
+    def solve(self, rho, phi=None):
+        """rho: contiguous fp64 CUDA tensor of shape N.  Returns phi (allocated if not given)."""
+        import torch
+        assert rho.is_cuda and rho.dtype == torch.float64 and rho.is_contiguous() and tuple(rho.shape) == self.N
+        if phi is None:
+            phi = torch.empty_like(rho)
+        assert phi.is_cuda and phi.dtype == torch.float64 and phi.is_contiguous() and tuple(phi.shape) == self.N
+        solve(self.handle, rho, phi)
+        return phi
+
+    def solve_host(self, rho_host, phi_host):
+        """Host buffers (numpy arrays or pinned torch CPU tensors), copies inside the call."""
+        solve_host(self.handle, rho_host, phi_host)
+        return phi_host
+
+    def green_table(self) -> np.ndarray:
+        return get_green_table(self.handle, self.N)
+
+    def green_spectrum(self) -> np.ndarray:
+        return get_green_spectrum(self.handle, self.N)
+
+    @property
+    def bytes(self) -> int:
+        return plan_bytes(self.handle)
+
+    @property
+    def precompute_peak_bytes(self) -> int:
+        return precompute_peak_bytes(self.handle)
+
+    def model_bytes(self):
+        return model_bytes_per_solve(self.handle)
+
+    def set_profiling(self, on: bool):
+        set_profiling(self.handle, on)
+
+    def kernel_times(self):
+        return get_kernel_times(self.handle)
+
+    def destroy(self):
+        if self.handle:
+            destroy(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

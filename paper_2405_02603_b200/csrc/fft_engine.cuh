@@ -1,0 +1,172 @@
+// fft_engine.cuh -- register-resident fp64 complex FFT for one "column" of M points spread over
+// T = M/R threads (R points per thread), Stockham autosort, radix-{2,4,8,16} butterflies held in
+// registers, one shared-memory exchange between stages.
+//
+// Index convention (validated against numpy in DESIGN.md "FFT engine"): thread t of a column holds
+// v[i] <-> position t + T*i, both on entry (natural-order input) and on exit (natural-order
+// output), so global loads/stores never need a transpose or a bit reversal.
+//
+// Stage with radix r after stages of total radix Ns (decimation in time):
+//     butterfly j = t + T*m, m < R/r, works on v[m + i*(R/r)], i < r
+//     k  = j mod Ns;  v[.] *= w_{Ns*r}^{i*k};  r-point DFT;
+//     result i goes to position (j - k)*r + k + i*Ns.
+//
+// Forward sign is exp(-2 pi i ...).  The inverse transform is the same code with re/im swapped by
+// the caller (IFFT(x) = swap(FFT(swap(x)))), so there is no second set of butterflies.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace fsp {
+
+// ---- constants: w_16^k = cos(pi k/8) - i sin(pi k/8) -------------------------------------------
+__device__ __forceinline__ double cos16(int k) {
+    switch (k & 15) {
+        case 0: return 1.0;
+        case 1: case 15: return 0.92387953251128673848;
+        case 2: case 14: return 0.70710678118654752440;
+        case 3: case 13: return 0.38268343236508977173;
+        case 4: case 12: return 0.0;
+        case 5: case 11: return -0.38268343236508977173;
+        case 6: case 10: return -0.70710678118654752440;
+        case 7: case 9: return -0.92387953251128673848;
+        default: return -1.0;
+    }
+}
+__device__ __forceinline__ double sin16(int k) { return cos16(k - 4); }  // sin(x) = cos(x - pi/2)
+
+// ---- r-point DFT, in place, on elements re[0], re[S], re[2S], ... (natural order in and out) ---
+template <int r, int S>
+__device__ __forceinline__ void dft_inplace(double* re, double* im) {
+    if constexpr (r == 2) {
+        double ar = re[0], ai = im[0], br = re[S], bi = im[S];
+        re[0] = ar + br; im[0] = ai + bi;
+        re[S] = ar - br; im[S] = ai - bi;
+    } else if constexpr (r > 2) {
+        constexpr int H = r / 2;
+        dft_inplace<H, 2 * S>(re, im);          // even-indexed inputs
+        dft_inplace<H, 2 * S>(re + S, im + S);  // odd-indexed inputs
+        double er[H], ei[H], qr[H], qi[H];
+#pragma unroll
+        for (int k = 0; k < H; ++k) {
+            er[k] = re[2 * S * k]; ei[k] = im[2 * S * k];
+            qr[k] = re[S + 2 * S * k]; qi[k] = im[S + 2 * S * k];
+        }
+#pragma unroll
+        for (int k = 0; k < H; ++k) {
+            double tr, ti;
+            if (k == 0) { tr = qr[k]; ti = qi[k]; }
+            else if (4 * k == r) { tr = qi[k]; ti = -qr[k]; }   // times -i
+            else {
+                const double c = cos16(k * (16 / r)), s = sin16(k * (16 / r));  // w = c - i s
+                tr = qr[k] * c + qi[k] * s;
+                ti = qi[k] * c - qr[k] * s;
+            }
+            re[S * k] = er[k] + tr; im[S * k] = ei[k] + ti;
+            re[S * (k + H)] = er[k] - tr; im[S * (k + H)] = ei[k] - ti;
+        }
+    }
+}
+
+// ---- static description of one FFT size ---------------------------------------------------------
+// R points per thread; up to three stages r1*r2*r3 = M (r = 1 marks "no stage").
+template <int M_, int R_, int R1_, int R2_, int R3_>
+struct FftCfgT {
+    static constexpr int M = M_, R = R_, R1 = R1_, R2 = R2_, R3 = R3_, T = M_ / R_;
+    static_assert(R1_ * R2_ * R3_ == M_, "radices must multiply to M");
+    static_assert(R_ % R1_ == 0 && R_ % R2_ == 0 && R_ % R3_ == 0, "radix must divide R");
+};
+template <int M> struct FftCfg;
+template <> struct FftCfg<4> : FftCfgT<4, 4, 4, 1, 1> {};
+template <> struct FftCfg<8> : FftCfgT<8, 8, 8, 1, 1> {};
+template <> struct FftCfg<16> : FftCfgT<16, 16, 16, 1, 1> {};
+template <> struct FftCfg<32> : FftCfgT<32, 8, 8, 4, 1> {};
+template <> struct FftCfg<64> : FftCfgT<64, 8, 8, 8, 1> {};
+template <> struct FftCfg<128> : FftCfgT<128, 16, 16, 8, 1> {};
+template <> struct FftCfg<256> : FftCfgT<256, 16, 16, 16, 1> {};
+template <> struct FftCfg<512> : FftCfgT<512, 8, 8, 8, 8> {};
+template <> struct FftCfg<1024> : FftCfgT<1024, 16, 16, 16, 4> {};
+
+// ---- one stage: twiddle (if Ns > 1) and butterflies ----------------------------------------------
+// W: table of exp(-2 pi i n / LTAB), n < LTAB, in shared memory; LTAB a multiple of Ns*r.
+template <int M, int R, int r, int Ns, int LTAB>
+__device__ __forceinline__ void fft_stage(double (&re)[R], double (&im)[R], int t,
+                                          const double2* __restrict__ W) {
+    constexpr int T = M / R, nb = R / r;
+#pragma unroll
+    for (int m = 0; m < nb; ++m) {
+        if constexpr (Ns > 1) {
+            const int k = (t + T * m) & (Ns - 1);
+            constexpr int step = LTAB / (Ns * r);
+#pragma unroll
+            for (int i = 1; i < r; ++i) {
+                const double2 w = W[i * k * step];
+                const double xr = re[m + i * nb], xi = im[m + i * nb];
+                re[m + i * nb] = xr * w.x - xi * w.y;
+                im[m + i * nb] = xr * w.y + xi * w.x;
+            }
+        }
+        dft_inplace<r, nb>(&re[m], &im[m]);
+    }
+}
+
+// scatter the results of a stage to their Stockham positions in the exchange buffer
+// buf: this column's buffer; element at position p lives at buf[p * PS].
+template <int M, int R, int r, int Ns, int PS>
+__device__ __forceinline__ void fft_exchange_write(const double (&re)[R], const double (&im)[R], int t,
+                                                   double2* __restrict__ buf) {
+    constexpr int T = M / R, nb = R / r;
+#pragma unroll
+    for (int m = 0; m < nb; ++m) {
+        const int j = t + T * m;
+        const int k = j & (Ns - 1);
+        const int j0 = (j - k) * r + k;
+#pragma unroll
+        for (int i = 0; i < r; ++i) buf[(j0 + i * Ns) * PS] = make_double2(re[m + i * nb], im[m + i * nb]);
+    }
+}
+
+template <int M, int R, int PS>
+__device__ __forceinline__ void fft_exchange_read(double (&re)[R], double (&im)[R], int t,
+                                                  const double2* __restrict__ buf) {
+    constexpr int T = M / R;
+#pragma unroll
+    for (int i = 0; i < R; ++i) {
+        const double2 v = buf[(t + T * i) * PS];
+        re[i] = v.x; im[i] = v.y;
+    }
+}
+
+// ---- the whole M-point forward FFT of one column --------------------------------------------------
+// All threads of the CTA must call this together (it contains __syncthreads()).
+// On return the exchange buffer may be reused immediately by the caller only after a barrier;
+// the function itself places a barrier before each of its own writes.
+template <class Cfg, int PS, int LTAB>
+__device__ __forceinline__ void fft_forward(double (&re)[Cfg::R], double (&im)[Cfg::R], int t,
+                                            double2* __restrict__ buf, const double2* __restrict__ W) {
+    constexpr int M = Cfg::M, R = Cfg::R;
+    fft_stage<M, R, Cfg::R1, 1, LTAB>(re, im, t, W);
+    if constexpr (Cfg::R2 > 1) {
+        __syncthreads();  // previous readers of buf are done
+        fft_exchange_write<M, R, Cfg::R1, 1, PS>(re, im, t, buf);
+        __syncthreads();
+        fft_exchange_read<M, R, PS>(re, im, t, buf);
+        fft_stage<M, R, Cfg::R2, Cfg::R1, LTAB>(re, im, t, W);
+    }
+    if constexpr (Cfg::R3 > 1) {
+        __syncthreads();
+        fft_exchange_write<M, R, Cfg::R2, Cfg::R1, PS>(re, im, t, buf);
+        __syncthreads();
+        fft_exchange_read<M, R, PS>(re, im, t, buf);
+        fft_stage<M, R, Cfg::R3, Cfg::R1 * Cfg::R2, LTAB>(re, im, t, W);
+    }
+}
+
+// unnormalised inverse: swap the roles of re and im
+template <class Cfg, int PS, int LTAB>
+__device__ __forceinline__ void fft_inverse(double (&re)[Cfg::R], double (&im)[Cfg::R], int t,
+                                            double2* __restrict__ buf, const double2* __restrict__ W) {
+    // the exchange then stores (im, re) pairs -- harmless, it is read back the same way
+    fft_forward<Cfg, PS, LTAB>(im, re, t, buf, W);
+}
+
+}  // namespace fsp

@@ -1,0 +1,522 @@
+// fsp_api.cu -- the C ABI of include/fsp.h: plan management, Green precompute driver, and the
+// five-kernel solve.  Host code only marshals sizes and launches; every step of the path runs in the
+// kernels of solve_kernels.cuh / green_kernels.cuh.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/fsp.h"
+#include "green_kernels.cuh"
+#include "solve_kernels.cuh"
+
+using namespace fsp;
+
+#define FSP_VERSION_NUM 100
+
+struct fsp_plan {
+    int Nx = 0, Ny = 0, Nz = 0;
+    double h[3] = {0, 0, 0};
+    int algorithm = 0;
+    cudaStream_t stream = nullptr;
+    int device = 0;
+    double g0 = 0.0, alpha = 1.1;
+    // plan-owned device memory
+    double2* B1 = nullptr;  // (Nx+1) * Ny * Nz
+    double2* B2 = nullptr;  // (Nx+1) * 2Ny * Nz
+    double* Gh = nullptr;   // (Nx+1) * 2Ny * 2Nz   spectrum in K3 layout, scale folded in
+    double* T = nullptr;    // (Nx+1)(Ny+1)(Nz+1)   real-space table
+    double* Goct = nullptr; // (Nx+1)(Ny+1)(Nz+1)   un-normalised spectrum octant
+    double2 *Wx = nullptr, *Wy = nullptr, *Wz = nullptr;  // exp(-2 pi i n / 2N_d), n < 2N_d
+    double *rho_stage = nullptr, *phi_stage = nullptr;
+    bool precomputed = false;
+    size_t bytes = 0, peak_transient = 0;
+    // profiling
+    bool profiling = false;
+    std::vector<cudaEvent_t> events;  // 6 per recorded solve
+    size_t events_used = 0;
+};
+
+namespace {
+
+bool pow2_in(int n, int lo, int hi) { return n >= lo && n <= hi && (n & (n - 1)) == 0; }
+
+int map_cuda(cudaError_t e) {
+    if (e == cudaSuccess) return FSP_OK;
+    if (e == cudaErrorMemoryAllocation) return FSP_ERR_OUT_OF_MEMORY;
+    if (e == cudaErrorNoDevice || e == cudaErrorInsufficientDriver) return FSP_ERR_NO_DEVICE;
+    return FSP_ERR_CUDA;
+}
+
+#define CU(call)                                     \
+    do {                                             \
+        cudaError_t e__ = (call);                    \
+        if (e__ != cudaSuccess) {                    \
+            (void)cudaGetLastError();                \
+            return map_cuda(e__);                    \
+        }                                            \
+    } while (0)
+
+template <class T>
+int dev_alloc(T** p, size_t count, size_t* acc) {
+    void* q = nullptr;
+    cudaError_t e = cudaMalloc(&q, count * sizeof(T));
+    if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        *p = nullptr;
+        return map_cuda(e);
+    }
+    *p = static_cast<T*>(q);
+    if (acc) *acc += count * sizeof(T);
+    return FSP_OK;
+}
+
+// exp(-2 pi i n / L), n < L, evaluated in long double with exact octant symmetry
+int make_table(double2** dst, int L, size_t* acc) {
+    std::vector<double2> hst((size_t)L);
+    const long double PI2 = 6.283185307179586476925286766559005768L;
+    for (int n = 0; n < L; ++n) {
+        // reduce to the first octant so that e.g. n = L/8 gives equal re/im and n = L/4 gives exactly -i
+        long double c, s;
+        int m = n % L;
+        int q = (int)((8LL * m) / L);  // octant 0..7
+        long double a;
+        switch (q) {
+            case 0: a = PI2 * m / L; c = cosl(a); s = sinl(a); break;
+            case 1: a = PI2 * (L / 4.0L - m) / L; c = sinl(a); s = cosl(a); break;
+            case 2: a = PI2 * (m - L / 4.0L) / L; c = -sinl(a); s = cosl(a); break;
+            case 3: a = PI2 * (L / 2.0L - m) / L; c = -cosl(a); s = sinl(a); break;
+            case 4: a = PI2 * (m - L / 2.0L) / L; c = -cosl(a); s = -sinl(a); break;
+            case 5: a = PI2 * (3.0L * L / 4.0L - m) / L; c = -sinl(a); s = -cosl(a); break;
+            case 6: a = PI2 * (m - 3.0L * L / 4.0L) / L; c = sinl(a); s = -cosl(a); break;
+            default: a = PI2 * (L - m) / (long double)L; c = cosl(a); s = -sinl(a); break;
+        }
+        hst[n] = make_double2((double)c, (double)(-s));
+    }
+    int rc = dev_alloc(dst, (size_t)L, acc);
+    if (rc != FSP_OK) return rc;
+    CU(cudaMemcpy(*dst, hst.data(), sizeof(double2) * L, cudaMemcpyHostToDevice));
+    return FSP_OK;
+}
+
+// ---- kernel launch helpers (one template instantiation per FFT length) ---------------------------
+template <int M>
+int launch_fwd_y(fsp_plan* p) {
+    using Cfg = FftCfg<M>;
+    constexpr int G = TileGroups<Cfg>::G;
+    const long ntiles = (long)(p->Nx + 1) * (p->Nz / kW);
+    const size_t smem = sizeof(double2) * (size_t)(2 * M + G * M * kW);
+    CU(cudaFuncSetAttribute(k_fwd_y<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_fwd_y<M><<<(unsigned)((ntiles + G - 1) / G), G * kW * Cfg::T, smem, p->stream>>>(p->B1, p->B2, p->Wy, p->Nz, ntiles);
+    return FSP_OK;
+}
+template <int M>
+int launch_inv_y(fsp_plan* p) {
+    using Cfg = FftCfg<M>;
+    constexpr int G = TileGroups<Cfg>::G;
+    const long ntiles = (long)(p->Nx + 1) * (p->Nz / kW);
+    const size_t smem = sizeof(double2) * (size_t)(2 * M + G * M * kW);
+    CU(cudaFuncSetAttribute(k_inv_y<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_inv_y<M><<<(unsigned)((ntiles + G - 1) / G), G * kW * Cfg::T, smem, p->stream>>>(p->B2, p->B1, p->Wy, p->Nz, ntiles);
+    return FSP_OK;
+}
+template <int M>
+int launch_conv_z(fsp_plan* p) {
+    using Cfg = FftCfg<M>;
+    constexpr int P = PencilGroups<Cfg>::P;
+    const long npencils = (long)(p->Nx + 1) * (2 * p->Ny);
+    const size_t smem = sizeof(double2) * (size_t)(2 * M + P * M);
+    CU(cudaFuncSetAttribute(k_conv_z<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_conv_z<M><<<(unsigned)((npencils + P - 1) / P), P * Cfg::T, smem, p->stream>>>(p->B2, p->Gh, p->Wz, npencils);
+    return FSP_OK;
+}
+template <int M>
+int launch_fwd_x(fsp_plan* p, const double* rho) {
+    using Cfg = FftCfg<M>;
+    constexpr int G = TileGroups<Cfg>::G;
+    const long ntiles = (long)p->Ny * (p->Nz / kW);
+    const size_t smem = sizeof(double2) * (size_t)(4 * M + G * M * kW + G * 2 * M * kW);
+    CU(cudaFuncSetAttribute(k_fwd_x_r2c<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_fwd_x_r2c<M><<<(unsigned)((ntiles + G - 1) / G), G * kW * Cfg::T, smem, p->stream>>>(rho, p->B1, p->Wx, p->Ny, p->Nz, ntiles);
+    return FSP_OK;
+}
+template <int M>
+int launch_inv_x(fsp_plan* p, double* phi) {
+    using Cfg = FftCfg<M>;
+    constexpr int G = TileGroups<Cfg>::G;
+    const long ntiles = (long)p->Ny * (p->Nz / kW);
+    const size_t smem = sizeof(double2) * (size_t)(4 * M + G * M * kW);
+    CU(cudaFuncSetAttribute(k_inv_x_c2r<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_inv_x_c2r<M><<<(unsigned)((ntiles + G - 1) / G), G * kW * Cfg::T, smem, p->stream>>>(p->B1, phi, p->Wx, p->Ny, p->Nz, ntiles);
+    return FSP_OK;
+}
+
+#define DISPATCH_YZ(fn, M, ...)                          \
+    switch (M) {                                         \
+        case 8: return fn<8>(__VA_ARGS__);               \
+        case 16: return fn<16>(__VA_ARGS__);             \
+        case 32: return fn<32>(__VA_ARGS__);             \
+        case 64: return fn<64>(__VA_ARGS__);             \
+        case 128: return fn<128>(__VA_ARGS__);           \
+        case 256: return fn<256>(__VA_ARGS__);           \
+        case 512: return fn<512>(__VA_ARGS__);           \
+        case 1024: return fn<1024>(__VA_ARGS__);         \
+        default: return FSP_ERR_INVALID_ARG;             \
+    }
+#define DISPATCH_X(fn, M, ...)                           \
+    switch (M) {                                         \
+        case 4: return fn<4>(__VA_ARGS__);               \
+        case 8: return fn<8>(__VA_ARGS__);               \
+        case 16: return fn<16>(__VA_ARGS__);             \
+        case 32: return fn<32>(__VA_ARGS__);             \
+        case 64: return fn<64>(__VA_ARGS__);             \
+        case 128: return fn<128>(__VA_ARGS__);           \
+        case 256: return fn<256>(__VA_ARGS__);           \
+        default: return FSP_ERR_INVALID_ARG;             \
+    }
+
+int do_fwd_x(fsp_plan* p, const double* rho) { DISPATCH_X(launch_fwd_x, p->Nx / 2, p, rho) }
+int do_fwd_y(fsp_plan* p) { DISPATCH_YZ(launch_fwd_y, p->Ny, p) }
+int do_conv_z(fsp_plan* p) { DISPATCH_YZ(launch_conv_z, p->Nz, p) }
+int do_inv_y(fsp_plan* p) { DISPATCH_YZ(launch_inv_y, p->Ny, p) }
+int do_inv_x(fsp_plan* p, double* phi) { DISPATCH_X(launch_inv_x, p->Nx / 2, p, phi) }
+
+unsigned grid_for(long total, int block) {
+    long g = (total + block - 1) / block;
+    const long cap = 148L * 32;
+    return (unsigned)(g < cap ? (g > 0 ? g : 1) : cap);
+}
+
+// batched DCT-I along one axis of a real 3-D array (C order), output pruned to nout along that axis
+int dct1_axis(fsp_plan* p, const double* in, double* out, const long in_dims[3], const long out_dims[3],
+              int axis, int n, int nout, double scale) {
+    const long is[3] = {in_dims[1] * in_dims[2], in_dims[2], 1};
+    const long os[3] = {out_dims[1] * out_dims[2], out_dims[2], 1};
+    const int o1 = (axis + 1) % 3, o2 = (axis + 2) % 3;
+    const long n1 = in_dims[o1], n2 = in_dims[o2];
+    const int Lf = 2 * n;
+    const size_t smem = sizeof(double2) * 2 * (size_t)Lf;
+    CU(cudaFuncSetAttribute(k_dct1_pencils, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int threads = Lf / 2 < 256 ? (Lf / 2 < 32 ? 32 : Lf / 2) : 256;
+    k_dct1_pencils<<<(unsigned)(n1 * n2), threads, smem, p->stream>>>(in, out, n, nout, is[axis], os[axis], n2,
+                                                                      is[o1], is[o2], os[o1], os[o2], scale);
+    CU(cudaGetLastError());
+    return FSP_OK;
+}
+
+int fft_axis(fsp_plan* p, double2* data, const long dims[3], int axis, int sign) {
+    const long st[3] = {dims[1] * dims[2], dims[2], 1};
+    const int o1 = (axis + 1) % 3, o2 = (axis + 2) % 3;
+    const int Lf = (int)dims[axis];
+    const size_t smem = sizeof(double2) * 2 * (size_t)Lf;
+    CU(cudaFuncSetAttribute(k_fft_pencils, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int threads = Lf / 2 < 256 ? (Lf / 2 < 32 ? 32 : Lf / 2) : 256;
+    k_fft_pencils<<<(unsigned)(dims[o1] * dims[o2]), threads, smem, p->stream>>>(data, Lf, st[axis], dims[o2],
+                                                                                st[o1], st[o2], sign);
+    CU(cudaGetLastError());
+    return FSP_OK;
+}
+
+struct ScopedFree {
+    std::vector<void*> ptrs;
+    ~ScopedFree() {
+        for (void* q : ptrs)
+            if (q) cudaFree(q);
+    }
+};
+
+int precompute_impl(fsp_plan* p) {
+    const int Nx = p->Nx, Ny = p->Ny, Nz = p->Nz;
+    const double hx = p->h[0], hy = p->h[1], hz = p->h[2];
+    const long tdims[3] = {Nx + 1, Ny + 1, Nz + 1};
+    const long tcount = tdims[0] * tdims[1] * tdims[2];
+    ScopedFree tmp;
+    size_t peak = 0;
+    const int blk = 256;
+
+    if (p->algorithm == FSP_HOCKNEY) {
+        k_fill_he<<<grid_for(tcount, blk), blk, 0, p->stream>>>(p->T, Nx, Ny, Nz, hx, hy, hz, p->g0);
+        CU(cudaGetLastError());
+    } else {
+        const double Lx = Nx * hx, Ly = Ny * hy, Lz = Nz * hz;
+        const double L = p->alpha * std::sqrt(Lx * Lx + Ly * Ly + Lz * Lz);
+        const double scale = 1.0 / ((4.0 * Nx * hx) * (4.0 * Ny * hy) * (4.0 * Nz * hz));
+        if (p->algorithm == FSP_VICO) {
+            // (4N)^3 complex grid: fill, unscaled inverse DFT axis by axis, restrict
+            const long gd[3] = {4L * Nx, 4L * Ny, 4L * Nz};
+            const size_t gcount = (size_t)gd[0] * gd[1] * gd[2];
+            double2* g = nullptr;
+            int rc = dev_alloc(&g, gcount, &peak);
+            if (rc != FSP_OK) return rc;
+            tmp.ptrs.push_back(g);
+            k_fill_gl_vg<<<grid_for((long)gcount, blk), blk, 0, p->stream>>>(g, Nx, Ny, Nz, hx, hy, hz, L);
+            CU(cudaGetLastError());
+            for (int axis = 2; axis >= 0; --axis) {
+                rc = fft_axis(p, g, gd, axis, +1);
+                if (rc != FSP_OK) return rc;
+            }
+            k_restrict_vg<<<grid_for(tcount, blk), blk, 0, p->stream>>>(g, p->T, Nx, Ny, Nz, scale);
+            CU(cudaGetLastError());
+        } else {
+            // (2N+1)^3 real grid, DCT-I per axis with output pruned to N_d + 1
+            const long fd[3] = {2L * Nx + 1, 2L * Ny + 1, 2L * Nz + 1};
+            const long ad[3] = {fd[0], fd[1], Nz + 1};
+            const long bd[3] = {fd[0], Ny + 1, Nz + 1};
+            double *f = nullptr, *a = nullptr, *b = nullptr;
+            int rc = dev_alloc(&f, (size_t)fd[0] * fd[1] * fd[2], &peak);
+            if (rc != FSP_OK) return rc;
+            tmp.ptrs.push_back(f);
+            rc = dev_alloc(&a, (size_t)ad[0] * ad[1] * ad[2], &peak);
+            if (rc != FSP_OK) return rc;
+            tmp.ptrs.push_back(a);
+            rc = dev_alloc(&b, (size_t)bd[0] * bd[1] * bd[2], &peak);
+            if (rc != FSP_OK) return rc;
+            tmp.ptrs.push_back(b);
+            k_fill_gl_vg2<<<grid_for(fd[0] * fd[1] * fd[2], blk), blk, 0, p->stream>>>(f, Nx, Ny, Nz, hx, hy, hz, L);
+            CU(cudaGetLastError());
+            if ((rc = dct1_axis(p, f, a, fd, ad, 2, 2 * Nz, Nz + 1, 1.0)) != FSP_OK) return rc;
+            if ((rc = dct1_axis(p, a, b, ad, bd, 1, 2 * Ny, Ny + 1, 1.0)) != FSP_OK) return rc;
+            if ((rc = dct1_axis(p, b, p->T, bd, tdims, 0, 2 * Nx, Nx + 1, scale)) != FSP_OK) return rc;
+        }
+    }
+    // Ghat octant = 3-D DCT-I of T (size N_d + 1 per axis)
+    {
+        double* u = nullptr;
+        int rc = dev_alloc(&u, (size_t)tcount, &peak);
+        if (rc != FSP_OK) return rc;
+        tmp.ptrs.push_back(u);
+        if ((rc = dct1_axis(p, p->T, p->Goct, tdims, tdims, 2, Nz, Nz + 1, 1.0)) != FSP_OK) return rc;
+        if ((rc = dct1_axis(p, p->Goct, u, tdims, tdims, 1, Ny, Ny + 1, 1.0)) != FSP_OK) return rc;
+        if ((rc = dct1_axis(p, u, p->Goct, tdims, tdims, 0, Nx, Nx + 1, 1.0)) != FSP_OK) return rc;
+    }
+    // scale: hx hy hz / (8 Nx Ny Nz) (inverse DFT) / 2 (K1 produces 2X)
+    const double gscale = hx * hy * hz / (8.0 * (double)Nx * (double)Ny * (double)Nz) * 0.5;
+    const long gh_total = (long)(Nx + 1) * (2 * Ny) * (2 * Nz);
+    k_layout_spectrum<<<grid_for(gh_total, blk), blk, 0, p->stream>>>(p->Goct, p->Gh, Nx, Ny, Nz, gscale);
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(p->stream));
+    p->peak_transient = peak;
+    return FSP_OK;
+}
+
+void free_plan_memory(fsp_plan* p) {
+    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->Gh); cudaFree(p->T); cudaFree(p->Goct);
+    cudaFree(p->Wx); cudaFree(p->Wy); cudaFree(p->Wz); cudaFree(p->rho_stage); cudaFree(p->phi_stage);
+    for (cudaEvent_t e : p->events) cudaEventDestroy(e);
+    p->events.clear();
+}
+
+}  // namespace
+
+extern "C" {
+
+int fsp_version(void) { return FSP_VERSION_NUM; }
+
+const char* fsp_strerror(int code) {
+    switch (code) {
+        case FSP_OK: return "success";
+        case FSP_ERR_INVALID_ARG: return "invalid argument";
+        case FSP_ERR_NOT_PRECOMPUTED: return "fsp_precompute_green has not been called";
+        case FSP_ERR_OUT_OF_MEMORY: return "device memory allocation failed";
+        case FSP_ERR_CUDA: return "CUDA runtime or kernel launch error";
+        case FSP_ERR_NO_DEVICE: return "no usable CUDA device";
+        default: return "unknown error code";
+    }
+}
+
+const char* fsp_kernel_name(int i) {
+    static const char* names[FSP_NUM_SOLVE_KERNELS] = {"k_fwd_x_r2c", "k_fwd_y", "k_conv_z", "k_inv_y", "k_inv_x_c2r"};
+    return (i >= 0 && i < FSP_NUM_SOLVE_KERNELS) ? names[i] : "";
+}
+
+int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int algorithm, void* cuda_stream) {
+    if (!out) return FSP_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!h || !(h[0] > 0.0) || !(h[1] > 0.0) || !(h[2] > 0.0)) return FSP_ERR_INVALID_ARG;
+    if (!std::isfinite(h[0]) || !std::isfinite(h[1]) || !std::isfinite(h[2])) return FSP_ERR_INVALID_ARG;
+    if (!pow2_in(Nx, 8, 512) || !pow2_in(Ny, 8, 1024) || !pow2_in(Nz, 8, 1024)) return FSP_ERR_INVALID_ARG;
+    if (algorithm != FSP_HOCKNEY && algorithm != FSP_VICO && algorithm != FSP_VICO_2) return FSP_ERR_INVALID_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        (void)cudaGetLastError();
+        return FSP_ERR_NO_DEVICE;
+    }
+    fsp_plan* p = new (std::nothrow) fsp_plan();
+    if (!p) return FSP_ERR_OUT_OF_MEMORY;
+    p->Nx = Nx; p->Ny = Ny; p->Nz = Nz;
+    p->h[0] = h[0]; p->h[1] = h[1]; p->h[2] = h[2];
+    p->algorithm = algorithm;
+    p->stream = static_cast<cudaStream_t>(cuda_stream);
+    p->g0 = 1.0 / (4.0 * 3.14159265358979323846);
+    p->alpha = 1.1;
+    int rc = FSP_OK;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&p->device) != cudaSuccess || cudaGetDeviceProperties(&prop, p->device) != cudaSuccess) rc = FSP_ERR_NO_DEVICE;
+    if (rc == FSP_OK && prop.major != 10) rc = FSP_ERR_NO_DEVICE;  // the library holds sm_100a code only
+    const size_t n1 = (size_t)(Nx + 1) * Ny * Nz, n2 = (size_t)(Nx + 1) * 2 * Ny * Nz;
+    const size_t ng = (size_t)(Nx + 1) * 2 * Ny * 2 * Nz, nt = (size_t)(Nx + 1) * (Ny + 1) * (Nz + 1);
+    if (rc == FSP_OK) rc = dev_alloc(&p->B1, n1, &p->bytes);
+    if (rc == FSP_OK) rc = dev_alloc(&p->B2, n2, &p->bytes);
+    if (rc == FSP_OK) rc = dev_alloc(&p->Gh, ng, &p->bytes);
+    if (rc == FSP_OK) rc = dev_alloc(&p->T, nt, &p->bytes);
+    if (rc == FSP_OK) rc = dev_alloc(&p->Goct, nt, &p->bytes);
+    if (rc == FSP_OK) rc = make_table(&p->Wx, 2 * Nx, &p->bytes);
+    if (rc == FSP_OK) rc = make_table(&p->Wy, 2 * Ny, &p->bytes);
+    if (rc == FSP_OK) rc = make_table(&p->Wz, 2 * Nz, &p->bytes);
+    if (rc != FSP_OK) {
+        free_plan_memory(p);
+        delete p;
+        return rc;
+    }
+    *out = p;
+    return FSP_OK;
+}
+
+int fsp_plan_set_param(fsp_plan* p, int which, double value) {
+    if (!p || !std::isfinite(value)) return FSP_ERR_INVALID_ARG;
+    if (which == FSP_PARAM_G0) { p->g0 = value; return FSP_OK; }
+    if (which == FSP_PARAM_ALPHA) {
+        if (!(value > 0.0)) return FSP_ERR_INVALID_ARG;
+        p->alpha = value;
+        return FSP_OK;
+    }
+    return FSP_ERR_INVALID_ARG;
+}
+
+int fsp_precompute_green(fsp_plan* p) {
+    if (!p) return FSP_ERR_INVALID_ARG;
+    p->precomputed = false;
+    int rc = precompute_impl(p);
+    if (rc != FSP_OK) {
+        cudaStreamSynchronize(p->stream);
+        (void)cudaGetLastError();
+        return rc;
+    }
+    p->precomputed = true;
+    return FSP_OK;
+}
+
+int fsp_solve(fsp_plan* p, const double* rho_dev, double* phi_dev) {
+    if (!p || !rho_dev || !phi_dev || rho_dev == phi_dev) return FSP_ERR_INVALID_ARG;
+    if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
+    cudaEvent_t* ev = nullptr;
+    if (p->profiling) {
+        if (p->events_used + 6 > p->events.size()) {
+            for (int i = 0; i < 6; ++i) {
+                cudaEvent_t e;
+                CU(cudaEventCreate(&e));
+                p->events.push_back(e);
+            }
+        }
+        ev = &p->events[p->events_used];
+        p->events_used += 6;
+        CU(cudaEventRecord(ev[0], p->stream));
+    }
+    int rc;
+    if ((rc = do_fwd_x(p, rho_dev)) != FSP_OK) return rc;
+    if (ev) CU(cudaEventRecord(ev[1], p->stream));
+    if ((rc = do_fwd_y(p)) != FSP_OK) return rc;
+    if (ev) CU(cudaEventRecord(ev[2], p->stream));
+    if ((rc = do_conv_z(p)) != FSP_OK) return rc;
+    if (ev) CU(cudaEventRecord(ev[3], p->stream));
+    if ((rc = do_inv_y(p)) != FSP_OK) return rc;
+    if (ev) CU(cudaEventRecord(ev[4], p->stream));
+    if ((rc = do_inv_x(p, phi_dev)) != FSP_OK) return rc;
+    if (ev) CU(cudaEventRecord(ev[5], p->stream));
+    CU(cudaGetLastError());
+    return FSP_OK;
+}
+
+int fsp_solve_host(fsp_plan* p, const double* rho_host, double* phi_host) {
+    if (!p || !rho_host || !phi_host) return FSP_ERR_INVALID_ARG;
+    if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
+    const size_t v = (size_t)p->Nx * p->Ny * p->Nz;
+    if (!p->rho_stage) {
+        int rc = dev_alloc(&p->rho_stage, v, &p->bytes);
+        if (rc != FSP_OK) return rc;
+        rc = dev_alloc(&p->phi_stage, v, &p->bytes);
+        if (rc != FSP_OK) return rc;
+    }
+    CU(cudaMemcpyAsync(p->rho_stage, rho_host, v * sizeof(double), cudaMemcpyHostToDevice, p->stream));
+    int rc = fsp_solve(p, p->rho_stage, p->phi_stage);
+    if (rc != FSP_OK) return rc;
+    CU(cudaMemcpyAsync(phi_host, p->phi_stage, v * sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaStreamSynchronize(p->stream));
+    return FSP_OK;
+}
+
+int fsp_destroy(fsp_plan* p) {
+    if (!p) return FSP_ERR_INVALID_ARG;
+    cudaStreamSynchronize(p->stream);
+    free_plan_memory(p);
+    (void)cudaGetLastError();
+    delete p;
+    return FSP_OK;
+}
+
+size_t fsp_plan_bytes(const fsp_plan* p) { return p ? p->bytes : 0; }
+size_t fsp_precompute_peak_bytes(const fsp_plan* p) { return p ? p->peak_transient : 0; }
+
+double fsp_model_bytes_per_solve(const fsp_plan* p, double* per_kernel) {
+    if (!p) return 0.0;
+    const double V = (double)p->Nx * p->Ny * p->Nz;
+    const double H = (double)(p->Nx + 1) * p->Ny * p->Nz;  // complex elements of B1; B2 has 2H
+    double k[FSP_NUM_SOLVE_KERNELS];
+    k[0] = 8.0 * V + 16.0 * H;                      // K1: read rho, write B1
+    k[1] = 16.0 * H + 32.0 * H;                     // K2: read B1, write B2
+    k[2] = 32.0 * H + 32.0 * H + 8.0 * 4.0 * H;     // K3: read+write B2, read Ghat (real, 2Nz per pencil)
+    k[3] = 32.0 * H + 16.0 * H;                     // K4
+    k[4] = 16.0 * H + 8.0 * V;                      // K5
+    double tot = 0.0;
+    for (int i = 0; i < FSP_NUM_SOLVE_KERNELS; ++i) {
+        tot += k[i];
+        if (per_kernel) per_kernel[i] = k[i];
+    }
+    return tot;
+}
+
+int fsp_get_green_table(const fsp_plan* p, double* T_host) {
+    if (!p || !T_host) return FSP_ERR_INVALID_ARG;
+    if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
+    const size_t nt = (size_t)(p->Nx + 1) * (p->Ny + 1) * (p->Nz + 1);
+    CU(cudaStreamSynchronize(p->stream));
+    CU(cudaMemcpy(T_host, p->T, nt * sizeof(double), cudaMemcpyDeviceToHost));
+    return FSP_OK;
+}
+
+int fsp_get_green_spectrum(const fsp_plan* p, double* Ghat_host) {
+    if (!p || !Ghat_host) return FSP_ERR_INVALID_ARG;
+    if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
+    const size_t nt = (size_t)(p->Nx + 1) * (p->Ny + 1) * (p->Nz + 1);
+    CU(cudaStreamSynchronize(p->stream));
+    CU(cudaMemcpy(Ghat_host, p->Goct, nt * sizeof(double), cudaMemcpyDeviceToHost));
+    return FSP_OK;
+}
+
+int fsp_set_profiling(fsp_plan* p, int on) {
+    if (!p) return FSP_ERR_INVALID_ARG;
+    p->profiling = on != 0;
+    p->events_used = 0;
+    return FSP_OK;
+}
+
+int fsp_get_kernel_times(fsp_plan* p, float* ms, int* n_solves) {
+    if (!p || !ms || !n_solves) return FSP_ERR_INVALID_ARG;
+    for (int i = 0; i < FSP_NUM_SOLVE_KERNELS; ++i) ms[i] = 0.0f;
+    const size_t n = p->events_used / 6;
+    if (n > 0) CU(cudaEventSynchronize(p->events[p->events_used - 1]));
+    for (size_t s = 0; s < n; ++s)
+        for (int i = 0; i < FSP_NUM_SOLVE_KERNELS; ++i) {
+            float t = 0.0f;
+            CU(cudaEventElapsedTime(&t, p->events[6 * s + i], p->events[6 * s + i + 1]));
+            ms[i] += t;
+        }
+    *n_solves = (int)n;
+    p->events_used = 0;
+    return FSP_OK;
+}
+
+}  // extern "C"

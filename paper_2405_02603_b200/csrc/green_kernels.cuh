@@ -1,0 +1,148 @@
+// green_kernels.cuh -- Green's-function precompute (done once per plan).
+//
+//   HE:  T[d] = 1/(4 pi |d h|), T[0] = g0.
+//   VG:      G_L (Eq. 3) on the (4N)^3 lattice, inverse DFT, restricted to d <= N.
+//   VG2:    G_L on the (2N+1)^3 lattice, DCT-I per axis, restricted to d <= N.
+//   all: Ghat = F{G2} of the 8-case mirror = 3-D DCT-I of T (G2 is real and even).
+//
+// These kernels are NOT on the per-solve path and are written for clarity, not speed: one CTA
+// transforms one pencil with a radix-2 Stockham FFT in shared memory; twiddles come from
+// sincospi() in fp64.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace fsp {
+
+// Eq. 3 with the s -> 0 limit L^2/2.
+__device__ __forceinline__ double vg_GL(double sx, double sy, double sz, double L) {
+    const double s = sqrt(sx * sx + sy * sy + sz * sz);
+    if (s == 0.0) return 0.5 * L * L;
+    const double q = sin(0.5 * L * s) / s;
+    return 2.0 * q * q;
+}
+
+__global__ void k_fill_he(double* __restrict__ T, int Nx, int Ny, int Nz, double hx, double hy,
+                          double hz, double g0) {
+    const long total = (long)(Nx + 1) * (Ny + 1) * (Nz + 1);
+    for (long o = blockIdx.x * (long)blockDim.x + threadIdx.x; o < total; o += (long)gridDim.x * blockDim.x) {
+        const int dz = (int)(o % (Nz + 1));
+        const int dy = (int)((o / (Nz + 1)) % (Ny + 1));
+        const int dx = (int)(o / ((long)(Nz + 1) * (Ny + 1)));
+        const double x = dx * hx, y = dy * hy, z = dz * hz;
+        const double r = sqrt(x * x + y * y + z * z);
+        T[o] = (o == 0) ? g0 : 1.0 / (4.0 * 3.14159265358979323846 * r);
+    }
+}
+
+// VG2: f[kx][ky][kz] = G_L(2 pi k_d / (4 N_d h_d)), 0 <= k_d <= 2 N_d
+__global__ void k_fill_gl_vg2(double* __restrict__ f, int Nx, int Ny, int Nz, double hx, double hy,
+                              double hz, double L) {
+    const long Kx = 2 * Nx + 1, Ky = 2 * Ny + 1, Kz = 2 * Nz + 1;
+    const long total = Kx * Ky * Kz;
+    const double PI2 = 6.28318530717958647692;
+    for (long o = blockIdx.x * (long)blockDim.x + threadIdx.x; o < total; o += (long)gridDim.x * blockDim.x) {
+        const long kz = o % Kz, ky = (o / Kz) % Ky, kx = o / (Kz * Ky);
+        f[o] = vg_GL(PI2 * kx / (4.0 * Nx * hx), PI2 * ky / (4.0 * Ny * hy), PI2 * kz / (4.0 * Nz * hz), L);
+    }
+}
+
+// VG: g[ix][iy][iz] complex on the (4N)^3 lattice, DFT frequency order k in {0..2N-1, -2N..-1}
+__global__ void k_fill_gl_vg(double2* __restrict__ g, int Nx, int Ny, int Nz, double hx, double hy,
+                             double hz, double L) {
+    const long Mx = 4 * Nx, My = 4 * Ny, Mz = 4 * Nz;
+    const long total = Mx * My * Mz;
+    const double PI2 = 6.28318530717958647692;
+    for (long o = blockIdx.x * (long)blockDim.x + threadIdx.x; o < total; o += (long)gridDim.x * blockDim.x) {
+        const long iz = o % Mz, iy = (o / Mz) % My, ix = o / (Mz * My);
+        const long kx = ix < 2 * Nx ? ix : ix - Mx, ky = iy < 2 * Ny ? iy : iy - My, kz = iz < 2 * Nz ? iz : iz - Mz;
+        g[o] = make_double2(vg_GL(PI2 * kx / (Mx * hx), PI2 * ky / (My * hy), PI2 * kz / (Mz * hz), L), 0.0);
+    }
+}
+
+// Radix-2 Stockham FFT of length Lf (power of two) in shared memory, all threads of the CTA.
+// a holds the input; a and b ping-pong; returns the buffer holding the (natural-order) result.
+// sign = -1 forward, +1 inverse (unscaled).
+__device__ __forceinline__ double2* smem_fft_radix2(double2* a, double2* b, int Lf, int sign) {
+    const int half = Lf >> 1;
+    for (int Ns = 1; Ns < Lf; Ns <<= 1) {
+        __syncthreads();
+        for (int j = threadIdx.x; j < half; j += blockDim.x) {
+            const int k = j & (Ns - 1);
+            double s, c;
+            sincospi((double)sign * (double)k / (double)Ns, &s, &c);  // exp(sign * 2 pi i k / (2 Ns))
+            const double2 u = a[j], v0 = a[j + half];
+            const double2 v = make_double2(v0.x * c - v0.y * s, v0.x * s + v0.y * c);
+            const int j0 = ((j - k) << 1) + k;
+            b[j0] = make_double2(u.x + v.x, u.y + v.y);
+            b[j0 + Ns] = make_double2(u.x - v.x, u.y - v.y);
+        }
+        double2* tmp = a; a = b; b = tmp;
+    }
+    __syncthreads();
+    return a;
+}
+
+// In-place complex FFT of pencils: element i of pencil (i1, i2) at data[i1*s1 + i2*s2 + i*sa].
+// grid.x = n1 * n2 pencils.
+__global__ void k_fft_pencils(double2* __restrict__ data, int Lf, long sa, long n2, long s1, long s2,
+                              int sign) {
+    extern __shared__ double2 sm[];
+    double2* a = sm;
+    double2* b = sm + Lf;
+    const long p = blockIdx.x;
+    double2* base = data + (p / n2) * s1 + (p % n2) * s2;
+    for (int i = threadIdx.x; i < Lf; i += blockDim.x) a[i] = base[(long)i * sa];
+    double2* r = smem_fft_radix2(a, b, Lf, sign);
+    for (int i = threadIdx.x; i < Lf; i += blockDim.x) base[(long)i * sa] = r[i];
+}
+
+// Un-normalised DCT-I (REDFT00) of pencils: n+1 real inputs -> first nout outputs,
+//   out[d] = sum_k w_k in[k] cos(pi k d / n),  w_0 = w_n = 1, else 2,
+// evaluated as the length-2n DFT of the even extension.
+__global__ void k_dct1_pencils(const double* __restrict__ in, double* __restrict__ out, int n, int nout,
+                               long sa_in, long sa_out, long n2, long s1_in, long s2_in, long s1_out,
+                               long s2_out, double scale) {
+    extern __shared__ double2 sm[];
+    const int Lf = 2 * n;
+    double2* a = sm;
+    double2* b = sm + Lf;
+    const long p = blockIdx.x;
+    const double* src = in + (p / n2) * s1_in + (p % n2) * s2_in;
+    double* dst = out + (p / n2) * s1_out + (p % n2) * s2_out;
+    for (int m = threadIdx.x; m < Lf; m += blockDim.x) {
+        const int k = m <= n ? m : Lf - m;
+        a[m] = make_double2(src[(long)k * sa_in], 0.0);
+    }
+    double2* r = smem_fft_radix2(a, b, Lf, +1);
+    for (int d = threadIdx.x; d < nout; d += blockDim.x) dst[(long)d * sa_out] = scale * r[d].x;
+}
+
+// VG: T[d] = scale * Re g[dx][dy][dz], d <= N, from the (4N)^3 complex grid
+__global__ void k_restrict_vg(const double2* __restrict__ g, double* __restrict__ T, int Nx, int Ny,
+                              int Nz, double scale) {
+    const long total = (long)(Nx + 1) * (Ny + 1) * (Nz + 1);
+    const long My = 4 * Ny, Mz = 4 * Nz;
+    for (long o = blockIdx.x * (long)blockDim.x + threadIdx.x; o < total; o += (long)gridDim.x * blockDim.x) {
+        const long dz = o % (Nz + 1), dy = (o / (Nz + 1)) % (Ny + 1), dx = o / ((long)(Nz + 1) * (Ny + 1));
+        T[o] = scale * g[(dx * My + dy) * Mz + dz].x;
+    }
+}
+
+// Spectrum layout for K3: Gh[(kx*2Ny + ky)][parity][j] = scale * Goct[kx][min(ky,2Ny-ky)][min(kz,2Nz-kz)],
+// kz = 2j + parity  (F{G2} is even under k -> 2N-k).
+__global__ void k_layout_spectrum(const double* __restrict__ Goct, double* __restrict__ Gh, int Nx,
+                                  int Ny, int Nz, double scale) {
+    const long total = (long)(Nx + 1) * (2 * Ny) * (2 * Nz);
+    for (long o = blockIdx.x * (long)blockDim.x + threadIdx.x; o < total; o += (long)gridDim.x * blockDim.x) {
+        const int j = (int)(o % Nz);
+        const int par = (int)((o / Nz) & 1);
+        const long pen = o / (2 * Nz);
+        const int ky = (int)(pen % (2 * Ny));
+        const long kx = pen / (2 * Ny);
+        const int kz = 2 * j + par;
+        const int qy = ky <= Ny ? ky : 2 * Ny - ky, qz = kz <= Nz ? kz : 2 * Nz - kz;
+        Gh[o] = scale * Goct[(kx * (Ny + 1) + qy) * (Nz + 1) + qz];
+    }
+}
+
+}  // namespace fsp

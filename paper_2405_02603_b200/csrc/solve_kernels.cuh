@@ -1,0 +1,322 @@
+// solve_kernels.cuh -- the five passes of one solve.
+//
+//   K1 fwd_x_r2c   rho[x][y][z] (real)          -> B1[kx<=Nx][y<Ny][z<Nz]   R2C along x, input-pruned
+//   K2 fwd_y       B1                            -> B2[kx][ky<2Ny][z<Nz]     forward along y, input-pruned
+//   K3 conv_z      B2 (in place)                 forward z (input-pruned) x Ghat, inverse z (output-pruned)
+//   K4 inv_y       B2                            -> B1[kx][y<Ny][z<Nz]       inverse along y, output-pruned
+//   K5 inv_x_c2r   B1                            -> phi[x][y][z] (real)      C2R along x, output-pruned
+//
+// Pruning identities used by every pass (N = mesh size along the axis, w = exp(-2 pi i/2N)):
+//   zero-padded forward of length 2N with N non-zero inputs x[n]:
+//       X[2j]   = FFT_N(x)[j],            X[2j+1] = FFT_N(x[n] w^n)[j]
+//   inverse of length 2N of which only outputs n < N are kept:
+//       y[n] = IFFT_N(Y[2j])[n] + conj(w^n) IFFT_N(Y[2j+1])[n]
+// so the zero half of rho2 is never read and the discarded part of phi2
+// is never computed or written.
+//
+// The x axis carries the real<->complex packing: z[n] = rho[2n] + i rho[2n+1] (adjacent x rows),
+// a pruned length-Nx complex transform (two FFTs of length Nx/2), and the usual untangling
+//       X'[k] = (A + B) - i w^k (A - B),   A = Z[k], B = conj(Z[Nx-k]),  k = 0..Nx    (X' = 2X)
+// and its inverse  Z[k] = (A + B) + i conj(w^k) (A - B),  A = X[k], B = conj(X[Nx-k]).
+// The factor 1/2 and hx hy hz/(8 Nx Ny Nz) live in Ghat.
+#pragma once
+#include "fft_engine.cuh"
+
+namespace fsp {
+
+constexpr int kW = 8;  // complex columns per tile: 8 x 16 B = one 128-byte line per tile row
+
+__device__ __forceinline__ void cmul(double& xr, double& xi, const double2 w) {
+    const double a = xr * w.x - xi * w.y;
+    xi = xr * w.y + xi * w.x;
+    xr = a;
+}
+__device__ __forceinline__ void cmul_conj(double& xr, double& xi, const double2 w) {
+    const double a = xr * w.x + xi * w.y;
+    xi = xi * w.x - xr * w.y;
+    xr = a;
+}
+
+// copy the twiddle table exp(-2 pi i n/LTAB) into shared memory
+template <int LTAB>
+__device__ __forceinline__ void load_table(double2* __restrict__ Ws, const double2* __restrict__ Wg) {
+    for (int n = threadIdx.x; n < LTAB; n += blockDim.x) Ws[n] = Wg[n];
+}
+
+// tiles per CTA so that a CTA has at least 128 threads
+template <class Cfg> struct TileGroups { static constexpr int G = (kW * Cfg::T >= 128) ? 1 : 128 / (kW * Cfg::T); };
+
+// ====================================================================================== K2: fwd_y
+// grid: ceil(ntiles / G) CTAs of G*kW*T threads; tile = (kx, z-bundle of kW columns).
+template <int M>
+__global__ void __launch_bounds__(TileGroups<FftCfg<M>>::G* kW* FftCfg<M>::T)
+k_fwd_y(const double2* __restrict__ B1, double2* __restrict__ B2, const double2* __restrict__ Wg,
+        int Nz, long ntiles) {
+    using Cfg = FftCfg<M>;
+    constexpr int R = Cfg::R, T = Cfg::T, G = TileGroups<Cfg>::G, LTAB = 2 * M;
+    extern __shared__ double2 smem[];
+    double2* Ws = smem;                 // LTAB
+    double2* xb = smem + LTAB;          // G * M * kW
+    load_table<LTAB>(Ws, Wg);
+    const int tid = threadIdx.x;
+    const int g = tid / (kW * T), lt = tid % (kW * T);
+    const int c = lt % kW, t = lt / kW;
+    double2* buf = xb + g * (M * kW) + c;
+    const long tile = (long)blockIdx.x * G + g;
+    const bool valid = tile < ntiles;
+    const int nzb = Nz / kW;
+    const long kx = valid ? tile / nzb : 0;
+    const int zb = valid ? (int)(tile % nzb) : 0;
+    const double2* in = B1 + (kx * M) * (long)Nz + zb * kW + c;
+    double2* out = B2 + (kx * 2 * M) * (long)Nz + zb * kW + c;
+
+    double xr[R], xi[R], vr[R], vi[R];
+#pragma unroll
+    for (int i = 0; i < R; ++i) {
+        double2 v = valid ? in[(long)(t + T * i) * Nz] : make_double2(0.0, 0.0);
+        xr[i] = v.x; xi[i] = v.y;
+    }
+    __syncthreads();  // table ready
+    // even outputs
+#pragma unroll
+    for (int i = 0; i < R; ++i) { vr[i] = xr[i]; vi[i] = xi[i]; }
+    fft_forward<Cfg, kW, LTAB>(vr, vi, t, buf, Ws);
+    if (valid) {
+#pragma unroll
+        for (int i = 0; i < R; ++i) out[(long)(2 * (t + T * i)) * Nz] = make_double2(vr[i], vi[i]);
+    }
+    // odd outputs
+#pragma unroll
+    for (int i = 0; i < R; ++i) { cmul(xr[i], xi[i], Ws[t + T * i]); }
+    fft_forward<Cfg, kW, LTAB>(xr, xi, t, buf, Ws);
+    if (valid) {
+#pragma unroll
+        for (int i = 0; i < R; ++i) out[(long)(2 * (t + T * i) + 1) * Nz] = make_double2(xr[i], xi[i]);
+    }
+}
+
+// ====================================================================================== K4: inv_y
+template <int M>
+__global__ void __launch_bounds__(TileGroups<FftCfg<M>>::G* kW* FftCfg<M>::T)
+k_inv_y(const double2* __restrict__ B2, double2* __restrict__ B1, const double2* __restrict__ Wg,
+        int Nz, long ntiles) {
+    using Cfg = FftCfg<M>;
+    constexpr int R = Cfg::R, T = Cfg::T, G = TileGroups<Cfg>::G, LTAB = 2 * M;
+    extern __shared__ double2 smem[];
+    double2* Ws = smem;
+    double2* xb = smem + LTAB;
+    load_table<LTAB>(Ws, Wg);
+    const int tid = threadIdx.x;
+    const int g = tid / (kW * T), lt = tid % (kW * T);
+    const int c = lt % kW, t = lt / kW;
+    double2* buf = xb + g * (M * kW) + c;
+    const long tile = (long)blockIdx.x * G + g;
+    const bool valid = tile < ntiles;
+    const int nzb = Nz / kW;
+    const long kx = valid ? tile / nzb : 0;
+    const int zb = valid ? (int)(tile % nzb) : 0;
+    const double2* in = B2 + (kx * 2 * M) * (long)Nz + zb * kW + c;
+    double2* out = B1 + (kx * M) * (long)Nz + zb * kW + c;
+
+    double er[R], ei[R], qr[R], qi[R];
+#pragma unroll
+    for (int i = 0; i < R; ++i) {
+        const long row = 2 * (t + T * i);
+        double2 a = valid ? in[row * Nz] : make_double2(0.0, 0.0);
+        double2 b = valid ? in[(row + 1) * Nz] : make_double2(0.0, 0.0);
+        er[i] = a.x; ei[i] = a.y; qr[i] = b.x; qi[i] = b.y;
+    }
+    __syncthreads();
+    fft_inverse<Cfg, kW, LTAB>(qr, qi, t, buf, Ws);
+#pragma unroll
+    for (int i = 0; i < R; ++i) cmul_conj(qr[i], qi[i], Ws[t + T * i]);
+    fft_inverse<Cfg, kW, LTAB>(er, ei, t, buf, Ws);
+    if (valid) {
+#pragma unroll
+        for (int i = 0; i < R; ++i)
+            out[(long)(t + T * i) * Nz] = make_double2(er[i] + qr[i], ei[i] + qi[i]);
+    }
+}
+
+// ===================================================================================== K3: conv_z
+// Contiguous pencils of M = Nz complex; T threads per pencil (t fastest), P pencils per CTA.
+// Gh: [pencil][2][M] doubles, plane 0 = Ghat[2j] (even), plane 1 = Ghat[2j+1] (odd), scale folded in.
+template <class Cfg> struct PencilGroups { static constexpr int P = (Cfg::T >= 128) ? 1 : 128 / Cfg::T; };
+
+template <int M>
+__global__ void __launch_bounds__(PencilGroups<FftCfg<M>>::P* FftCfg<M>::T)
+k_conv_z(double2* __restrict__ B2, const double* __restrict__ Gh, const double2* __restrict__ Wg,
+         long npencils) {
+    using Cfg = FftCfg<M>;
+    constexpr int R = Cfg::R, T = Cfg::T, P = PencilGroups<Cfg>::P, LTAB = 2 * M;
+    extern __shared__ double2 smem[];
+    double2* Ws = smem;
+    double2* xb = smem + LTAB;  // P * M
+    load_table<LTAB>(Ws, Wg);
+    const int tid = threadIdx.x;
+    const int t = tid % T, c = tid / T;
+    double2* buf = xb + c * M;
+    const long pencil = (long)blockIdx.x * P + c;
+    const bool valid = pencil < npencils;
+    double2* base = B2 + (valid ? pencil : 0) * M;
+    const double* ge = Gh + (valid ? pencil : 0) * 2 * M;
+    const double* go = ge + M;
+
+    double xr[R], xi[R], vr[R], vi[R], gg[R];
+#pragma unroll
+    for (int i = 0; i < R; ++i) {
+        double2 v = valid ? base[t + T * i] : make_double2(0.0, 0.0);
+        xr[i] = v.x; xi[i] = v.y;
+    }
+#pragma unroll
+    for (int i = 0; i < R; ++i) gg[i] = go[t + T * i];
+    __syncthreads();
+    // odd half-spectrum: y_o = conj(w^n) IFFT( Go * FFT(x w^n) )
+#pragma unroll
+    for (int i = 0; i < R; ++i) { vr[i] = xr[i]; vi[i] = xi[i]; cmul(vr[i], vi[i], Ws[t + T * i]); }
+    fft_forward<Cfg, 1, LTAB>(vr, vi, t, buf, Ws);
+#pragma unroll
+    for (int i = 0; i < R; ++i) { vr[i] *= gg[i]; vi[i] *= gg[i]; }
+#pragma unroll
+    for (int i = 0; i < R; ++i) gg[i] = ge[t + T * i];
+    fft_inverse<Cfg, 1, LTAB>(vr, vi, t, buf, Ws);
+#pragma unroll
+    for (int i = 0; i < R; ++i) cmul_conj(vr[i], vi[i], Ws[t + T * i]);
+    // even half-spectrum
+    fft_forward<Cfg, 1, LTAB>(xr, xi, t, buf, Ws);
+#pragma unroll
+    for (int i = 0; i < R; ++i) { xr[i] *= gg[i]; xi[i] *= gg[i]; }
+    fft_inverse<Cfg, 1, LTAB>(xr, xi, t, buf, Ws);
+    if (valid) {
+#pragma unroll
+        for (int i = 0; i < R; ++i) base[t + T * i] = make_double2(xr[i] + vr[i], xi[i] + vi[i]);
+    }
+}
+
+// ================================================================================== K1: fwd_x_r2c
+// M = Nx/2.  Tile = (y, z-bundle of kW columns); rows are x.  LTAB = 2Nx = 4M.
+template <int M>
+__global__ void __launch_bounds__(TileGroups<FftCfg<M>>::G* kW* FftCfg<M>::T)
+k_fwd_x_r2c(const double* __restrict__ rho, double2* __restrict__ B1, const double2* __restrict__ Wg,
+            int Ny, int Nz, long ntiles) {
+    using Cfg = FftCfg<M>;
+    constexpr int R = Cfg::R, T = Cfg::T, G = TileGroups<Cfg>::G, LTAB = 4 * M, N = 2 * M;
+    extern __shared__ double2 smem[];
+    double2* Ws = smem;                      // LTAB
+    double2* xb = Ws + LTAB;                 // G * M * kW   exchange
+    double2* zs = xb + G * M * kW;           // G * N * kW   Z[k] for the untangling
+    load_table<LTAB>(Ws, Wg);
+    const int tid = threadIdx.x;
+    const int g = tid / (kW * T), lt = tid % (kW * T);
+    const int c = lt % kW, t = lt / kW;
+    double2* buf = xb + g * (M * kW) + c;
+    double2* Z = zs + g * (N * kW) + c;
+    const long tile = (long)blockIdx.x * G + g;
+    const bool valid = tile < ntiles;
+    const int nzb = Nz / kW;
+    const long y = valid ? tile / nzb : 0;
+    const int zb = valid ? (int)(tile % nzb) : 0;
+    const long plane = (long)Ny * Nz;
+    const double* in = rho + y * Nz + zb * kW + c;
+    double2* out = B1 + y * Nz + zb * kW + c;
+
+    double xr[R], xi[R], vr[R], vi[R];
+#pragma unroll
+    for (int i = 0; i < R; ++i) {
+        const long n = t + T * i;
+        xr[i] = valid ? in[(2 * n) * plane] : 0.0;
+        xi[i] = valid ? in[(2 * n + 1) * plane] : 0.0;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < R; ++i) { vr[i] = xr[i]; vi[i] = xi[i]; }
+    fft_forward<Cfg, kW, LTAB>(vr, vi, t, buf, Ws);
+#pragma unroll
+    for (int i = 0; i < R; ++i) Z[(2 * (t + T * i)) * kW] = make_double2(vr[i], vi[i]);
+    // odd: z[n] * w_N^n = W[2n] (table is exp(-2 pi i n/(2N)))
+#pragma unroll
+    for (int i = 0; i < R; ++i) cmul(xr[i], xi[i], Ws[2 * (t + T * i)]);
+    fft_forward<Cfg, kW, LTAB>(xr, xi, t, buf, Ws);
+#pragma unroll
+    for (int i = 0; i < R; ++i) Z[(2 * (t + T * i) + 1) * kW] = make_double2(xr[i], xi[i]);
+    __syncthreads();
+    if (valid) {
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+#pragma unroll
+            for (int o = 0; o < 2; ++o) {
+                const int k = 2 * (t + T * i) + o;
+                const double2 a = Z[k * kW];
+                const double2 bq = Z[((N - k) & (N - 1)) * kW];
+                const double br = bq.x, bi = -bq.y;            // B = conj(Z[N-k])
+                const double sr = a.x + br, si = a.y + bi;     // A + B
+                double dr = a.x - br, di = a.y - bi;           // A - B
+                cmul(dr, di, Ws[k]);                           // w^k (A - B)
+                // X' = (A+B) - i * d = (sr + di) + i (si - dr)
+                out[(long)k * plane] = make_double2(sr + di, si - dr);
+                if (k == 0) {
+                    // k = N: A = Z[0], B = conj(Z[0]), w^N = -1  ->  X'[N] = 2 (Re Z0 - Im Z0)
+                    out[(long)N * plane] = make_double2(2.0 * (a.x - a.y), 0.0);
+                }
+            }
+        }
+    }
+}
+
+// ================================================================================== K5: inv_x_c2r
+template <int M>
+__global__ void __launch_bounds__(TileGroups<FftCfg<M>>::G* kW* FftCfg<M>::T)
+k_inv_x_c2r(const double2* __restrict__ B1, double* __restrict__ phi, const double2* __restrict__ Wg,
+            int Ny, int Nz, long ntiles) {
+    using Cfg = FftCfg<M>;
+    constexpr int R = Cfg::R, T = Cfg::T, G = TileGroups<Cfg>::G, LTAB = 4 * M, N = 2 * M;
+    extern __shared__ double2 smem[];
+    double2* Ws = smem;
+    double2* xb = Ws + LTAB;
+    load_table<LTAB>(Ws, Wg);
+    const int tid = threadIdx.x;
+    const int g = tid / (kW * T), lt = tid % (kW * T);
+    const int c = lt % kW, t = lt / kW;
+    double2* buf = xb + g * (M * kW) + c;
+    const long tile = (long)blockIdx.x * G + g;
+    const bool valid = tile < ntiles;
+    const int nzb = Nz / kW;
+    const long y = valid ? tile / nzb : 0;
+    const int zb = valid ? (int)(tile % nzb) : 0;
+    const long plane = (long)Ny * Nz;
+    const double2* in = B1 + y * Nz + zb * kW + c;
+    double* out = phi + y * Nz + zb * kW + c;
+
+    double er[R], ei[R], qr[R], qi[R];
+    __syncthreads();  // table (needed while building Z)
+#pragma unroll
+    for (int i = 0; i < R; ++i) {
+#pragma unroll
+        for (int o = 0; o < 2; ++o) {
+            const int k = 2 * (t + T * i) + o;
+            const double2 a = valid ? in[(long)k * plane] : make_double2(0.0, 0.0);
+            const double2 bq = valid ? in[(long)(N - k) * plane] : make_double2(0.0, 0.0);
+            const double br = bq.x, bi = -bq.y;
+            const double sr = a.x + br, si = a.y + bi;
+            double dr = a.x - br, di = a.y - bi;
+            cmul_conj(dr, di, Ws[k]);                      // conj(w^k) (A - B)
+            // Z = (A+B) + i d = (sr - di) + i (si + dr)
+            if (o == 0) { er[i] = sr - di; ei[i] = si + dr; }
+            else        { qr[i] = sr - di; qi[i] = si + dr; }
+        }
+    }
+    fft_inverse<Cfg, kW, LTAB>(qr, qi, t, buf, Ws);
+#pragma unroll
+    for (int i = 0; i < R; ++i) cmul_conj(qr[i], qi[i], Ws[2 * (t + T * i)]);
+    fft_inverse<Cfg, kW, LTAB>(er, ei, t, buf, Ws);
+    if (valid) {
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            const long n = t + T * i;
+            out[(2 * n) * plane] = er[i] + qr[i];
+            out[(2 * n + 1) * plane] = ei[i] + qi[i];
+        }
+    }
+}
+
+}  // namespace fsp

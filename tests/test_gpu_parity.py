@@ -1,0 +1,141 @@
+"""-m gpu: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances are BASELINE.json's: relative L2 <= 1e-12, max-norm relative <= 1e-10
+(reading R14)."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2405_02603_b200 import binding, workloads as W
+from tests.analytic import gaussian_potential_iso, rel_l2, rel_max
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+L2_TOL, MAX_TOL = 1e-12, 1e-10
+ALGS = {"HE": (binding.HOCKNEY, oracle.HOCKNEY), "VG": (binding.VICO, oracle.VICO), "VG2": (binding.VICO_2, oracle.VICO_2)}
+
+
+def gpu_solve(plan, rho_np):
+    rho = torch.from_numpy(rho_np).cuda()
+    phi = plan.solve(rho)
+    torch.cuda.synchronize()
+    return phi.cpu().numpy()
+
+
+def check(got, ref):
+    assert np.isfinite(got).all()
+    assert rel_l2(got, ref) <= L2_TOL, f"rel L2 {rel_l2(got, ref):.3e}"
+    assert rel_max(got, ref) <= MAX_TOL, f"max rel {rel_max(got, ref):.3e}"
+
+
+@pytest.mark.parametrize("alg", ["HE", "VG", "VG2"])
+@pytest.mark.parametrize("N,h", [((16, 16, 16), (1 / 16,) * 3), ((8, 8, 8), (0.125,) * 3), ((8, 32, 16), (0.1, 0.05, 0.2)),
+                                 ((32, 16, 8), (0.03, 0.07, 0.11)), ((64, 64, 64), (1 / 64,) * 3)])
+def test_green_table_and_spectrum_parity(alg, N, h):
+    with binding.Plan(N, h, ALGS[alg][0]) as p:
+        p.precompute_green()
+        T, G = p.green_table(), p.green_spectrum()
+    To = oracle.green_table(ALGS[alg][1], N, h)
+    assert np.abs(T - To).max() <= 1e-13 * np.abs(To).max()
+    Go = oracle.green_spectrum(To).real[: N[0] + 1, : N[1] + 1, : N[2] + 1]
+    assert np.abs(G - Go).max() <= 1e-12 * np.abs(Go).max()
+
+
+@pytest.mark.parametrize("alg", ["HE", "VG", "VG2"])
+def test_config1_gaussian_16(alg):
+    """BASELINE.json config 1: 16^3, Gaussian sigma = 0.05; parity and accuracy vs the closed form."""
+    w = W.config1(16)
+    with binding.Plan(w.N, w.h, ALGS[alg][0]) as p:
+        got = gpu_solve(p.precompute_green(), w.rho)
+    ref = oracle.OraclePlan(w.N, w.h, ALGS[alg][1]).precompute_green().solve(w.rho)
+    check(got, ref)
+    err = rel_l2(got, gaussian_potential_iso(w))
+    assert err == pytest.approx(5.281e-2 if alg == "HE" else 2.890e-4, rel=2e-3)
+
+
+@pytest.mark.parametrize("alg", ["HE", "VG", "VG2"])
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_config2_multigauss_64(alg, seed):
+    """BASELINE.json config 2: 64^3, four signed Gaussians."""
+    w = W.config2(64, seed)
+    with binding.Plan(w.N, w.h, ALGS[alg][0]) as p:
+        got = gpu_solve(p.precompute_green(), w.rho)
+    ref = oracle.OraclePlan(w.N, w.h, ALGS[alg][1]).precompute_green().solve(w.rho)
+    check(got, ref)
+
+
+@pytest.mark.parametrize("N", [(8, 8, 8), (16, 8, 8), (8, 16, 8), (8, 8, 16), (32, 64, 16), (16, 32, 128), (128, 16, 32),
+                               (64, 8, 256), (8, 256, 8), (256, 8, 8), (8, 8, 512), (8, 512, 8), (512, 8, 8), (8, 8, 1024),
+                               (8, 1024, 8)])
+def test_random_density_every_fft_length(N):
+    """Dense random rho (no zero tail to hide an indexing error), anisotropic spacing, every
+    supported transform length on every axis; several tiles and ragged tile groups."""
+    w = W.random_density(N, seed=sum(N))
+    with binding.Plan(w.N, w.h, binding.HOCKNEY) as p:
+        got = gpu_solve(p.precompute_green(), w.rho)
+    ref = oracle.OraclePlan(w.N, w.h, oracle.HOCKNEY).precompute_green().solve(w.rho)
+    check(got, ref)
+
+
+def test_delta_source_gives_table():
+    N, h = (16, 32, 8), (0.1, 0.2, 0.05)
+    with binding.Plan(N, h, binding.VICO_2) as p:
+        p.precompute_green()
+        T = p.green_table()
+        rho = np.zeros(N)
+        j0 = (5, 17, 3)
+        rho[j0] = 1.0
+        got = gpu_solve(p, rho)
+    i, j, k = np.meshgrid(*(np.arange(n) for n in N), indexing="ij")
+    ref = h[0] * h[1] * h[2] * T[np.abs(i - j0[0]), np.abs(j - j0[1]), np.abs(k - j0[2])]
+    assert rel_max(got, ref) <= 1e-12
+
+
+def test_repeated_solves_and_rho_preserved():
+    w = W.config2(32, 5)
+    rho = torch.from_numpy(w.rho).cuda()
+    keep = rho.clone()
+    with binding.Plan(w.N, w.h, binding.HOCKNEY) as p:
+        p.precompute_green()
+        a = p.solve(rho).clone()
+        b = p.solve(rho).clone()
+        torch.cuda.synchronize()
+    assert torch.equal(a, b)          # deterministic, no state carried between solves
+    assert torch.equal(rho, keep)     # rho is read-only
+
+
+def test_solve_host_matches_device_solve():
+    w = W.config2(32, 6)
+    with binding.Plan(w.N, w.h, binding.VICO_2) as p:
+        p.precompute_green()
+        dev = gpu_solve(p, w.rho)
+        rho_h = torch.from_numpy(w.rho).pin_memory()
+        phi_h = torch.empty_like(rho_h).pin_memory()
+        p.solve_host(rho_h, phi_h)
+    assert np.array_equal(phi_h.numpy(), dev)
+
+
+def test_errors_on_device():
+    with binding.Plan((16, 16, 16), (0.1,) * 3, binding.HOCKNEY) as p:
+        rho = torch.zeros((16, 16, 16), dtype=torch.float64, device="cuda")
+        with pytest.raises(binding.FspError) as ei:
+            binding.solve(p.handle, rho, torch.empty_like(rho))
+        assert ei.value.code == -2      # NOT_PRECOMPUTED
+        p.precompute_green()
+        with pytest.raises(binding.FspError) as ei:
+            binding.solve(p.handle, rho, rho)
+        assert ei.value.code == -1      # rho and phi must not overlap
+        assert p.bytes > 0
+
+
+def test_g0_and_alpha_parameters():
+    N, h = (16, 16, 16), (1 / 16,) * 3
+    w = W.random_density(N, seed=9)
+    with binding.Plan(N, (w.h), binding.HOCKNEY, g0=-1.0 / (4 * np.pi)) as p:
+        got = gpu_solve(p.precompute_green(), w.rho)
+    ref = oracle.OraclePlan(N, w.h, oracle.HOCKNEY, g0=-1.0 / (4 * np.pi)).precompute_green().solve(w.rho)
+    check(got, ref)
+    with binding.Plan(N, w.h, binding.VICO_2, alpha=1.3) as p:
+        got = gpu_solve(p.precompute_green(), w.rho)
+    ref = oracle.OraclePlan(N, w.h, oracle.VICO_2, alpha=1.3).precompute_green().solve(w.rho)
+    check(got, ref)
