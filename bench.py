@@ -1,0 +1,390 @@
+#!/usr/bin/env python
+"""bench.py -- times the free-space Poisson solve (the whole hot path: five fused/pruned FFT passes,
+include/fsp.h `fsp_solve`) on B200 and prints ONE JSON line (contract: see DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 512|256|beam] [--alg HE|VG2]
+    python bench.py --impl reference ...      # the CPU oracle, as it stands, on a bounded sample
+
+A step = one solve of one batch (one density) with the Green spectrum already precomputed
+(computed once, reused every time step).  N > 1 = N independent replicas ("replicas
+only"): no data-path collective, value = solves of all ranks / max time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+WORKLOADS = {
+    # name -> (BASELINE.json config index, builder name, kwargs, description)
+    "512": (4, "config5", {}, "configs[4]: 512^3 fp64 unit cube, Gaussian sigma=0.05 (doubled grid 1024^3)"),
+    "256": (2, "config3", {}, "configs[2]: 256^3 fp64 unit cube, Gaussian sigma=0.05 + 1e-6 seeded noise (doubled grid 512^3)"),
+    "beam": (3, "config4", {}, "configs[3]: 128x128x512 fp64, beam-like Gaussian"),
+    "64": (1, "config2", {}, "configs[1]: 64^3 fp64, 4 seeded Gaussians (L2-resident, launch-bound)"),
+}
+ALGS = {"HE": 0, "VG": 1, "VG2": 2}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="512", choices=sorted(WORKLOADS))
+    ap.add_argument("--alg", default="HE", choices=sorted(ALGS))
+    ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
+    ap.add_argument("--no-extras", action="store_true", help="skip the 256^3 / VG2 side measurements")
+    return ap.parse_args()
+
+
+def peaks():
+    """Measured roofline denominators (driver-written), else the profiling guide's fallback."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, STREAM-style copy)"
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc = index, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "50"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, smax, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(smax), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle legs (the ONLY places bench.py touches oracle/): cpu_baseline and --impl reference
+# ------------------------------------------------------------------------------------------------
+def _sample_workload(wname: str, edge: int):
+    """The same analytic density as the bench workload, sampled on a smaller mesh (bounded sample)."""
+    from paper_2405_02603_b200 import workloads as W
+    if wname == "beam":
+        return W.config4((edge // 4, edge // 4, edge))
+    if wname == "64":
+        return W.config2(min(edge, 64), 1)
+    if wname == "256":
+        return W.config3(edge, 4)
+    return W.config1(edge)
+
+
+def oracle_time_solves(wname: str, alg: str, steps: int, warmup: int, budget_s: float):
+    """Times the oracle's solve (PAPER.md:67-82 steps 1-5, un-pruned, radix-2 FFT) as it stands on the
+    host cores.  Returns (seconds per solve of the sample, sample workload, threads, description)."""
+    import oracle
+    oalg = {"HE": oracle.HOCKNEY, "VG": oracle.VICO, "VG2": oracle.VICO_2}[alg]
+    # calibrate on 32^3, then take the largest edge whose (steps+warmup) solves fit the budget
+    w = _sample_workload(wname, 32)
+    pl = oracle.OraclePlan(w.N, w.h, oracle.HOCKNEY).precompute_green()
+    pl.solve(w.rho)
+    t0 = time.perf_counter(); pl.solve(w.rho); t32 = time.perf_counter() - t0
+    edge = 32
+    for cand in (64, 128):
+        est = t32 * (cand / 32) ** 3 * 1.4 * (steps + warmup + 1)   # +1: spectrum build; 1.4: log factor, cache
+        if est <= budget_s:
+            edge = cand
+    w = _sample_workload(wname, edge)
+    # VICO's (4N)^3 table is not needed for timing the solve: the solve is identical for every
+    # algorithm given the spectrum; VG spectra are built with the cheap VICO_2 route.
+    pl = oracle.OraclePlan(w.N, w.h, oracle.VICO_2 if oalg != oracle.HOCKNEY else oalg).precompute_green()
+    for _ in range(warmup):
+        pl.solve(w.rho)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        pl.solve(w.rho)
+    dt = (time.perf_counter() - t0) / max(steps, 1)
+    desc = (f"oracle O2 (oracle/fsp_oracle.c, un-pruned radix-2 FFT convolution) full solve of the same "
+            f"density on a {w.N[0]}x{w.N[1]}x{w.N[2]} mesh, {steps} solve(s); grid-points/s scaled to the "
+            f"workload's V (FFT log factor ignored: flatters the CPU by <= 25%)")
+    return dt, w, oracle.num_threads(), desc
+
+
+def run_reference(args):
+    """--impl reference: the oracle is the reference arm for this tier (no reference code exists)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2405_02603_b200 import workloads as W  # noqa: F401  (input generators only)
+    cfg_idx, _, _, wdesc = WORKLOADS[args.workload]
+    dt, w, threads, desc = oracle_time_solves(args.workload, args.alg, args.steps, args.warmup, budget_s=150.0)
+    Vs = w.N[0] * w.N[1] * w.N[2]
+    V = workload_points(args.workload)
+    pts_per_s = Vs / dt
+    value = pts_per_s / V
+    line = {
+        "impl": "reference", "metric": "solves/s", "value": value, "unit": "solves/s",
+        "grid_points_per_s": pts_per_s, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": dt * 1e3 * (V / Vs), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wdesc, "baseline_config_index": cfg_idx, "algorithm": args.alg,
+                   "note": "ms_per_step is the sample's time scaled by V_workload/V_sample"},
+        "cpu_baseline": {"value": value, "unit": "solves/s", "cores": threads, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": "solves/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def workload_points(wname: str) -> int:
+    return {"512": 512 ** 3, "256": 256 ** 3, "beam": 128 * 128 * 512, "64": 64 ** 3}[wname]
+
+
+# ------------------------------------------------------------------------------------------------
+# GPU arm
+# ------------------------------------------------------------------------------------------------
+def _analytic_error(w, phi):
+    """rel. L2 error of phi against the closed-form potential erf(r/(sqrt2 s))/(4 pi r) of the
+    isotropic Gaussian, evaluated with torch on the device.  A guard that the timed
+    kernels did the work, not a parity claim (parity lives in tests/)."""
+    import math
+    import torch
+    if len(w.gaussians) != 1 or len(set(w.gaussians[0][2])) != 1:
+        return None
+    amp, c, s = w.gaussians[0]
+    xs = [torch.from_numpy(__import__("paper_2405_02603_b200").workloads.cell_centres(w.N, w.lo, w.hi)[d]).cuda() - c[d]
+          for d in range(3)]
+    num = torch.zeros((), dtype=torch.float64, device="cuda")
+    den = torch.zeros((), dtype=torch.float64, device="cuda")
+    for i in range(w.N[0]):  # plane by plane: bounded temporaries
+        r = torch.sqrt(xs[0][i] ** 2 + xs[1][:, None] ** 2 + xs[2][None, :] ** 2)
+        ex = amp * torch.erf(r / (math.sqrt(2.0) * s[0])) / (4.0 * math.pi * r)
+        num += ((phi[i] - ex) ** 2).sum()
+        den += (ex ** 2).sum()
+    return float(torch.sqrt(num / den))
+
+
+def time_solves(plan, rho, phi, steps, warmup, sampler=None, barrier=None):
+    """W untimed + exactly K timed solves between two CUDA events on the plan's stream."""
+    import torch
+    for _ in range(warmup):
+        plan.solve(rho, phi)
+    torch.cuda.synchronize()
+    if barrier:
+        barrier()
+        torch.cuda.synchronize()
+    if sampler:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        plan.solve(rho, phi)
+    e1.record()
+    torch.cuda.synchronize()
+    if barrier:
+        barrier()
+    clocks = sampler.stop() if sampler else None
+    return e0.elapsed_time(e1) / steps, clocks
+
+
+def kernel_breakdown(plan, rho, phi, nsolves):
+    """Per-kernel CUDA-event durations (events recorded by libfsp on its own stream)."""
+    import torch
+    plan.set_profiling(True)
+    for _ in range(nsolves):
+        plan.solve(rho, phi)
+    torch.cuda.synchronize()
+    ms, n = plan.kernel_times()
+    plan.set_profiling(False)
+    return [m / max(n, 1) for m in ms]
+
+
+def run_b200(args):
+    import numpy as np
+    import torch
+    from paper_2405_02603_b200 import binding, workloads as W
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    barrier = (lambda: dist.barrier()) if dist else None
+
+    cfg_idx, builder, kw, wdesc = WORKLOADS[args.workload]
+    w = getattr(W, builder)(**kw)
+    V = int(np.prod(w.N))
+    peak, peak_src = peaks()
+
+    plan = binding.Plan(w.N, w.h, ALGS[args.alg])
+    t0 = time.perf_counter()
+    plan.precompute_green()
+    torch.cuda.synchronize()
+    t_pre = time.perf_counter() - t0
+    rho_h = torch.from_numpy(w.rho).pin_memory()
+    rho = rho_h.cuda(non_blocking=True)
+    phi = torch.empty_like(rho)
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    ms, clocks = time_solves(plan, rho, phi, args.steps, args.warmup, sampler, barrier)
+    if dist:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * 1e3 / ms
+
+    # per-kernel roofline (events on the launching stream, inside libfsp)
+    model_total, model_k = plan.model_bytes()
+    kms = kernel_breakdown(plan, rho, phi, max(3, min(args.steps, 10)))
+    names = [binding.kernel_name(i) for i in range(binding.NUM_SOLVE_KERNELS)]
+    dom = max(range(len(kms)), key=lambda i: kms[i])
+    kernels = [{"name": names[i], "ms": kms[i], "model_bytes": model_k[i],
+                "achieved_gbs": model_k[i] / (kms[i] * 1e-3) / 1e9 if kms[i] > 0 else None,
+                "share": kms[i] / sum(kms)} for i in range(len(kms))]
+    roofline = {"bound": "hbm", "kernel": names[dom], "achieved": kernels[dom]["achieved_gbs"], "peak": peak,
+                "unit": "GB/s", "frac": kernels[dom]["achieved_gbs"] / peak, "traffic": _ncu_traffic(names[dom], args.workload),
+                "peak_source": peak_src,
+                "whole_solve": {"model_bytes": model_total, "achieved": model_total / (ms * 1e-3) / 1e9,
+                                "frac": model_total / (ms * 1e-3) / 1e9 / peak,
+                                "frac_of_nominal_8TBs": model_total / (ms * 1e-3) / 1e9 / 8000.0},
+                "kernels": kernels}
+
+    err = _analytic_error(w, phi)
+
+    # e2e: the public host-buffer call, H2D of rho and D2H of phi inside the timed region
+    phi_h = torch.empty_like(rho_h).pin_memory()
+    for _ in range(2):
+        plan.solve_host(rho_h, phi_h)
+    if barrier:
+        barrier()
+    ne = args.steps
+    t0 = time.perf_counter()
+    for _ in range(ne):
+        plan.solve_host(rho_h, phi_h)       # synchronises the stream before returning
+    torch.cuda.synchronize()
+    t_e2e = (time.perf_counter() - t0) / ne
+    if dist:
+        t = torch.tensor([t_e2e], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        t_e2e = float(t.item())
+    e2e_ok = bool(torch.equal(phi_h.cuda(), phi))
+    e2e = {"value": world / t_e2e, "unit": "solves/s", "h2d_bytes_per_step": 8 * V, "d2h_bytes_per_step": 8 * V,
+           "ms_per_step": t_e2e * 1e3, "matches_device_solve": e2e_ok, "host_memory": "pinned"}
+    plan_bytes, pre_peak = plan.bytes, plan.precompute_peak_bytes
+    plan.destroy()
+    del rho, phi, phi_h, rho_h
+
+    line = {
+        "metric": "solves/s", "value": value, "unit": "solves/s", "grid_points_per_s": value * V,
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wdesc, "baseline_config_index": cfg_idx, "algorithm": args.alg,
+                   "mesh": list(w.N), "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2": "no flush: each pass streams > 2 GB (> 126 MB L2) at 512^3 / >= 400 MB at 256^3"},
+        "clocks": clocks, "roofline": roofline, "e2e": e2e,
+        "gpu_launches": binding.NUM_SOLVE_KERNELS * args.steps,
+        "precompute_green_s": t_pre, "plan_bytes": plan_bytes, "precompute_peak_bytes": pre_peak,
+        "rel_l2_vs_closed_form": err,
+    }
+    if world == 1 and not args.no_extras:
+        line["also"] = extras(args, peak)
+    if world == 1 and rank == 0 and not args.no_cpu_baseline:
+        dt, ws, threads, desc = oracle_time_solves(args.workload, args.alg, steps=2, warmup=1, budget_s=25.0)
+        pts = ws.N[0] * ws.N[1] * ws.N[2] / dt
+        line["cpu_baseline"] = {"value": pts / V, "unit": "solves/s", "cores": threads, "kind": "oracle",
+                                "sample": desc, "grid_points_per_s": pts}
+    if rank == 0:
+        print(json.dumps(line))
+    if dist:
+        dist.destroy_process_group()
+    return 0
+
+
+def _ncu_traffic(kernel: str, wname: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
+    committed `ncu --set full` summary under profiles/ (null until one exists for this workload)."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if not os.path.exists(path):
+        return None
+    try:
+        return json.load(open(path)).get(wname, {}).get(kernel)
+    except Exception:
+        return None
+
+
+def extras(args, peak):
+    """Side measurements (N = 1 only): the other HBM-bound BASELINE configs and the VG spectrum, same
+    timing loop.  Not bench lines of their own."""
+    import numpy as np
+    import torch
+    from paper_2405_02603_b200 import binding, workloads as W
+    out = {}
+    todo = [("256", "HE"), ("beam", "HE"), (args.workload, "VG2" if args.alg == "HE" else "HE")]
+    for wname, alg in todo:
+        if (wname, alg) == (args.workload, args.alg):
+            continue
+        _, builder, kw, wdesc = WORKLOADS[wname]
+        w = getattr(W, builder)(**kw)
+        V = int(np.prod(w.N))
+        with binding.Plan(w.N, w.h, ALGS[alg]) as plan:
+            t0 = time.perf_counter(); plan.precompute_green(); torch.cuda.synchronize()
+            t_pre = time.perf_counter() - t0
+            rho = torch.from_numpy(w.rho).cuda()
+            phi = torch.empty_like(rho)
+            steps = 100 if V <= 256 ** 3 else args.steps
+            ms, _ = time_solves(plan, rho, phi, steps, 10)
+            model_total, _ = plan.model_bytes()
+            out[f"{wname}_{alg}"] = {"workload": wdesc, "ms_per_solve": ms, "solves_per_s": 1e3 / ms,
+                                     "grid_points_per_s": V * 1e3 / ms, "steps": steps,
+                                     "model_gbs": model_total / (ms * 1e-3) / 1e9,
+                                     "frac_of_measured_peak": model_total / (ms * 1e-3) / 1e9 / peak,
+                                     "precompute_green_s": t_pre, "rel_l2_vs_closed_form": _analytic_error(w, phi)}
+        del rho, phi
+    return out
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    sys.exit(run_reference(a) if a.impl == "reference" else run_b200(a))
