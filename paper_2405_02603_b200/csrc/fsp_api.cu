@@ -27,7 +27,11 @@ struct fsp_plan {
     // plan-owned device memory
     double2* B1 = nullptr;  // (Nx+1) * Ny * Nz
     double2* B2 = nullptr;  // (Nx+1) * 2Ny * Nz
-    double* Gh = nullptr;   // (Nx+1) * 2Ny * 2Nz   spectrum in K3 layout, scale folded in
+    double* Gh = nullptr;   // (Nx+1) * 2Ny * 2Nz   spectrum, full K3-v1 layout (only when Nz = 1024)
+    double* Gk = nullptr;   // (Nx+1)(Ny+1)(Nz+2)   spectrum octant in K3-v2 layout, scale folded in
+    double2* TWz = nullptr; // Nz                   stage-2 twiddles of the z transform (fft_warp.cuh)
+    bool z_warp = false;    // K3 v2 (k_conv_z_w) is used
+    int sm_count = 148;
     double* T = nullptr;    // (Nx+1)(Ny+1)(Nz+1)   real-space table
     double* Goct = nullptr; // (Nx+1)(Ny+1)(Nz+1)   un-normalised spectrum octant
     double2 *Wx = nullptr, *Wy = nullptr, *Wz = nullptr;  // exp(-2 pi i n / 2N_d), n < 2N_d
@@ -74,33 +78,51 @@ int dev_alloc(T** p, size_t count, size_t* acc) {
     return FSP_OK;
 }
 
-// exp(-2 pi i n / L), n < L, evaluated in long double with exact octant symmetry
-int make_table(double2** dst, int L, size_t* acc) {
-    std::vector<double2> hst((size_t)L);
+// exp(-2 pi i m / L) evaluated in long double with exact octant symmetry
+double2 unit_root(long m, long L) {
     const long double PI2 = 6.283185307179586476925286766559005768L;
-    for (int n = 0; n < L; ++n) {
-        // reduce to the first octant so that e.g. n = L/8 gives equal re/im and n = L/4 gives exactly -i
-        long double c, s;
-        int m = n % L;
-        int q = (int)((8LL * m) / L);  // octant 0..7
-        long double a;
-        switch (q) {
-            case 0: a = PI2 * m / L; c = cosl(a); s = sinl(a); break;
-            case 1: a = PI2 * (L / 4.0L - m) / L; c = sinl(a); s = cosl(a); break;
-            case 2: a = PI2 * (m - L / 4.0L) / L; c = -sinl(a); s = cosl(a); break;
-            case 3: a = PI2 * (L / 2.0L - m) / L; c = -cosl(a); s = sinl(a); break;
-            case 4: a = PI2 * (m - L / 2.0L) / L; c = -cosl(a); s = -sinl(a); break;
-            case 5: a = PI2 * (3.0L * L / 4.0L - m) / L; c = -sinl(a); s = -cosl(a); break;
-            case 6: a = PI2 * (m - 3.0L * L / 4.0L) / L; c = sinl(a); s = -cosl(a); break;
-            default: a = PI2 * (L - m) / (long double)L; c = cosl(a); s = -sinl(a); break;
-        }
-        hst[n] = make_double2((double)c, (double)(-s));
+    m %= L;
+    // reduce to the first octant so that e.g. m = L/8 gives equal re/im and m = L/4 gives exactly -i
+    long double c, s, a;
+    const int q = (int)((8LL * m) / L);  // octant 0..7
+    switch (q) {
+        case 0: a = PI2 * m / L; c = cosl(a); s = sinl(a); break;
+        case 1: a = PI2 * (L / 4.0L - m) / L; c = sinl(a); s = cosl(a); break;
+        case 2: a = PI2 * (m - L / 4.0L) / L; c = -sinl(a); s = cosl(a); break;
+        case 3: a = PI2 * (L / 2.0L - m) / L; c = -cosl(a); s = sinl(a); break;
+        case 4: a = PI2 * (m - L / 2.0L) / L; c = -cosl(a); s = -sinl(a); break;
+        case 5: a = PI2 * (3.0L * L / 4.0L - m) / L; c = -sinl(a); s = -cosl(a); break;
+        case 6: a = PI2 * (m - 3.0L * L / 4.0L) / L; c = sinl(a); s = -cosl(a); break;
+        default: a = PI2 * (L - m) / (long double)L; c = cosl(a); s = -sinl(a); break;
     }
-    int rc = dev_alloc(dst, (size_t)L, acc);
+    return make_double2((double)c, (double)(-s));
+}
+
+int upload_table(double2** dst, const std::vector<double2>& hst, size_t* acc) {
+    int rc = dev_alloc(dst, hst.size(), acc);
     if (rc != FSP_OK) return rc;
-    CU(cudaMemcpy(*dst, hst.data(), sizeof(double2) * L, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(*dst, hst.data(), sizeof(double2) * hst.size(), cudaMemcpyHostToDevice));
     return FSP_OK;
 }
+
+// exp(-2 pi i n / L), n < L
+int make_table(double2** dst, int L, size_t* acc) {
+    std::vector<double2> hst((size_t)L);
+    for (int n = 0; n < L; ++n) hst[n] = unit_root(n, L);
+    return upload_table(dst, hst, acc);
+}
+
+// stage-2 twiddles of the two-stage transform of fft_warp.cuh: tw[i*R1 + j] = exp(-2 pi i (i j) / M)
+int make_stage2_table(double2** dst, int M, int R1, size_t* acc) {
+    std::vector<double2> hst((size_t)M);
+    const int R2 = M / R1;
+    for (int i = 0; i < R2; ++i)
+        for (int j = 0; j < R1; ++j) hst[(size_t)i * R1 + j] = unit_root((long)i * j, M);
+    return upload_table(dst, hst, acc);
+}
+
+template <int M>
+int stage2_table_for(double2** dst, size_t* acc) { return make_stage2_table(dst, M, Fft2Cfg<M>::R1, acc); }
 
 // ---- kernel launch helpers (one template instantiation per FFT length) ---------------------------
 template <int M>
@@ -131,6 +153,23 @@ int launch_conv_z(fsp_plan* p) {
     const size_t smem = sizeof(double2) * (size_t)(2 * M + P * M);
     CU(cudaFuncSetAttribute(k_conv_z<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k_conv_z<M><<<(unsigned)((npencils + P - 1) / P), P * Cfg::T, smem, p->stream>>>(p->B2, p->Gh, p->Wz, npencils);
+    return FSP_OK;
+}
+template <int M>
+int launch_conv_z_w(fsp_plan* p) {
+    using Z = ConvZ<M>;
+    const long ngroups = (long)(p->Nx + 1) * (2 * p->Ny) / Z::G;
+    const size_t smem = Z::smem_bytes();
+    static int occ = 0;  // CTAs per SM, queried once per transform length
+    if (occ == 0) {
+        CU(cudaFuncSetAttribute(k_conv_z_w<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_conv_z_w<M>, Z::WARPS * 32, smem));
+        if (occ < 1) return FSP_ERR_CUDA;
+    }
+    long grid = (long)p->sm_count * occ;
+    const long need = (ngroups + Z::WARPS - 1) / Z::WARPS;
+    if (grid > need) grid = need;
+    k_conv_z_w<M><<<(unsigned)grid, Z::WARPS * 32, smem, p->stream>>>(p->B2, p->Gk, p->TWz, p->Wz, p->Ny, ngroups);
     return FSP_OK;
 }
 template <int M>
@@ -180,7 +219,21 @@ int launch_inv_x(fsp_plan* p, double* phi) {
 
 int do_fwd_x(fsp_plan* p, const double* rho) { DISPATCH_X(launch_fwd_x, p->Nx / 2, p, rho) }
 int do_fwd_y(fsp_plan* p) { DISPATCH_YZ(launch_fwd_y, p->Ny, p) }
-int do_conv_z(fsp_plan* p) { DISPATCH_YZ(launch_conv_z, p->Nz, p) }
+#define DISPATCH_W(fn, M, ...)                           \
+    switch (M) {                                         \
+        case 8: return fn<8>(__VA_ARGS__);               \
+        case 16: return fn<16>(__VA_ARGS__);             \
+        case 32: return fn<32>(__VA_ARGS__);             \
+        case 64: return fn<64>(__VA_ARGS__);             \
+        case 128: return fn<128>(__VA_ARGS__);           \
+        case 256: return fn<256>(__VA_ARGS__);           \
+        case 512: return fn<512>(__VA_ARGS__);           \
+        default: return FSP_ERR_INVALID_ARG;             \
+    }
+int do_conv_z_v1(fsp_plan* p) { DISPATCH_YZ(launch_conv_z, p->Nz, p) }
+int do_conv_z_w(fsp_plan* p) { DISPATCH_W(launch_conv_z_w, p->Nz, p) }
+int do_conv_z(fsp_plan* p) { return p->z_warp ? do_conv_z_w(p) : do_conv_z_v1(p); }
+int make_z_stage2_table(fsp_plan* p) { DISPATCH_W(stage2_table_for, p->Nz, &p->TWz, &p->bytes) }
 int do_inv_y(fsp_plan* p) { DISPATCH_YZ(launch_inv_y, p->Ny, p) }
 int do_inv_x(fsp_plan* p, double* phi) { DISPATCH_X(launch_inv_x, p->Nx / 2, p, phi) }
 
@@ -294,8 +347,13 @@ int precompute_impl(fsp_plan* p) {
     }
     // scale: hx hy hz / (8 Nx Ny Nz) (inverse DFT) / 2 (K1 produces 2X)
     const double gscale = hx * hy * hz / (8.0 * (double)Nx * (double)Ny * (double)Nz) * 0.5;
-    const long gh_total = (long)(Nx + 1) * (2 * Ny) * (2 * Nz);
-    k_layout_spectrum<<<grid_for(gh_total, blk), blk, 0, p->stream>>>(p->Goct, p->Gh, Nx, Ny, Nz, gscale);
+    if (p->z_warp) {
+        const long gk_total = (long)(Nx + 1) * (Ny + 1) * (Nz + 2);
+        k_layout_spectrum_oct<<<grid_for(gk_total, blk), blk, 0, p->stream>>>(p->Goct, p->Gk, Nx, Ny, Nz, gscale);
+    } else {
+        const long gh_total = (long)(Nx + 1) * (2 * Ny) * (2 * Nz);
+        k_layout_spectrum<<<grid_for(gh_total, blk), blk, 0, p->stream>>>(p->Goct, p->Gh, Nx, Ny, Nz, gscale);
+    }
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(p->stream));
     p->peak_transient = peak;
@@ -303,7 +361,7 @@ int precompute_impl(fsp_plan* p) {
 }
 
 void free_plan_memory(fsp_plan* p) {
-    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->Gh); cudaFree(p->T); cudaFree(p->Goct);
+    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->Gh); cudaFree(p->Gk); cudaFree(p->TWz); cudaFree(p->T); cudaFree(p->Goct);
     cudaFree(p->Wx); cudaFree(p->Wy); cudaFree(p->Wz); cudaFree(p->rho_stage); cudaFree(p->phi_stage);
     for (cudaEvent_t e : p->events) cudaEventDestroy(e);
     p->events.clear();
@@ -353,14 +411,18 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
     p->g0 = 1.0 / (4.0 * 3.14159265358979323846);
     p->alpha = 1.1;
     int rc = FSP_OK;
-    cudaDeviceProp prop;
+    cudaDeviceProp prop{};
     if (cudaGetDevice(&p->device) != cudaSuccess || cudaGetDeviceProperties(&prop, p->device) != cudaSuccess) rc = FSP_ERR_NO_DEVICE;
     if (rc == FSP_OK && prop.major != 10) rc = FSP_ERR_NO_DEVICE;  // the library holds sm_100a code only
     const size_t n1 = (size_t)(Nx + 1) * Ny * Nz, n2 = (size_t)(Nx + 1) * 2 * Ny * Nz;
     const size_t ng = (size_t)(Nx + 1) * 2 * Ny * 2 * Nz, nt = (size_t)(Nx + 1) * (Ny + 1) * (Nz + 1);
     if (rc == FSP_OK) rc = dev_alloc(&p->B1, n1, &p->bytes);
     if (rc == FSP_OK) rc = dev_alloc(&p->B2, n2, &p->bytes);
-    if (rc == FSP_OK) rc = dev_alloc(&p->Gh, ng, &p->bytes);
+    p->z_warp = Nz <= 512;
+    p->sm_count = prop.multiProcessorCount > 0 ? prop.multiProcessorCount : 148;
+    if (rc == FSP_OK && !p->z_warp) rc = dev_alloc(&p->Gh, ng, &p->bytes);
+    if (rc == FSP_OK && p->z_warp) rc = dev_alloc(&p->Gk, (size_t)(Nx + 1) * (Ny + 1) * (Nz + 2), &p->bytes);
+    if (rc == FSP_OK && p->z_warp) rc = make_z_stage2_table(p);
     if (rc == FSP_OK) rc = dev_alloc(&p->T, nt, &p->bytes);
     if (rc == FSP_OK) rc = dev_alloc(&p->Goct, nt, &p->bytes);
     if (rc == FSP_OK) rc = make_table(&p->Wx, 2 * Nx, &p->bytes);
@@ -467,7 +529,9 @@ double fsp_model_bytes_per_solve(const fsp_plan* p, double* per_kernel) {
     double k[FSP_NUM_SOLVE_KERNELS];
     k[0] = 8.0 * V + 16.0 * H;                      // K1: read rho, write B1
     k[1] = 16.0 * H + 32.0 * H;                     // K2: read B1, write B2
-    k[2] = 32.0 * H + 32.0 * H + 8.0 * 4.0 * H;     // K3: read+write B2, read Ghat (real, 2Nz per pencil)
+    // K3: read+write B2, read Ghat (real): the unique octant once (v2), or 2Nz values per pencil (v1)
+    k[2] = 32.0 * H + 32.0 * H +
+           (p->z_warp ? 8.0 * (double)(p->Nx + 1) * (p->Ny + 1) * (p->Nz + 2) : 8.0 * 4.0 * H);
     k[3] = 32.0 * H + 16.0 * H;                     // K4
     k[4] = 16.0 * H + 8.0 * V;                      // K5
     double tot = 0.0;

@@ -145,4 +145,21 @@ __global__ void k_layout_spectrum(const double* __restrict__ Goct, double* __res
     }
 }
 
+// Spectrum layout for K3 v2 (k_conv_z_w): the unique octant only, rows de-interleaved by parity of kz:
+//   Gk[(kx*(Ny+1) + qy)*(Nz+2) + m]              = scale * Goct[kx][qy][2m],    m <= Nz/2   (E)
+//   Gk[(kx*(Ny+1) + qy)*(Nz+2) + Nz/2 + 1 + m]   = scale * Goct[kx][qy][2m+1],  m <  Nz/2   (O)
+__global__ void k_layout_spectrum_oct(const double* __restrict__ Goct, double* __restrict__ Gk, int Nx,
+                                      int Ny, int Nz, double scale) {
+    const long row = Nz + 2;
+    const long total = (long)(Nx + 1) * (Ny + 1) * row;
+    for (long o = blockIdx.x * (long)blockDim.x + threadIdx.x; o < total; o += (long)gridDim.x * blockDim.x) {
+        const int c = (int)(o % row);
+        const long pr = o / row;
+        double v = 0.0;
+        if (c <= Nz / 2) v = Goct[pr * (Nz + 1) + 2 * c];
+        else if (c <= Nz) v = Goct[pr * (Nz + 1) + 2 * (c - Nz / 2 - 1) + 1];
+        Gk[o] = scale * v;
+    }
+}
+
 }  // namespace fsp

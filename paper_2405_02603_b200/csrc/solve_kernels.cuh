@@ -21,6 +21,7 @@
 // The factor 1/2 and hx hy hz/(8 Nx Ny Nz) live in Ghat.
 #pragma once
 #include "fft_engine.cuh"
+#include "fft_warp.cuh"
 
 namespace fsp {
 
@@ -190,6 +191,103 @@ k_conv_z(double2* __restrict__ B2, const double* __restrict__ Gh, const double2*
     if (valid) {
 #pragma unroll
         for (int i = 0; i < R; ++i) base[t + T * i] = make_double2(xr[i] + vr[i], xi[i] + vi[i]);
+    }
+}
+
+// ============================================================================== K3 (v2): conv_z_w
+// One pencil per group of 2T lanes of a warp: lanes with b = 0 run the even
+// half-spectrum branch, lanes with b = 1 the odd one, each a two-stage single-exchange FFT of
+// fft_warp.cuh over T lanes with R points per lane.  Both branches read the same x (one fetch,
+// broadcast), read their half of the spectrum row (E or O), and the final sum y = y_e + conj(w^n) y_o
+// is formed with one shuffle per value; each branch then stores half of the pencil.
+//
+// Spectrum layout Gk (k_layout_spectrum_oct): only the unique octant of the real, even spectrum is
+// stored, row (kx, qy) = [ E[0..M/2] | O[0..M/2-1] | pad ], E[m] = Ghat[2m], O[m] = Ghat[2m+1], so
+//     Ghat[kz = 2j]   = E[min(j, M - j)],      Ghat[kz = 2j+1] = O[min(j, M-1-j)],     row of ky = row of 2Ny-ky.
+// Pencils are visited in the order ky = 0, 2Ny-1, 1, 2Ny-2, 2, ... so that the two pencils sharing a
+// spectrum row are processed back to back by neighbouring warps (second read hits L2).
+//
+// Persistent warps: warp w of the grid handles pencil groups w, w + nwarps, ... (no CTA barrier after
+// the tables are loaded).  The next group's x is prefetched into L2 while this one is transformed.
+template <int M>
+struct ConvZ {
+    using Cfg = Fft2Cfg<M>;
+    static constexpr int T = Cfg::T, R = Cfg::R;
+    static constexpr int G = 16 / T;                 // pencils per warp at a time
+    static constexpr int WARPS = 4;                  // warps per CTA
+    static constexpr int ROW = M + 2;                // doubles per spectrum row (E: M/2+1, O: M/2, pad 1)
+    static constexpr size_t smem_bytes() { return sizeof(double2) * (size_t)(2 * M + WARPS * 2 * G * Cfg::BUF); }
+};
+
+template <int M>
+__global__ void __launch_bounds__(ConvZ<M>::WARPS * 32, (M >= 512 ? 2 : 3))
+k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double2* __restrict__ tw_g,
+           const double2* __restrict__ wp_g, int Ny, long ngroups) {
+    using Z = ConvZ<M>;
+    using Cfg = typename Z::Cfg;
+    constexpr int R = Z::R, T = Z::T, G = Z::G, WARPS = Z::WARPS, H = R / 2;
+    extern __shared__ double2 smem[];
+    double2* tw = smem;          // M: stage-2 twiddles tw[i*R1 + j] = w_M^(i j)
+    double2* wp = smem + M;      // M: w_2M^n, n < M
+    for (int n = threadIdx.x; n < M; n += blockDim.x) { tw[n] = tw_g[n]; wp[n] = wp_g[n]; }
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int g = lane / (2 * T), b = (lane / T) & 1, t = lane % T;
+    double2* buf = smem + 2 * M + ((warp * G + g) * 2 + b) * Cfg::BUF;
+    const long nwarps = (long)gridDim.x * WARPS;
+    const int ny2 = 2 * Ny;
+    for (long grp = (long)blockIdx.x * WARPS + warp; grp < ngroups; grp += nwarps) {
+        const long s = grp * G + g;                       // position in the visiting order
+        const long kx = s / ny2;
+        const int r = (int)(s - kx * ny2);
+        const int ky = (r & 1) ? ny2 - ((r + 1) >> 1) : (r >> 1);
+        const int qy = ky <= Ny ? ky : ny2 - ky;
+        double2* base = B2 + (kx * ny2 + ky) * M;
+        const double* grow = Gk + (kx * (Ny + 1) + qy) * Z::ROW + (b ? M / 2 + 1 : 0);
+
+        double vr[R], vi[R];
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            const double2 v = base[t + T * i];
+            vr[i] = v.x; vi[i] = v.y;
+        }
+        {   // L2 prefetch of the next group's pencil(s): 16-byte elements, one 128-byte line per 8
+            const long s2 = s + nwarps * G;
+            if (s2 < ngroups * G) {
+                const long kx2 = s2 / ny2;
+                const int r2 = (int)(s2 - kx2 * ny2);
+                const int ky2 = (r2 & 1) ? ny2 - ((r2 + 1) >> 1) : (r2 >> 1);
+                const double2* nb = B2 + (kx2 * ny2 + ky2) * M;
+                for (int e = (b * T + t) * 8; e < M; e += 2 * T * 8)
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(nb + e));
+            }
+        }
+        if (b) {
+#pragma unroll
+            for (int i = 0; i < R; ++i) cmul(vr[i], vi[i], wp[t + T * i]);
+        }
+        fft2_forward<Cfg>(vr, vi, t, buf, tw);
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            const int j = t + T * i;
+            const int m = b ? (j < M - 1 - j ? j : M - 1 - j) : (j < M - j ? j : M - j);
+            const double gk = __ldg(grow + m);
+            vr[i] *= gk; vi[i] *= gk;
+        }
+        fft2_inverse<Cfg>(vr, vi, t, buf, tw);
+        if (b) {
+#pragma unroll
+            for (int i = 0; i < R; ++i) cmul_conj(vr[i], vi[i], wp[t + T * i]);
+        }
+        // y[n] = y_e[n] + y_o[n]: branch 0 finishes n = t + T*i for i < R/2, branch 1 for i >= R/2
+#pragma unroll
+        for (int i = 0; i < H; ++i) {
+            const double sr = b ? vr[i] : vr[i + H], si = b ? vi[i] : vi[i + H];
+            const double pr = __shfl_xor_sync(0xffffffffu, sr, T), pi = __shfl_xor_sync(0xffffffffu, si, T);
+            const int o = b ? i + H : i;
+            const double kr = b ? vr[i + H] : vr[i], ki = b ? vi[i + H] : vi[i];
+            base[t + T * o] = make_double2(kr + pr, ki + pi);
+        }
     }
 }
 
