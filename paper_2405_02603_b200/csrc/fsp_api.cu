@@ -131,8 +131,15 @@ int launch_fwd_y(fsp_plan* p) {
     constexpr int G = TileGroups<Cfg>::G;
     const long ntiles = (long)(p->Nx + 1) * (p->Nz / kW);
     const size_t smem = sizeof(double2) * (size_t)(2 * M + G * M * kW);
-    CU(cudaFuncSetAttribute(k_fwd_y<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_fwd_y<M><<<(unsigned)((ntiles + G - 1) / G), G * kW * Cfg::T, smem, p->stream>>>(p->B1, p->B2, p->Wy, p->Nz, ntiles);
+    static int occ = 0;
+    if (occ == 0) {
+        CU(cudaFuncSetAttribute(k_fwd_y<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_fwd_y<M>, G * kW * Cfg::T, smem));
+        if (occ < 1) return FSP_ERR_CUDA;
+    }
+    long grid = (ntiles + G - 1) / G;
+    if (grid > (long)p->sm_count * occ) grid = (long)p->sm_count * occ;
+    k_fwd_y<M><<<(unsigned)grid, G * kW * Cfg::T, smem, p->stream>>>(p->B1, p->B2, p->Wy, p->Nz, ntiles);
     return FSP_OK;
 }
 template <int M>
@@ -141,8 +148,15 @@ int launch_inv_y(fsp_plan* p) {
     constexpr int G = TileGroups<Cfg>::G;
     const long ntiles = (long)(p->Nx + 1) * (p->Nz / kW);
     const size_t smem = sizeof(double2) * (size_t)(2 * M + G * M * kW);
-    CU(cudaFuncSetAttribute(k_inv_y<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_inv_y<M><<<(unsigned)((ntiles + G - 1) / G), G * kW * Cfg::T, smem, p->stream>>>(p->B2, p->B1, p->Wy, p->Nz, ntiles);
+    static int occ = 0;
+    if (occ == 0) {
+        CU(cudaFuncSetAttribute(k_inv_y<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_inv_y<M>, G * kW * Cfg::T, smem));
+        if (occ < 1) return FSP_ERR_CUDA;
+    }
+    long grid = (ntiles + G - 1) / G;
+    if (grid > (long)p->sm_count * occ) grid = (long)p->sm_count * occ;
+    k_inv_y<M><<<(unsigned)grid, G * kW * Cfg::T, smem, p->stream>>>(p->B2, p->B1, p->Wy, p->Nz, ntiles);
     return FSP_OK;
 }
 template <int M>

@@ -63,36 +63,48 @@ k_fwd_y(const double2* __restrict__ B1, double2* __restrict__ B2, const double2*
     const int g = tid / (kW * T), lt = tid % (kW * T);
     const int c = lt % kW, t = lt / kW;
     double2* buf = xb + g * (M * kW) + c;
-    const long tile = (long)blockIdx.x * G + g;
-    const bool valid = tile < ntiles;
     const int nzb = Nz / kW;
-    const long kx = valid ? tile / nzb : 0;
-    const int zb = valid ? (int)(tile % nzb) : 0;
-    const double2* in = B1 + (kx * M) * (long)Nz + zb * kW + c;
-    double2* out = B2 + (kx * 2 * M) * (long)Nz + zb * kW + c;
-
-    double xr[R], xi[R], vr[R], vi[R];
-#pragma unroll
-    for (int i = 0; i < R; ++i) {
-        double2 v = valid ? in[(long)(t + T * i) * Nz] : make_double2(0.0, 0.0);
-        xr[i] = v.x; xi[i] = v.y;
-    }
     __syncthreads();  // table ready
-    // even outputs
+    // persistent CTAs: tile groups blockIdx.x, blockIdx.x + gridDim.x, ...; the next group's rows are
+    // prefetched into L2 while this one is transformed
+    for (long tile0 = (long)blockIdx.x * G; tile0 < ntiles; tile0 += (long)gridDim.x * G) {
+        const long tile = tile0 + g;
+        const bool valid = tile < ntiles;
+        const long kx = valid ? tile / nzb : 0;
+        const int zb = valid ? (int)(tile % nzb) : 0;
+        const double2* in = B1 + (kx * M) * (long)Nz + zb * kW + c;
+        double2* out = B2 + (kx * 2 * M) * (long)Nz + zb * kW + c;
+
+        double xr[R], xi[R], vr[R], vi[R];
 #pragma unroll
-    for (int i = 0; i < R; ++i) { vr[i] = xr[i]; vi[i] = xi[i]; }
-    fft_forward<Cfg, kW, LTAB>(vr, vi, t, buf, Ws);
-    if (valid) {
+        for (int i = 0; i < R; ++i) {
+            double2 v = valid ? in[(long)(t + T * i) * Nz] : make_double2(0.0, 0.0);
+            xr[i] = v.x; xi[i] = v.y;
+        }
+        {
+            const long tn = tile + (long)gridDim.x * G;
+            if (c == 0 && tn < ntiles) {
+                const double2* nin = B1 + ((tn / nzb) * M) * (long)Nz + (tn % nzb) * kW;
 #pragma unroll
-        for (int i = 0; i < R; ++i) out[(long)(2 * (t + T * i)) * Nz] = make_double2(vr[i], vi[i]);
-    }
-    // odd outputs
+                for (int i = 0; i < R; ++i) asm volatile("prefetch.global.L2 [%0];" ::"l"(nin + (long)(t + T * i) * Nz));
+            }
+        }
+        // even outputs
 #pragma unroll
-    for (int i = 0; i < R; ++i) { cmul(xr[i], xi[i], Ws[t + T * i]); }
-    fft_forward<Cfg, kW, LTAB>(xr, xi, t, buf, Ws);
-    if (valid) {
+        for (int i = 0; i < R; ++i) { vr[i] = xr[i]; vi[i] = xi[i]; }
+        fft_forward<Cfg, kW, LTAB>(vr, vi, t, buf, Ws);
+        if (valid) {
 #pragma unroll
-        for (int i = 0; i < R; ++i) out[(long)(2 * (t + T * i) + 1) * Nz] = make_double2(xr[i], xi[i]);
+            for (int i = 0; i < R; ++i) out[(long)(2 * (t + T * i)) * Nz] = make_double2(vr[i], vi[i]);
+        }
+        // odd outputs
+#pragma unroll
+        for (int i = 0; i < R; ++i) { cmul(xr[i], xi[i], Ws[t + T * i]); }
+        fft_forward<Cfg, kW, LTAB>(xr, xi, t, buf, Ws);
+        if (valid) {
+#pragma unroll
+            for (int i = 0; i < R; ++i) out[(long)(2 * (t + T * i) + 1) * Nz] = make_double2(xr[i], xi[i]);
+        }
     }
 }
 
@@ -111,31 +123,41 @@ k_inv_y(const double2* __restrict__ B2, double2* __restrict__ B1, const double2*
     const int g = tid / (kW * T), lt = tid % (kW * T);
     const int c = lt % kW, t = lt / kW;
     double2* buf = xb + g * (M * kW) + c;
-    const long tile = (long)blockIdx.x * G + g;
-    const bool valid = tile < ntiles;
     const int nzb = Nz / kW;
-    const long kx = valid ? tile / nzb : 0;
-    const int zb = valid ? (int)(tile % nzb) : 0;
-    const double2* in = B2 + (kx * 2 * M) * (long)Nz + zb * kW + c;
-    double2* out = B1 + (kx * M) * (long)Nz + zb * kW + c;
+    __syncthreads();  // table ready
+    for (long tile0 = (long)blockIdx.x * G; tile0 < ntiles; tile0 += (long)gridDim.x * G) {
+        const long tile = tile0 + g;
+        const bool valid = tile < ntiles;
+        const long kx = valid ? tile / nzb : 0;
+        const int zb = valid ? (int)(tile % nzb) : 0;
+        const double2* in = B2 + (kx * 2 * M) * (long)Nz + zb * kW + c;
+        double2* out = B1 + (kx * M) * (long)Nz + zb * kW + c;
 
-    double er[R], ei[R], qr[R], qi[R];
+        double er[R], ei[R], qr[R], qi[R];
 #pragma unroll
-    for (int i = 0; i < R; ++i) {
-        const long row = 2 * (t + T * i);
-        double2 a = valid ? in[row * Nz] : make_double2(0.0, 0.0);
-        double2 b = valid ? in[(row + 1) * Nz] : make_double2(0.0, 0.0);
-        er[i] = a.x; ei[i] = a.y; qr[i] = b.x; qi[i] = b.y;
-    }
-    __syncthreads();
-    fft_inverse<Cfg, kW, LTAB>(qr, qi, t, buf, Ws);
+        for (int i = 0; i < R; ++i) {
+            const long row = 2 * (t + T * i);
+            double2 a = valid ? in[row * Nz] : make_double2(0.0, 0.0);
+            double2 b = valid ? in[(row + 1) * Nz] : make_double2(0.0, 0.0);
+            er[i] = a.x; ei[i] = a.y; qr[i] = b.x; qi[i] = b.y;
+        }
+        {
+            const long tn = tile + (long)gridDim.x * G;
+            if (c == 0 && tn < ntiles) {
+                const double2* nin = B2 + ((tn / nzb) * 2 * M) * (long)Nz + (tn % nzb) * kW;
 #pragma unroll
-    for (int i = 0; i < R; ++i) cmul_conj(qr[i], qi[i], Ws[t + T * i]);
-    fft_inverse<Cfg, kW, LTAB>(er, ei, t, buf, Ws);
-    if (valid) {
+                for (int i = 0; i < 2 * R; ++i) asm volatile("prefetch.global.L2 [%0];" ::"l"(nin + (long)(2 * t + 2 * T * (i >> 1) + (i & 1)) * Nz));
+            }
+        }
+        fft_inverse<Cfg, kW, LTAB>(qr, qi, t, buf, Ws);
 #pragma unroll
-        for (int i = 0; i < R; ++i)
-            out[(long)(t + T * i) * Nz] = make_double2(er[i] + qr[i], ei[i] + qi[i]);
+        for (int i = 0; i < R; ++i) cmul_conj(qr[i], qi[i], Ws[t + T * i]);
+        fft_inverse<Cfg, kW, LTAB>(er, ei, t, buf, Ws);
+        if (valid) {
+#pragma unroll
+            for (int i = 0; i < R; ++i)
+                out[(long)(t + T * i) * Nz] = make_double2(er[i] + qr[i], ei[i] + qi[i]);
+        }
     }
 }
 
@@ -266,18 +288,25 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
 #pragma unroll
             for (int i = 0; i < R; ++i) cmul(vr[i], vi[i], wp[t + T * i]);
         }
-        fft2_forward<Cfg>(vr, vi, t, buf, tw);
+        // Two passes over ONE copy of the transform code (the kernel would not fit the instruction
+        // cache otherwise): IFFT(Y) = conj(FFT(conj(Y))).  Pass 0 ends with Y = conj(Ghat * X).
+#pragma unroll 1
+        for (int pass = 0; pass < 2; ++pass) {
+            fft2_forward<Cfg>(vr, vi, t, buf, tw);
+            if (pass == 0) {
 #pragma unroll
-        for (int i = 0; i < R; ++i) {
-            const int j = t + T * i;
-            const int m = b ? (j < M - 1 - j ? j : M - 1 - j) : (j < M - j ? j : M - j);
-            const double gk = __ldg(grow + m);
-            vr[i] *= gk; vi[i] *= gk;
+                for (int i = 0; i < R; ++i) {
+                    const int j = t + T * i;
+                    const int m = b ? (j < M - 1 - j ? j : M - 1 - j) : (j < M - j ? j : M - j);
+                    const double gk = __ldg(grow + m);
+                    vr[i] *= gk; vi[i] *= -gk;
+                }
+            }
         }
-        fft2_inverse<Cfg>(vr, vi, t, buf, tw);
+        // now (vr, -vi) = IFFT(Ghat X); the odd branch still needs conj(w^n): conj(v) conj(w) = conj(v w)
         if (b) {
 #pragma unroll
-            for (int i = 0; i < R; ++i) cmul_conj(vr[i], vi[i], wp[t + T * i]);
+            for (int i = 0; i < R; ++i) cmul(vr[i], vi[i], wp[t + T * i]);
         }
         // y[n] = y_e[n] + y_o[n]: branch 0 finishes n = t + T*i for i < R/2, branch 1 for i >= R/2
 #pragma unroll
@@ -286,7 +315,7 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
             const double pr = __shfl_xor_sync(0xffffffffu, sr, T), pi = __shfl_xor_sync(0xffffffffu, si, T);
             const int o = b ? i + H : i;
             const double kr = b ? vr[i + H] : vr[i], ki = b ? vi[i + H] : vi[i];
-            base[t + T * o] = make_double2(kr + pr, ki + pi);
+            base[t + T * o] = make_double2(kr + pr, -ki - pi);
         }
     }
 }
