@@ -56,7 +56,9 @@ enum {
 /* parameters settable before fsp_precompute_green */
 enum {
     FSP_PARAM_G0 = 0,    /* HE value at the origin, default +1/(4 pi)  (R5) */
-    FSP_PARAM_ALPHA = 1  /* VG window factor, default 1.1               */
+    FSP_PARAM_ALPHA = 1, /* VG window factor, default 1.1               */
+    FSP_PARAM_CHUNK_PLANES = 2 /* kx-planes per pass of the y-z-y middle (0 = all at once); takes
+                                  effect at the next fsp_solve; does not change results             */
 };
 
 /* number of kernels one fsp_solve launches (the five passes of DESIGN.md "The path") */

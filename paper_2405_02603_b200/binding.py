@@ -15,7 +15,7 @@ import os
 import numpy as np
 
 HOCKNEY, VICO, VICO_2 = 0, 1, 2                       # include/fsp.h
-PARAM_G0, PARAM_ALPHA = 0, 1
+PARAM_G0, PARAM_ALPHA, PARAM_CHUNK_PLANES = 0, 1, 2
 NUM_SOLVE_KERNELS = 5
 ERRORS = {0: "FSP_OK", -1: "FSP_ERR_INVALID_ARG", -2: "FSP_ERR_NOT_PRECOMPUTED",
           -3: "FSP_ERR_OUT_OF_MEMORY", -4: "FSP_ERR_CUDA", -5: "FSP_ERR_NO_DEVICE"}

@@ -87,6 +87,51 @@ __device__ __forceinline__ void dft_inplace(double* re, double* im) {
     }
 }
 
+// ---- r-point DFT, strictly in place ------------------------------------------------------------
+// Input x_i at re[S*i]; output X_k at re[S*brev_r(k)] (bit-reversed PLACEMENT, natural values): the
+// iterative decimation-in-time network on the working array a[p] = element brev_r(p), whose butterflies
+// (a[q], a[q+h]) -> (a[q] + w a[q+h], a[q] - w a[q+h]) overwrite their own operands, so the live set is
+// the 2r data registers plus two temporaries per butterfly in flight (the recursive dft_inplace above
+// gathers copies at every level and needs half as many registers again).  All indices are compile-time.
+__host__ __device__ constexpr int brev(int v, int r) {
+    int o = 0;
+    for (int b = 1; b < r; b <<= 1) { o = (o << 1) | (v & 1); v >>= 1; }
+    return o;
+}
+
+template <int r, int S>
+__device__ __forceinline__ void dft_br(double* re, double* im) {
+#pragma unroll
+    for (int len = 2; len <= r; len *= 2) {
+        const int half = len / 2;
+#pragma unroll
+        for (int blk = 0; blk < r; blk += len) {
+#pragma unroll
+            for (int k = 0; k < half; ++k) {
+                const int p = S * brev(blk + k, r), q = S * brev(blk + k + half, r);
+                const double ar = re[p], ai = im[p], br = re[q], bi = im[q];
+                if (k == 0) {
+                    re[p] = ar + br; im[p] = ai + bi; re[q] = ar - br; im[q] = ai - bi;
+                } else if (4 * k == len) {  // w = -i
+                    re[p] = ar + bi; im[p] = ai - br; re[q] = ar - bi; im[q] = ai + br;
+                } else {
+                    const double c = cos32(k * (32 / len)), s = sin32(k * (32 / len));
+                    double ur, ui, f;
+                    if (c * c >= s * s) {
+                        const double tn = s / c;
+                        ur = fma(bi, tn, br); ui = fma(-br, tn, bi); f = c;
+                    } else {
+                        const double ct = c / s;
+                        ur = fma(br, ct, bi); ui = fma(bi, ct, -br); f = s;
+                    }
+                    re[q] = fma(-f, ur, ar); im[q] = fma(-f, ui, ai);
+                    re[p] = fma(f, ur, ar); im[p] = fma(f, ui, ai);
+                }
+            }
+        }
+    }
+}
+
 // ---- static description of one FFT size ---------------------------------------------------------
 // R points per thread; up to three stages r1*r2*r3 = M (r = 1 marks "no stage").
 template <int M_, int R_, int R1_, int R2_, int R3_>

@@ -17,6 +17,7 @@
 //            output at position j + R1*i = t + T*(m + i*nb2): the register it already sits in.
 #pragma once
 #include "fft_engine.cuh"
+#include "tma.cuh"
 
 namespace fsp {
 
@@ -80,6 +81,117 @@ __device__ __forceinline__ void fft2_forward(double (&re)[Cfg::R], double (&im)[
         }
         dft_inplace<R2, NB2>(&re[m], &im[m]);
     }
+}
+
+// ---- stage 2 with lane-constant twiddles ------------------------------------------------------------
+// The stage-2 butterfly j computes  Y_k = sum_i x_i om^i w_R2^(i k),  om = w_M^j  (the input twiddles of
+// fft2_forward folded into the transform: a DFT at the shifted frequencies k + j/R1).  Decimation in time
+// keeps that form at every level: with b_r = om^(R2/r),
+//     Y_k = E_k + (b_r w_r^k) O_k,   Y_(k+r/2) = E_k - (b_r w_r^k) O_k,   k < r/2,
+// E, O the size-r/2 transforms (base b_r^2) of the even / odd inputs.  Since w_r^(k + r/4) = -i w_r^k, a
+// size-r level needs only max(1, r/4) distinct twiddles b_r w_r^k, R2/2 in total over all levels.  They
+// depend on j only, i.e. they are per-lane constants for the whole kernel: held in registers as
+// (cos, tan) pairs, each twiddle + butterfly is 6 FMAs and stage 2 reads no twiddle table at all
+// (the LSU data pipe, not HBM, is the first roof of these kernels).
+// Constant i of level r (r >= 4) sits at index r/4 + (k mod r/4); level 2 at index 0.
+template <int R2> struct LaneTw { static constexpr int NC = R2 >= 4 ? R2 / 2 : 1; };
+
+template <int r, int S>
+__device__ __forceinline__ void dft_lane(double* re, double* im, const double* __restrict__ cc,
+                                         const double* __restrict__ tn) {
+    // in place: input x_i at re[S*brev_r(i)] (the caller loads it there), output Y_k at re[S*k]
+#pragma unroll
+    for (int len = 2; len <= r; len *= 2) {
+        const int half = len / 2;
+        const int OFS = len >= 4 ? len / 4 : 0, Q = len >= 4 ? len / 4 : 1;
+#pragma unroll
+        for (int blk = 0; blk < r; blk += len) {
+#pragma unroll
+            for (int k = 0; k < half; ++k) {
+                const int p = S * (blk + k), q = S * (blk + k + half);
+                const double c = cc[OFS + (k % Q)], tg = tn[OFS + (k % Q)];
+                const double ar = re[p], ai = im[p], br = re[q], bi = im[q];
+                // b (c - i s) = c [(br + bi tg) + i (bi - br tg)],  tg = s / c
+                const double ur = fma(bi, tg, br), ui = fma(-br, tg, bi);
+                if (((k / Q) & 1) == 0) {
+                    re[q] = fma(-c, ur, ar); im[q] = fma(-c, ui, ai);
+                    re[p] = fma(c, ur, ar); im[p] = fma(c, ui, ai);
+                } else {  // twiddle times -i:  c (ui - i ur)
+                    re[q] = fma(-c, ui, ar); im[q] = fma(c, ur, ai);
+                    re[p] = fma(c, ui, ar); im[p] = fma(-c, ur, ai);
+                }
+            }
+        }
+    }
+}
+
+// fft2_forward with the lane-constant stage 2 and in-place butterflies.
+// Natural order in and out (lane t holds position t + T*i in register i): stage 1 leaves output k of
+// butterfly m in register m + NB1*brev(k), which is where the exchange write takes it from; the exchange
+// read puts input e of stage-2 butterfly m into register m + NB2*brev(e), so that the in-place stage 2
+// ends in natural order.  cc/tn: [NB2][LaneTw<R2>::NC] constants of this lane's butterflies j = t + T*m
+// (host table make_lane_table, loaded once per kernel).
+template <class Cfg>
+__device__ __forceinline__ void fft2_forward_lc(double (&re)[Cfg::R], double (&im)[Cfg::R], int t,
+                                                double2* __restrict__ buf,
+                                                const double (&cc)[Cfg::NB2][LaneTw<Cfg::R2>::NC],
+                                                const double (&tn)[Cfg::NB2][LaneTw<Cfg::R2>::NC]) {
+    constexpr int R = Cfg::R, R1 = Cfg::R1, R2 = Cfg::R2, T = Cfg::T, NB1 = Cfg::NB1, NB2 = Cfg::NB2;
+#pragma unroll
+    for (int m = 0; m < NB1; ++m) dft_br<R1, NB1>(&re[m], &im[m]);
+    __syncwarp();  // earlier readers of buf are done
+#pragma unroll
+    for (int m = 0; m < NB1; ++m) {
+        double2* dst = buf + (t + T * m) * (R1 + 1);
+#pragma unroll
+        for (int i = 0; i < R1; ++i)   // output i of butterfly m sits in register m + NB1*brev(i)
+            dst[i] = make_double2(re[m + brev(i, R1) * NB1], im[m + brev(i, R1) * NB1]);
+    }
+    __syncwarp();
+#pragma unroll
+    for (int i = 0; i < R; ++i) {
+        int a;
+        if constexpr (R1 % T == 0) a = t + T * i + (T * i) / R1;
+        else a = pad_pos<R1>(t + T * i);
+        const double2 v = buf[a];
+        const int d = (i % NB2) + NB2 * brev(i / NB2, R2);
+        re[d] = v.x; im[d] = v.y;
+    }
+#pragma unroll
+    for (int m = 0; m < NB2; ++m) dft_lane<R2, NB2>(&re[m], &im[m], cc[m], tn[m]);
+}
+
+// The same transform for the tile kernels (strided axes): a GROUP of CW*T threads transforms CW adjacent
+// columns at once, thread (c, t) = (column, lane of the column), c fastest, so that a quarter-warp is
+// 8 columns of one position: every exchange access is one contiguous 128-byte row of the buffer
+// E[position][CW] (conflict free without padding) and every global access a full line.  The T lanes of
+// a column sit in different warps, so the two syncs are named barriers over the group.
+// Ec = E + c;  bar_id: the group's barrier.
+template <class Cfg, int CW>
+__device__ __forceinline__ void fft2_forward_tile(double (&re)[Cfg::R], double (&im)[Cfg::R], int t,
+                                                  double2* __restrict__ Ec, int bar_id,
+                                                  const double (&cc)[Cfg::NB2][LaneTw<Cfg::R2>::NC],
+                                                  const double (&tn)[Cfg::NB2][LaneTw<Cfg::R2>::NC]) {
+    constexpr int R = Cfg::R, R1 = Cfg::R1, R2 = Cfg::R2, T = Cfg::T, NB1 = Cfg::NB1, NB2 = Cfg::NB2;
+#pragma unroll
+    for (int m = 0; m < NB1; ++m) dft_br<R1, NB1>(&re[m], &im[m]);
+    bar_sync(bar_id, CW * T);  // earlier readers of E are done
+#pragma unroll
+    for (int m = 0; m < NB1; ++m) {
+        double2* dst = Ec + (t + T * m) * (R1 * CW);
+#pragma unroll
+        for (int i = 0; i < R1; ++i)
+            dst[i * CW] = make_double2(re[m + brev(i, R1) * NB1], im[m + brev(i, R1) * NB1]);
+    }
+    bar_sync(bar_id, CW * T);
+#pragma unroll
+    for (int i = 0; i < R; ++i) {
+        const double2 v = Ec[(t + T * i) * CW];
+        const int d = (i % NB2) + NB2 * brev(i / NB2, R2);
+        re[d] = v.x; im[d] = v.y;
+    }
+#pragma unroll
+    for (int m = 0; m < NB2; ++m) dft_lane<R2, NB2>(&re[m], &im[m], cc[m], tn[m]);
 }
 
 // unnormalised inverse: swap the roles of re and im (IFFT(x) = swap(FFT(swap(x))))

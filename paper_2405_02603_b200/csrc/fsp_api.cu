@@ -7,6 +7,7 @@
 #include <new>
 #include <vector>
 
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include "../../include/fsp.h"
@@ -29,8 +30,12 @@ struct fsp_plan {
     double2* B2 = nullptr;  // (Nx+1) * 2Ny * Nz
     double* Gh = nullptr;   // (Nx+1) * 2Ny * 2Nz   spectrum, full K3-v1 layout (only when Nz = 1024)
     double* Gk = nullptr;   // (Nx+1)(Ny+1)(Nz+2)   spectrum octant in K3-v2 layout, scale folded in
-    double2* TWz = nullptr; // Nz                   stage-2 twiddles of the z transform (fft_warp.cuh)
+    double* LTz = nullptr;  // lane-constant stage-2 twiddles of the z transform (fft_warp.cuh dft_lane)
+    double* LTy = nullptr;  // the same for the y transform (tile kernels)
+    bool tile_y = false;    // K2/K4 tile kernels (TMA-staged) are used
+    CUtensorMap tmB1y;      // B1 as [kx][y][2 Nz doubles], box = 8 columns x <=256 rows (K2 input)
     bool z_warp = false;    // K3 v2 (k_conv_z_w) is used
+    int chunk_planes = 0;   // > 0: K2-K3-K4 run chunk_planes kx-planes at a time (L2-resident B2)
     int sm_count = 148;
     double* T = nullptr;    // (Nx+1)(Ny+1)(Nz+1)   real-space table
     double* Goct = nullptr; // (Nx+1)(Ny+1)(Nz+1)   un-normalised spectrum octant
@@ -112,24 +117,96 @@ int make_table(double2** dst, int L, size_t* acc) {
     return upload_table(dst, hst, acc);
 }
 
-// stage-2 twiddles of the two-stage transform of fft_warp.cuh: tw[i*R1 + j] = exp(-2 pi i (i j) / M)
-int make_stage2_table(double2** dst, int M, int R1, size_t* acc) {
-    std::vector<double2> hst((size_t)M);
-    const int R2 = M / R1;
-    for (int i = 0; i < R2; ++i)
-        for (int j = 0; j < R1; ++j) hst[(size_t)i * R1 + j] = unit_root((long)i * j, M);
-    return upload_table(dst, hst, acc);
+// (cos, tan) of exp(-2 pi i m / L) in long double; an exactly vanishing cosine is replaced by 2^-200 so
+// that c * (x + y * (s/c)) still evaluates to s * y (fft_warp.cuh dft_lane, "tan form")
+void cos_tan(long m, long L, double* c_out, double* t_out) {
+    const long double PI2 = 6.283185307179586476925286766559005768L;
+    m %= L;
+    long double c, s;
+    if (4 * m == L) { c = 0.0L; s = 1.0L; }
+    else if (2 * m == L) { c = -1.0L; s = 0.0L; }
+    else if (4 * m == 3 * L) { c = 0.0L; s = -1.0L; }
+    else if (m == 0) { c = 1.0L; s = 0.0L; }
+    else { const long double a = PI2 * (long double)m / (long double)L; c = cosl(a); s = sinl(a); }
+    if (c == 0.0L) c = ldexpl(1.0L, -200);
+    *c_out = (double)c;
+    *t_out = (double)(s / c);
+}
+
+// lane-constant stage-2 twiddles of fft_warp.cuh: for butterfly j < R1, level r = 2,4,..,R2, k < max(1,r/4):
+//   b_r w_r^k = exp(-2 pi i (j R2 + k M) / (r M)),  stored as [j][cos(NC) | tan(NC)], index r/4 + k (level 2: 0)
+int make_lane_table(double** dst, int M, int R1, size_t* acc) {
+    const int R2 = M / R1, NC = R2 >= 4 ? R2 / 2 : 1;
+    std::vector<double> hst((size_t)R1 * 2 * NC, 0.0);
+    for (int j = 0; j < R1; ++j)
+        for (int r = 2; r <= R2; r *= 2) {
+            const int ofs = r >= 4 ? r / 4 : 0, q = r >= 4 ? r / 4 : 1;
+            for (int k = 0; k < q; ++k)
+                cos_tan((long)j * R2 + (long)k * M, (long)r * M, &hst[(size_t)j * 2 * NC + ofs + k],
+                        &hst[(size_t)j * 2 * NC + NC + ofs + k]);
+        }
+    int rc = dev_alloc(dst, hst.size(), acc);
+    if (rc != FSP_OK) return rc;
+    CU(cudaMemcpy(*dst, hst.data(), sizeof(double) * hst.size(), cudaMemcpyHostToDevice));
+    return FSP_OK;
 }
 
 template <int M>
-int stage2_table_for(double2** dst, size_t* acc) { return make_stage2_table(dst, M, Fft2Cfg<M>::R1, acc); }
+int lane_table_for(double** dst, size_t* acc) { return make_lane_table(dst, M, Fft2Cfg<M>::R1, acc); }
+
+// ---- TMA tensor maps ---------------------------------------------------------------------------------
+// cuTensorMapEncodeTiled is fetched through the runtime so that libfsp.so does not link libcuda directly.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* q = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &q, cudaEnableDefault, &qr) != cudaSuccess ||
+            qr != cudaDriverEntryPointSuccess) {
+            (void)cudaGetLastError();
+            return nullptr;
+        }
+        fn = reinterpret_cast<EncodeTiledFn>(q);
+    }
+    return fn;
+}
+// fp64 tensor of `rank` dimensions (dims[0] fastest, strides in bytes for dims 1..rank-1), no swizzle
+int make_tensor_map(CUtensorMap* tm, void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides,
+                    const cuuint32_t* box) {
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return FSP_ERR_CUDA;
+    cuuint32_t es[5] = {1, 1, 1, 1, 1};
+    CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, (cuuint32_t)rank, base, dims, strides, box, es,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? FSP_OK : FSP_ERR_CUDA;
+}
 
 // ---- kernel launch helpers (one template instantiation per FFT length) ---------------------------
 template <int M>
-int launch_fwd_y(fsp_plan* p) {
+int launch_fwd_y_t(fsp_plan* p, int kx0, double2* B2, int nplanes) {
+    using Y = TileY<M>;
+    const long ntiles = (long)nplanes * (p->Nz / kW);
+    const size_t smem = Y::smem_bytes();
+    static int occ = 0;
+    if (occ == 0) {
+        CU(cudaFuncSetAttribute(k_fwd_y_t<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_fwd_y_t<M>, Y::THREADS, smem));
+        if (occ < 1) return FSP_ERR_CUDA;
+    }
+    long grid = (long)p->sm_count * occ;
+    if (grid > ntiles) grid = ntiles;
+    k_fwd_y_t<M><<<(unsigned)grid, Y::THREADS, smem, p->stream>>>(p->tmB1y, B2, p->LTy, p->Wy, p->Nz, kx0, ntiles);
+    return FSP_OK;
+}
+template <int M>
+int launch_fwd_y(fsp_plan* p, const double2* B1, double2* B2, int nplanes) {
     using Cfg = FftCfg<M>;
     constexpr int G = TileGroups<Cfg>::G;
-    const long ntiles = (long)(p->Nx + 1) * (p->Nz / kW);
+    const long ntiles = (long)nplanes * (p->Nz / kW);
     const size_t smem = sizeof(double2) * (size_t)(2 * M + G * M * kW);
     static int occ = 0;
     if (occ == 0) {
@@ -139,14 +216,14 @@ int launch_fwd_y(fsp_plan* p) {
     }
     long grid = (ntiles + G - 1) / G;
     if (grid > (long)p->sm_count * occ) grid = (long)p->sm_count * occ;
-    k_fwd_y<M><<<(unsigned)grid, G * kW * Cfg::T, smem, p->stream>>>(p->B1, p->B2, p->Wy, p->Nz, ntiles);
+    k_fwd_y<M><<<(unsigned)grid, G * kW * Cfg::T, smem, p->stream>>>(B1, B2, p->Wy, p->Nz, ntiles);
     return FSP_OK;
 }
 template <int M>
-int launch_inv_y(fsp_plan* p) {
+int launch_inv_y(fsp_plan* p, const double2* B2, double2* B1, int nplanes) {
     using Cfg = FftCfg<M>;
     constexpr int G = TileGroups<Cfg>::G;
-    const long ntiles = (long)(p->Nx + 1) * (p->Nz / kW);
+    const long ntiles = (long)nplanes * (p->Nz / kW);
     const size_t smem = sizeof(double2) * (size_t)(2 * M + G * M * kW);
     static int occ = 0;
     if (occ == 0) {
@@ -156,23 +233,23 @@ int launch_inv_y(fsp_plan* p) {
     }
     long grid = (ntiles + G - 1) / G;
     if (grid > (long)p->sm_count * occ) grid = (long)p->sm_count * occ;
-    k_inv_y<M><<<(unsigned)grid, G * kW * Cfg::T, smem, p->stream>>>(p->B2, p->B1, p->Wy, p->Nz, ntiles);
+    k_inv_y<M><<<(unsigned)grid, G * kW * Cfg::T, smem, p->stream>>>(B2, B1, p->Wy, p->Nz, ntiles);
     return FSP_OK;
 }
 template <int M>
-int launch_conv_z(fsp_plan* p) {
+int launch_conv_z(fsp_plan* p, double2* B2, const double* G, int nplanes) {
     using Cfg = FftCfg<M>;
     constexpr int P = PencilGroups<Cfg>::P;
-    const long npencils = (long)(p->Nx + 1) * (2 * p->Ny);
+    const long npencils = (long)nplanes * (2 * p->Ny);
     const size_t smem = sizeof(double2) * (size_t)(2 * M + P * M);
     CU(cudaFuncSetAttribute(k_conv_z<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_conv_z<M><<<(unsigned)((npencils + P - 1) / P), P * Cfg::T, smem, p->stream>>>(p->B2, p->Gh, p->Wz, npencils);
+    k_conv_z<M><<<(unsigned)((npencils + P - 1) / P), P * Cfg::T, smem, p->stream>>>(B2, G, p->Wz, npencils);
     return FSP_OK;
 }
 template <int M>
-int launch_conv_z_w(fsp_plan* p) {
+int launch_conv_z_w(fsp_plan* p, double2* B2, const double* G, int nplanes) {
     using Z = ConvZ<M>;
-    const long ngroups = (long)(p->Nx + 1) * (2 * p->Ny) / Z::G;
+    const long ngroups = (long)nplanes * (2 * p->Ny) / Z::G;
     const size_t smem = Z::smem_bytes();
     static int occ = 0;  // CTAs per SM, queried once per transform length
     if (occ == 0) {
@@ -183,7 +260,7 @@ int launch_conv_z_w(fsp_plan* p) {
     long grid = (long)p->sm_count * occ;
     const long need = (ngroups + Z::WARPS - 1) / Z::WARPS;
     if (grid > need) grid = need;
-    k_conv_z_w<M><<<(unsigned)grid, Z::WARPS * 32, smem, p->stream>>>(p->B2, p->Gk, p->TWz, p->Wz, p->Ny, ngroups);
+    k_conv_z_w<M><<<(unsigned)grid, Z::WARPS * 32, smem, p->stream>>>(B2, G, p->LTz, p->Wz, p->Ny, ngroups);
     return FSP_OK;
 }
 template <int M>
@@ -232,7 +309,14 @@ int launch_inv_x(fsp_plan* p, double* phi) {
     }
 
 int do_fwd_x(fsp_plan* p, const double* rho) { DISPATCH_X(launch_fwd_x, p->Nx / 2, p, rho) }
-int do_fwd_y(fsp_plan* p) { DISPATCH_YZ(launch_fwd_y, p->Ny, p) }
+int do_fwd_y(fsp_plan* p, int kx0, double2* B2, int np) {
+    if (p->tile_y) {
+        if (p->Ny == 512) return launch_fwd_y_t<512>(p, kx0, B2, np);
+        return launch_fwd_y_t<256>(p, kx0, B2, np);
+    }
+    const double2* B1 = p->B1 + (size_t)kx0 * p->Ny * p->Nz;
+    DISPATCH_YZ(launch_fwd_y, p->Ny, p, B1, B2, np)
+}
 #define DISPATCH_W(fn, M, ...)                           \
     switch (M) {                                         \
         case 8: return fn<8>(__VA_ARGS__);               \
@@ -244,11 +328,16 @@ int do_fwd_y(fsp_plan* p) { DISPATCH_YZ(launch_fwd_y, p->Ny, p) }
         case 512: return fn<512>(__VA_ARGS__);           \
         default: return FSP_ERR_INVALID_ARG;             \
     }
-int do_conv_z_v1(fsp_plan* p) { DISPATCH_YZ(launch_conv_z, p->Nz, p) }
-int do_conv_z_w(fsp_plan* p) { DISPATCH_W(launch_conv_z_w, p->Nz, p) }
-int do_conv_z(fsp_plan* p) { return p->z_warp ? do_conv_z_w(p) : do_conv_z_v1(p); }
-int make_z_stage2_table(fsp_plan* p) { DISPATCH_W(stage2_table_for, p->Nz, &p->TWz, &p->bytes) }
-int do_inv_y(fsp_plan* p) { DISPATCH_YZ(launch_inv_y, p->Ny, p) }
+int do_conv_z_v1(fsp_plan* p, double2* B2, const double* G, int np) { DISPATCH_YZ(launch_conv_z, p->Nz, p, B2, G, np) }
+int do_conv_z_w(fsp_plan* p, double2* B2, const double* G, int np) { DISPATCH_W(launch_conv_z_w, p->Nz, p, B2, G, np) }
+// planes [kx0, kx0 + np) of the spectrum go with the np planes stored at B2
+int do_conv_z(fsp_plan* p, double2* B2, int kx0, int np) {
+    if (p->z_warp) return do_conv_z_w(p, B2, p->Gk + (size_t)kx0 * (p->Ny + 1) * (p->Nz + 2), np);
+    return do_conv_z_v1(p, B2, p->Gh + (size_t)kx0 * (2 * p->Ny) * (2 * p->Nz), np);
+}
+int make_z_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Nz, &p->LTz, &p->bytes) }
+int make_y_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Ny, &p->LTy, &p->bytes) }
+int do_inv_y(fsp_plan* p, const double2* B2, double2* B1, int np) { DISPATCH_YZ(launch_inv_y, p->Ny, p, B2, B1, np) }
 int do_inv_x(fsp_plan* p, double* phi) { DISPATCH_X(launch_inv_x, p->Nx / 2, p, phi) }
 
 unsigned grid_for(long total, int block) {
@@ -375,7 +464,7 @@ int precompute_impl(fsp_plan* p) {
 }
 
 void free_plan_memory(fsp_plan* p) {
-    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->Gh); cudaFree(p->Gk); cudaFree(p->TWz); cudaFree(p->T); cudaFree(p->Goct);
+    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->Gh); cudaFree(p->Gk); cudaFree(p->LTz); cudaFree(p->LTy); cudaFree(p->T); cudaFree(p->Goct);
     cudaFree(p->Wx); cudaFree(p->Wy); cudaFree(p->Wz); cudaFree(p->rho_stage); cudaFree(p->phi_stage);
     for (cudaEvent_t e : p->events) cudaEventDestroy(e);
     p->events.clear();
@@ -436,7 +525,15 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
     p->sm_count = prop.multiProcessorCount > 0 ? prop.multiProcessorCount : 148;
     if (rc == FSP_OK && !p->z_warp) rc = dev_alloc(&p->Gh, ng, &p->bytes);
     if (rc == FSP_OK && p->z_warp) rc = dev_alloc(&p->Gk, (size_t)(Nx + 1) * (Ny + 1) * (Nz + 2), &p->bytes);
-    if (rc == FSP_OK && p->z_warp) rc = make_z_stage2_table(p);
+    if (rc == FSP_OK && p->z_warp) rc = make_z_lane_table(p);
+    p->tile_y = (Ny == 256 || Ny == 512) && Nz >= kW;
+    if (rc == FSP_OK && p->tile_y) rc = make_y_lane_table(p);
+    if (rc == FSP_OK && p->tile_y) {
+        const cuuint64_t dims[3] = {(cuuint64_t)2 * Nz, (cuuint64_t)Ny, (cuuint64_t)(Nx + 1)};
+        const cuuint64_t strides[2] = {(cuuint64_t)Nz * 16, (cuuint64_t)Ny * Nz * 16};
+        const cuuint32_t box[3] = {2 * kW, (cuuint32_t)(Ny < 256 ? Ny : 256), 1};
+        rc = make_tensor_map(&p->tmB1y, p->B1, 3, dims, strides, box);
+    }
     if (rc == FSP_OK) rc = dev_alloc(&p->T, nt, &p->bytes);
     if (rc == FSP_OK) rc = dev_alloc(&p->Goct, nt, &p->bytes);
     if (rc == FSP_OK) rc = make_table(&p->Wx, 2 * Nx, &p->bytes);
@@ -454,6 +551,11 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
 int fsp_plan_set_param(fsp_plan* p, int which, double value) {
     if (!p || !std::isfinite(value)) return FSP_ERR_INVALID_ARG;
     if (which == FSP_PARAM_G0) { p->g0 = value; return FSP_OK; }
+    if (which == FSP_PARAM_CHUNK_PLANES) {
+        if (value < 0.0 || value > 4096.0) return FSP_ERR_INVALID_ARG;
+        p->chunk_planes = (int)value;
+        return FSP_OK;
+    }
     if (which == FSP_PARAM_ALPHA) {
         if (!(value > 0.0)) return FSP_ERR_INVALID_ARG;
         p->alpha = value;
@@ -494,12 +596,26 @@ int fsp_solve(fsp_plan* p, const double* rho_dev, double* phi_dev) {
     int rc;
     if ((rc = do_fwd_x(p, rho_dev)) != FSP_OK) return rc;
     if (ev) CU(cudaEventRecord(ev[1], p->stream));
-    if ((rc = do_fwd_y(p)) != FSP_OK) return rc;
+    const int planes = p->Nx + 1;
+    if (p->chunk_planes > 0 && p->chunk_planes < planes) {
+        // plane-chunked middle: K2 -> K3 -> K4 on chunk_planes kx-planes at a time through the head of
+        // B2, so that B2 stays resident in L2 between the three passes
+        const size_t plane1 = (size_t)p->Ny * p->Nz;
+        for (int kx0 = 0; kx0 < planes; kx0 += p->chunk_planes) {
+            const int np = planes - kx0 < p->chunk_planes ? planes - kx0 : p->chunk_planes;
+            if ((rc = do_fwd_y(p, kx0, p->B2, np)) != FSP_OK) return rc;
+            if ((rc = do_conv_z(p, p->B2, kx0, np)) != FSP_OK) return rc;
+            if ((rc = do_inv_y(p, p->B2, p->B1 + kx0 * plane1, np)) != FSP_OK) return rc;
+        }
+        if (ev) { CU(cudaEventRecord(ev[2], p->stream)); CU(cudaEventRecord(ev[3], p->stream)); CU(cudaEventRecord(ev[4], p->stream)); }
+    } else {
+    if ((rc = do_fwd_y(p, 0, p->B2, planes)) != FSP_OK) return rc;
     if (ev) CU(cudaEventRecord(ev[2], p->stream));
-    if ((rc = do_conv_z(p)) != FSP_OK) return rc;
+    if ((rc = do_conv_z(p, p->B2, 0, planes)) != FSP_OK) return rc;
     if (ev) CU(cudaEventRecord(ev[3], p->stream));
-    if ((rc = do_inv_y(p)) != FSP_OK) return rc;
+    if ((rc = do_inv_y(p, p->B2, p->B1, planes)) != FSP_OK) return rc;
     if (ev) CU(cudaEventRecord(ev[4], p->stream));
+    }
     if ((rc = do_inv_x(p, phi_dev)) != FSP_OK) return rc;
     if (ev) CU(cudaEventRecord(ev[5], p->stream));
     CU(cudaGetLastError());

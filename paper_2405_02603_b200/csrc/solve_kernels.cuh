@@ -108,6 +108,86 @@ k_fwd_y(const double2* __restrict__ B1, double2* __restrict__ B2, const double2*
     }
 }
 
+// ================================================================================= K2 (v2): fwd_y_t
+// Tile kernel: one CTA = two groups of kW*T threads, group 0 computes the even
+// outputs of the pruned transform, group 1 the odd ones (input times w^n first).  The tile
+// [M rows][kW columns] arrives by TMA (tensor map over B1 viewed as [kx][y][2 Nz doubles]) into X; both
+// groups copy it to registers, after which X is handed back to the TMA for the NEXT tile while this one
+// is transformed: global-load latency never reaches the FFT.  Results go straight from registers to
+// global memory, four full 128-byte lines per warp instruction.
+template <int M>
+struct TileY {
+    using Cfg = Fft2Cfg<M>;
+    static constexpr int T = Cfg::T, R = Cfg::R;
+    static constexpr int GT = kW * T;             // threads per group
+    static constexpr int THREADS = 2 * GT;
+    static constexpr int NC = LaneTw<Cfg::R2>::NC;
+    static constexpr int MINB = (M >= 512) ? 1 : 2;
+    static constexpr int BOXR = M < 256 ? M : 256;   // rows per TMA box (box dimensions are limited to 256)
+    // [mbarriers: 128 B][X: M*kW][E: 2 groups x M*kW][wp: M]
+    static constexpr size_t smem_bytes() { return 128 + sizeof(double2) * (size_t)(3 * M * kW + M); }
+};
+
+template <int M>
+__global__ void __launch_bounds__(TileY<M>::THREADS, TileY<M>::MINB)
+k_fwd_y_t(const __grid_constant__ CUtensorMap tmB1, double2* __restrict__ B2, const double* __restrict__ lane_g,
+          const double2* __restrict__ wp_g, int Nz, int kx0, long ntiles) {
+    using Y = TileY<M>;
+    using Cfg = typename Y::Cfg;
+    constexpr int R = Y::R, T = Y::T, GT = Y::GT, NC = Y::NC, NB2 = Cfg::NB2;
+    extern __shared__ __align__(128) unsigned char smraw[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smraw);
+    double2* X = reinterpret_cast<double2*>(smraw + 128);
+    double2* E = X + M * kW;
+    double2* wp = E + 2 * M * kW;
+    const int tid = threadIdx.x;
+    const int grp = tid / GT, gt = tid % GT, c = gt % kW, t = gt / kW;
+    for (int n = tid; n < M; n += Y::THREADS) wp[n] = wp_g[n];
+    double cc[NB2][NC], tn[NB2][NC];
+#pragma unroll
+    for (int m = 0; m < NB2; ++m)
+#pragma unroll
+        for (int i = 0; i < NC; ++i) {
+            cc[m][i] = lane_g[(t + T * m) * 2 * NC + i];
+            tn[m][i] = lane_g[(t + T * m) * 2 * NC + NC + i];
+        }
+    if (tid == 0) { mbar_init(full, 1); mbar_fence_init(); }
+    __syncthreads();
+    const int nzb = Nz / kW;
+    auto issue = [&](long tile) {   // one thread: arm the barrier, then one TMA per box of rows
+        const int kx = (int)(tile / nzb), zb = (int)(tile % nzb);
+        mbar_arrive_expect_tx(full, (uint32_t)(M * kW * sizeof(double2)));
+#pragma unroll
+        for (int r0 = 0; r0 < M; r0 += Y::BOXR) tma_load_3d(X + r0 * kW, &tmB1, full, zb * kW * 2, r0, kx0 + kx);
+    };
+    long tile = blockIdx.x;
+    if (tid == 0 && tile < ntiles) issue(tile);
+    uint32_t parity = 0;
+    double2* Ec = E + grp * (M * kW) + c;
+    for (; tile < ntiles; tile += gridDim.x) {
+        const long kx = tile / nzb;
+        const int zb = (int)(tile % nzb);
+        double vr[R], vi[R];
+        mbar_wait(full, parity);
+        parity ^= 1;
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            const double2 v = X[(t + T * i) * kW + c];
+            vr[i] = v.x; vi[i] = v.y;
+        }
+        __syncthreads();   // every thread holds its part of the tile: X may be refilled
+        if (tid == 0 && tile + gridDim.x < ntiles) issue(tile + gridDim.x);
+        if (grp) {
+#pragma unroll
+            for (int i = 0; i < R; ++i) cmul(vr[i], vi[i], wp[t + T * i]);
+        }
+        fft2_forward_tile<Cfg, kW>(vr, vi, t, Ec, 1 + grp, cc, tn);
+        double2* out = B2 + ((kx * 2 * M + grp) * (long)Nz + zb * kW + c);
+#pragma unroll
+        for (int i = 0; i < R; ++i) out[(long)(2 * (t + T * i)) * Nz] = make_double2(vr[i], vi[i]);
+    }
+}
+
 // ====================================================================================== K4: inv_y
 template <int M>
 __global__ void __launch_bounds__(TileGroups<FftCfg<M>>::G* kW* FftCfg<M>::T)
@@ -238,24 +318,33 @@ struct ConvZ {
     static constexpr int G = 16 / T;                 // pencils per warp at a time
     static constexpr int WARPS = 4;                  // warps per CTA
     static constexpr int ROW = M + 2;                // doubles per spectrum row (E: M/2+1, O: M/2, pad 1)
-    static constexpr size_t smem_bytes() { return sizeof(double2) * (size_t)(2 * M + WARPS * 2 * G * Cfg::BUF); }
+    static constexpr int NC = LaneTw<Cfg::R2>::NC;   // lane-constant twiddles per stage-2 butterfly
+    static constexpr size_t smem_bytes() { return sizeof(double2) * (size_t)(M + WARPS * 2 * G * Cfg::BUF); }
 };
 
 template <int M>
 __global__ void __launch_bounds__(ConvZ<M>::WARPS * 32, (M >= 512 ? 2 : 3))
-k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double2* __restrict__ tw_g,
+k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double* __restrict__ lane_g,
            const double2* __restrict__ wp_g, int Ny, long ngroups) {
     using Z = ConvZ<M>;
     using Cfg = typename Z::Cfg;
-    constexpr int R = Z::R, T = Z::T, G = Z::G, WARPS = Z::WARPS, H = R / 2;
+    constexpr int R = Z::R, T = Z::T, G = Z::G, WARPS = Z::WARPS, H = R / 2, NC = Z::NC, NB2 = Cfg::NB2;
     extern __shared__ double2 smem[];
-    double2* tw = smem;          // M: stage-2 twiddles tw[i*R1 + j] = w_M^(i j)
-    double2* wp = smem + M;      // M: w_2M^n, n < M
-    for (int n = threadIdx.x; n < M; n += blockDim.x) { tw[n] = tw_g[n]; wp[n] = wp_g[n]; }
+    double2* wp = smem;          // M: w_2M^n, n < M
+    for (int n = threadIdx.x; n < M; n += blockDim.x) wp[n] = wp_g[n];
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int g = lane / (2 * T), b = (lane / T) & 1, t = lane % T;
-    double2* buf = smem + 2 * M + ((warp * G + g) * 2 + b) * Cfg::BUF;
+    double2* buf = smem + M + ((warp * G + g) * 2 + b) * Cfg::BUF;
+    // stage-2 twiddles of this lane's butterflies j = t + T*m, kept in registers for the whole kernel
+    double cc[NB2][NC], tn[NB2][NC];
+#pragma unroll
+    for (int m = 0; m < NB2; ++m)
+#pragma unroll
+        for (int i = 0; i < NC; ++i) {
+            cc[m][i] = lane_g[(t + T * m) * 2 * NC + i];
+            tn[m][i] = lane_g[(t + T * m) * 2 * NC + NC + i];
+        }
     const long nwarps = (long)gridDim.x * WARPS;
     const int ny2 = 2 * Ny;
     for (long grp = (long)blockIdx.x * WARPS + warp; grp < ngroups; grp += nwarps) {
@@ -286,36 +375,47 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
         }
         if (b) {
 #pragma unroll
-            for (int i = 0; i < R; ++i) cmul(vr[i], vi[i], wp[t + T * i]);
+            for (int i = 0; i < R; ++i) {
+                cmul(vr[i], vi[i], wp[t + T * i]);
+                if ((i & 7) == 7) asm volatile("" ::: "memory");
+            }
         }
-        // Two passes over ONE copy of the transform code (the kernel would not fit the instruction
-        // cache otherwise): IFFT(Y) = conj(FFT(conj(Y))).  Pass 0 ends with Y = conj(Ghat * X).
+        // Two passes over ONE copy of the transform code: IFFT(Y) = conj(FFT(conj(Y))).
+        // Pass 0 ends with Y = conj(Ghat * X).
 #pragma unroll 1
         for (int pass = 0; pass < 2; ++pass) {
-            fft2_forward<Cfg>(vr, vi, t, buf, tw);
+            fft2_forward_lc<Cfg>(vr, vi, t, buf, cc, tn);
             if (pass == 0) {
 #pragma unroll
-                for (int i = 0; i < R; ++i) {
-                    const int j = t + T * i;
-                    const int m = b ? (j < M - 1 - j ? j : M - 1 - j) : (j < M - j ? j : M - j);
-                    const double gk = __ldg(grow + m);
-                    vr[i] *= gk; vi[i] *= -gk;
+                for (int i0 = 0; i0 < R; i0 += 8) {
+                    double gk[8];
+#pragma unroll
+                    for (int i = i0; i < i0 + 8 && i < R; ++i) {
+                        const int j = t + T * i;
+                        const int m = b ? (j < M - 1 - j ? j : M - 1 - j) : (j < M - j ? j : M - j);
+                        gk[i - i0] = __ldg(grow + m);
+                    }
+#pragma unroll
+                    for (int i = i0; i < i0 + 8 && i < R; ++i) { vr[i] *= gk[i - i0]; vi[i] *= -gk[i - i0]; }
+                    asm volatile("" ::: "memory");
                 }
             }
         }
-        // now (vr, -vi) = IFFT(Ghat X); the odd branch still needs conj(w^n): conj(v) conj(w) = conj(v w)
-        if (b) {
-#pragma unroll
-            for (int i = 0; i < R; ++i) cmul(vr[i], vi[i], wp[t + T * i]);
-        }
-        // y[n] = y_e[n] + y_o[n]: branch 0 finishes n = t + T*i for i < R/2, branch 1 for i >= R/2
+        // now v = FFT(conj(Ghat X)), i.e. IFFT(Ghat X) = conj(v) on each branch, and
+        //     y[n] = y_e[n] + conj(w^n) y_o[n] = conj( v_e[n] + w^n v_o[n] ).
+        // Branch 0 finishes n = t + T*i for i < R/2, branch 1 for i >= R/2: one exchange of the halves,
+        // then 4 FMAs per value on every lane.
 #pragma unroll
         for (int i = 0; i < H; ++i) {
             const double sr = b ? vr[i] : vr[i + H], si = b ? vi[i] : vi[i + H];
             const double pr = __shfl_xor_sync(0xffffffffu, sr, T), pi = __shfl_xor_sync(0xffffffffu, si, T);
             const int o = b ? i + H : i;
-            const double kr = b ? vr[i + H] : vr[i], ki = b ? vi[i + H] : vi[i];
-            base[t + T * o] = make_double2(kr + pr, -ki - pi);
+            const double ar = b ? pr : vr[i], ai = b ? pi : vi[i];            // v_e[n]
+            const double qr = b ? vr[i + H] : pr, qi = b ? vi[i + H] : pi;    // v_o[n]
+            const double2 w = wp[t + T * o];
+            const double zr = fma(-w.y, qi, fma(w.x, qr, ar));
+            const double zi = fma(w.y, qr, fma(w.x, qi, ai));
+            base[t + T * o] = make_double2(zr, -zi);
         }
     }
 }
