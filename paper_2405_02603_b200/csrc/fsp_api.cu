@@ -34,6 +34,7 @@ struct fsp_plan {
     double* LTy = nullptr;  // the same for the y transform (tile kernels)
     bool tile_y = false;    // K2/K4 tile kernels (TMA-staged) are used
     CUtensorMap tmB1y;      // B1 as [kx][y][2 Nz doubles], box = 8 columns x <=256 rows (K2 input)
+    CUtensorMap tmB2y;      // B2 as [kx][j][parity][2 Nz doubles], box = 8 columns x 1 parity x <=256 j (K4 input)
     bool z_warp = false;    // K3 v2 (k_conv_z_w) is used
     int chunk_planes = 0;   // > 0: K2-K3-K4 run chunk_planes kx-planes at a time (L2-resident B2)
     int sm_count = 148;
@@ -337,7 +338,30 @@ int do_conv_z(fsp_plan* p, double2* B2, int kx0, int np) {
 }
 int make_z_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Nz, &p->LTz, &p->bytes) }
 int make_y_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Ny, &p->LTy, &p->bytes) }
-int do_inv_y(fsp_plan* p, const double2* B2, double2* B1, int np) { DISPATCH_YZ(launch_inv_y, p->Ny, p, B2, B1, np) }
+template <int M>
+int launch_inv_y_t(fsp_plan* p, double2* B1, int nplanes) {
+    using Y = TileYI<M>;
+    const long ntiles = (long)nplanes * (p->Nz / kW);
+    const size_t smem = Y::smem_bytes();
+    static int occ = 0;
+    if (occ == 0) {
+        CU(cudaFuncSetAttribute(k_inv_y_t<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_inv_y_t<M>, Y::THREADS, smem));
+        if (occ < 1) return FSP_ERR_CUDA;
+    }
+    long grid = (long)p->sm_count * occ;
+    if (grid > ntiles) grid = ntiles;
+    k_inv_y_t<M><<<(unsigned)grid, Y::THREADS, smem, p->stream>>>(p->tmB2y, B1, p->LTy, p->Wy, p->Nz, ntiles);
+    return FSP_OK;
+}
+// B2 must be the plan's own B2 (the tile kernel reads it through the plan's tensor map)
+int do_inv_y(fsp_plan* p, const double2* B2, double2* B1, int np) {
+    if (p->tile_y && B2 == p->B2) {
+        if (p->Ny == 512) return launch_inv_y_t<512>(p, B1, np);
+        return launch_inv_y_t<256>(p, B1, np);
+    }
+    DISPATCH_YZ(launch_inv_y, p->Ny, p, B2, B1, np)
+}
 int do_inv_x(fsp_plan* p, double* phi) { DISPATCH_X(launch_inv_x, p->Nx / 2, p, phi) }
 
 unsigned grid_for(long total, int block) {
@@ -533,6 +557,12 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
         const cuuint64_t strides[2] = {(cuuint64_t)Nz * 16, (cuuint64_t)Ny * Nz * 16};
         const cuuint32_t box[3] = {2 * kW, (cuuint32_t)(Ny < 256 ? Ny : 256), 1};
         rc = make_tensor_map(&p->tmB1y, p->B1, 3, dims, strides, box);
+    }
+    if (rc == FSP_OK && p->tile_y) {
+        const cuuint64_t dims[4] = {(cuuint64_t)2 * Nz, 2, (cuuint64_t)Ny, (cuuint64_t)(Nx + 1)};
+        const cuuint64_t strides[3] = {(cuuint64_t)Nz * 16, (cuuint64_t)2 * Nz * 16, (cuuint64_t)2 * Ny * Nz * 16};
+        const cuuint32_t box[4] = {2 * kW, 1, (cuuint32_t)(Ny < 256 ? Ny : 256), 1};
+        rc = make_tensor_map(&p->tmB2y, p->B2, 4, dims, strides, box);
     }
     if (rc == FSP_OK) rc = dev_alloc(&p->T, nt, &p->bytes);
     if (rc == FSP_OK) rc = dev_alloc(&p->Goct, nt, &p->bytes);

@@ -241,6 +241,111 @@ k_inv_y(const double2* __restrict__ B2, double2* __restrict__ B1, const double2*
     }
 }
 
+// ================================================================================= K4 (v2): inv_y_t
+// Tile kernel, mirror image of k_fwd_y_t: group 0 inverse-transforms the even rows of the tile
+// [2M rows][kW columns] of B2, group 1 the odd rows; then y[n] = y_e[n] + conj(w^n) y_o[n] for n < M.
+// B2 is seen through a 4-D tensor map [plane][j][parity][2 Nz doubles], so that each group's TMA box
+// holds the rows of one parity only.  Each group's buffer X_g receives the tile and then serves as the
+// group's exchange buffer (same [position][kW] layout); once the exchange has been read back the buffer
+// is handed to the TMA for the next tile (whose lines were prefetched into L2 when this tile started).
+// The halves of y_e / y_o that the other group finishes travel through C.
+template <int M>
+struct TileYI {
+    using Cfg = Fft2Cfg<M>;
+    static constexpr int T = Cfg::T, R = Cfg::R;
+    static constexpr int GT = kW * T, THREADS = 2 * GT;
+    static constexpr int NC = LaneTw<Cfg::R2>::NC;
+    static constexpr int MINB = (M >= 512) ? 1 : 2;
+    static constexpr int BOXR = M < 256 ? M : 256;
+    // [mbarriers: 128 B][X: 2 groups x M*kW][C: 2 groups x (M/2)*kW][wp: M]
+    static constexpr size_t smem_bytes() { return 128 + sizeof(double2) * (size_t)(3 * M * kW + M); }
+};
+
+template <int M>
+__global__ void __launch_bounds__(TileYI<M>::THREADS, TileYI<M>::MINB)
+k_inv_y_t(const __grid_constant__ CUtensorMap tmB2, double2* __restrict__ B1, const double* __restrict__ lane_g,
+          const double2* __restrict__ wp_g, int Nz, long ntiles) {
+    using Y = TileYI<M>;
+    using Cfg = typename Y::Cfg;
+    constexpr int R = Y::R, T = Y::T, GT = Y::GT, NC = Y::NC, NB2 = Cfg::NB2, H = R / 2;
+    extern __shared__ __align__(128) unsigned char smraw[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smraw);   // full[0], full[1]
+    double2* X = reinterpret_cast<double2*>(smraw + 128);
+    double2* C = X + 2 * M * kW;
+    double2* wp = C + M * kW;
+    const int tid = threadIdx.x;
+    const int grp = tid / GT, gt = tid % GT, c = gt % kW, t = gt / kW;
+    for (int n = tid; n < M; n += Y::THREADS) wp[n] = wp_g[n];
+    double cc[NB2][NC], tn[NB2][NC];
+#pragma unroll
+    for (int m = 0; m < NB2; ++m)
+#pragma unroll
+        for (int i = 0; i < NC; ++i) {
+            cc[m][i] = lane_g[(t + T * m) * 2 * NC + i];
+            tn[m][i] = lane_g[(t + T * m) * 2 * NC + NC + i];
+        }
+    if (tid == 0) { mbar_init(&full[0], 1); mbar_init(&full[1], 1); mbar_fence_init(); }
+    __syncthreads();
+    const int nzb = Nz / kW;
+    double2* Xg = X + grp * (M * kW);
+    auto issue = [&](long tile) {   // one thread of the group: this group's rows of the tile
+        const int kx = (int)(tile / nzb), zb = (int)(tile % nzb);
+        mbar_arrive_expect_tx(&full[grp], (uint32_t)(M * kW * sizeof(double2)));
+#pragma unroll
+        for (int r0 = 0; r0 < M; r0 += Y::BOXR) tma_load_4d(Xg + r0 * kW, &tmB2, &full[grp], zb * kW * 2, grp, r0, kx);
+    };
+    auto prefetch = [&](long tile) {
+        const int kx = (int)(tile / nzb), zb = (int)(tile % nzb);
+#pragma unroll
+        for (int r0 = 0; r0 < M; r0 += Y::BOXR) tma_prefetch_4d(&tmB2, zb * kW * 2, grp, r0, kx);
+    };
+    long tile = blockIdx.x;
+    if (gt == 0 && tile < ntiles) issue(tile);
+    uint32_t parity = 0;
+    double2* Ec = Xg + c;
+    double2* Cmine = C + grp * (M / 2 * kW) + c;          // what this group gives away
+    double2* Ctheirs = C + (grp ^ 1) * (M / 2 * kW) + c;  // what it receives
+    for (; tile < ntiles; tile += gridDim.x) {
+        const long kx = tile / nzb;
+        const int zb = (int)(tile % nzb);
+        const bool more = tile + gridDim.x < ntiles;
+        if (gt == 0 && more) prefetch(tile + gridDim.x);
+        double vr[R], vi[R];
+        mbar_wait(&full[grp], parity);
+        parity ^= 1;
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            const double2 v = Ec[(t + T * i) * kW];
+            vr[i] = v.x; vi[i] = v.y;
+        }
+        // inverse transform = forward transform with the roles of re and im swapped; the first barrier
+        // inside also separates the reads of X_g above from its reuse as exchange buffer
+        fft2_forward_tile<Cfg, kW>(vi, vr, t, Ec, 1 + grp, cc, tn);
+        bar_sync(1 + grp, GT);   // exchange read back by the whole group: X_g is free
+        if (gt == 0 && more) { fence_proxy_async(); issue(tile + gridDim.x); }
+        __syncthreads();         // C of the previous tile has been consumed by both groups
+#pragma unroll
+        for (int i = 0; i < H; ++i) {
+            const int s = grp ? i : i + H;    // group 1 gives away y_o[n], i < H; group 0 gives y_e[n], i >= H
+            Cmine[(t + T * i) * kW] = make_double2(vr[s], vi[s]);
+        }
+        __syncthreads();
+        double2* out = B1 + ((kx * M) * (long)Nz + zb * kW + c);
+#pragma unroll
+        for (int i = 0; i < H; ++i) {
+            const double2 pv = Ctheirs[(t + T * i) * kW];
+            const int o = grp ? i + H : i;
+            const double er = grp ? pv.x : vr[i], ei = grp ? pv.y : vi[i];                 // y_e[n]
+            const double qr = grp ? vr[i + H] : pv.x, qi = grp ? vi[i + H] : pv.y;         // y_o[n]
+            const double2 w = wp[t + T * o];
+            // y = y_e + conj(w) y_o
+            const double yr = fma(w.y, qi, fma(w.x, qr, er));
+            const double yi = fma(-w.y, qr, fma(w.x, qi, ei));
+            out[(long)(t + T * o) * Nz] = make_double2(yr, yi);
+        }
+    }
+}
+
 // ===================================================================================== K3: conv_z
 // Contiguous pencils of M = Nz complex; T threads per pencil (t fastest), P pencils per CTA.
 // Gh: [pencil][2][M] doubles, plane 0 = Ghat[2j] (even), plane 1 = Ghat[2j+1] (odd), scale folded in.
