@@ -424,7 +424,14 @@ struct ConvZ {
     static constexpr int WARPS = 4;                  // warps per CTA
     static constexpr int ROW = M + 2;                // doubles per spectrum row (E: M/2+1, O: M/2, pad 1)
     static constexpr int NC = LaneTw<Cfg::R2>::NC;   // lane-constant twiddles per stage-2 butterfly
-    static constexpr size_t smem_bytes() { return sizeof(double2) * (size_t)(M + WARPS * 2 * G * Cfg::BUF); }
+    // the spectrum row of the current pencil is staged in shared memory by a bulk async copy issued when
+    // the pencil starts, so that its (HBM) latency is spent under the forward transform (only G == 1)
+    static constexpr bool GSTAGE = (G == 1);
+    static constexpr int GROW = GSTAGE ? ROW : 0;    // doubles of staging per warp
+    // [wp: M double2][exchange: WARPS*2*G*BUF double2][G rows: WARPS*GROW doubles][mbarriers: WARPS]
+    static constexpr size_t smem_bytes() {
+        return sizeof(double2) * (size_t)(M + WARPS * 2 * G * Cfg::BUF) + sizeof(double) * (size_t)(WARPS * GROW) + 8 * WARPS;
+    }
 };
 
 template <int M>
@@ -441,6 +448,11 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int g = lane / (2 * T), b = (lane / T) & 1, t = lane % T;
     double2* buf = smem + M + ((warp * G + g) * 2 + b) * Cfg::BUF;
+    double* gst = reinterpret_cast<double*>(smem + M + WARPS * 2 * G * Cfg::BUF) + warp * Z::GROW;
+    uint64_t* gbar = reinterpret_cast<uint64_t*>(reinterpret_cast<double*>(smem + M + WARPS * 2 * G * Cfg::BUF) + WARPS * Z::GROW) + warp;
+    if (Z::GSTAGE && lane == 0) { mbar_init(gbar, 1); mbar_fence_init(); }
+    __syncwarp();
+    uint32_t gpar = 0;
     // stage-2 twiddles of this lane's butterflies j = t + T*m, kept in registers for the whole kernel
     double cc[NB2][NC], tn[NB2][NC];
 #pragma unroll
@@ -460,6 +472,13 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
         const int qy = ky <= Ny ? ky : ny2 - ky;
         double2* base = B2 + (kx * ny2 + ky) * M;
         const double* grow = Gk + (kx * (Ny + 1) + qy) * Z::ROW + (b ? M / 2 + 1 : 0);
+        if constexpr (Z::GSTAGE) {
+            // all lanes are past the previous pencil's reads of gst (the shuffles of the final combine)
+            if (lane == 0) {
+                mbar_arrive_expect_tx(gbar, Z::ROW * 8);
+                bulk_load(gst, Gk + (kx * (Ny + 1) + qy) * Z::ROW, Z::ROW * 8, gbar);
+            }
+        }
 
         double vr[R], vi[R];
 #pragma unroll
@@ -480,10 +499,7 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
         }
         if (b) {
 #pragma unroll
-            for (int i = 0; i < R; ++i) {
-                cmul(vr[i], vi[i], wp[t + T * i]);
-                if ((i & 7) == 7) asm volatile("" ::: "memory");
-            }
+            for (int i = 0; i < R; ++i) cmul(vr[i], vi[i], wp[t + T * i]);
         }
         // Two passes over ONE copy of the transform code: IFFT(Y) = conj(FFT(conj(Y))).
         // Pass 0 ends with Y = conj(Ghat * X).
@@ -491,18 +507,18 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
         for (int pass = 0; pass < 2; ++pass) {
             fft2_forward_lc<Cfg>(vr, vi, t, buf, cc, tn);
             if (pass == 0) {
+                const double* gsrc = grow;
+                if constexpr (Z::GSTAGE) {
+                    mbar_wait(gbar, gpar);
+                    gpar ^= 1;
+                    gsrc = gst + (b ? M / 2 + 1 : 0);
+                }
 #pragma unroll
-                for (int i0 = 0; i0 < R; i0 += 8) {
-                    double gk[8];
-#pragma unroll
-                    for (int i = i0; i < i0 + 8 && i < R; ++i) {
-                        const int j = t + T * i;
-                        const int m = b ? (j < M - 1 - j ? j : M - 1 - j) : (j < M - j ? j : M - j);
-                        gk[i - i0] = __ldg(grow + m);
-                    }
-#pragma unroll
-                    for (int i = i0; i < i0 + 8 && i < R; ++i) { vr[i] *= gk[i - i0]; vi[i] *= -gk[i - i0]; }
-                    asm volatile("" ::: "memory");
+                for (int i = 0; i < R; ++i) {
+                    const int j = t + T * i;
+                    const int m = b ? (j < M - 1 - j ? j : M - 1 - j) : (j < M - j ? j : M - j);
+                    const double gk = Z::GSTAGE ? gsrc[m] : __ldg(gsrc + m);
+                    vr[i] *= gk; vi[i] *= -gk;
                 }
             }
         }
