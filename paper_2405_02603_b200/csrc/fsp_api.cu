@@ -2,6 +2,7 @@
 // five-kernel solve.  Host code only marshals sizes and launches; every step of the path runs in the
 // kernels of solve_kernels.cuh / green_kernels.cuh.
 #include <cmath>
+#include <cstdint>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -33,6 +34,10 @@ struct fsp_plan {
     double* LTz = nullptr;  // lane-constant stage-2 twiddles of the z transform (fft_warp.cuh dft_lane)
     double* LTy = nullptr;  // the same for the y transform (tile kernels)
     bool tile_y = false;    // K2/K4 tile kernels (TMA-staged) are used
+    double* LTx = nullptr;  // lane-constant twiddles of the x transform (length Nx/2)
+    bool tile_x = false;    // K1 tile kernel is used
+    CUtensorMap tmRho;      // rho as [x][Ny*Nz doubles], box = 16 columns x <=256 rows; re-encoded when rho moves
+    const double* tmRho_ptr = nullptr;
     CUtensorMap tmB1y;      // B1 as [kx][y][2 Nz doubles], box = 8 columns x <=256 rows (K2 input)
     CUtensorMap tmB2y;      // B2 as [kx][j][parity][2 Nz doubles], box = 8 columns x 1 parity x <=256 j (K4 input)
     bool z_warp = false;    // K3 v2 (k_conv_z_w) is used
@@ -309,7 +314,37 @@ int launch_inv_x(fsp_plan* p, double* phi) {
         default: return FSP_ERR_INVALID_ARG;             \
     }
 
-int do_fwd_x(fsp_plan* p, const double* rho) { DISPATCH_X(launch_fwd_x, p->Nx / 2, p, rho) }
+template <int M>
+int launch_fwd_x_t(fsp_plan* p) {
+    using X_ = TileX<M>;
+    const long plane = (long)p->Ny * p->Nz, ntiles = plane / kC;
+    const size_t smem = X_::smem_bytes();
+    static int occ = 0;
+    if (occ == 0) {
+        CU(cudaFuncSetAttribute(k_fwd_x_t<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_fwd_x_t<M>, X_::THREADS, smem));
+        if (occ < 1) return FSP_ERR_CUDA;
+    }
+    long grid = (long)p->sm_count * occ;
+    if (grid > ntiles) grid = ntiles;
+    k_fwd_x_t<M><<<(unsigned)grid, X_::THREADS, smem, p->stream>>>(p->tmRho, p->B1, p->LTx, p->Wx, plane, ntiles);
+    return FSP_OK;
+}
+int do_fwd_x(fsp_plan* p, const double* rho) {
+    if (p->tile_x && (reinterpret_cast<uintptr_t>(rho) & 15) == 0) {
+        if (rho != p->tmRho_ptr) {   // the caller owns rho: encode the map for this address (host only, ~1 us)
+            const cuuint64_t dims[2] = {(cuuint64_t)p->Ny * p->Nz, (cuuint64_t)p->Nx};
+            const cuuint64_t strides[1] = {(cuuint64_t)p->Ny * p->Nz * 8};
+            const cuuint32_t box[2] = {kC, (cuuint32_t)(p->Nx < 256 ? p->Nx : 256)};
+            int rc = make_tensor_map(&p->tmRho, const_cast<double*>(rho), 2, dims, strides, box);
+            if (rc != FSP_OK) return rc;
+            p->tmRho_ptr = rho;
+        }
+        if (p->Nx == 512) return launch_fwd_x_t<256>(p);
+        return launch_fwd_x_t<128>(p);
+    }
+    DISPATCH_X(launch_fwd_x, p->Nx / 2, p, rho)
+}
 int do_fwd_y(fsp_plan* p, int kx0, double2* B2, int np) {
     if (p->tile_y) {
         if (p->Ny == 512) return launch_fwd_y_t<512>(p, kx0, B2, np);
@@ -337,6 +372,7 @@ int do_conv_z(fsp_plan* p, double2* B2, int kx0, int np) {
     return do_conv_z_v1(p, B2, p->Gh + (size_t)kx0 * (2 * p->Ny) * (2 * p->Nz), np);
 }
 int make_z_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Nz, &p->LTz, &p->bytes) }
+int make_x_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Nx / 2, &p->LTx, &p->bytes) }
 int make_y_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Ny, &p->LTy, &p->bytes) }
 template <int M>
 int launch_inv_y_t(fsp_plan* p, double2* B1, int nplanes) {
@@ -488,7 +524,7 @@ int precompute_impl(fsp_plan* p) {
 }
 
 void free_plan_memory(fsp_plan* p) {
-    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->Gh); cudaFree(p->Gk); cudaFree(p->LTz); cudaFree(p->LTy); cudaFree(p->T); cudaFree(p->Goct);
+    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->Gh); cudaFree(p->Gk); cudaFree(p->LTz); cudaFree(p->LTy); cudaFree(p->LTx); cudaFree(p->T); cudaFree(p->Goct);
     cudaFree(p->Wx); cudaFree(p->Wy); cudaFree(p->Wz); cudaFree(p->rho_stage); cudaFree(p->phi_stage);
     for (cudaEvent_t e : p->events) cudaEventDestroy(e);
     p->events.clear();
@@ -550,6 +586,8 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
     if (rc == FSP_OK && !p->z_warp) rc = dev_alloc(&p->Gh, ng, &p->bytes);
     if (rc == FSP_OK && p->z_warp) rc = dev_alloc(&p->Gk, (size_t)(Nx + 1) * (Ny + 1) * (Nz + 2), &p->bytes);
     if (rc == FSP_OK && p->z_warp) rc = make_z_lane_table(p);
+    p->tile_x = (Nx == 256 || Nx == 512) && ((long)Ny * Nz) % kC == 0;
+    if (rc == FSP_OK && p->tile_x) rc = make_x_lane_table(p);
     p->tile_y = (Ny == 256 || Ny == 512) && Nz >= kW;
     if (rc == FSP_OK && p->tile_y) rc = make_y_lane_table(p);
     if (rc == FSP_OK && p->tile_y) {

@@ -20,6 +20,7 @@
 // and its inverse  Z[k] = (A + B) + i conj(w^k) (A - B),  A = X[k], B = conj(X[Nx-k]).
 // The factor 1/2 and hx hy hz/(8 Nx Ny Nz) live in Ghat.
 #pragma once
+#include <type_traits>
 #include "fft_engine.cuh"
 #include "fft_warp.cuh"
 
@@ -538,6 +539,130 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
             const double zi = fma(w.y, qr, fma(w.x, qi, ai));
             base[t + T * o] = make_double2(zr, -zi);
         }
+    }
+}
+
+// ================================================================================ K1 (v2): fwd_x_r2c_t
+// Tile kernel for the real-to-complex pass along x (M = Nx/2 complex points z[n] = rho[2n] + i rho[2n+1]).
+// Tile = all Nx rows of kC = 16 adjacent columns of the flattened (y, z) plane (one 128-byte line of
+// doubles per row), delivered by TMA through a 2-D tensor map over rho.  Group 0 computes Z[2j], group 1
+// Z[2j+1] (input times w_N^n); the untangling partner Z[N-k] has the parity of k, so it is found inside
+// the group: the group's exchange buffer is reused to look it up.  The twiddles w_2N^k and w_N^n factor
+// into a per-lane constant times a compile-time 32nd root of unity (k = (2t+g) + 2T i, n = t + T i,
+// N/T = 32), so no twiddle table is read.
+constexpr int kC = 16;
+template <int M>
+struct TileX {
+    using Cfg = Fft2Cfg<M>;
+    static constexpr int T = Cfg::T, R = Cfg::R;
+    static_assert(2 * M / T == 32, "tile x kernels assume N/T = 32");
+    static constexpr int GT = kC * T, THREADS = 2 * GT;
+    static constexpr int NC = LaneTw<Cfg::R2>::NC;
+    static constexpr int MINB = (M >= 256) ? 1 : 2;
+    // [mbarriers: 128 B][X: 2M rows x kC doubles = M*kC double2][E: 2 groups x M*kC double2]
+    static constexpr size_t smem_bytes() { return 128 + sizeof(double2) * (size_t)(3 * M * kC); }
+};
+
+// x * w_32^i (compile-time i)
+template <int i>
+__device__ __forceinline__ void cmul_w32(double& xr, double& xi) {
+    if constexpr ((i & 31) == 0) {
+    } else if constexpr ((i & 31) == 8) {   // -i
+        const double a = xi; xi = -xr; xr = a;
+    } else {
+        const double c = cos32(i), sn = sin32(i);
+        const double a = fma(xi, sn, xr * c);
+        xi = fma(-xr, sn, xi * c);
+        xr = a;
+    }
+}
+
+template <int M, int I = 0>
+struct UntangleFwd {   // unrolled over the register index with compile-time roots
+    template <class F>
+    __device__ __forceinline__ static void run(F&& f) {
+        if constexpr (I < Fft2Cfg<M>::R) {
+            f(std::integral_constant<int, I>{});
+            UntangleFwd<M, I + 1>::run(f);
+        }
+    }
+};
+
+template <int M>
+__global__ void __launch_bounds__(TileX<M>::THREADS, TileX<M>::MINB)
+k_fwd_x_t(const __grid_constant__ CUtensorMap tmRho, double2* __restrict__ B1, const double* __restrict__ lane_g,
+          const double2* __restrict__ Wg, long plane, long ntiles) {
+    using X_ = TileX<M>;
+    using Cfg = typename X_::Cfg;
+    constexpr int R = X_::R, T = X_::T, GT = X_::GT, NC = X_::NC, NB2 = Cfg::NB2, N = 2 * M;
+    constexpr int BOXR = N < 256 ? N : 256;
+    extern __shared__ __align__(128) unsigned char smraw[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smraw);
+    double* Xd = reinterpret_cast<double*>(smraw + 128);
+    double2* E = reinterpret_cast<double2*>(smraw + 128) + M * kC;
+    const int tid = threadIdx.x;
+    const int grp = tid / GT, gt = tid % GT, c = gt % kC, t = gt / kC;
+    double cc[NB2][NC], tn[NB2][NC];
+#pragma unroll
+    for (int m = 0; m < NB2; ++m)
+#pragma unroll
+        for (int i = 0; i < NC; ++i) {
+            cc[m][i] = lane_g[(t + T * m) * 2 * NC + i];
+            tn[m][i] = lane_g[(t + T * m) * 2 * NC + NC + i];
+        }
+    const double2 lam_n = Wg[2 * t];          // w_N^t     (Wg[m] = exp(-2 pi i m / 2N))
+    const double2 lam_k = Wg[2 * t + grp];    // w_2N^(2t+g)
+    if (tid == 0) { mbar_init(full, 1); mbar_fence_init(); }
+    __syncthreads();
+    auto issue = [&](long tile) {
+        mbar_arrive_expect_tx(full, (uint32_t)(N * kC * sizeof(double)));
+#pragma unroll
+        for (int r0 = 0; r0 < N; r0 += BOXR) tma_load_2d(Xd + r0 * kC, &tmRho, full, (int)(tile * kC), r0);
+    };
+    long tile = blockIdx.x;
+    if (tid == 0 && tile < ntiles) issue(tile);
+    uint32_t parity = 0;
+    double2* Ec = E + grp * (M * kC) + c;
+    for (; tile < ntiles; tile += gridDim.x) {
+        double vr[R], vi[R];
+        mbar_wait(full, parity);
+        parity ^= 1;
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            const int n = t + T * i;
+            vr[i] = Xd[(2 * n) * kC + c];
+            vi[i] = Xd[(2 * n + 1) * kC + c];
+        }
+        __syncthreads();   // X may be refilled
+        if (tid == 0 && tile + gridDim.x < ntiles) issue(tile + gridDim.x);
+        if (grp) {   // z[n] w_N^n,  w_N^n = w_N^t w_32^i
+            UntangleFwd<M>::run([&](auto ic) {
+                constexpr int i = decltype(ic)::value;
+                cmul(vr[i], vi[i], lam_n);
+                cmul_w32<i>(vr[i], vi[i]);
+            });
+        }
+        fft2_forward_tile<Cfg, kC>(vr, vi, t, Ec, 1 + grp, cc, tn);
+        // untangle: X'[k] = (A + B) - i w_2N^k (A - B), A = Z[k], B = conj(Z[N-k]), k = 2j + g, j = t + T i
+        bar_sync(1 + grp, GT);   // exchange buffer read back by the whole group
+#pragma unroll
+        for (int i = 0; i < R; ++i) Ec[(t + T * i) * kC] = make_double2(vr[i], vi[i]);
+        bar_sync(1 + grp, GT);
+        double2* out = B1 + tile * kC + c;
+        UntangleFwd<M>::run([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            const int j = t + T * i;
+            const int jp = grp ? M - 1 - j : (M - j) & (M - 1);
+            const double2 bq = Ec[jp * kC];
+            const double ar = vr[i], ai = vi[i], br = bq.x, bi = -bq.y;
+            const double sr = ar + br, si = ai + bi;
+            double dr = ar - br, di = ai - bi;
+            cmul(dr, di, lam_k);
+            cmul_w32<i>(dr, di);
+            const long k = 2 * j + grp;
+            out[k * plane] = make_double2(sr + di, si - dr);
+            if (i == 0 && grp == 0 && t == 0) out[(long)N * plane] = make_double2(2.0 * (ar - ai), 0.0);
+        });
     }
 }
 
