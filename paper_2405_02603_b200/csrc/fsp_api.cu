@@ -38,6 +38,7 @@ struct fsp_plan {
     bool tile_x = false;    // K1 tile kernel is used
     CUtensorMap tmRho;      // rho as [x][Ny*Nz doubles], box = 16 columns x <=256 rows; re-encoded when rho moves
     const double* tmRho_ptr = nullptr;
+    CUtensorMap tmB1x;      // B1 as [j][parity][2 Ny Nz doubles] (row = 2j + parity), box = 16 columns x 1 x <=256 (K5 input)
     CUtensorMap tmB1y;      // B1 as [kx][y][2 Nz doubles], box = 8 columns x <=256 rows (K2 input)
     CUtensorMap tmB2y;      // B2 as [kx][j][parity][2 Nz doubles], box = 8 columns x 1 parity x <=256 j (K4 input)
     bool z_warp = false;    // K3 v2 (k_conv_z_w) is used
@@ -398,7 +399,29 @@ int do_inv_y(fsp_plan* p, const double2* B2, double2* B1, int np) {
     }
     DISPATCH_YZ(launch_inv_y, p->Ny, p, B2, B1, np)
 }
-int do_inv_x(fsp_plan* p, double* phi) { DISPATCH_X(launch_inv_x, p->Nx / 2, p, phi) }
+template <int M>
+int launch_inv_x_t(fsp_plan* p, double* phi) {
+    using X_ = TileXI<M>;
+    const long plane = (long)p->Ny * p->Nz, ntiles = plane / kC;
+    const size_t smem = X_::smem_bytes();
+    static int occ = 0;
+    if (occ == 0) {
+        CU(cudaFuncSetAttribute(k_inv_x_t<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_inv_x_t<M>, X_::THREADS, smem));
+        if (occ < 1) return FSP_ERR_CUDA;
+    }
+    long grid = (long)p->sm_count * occ;
+    if (grid > ntiles) grid = ntiles;
+    k_inv_x_t<M><<<(unsigned)grid, X_::THREADS, smem, p->stream>>>(p->tmB1x, p->B1, phi, p->LTx, p->Wx, plane, ntiles);
+    return FSP_OK;
+}
+int do_inv_x(fsp_plan* p, double* phi) {
+    if (p->tile_x) {
+        if (p->Nx == 512) return launch_inv_x_t<256>(p, phi);
+        return launch_inv_x_t<128>(p, phi);
+    }
+    DISPATCH_X(launch_inv_x, p->Nx / 2, p, phi)
+}
 
 unsigned grid_for(long total, int block) {
     long g = (total + block - 1) / block;
@@ -588,6 +611,13 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
     if (rc == FSP_OK && p->z_warp) rc = make_z_lane_table(p);
     p->tile_x = (Nx == 256 || Nx == 512) && ((long)Ny * Nz) % kC == 0;
     if (rc == FSP_OK && p->tile_x) rc = make_x_lane_table(p);
+    if (rc == FSP_OK && p->tile_x) {
+        const cuuint64_t plane = (cuuint64_t)Ny * Nz;
+        const cuuint64_t dims[3] = {2 * plane, 2, (cuuint64_t)(Nx / 2)};
+        const cuuint64_t strides[2] = {plane * 16, 2 * plane * 16};
+        const cuuint32_t box[3] = {2 * kC, 1, (cuuint32_t)(Nx / 2 < 256 ? Nx / 2 : 256)};
+        rc = make_tensor_map(&p->tmB1x, p->B1, 3, dims, strides, box);
+    }
     p->tile_y = (Ny == 256 || Ny == 512) && Nz >= kW;
     if (rc == FSP_OK && p->tile_y) rc = make_y_lane_table(p);
     if (rc == FSP_OK && p->tile_y) {

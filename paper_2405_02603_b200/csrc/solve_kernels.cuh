@@ -666,6 +666,131 @@ k_fwd_x_t(const __grid_constant__ CUtensorMap tmRho, double2* __restrict__ B1, c
     }
 }
 
+// ================================================================================ K5 (v2): inv_x_c2r_t
+// Tile kernel for the complex-to-real pass along x, mirror image of k_fwd_x_t.  Group g rebuilds
+// Z[2j+g] = (A + B) + i conj(w_2N^k)(A - B), A = X[k], B = conj(X[N-k]) (N - k has the parity of k, so each
+// group needs the rows of its own parity only: 3-D tensor map [j][parity][2 plane doubles]; row N, needed
+// by k = 0, comes by a separate bulk copy), inverse-transforms it in place in its buffer, and
+// y[n] = y_e[n] + conj(w_N^n) y_o[n] gives phi[2n] = Re y[n], phi[2n+1] = Im y[n]: the restriction of
+// PAPER.md:82 is simply that rows n >= Nx/2 are never formed.
+template <int i>
+__device__ __forceinline__ void cmul_w32c(double& xr, double& xi) {   // x * conj(w_32^i)
+    if constexpr ((i & 31) == 0) {
+    } else if constexpr ((i & 31) == 8) {   // +i
+        const double a = -xi; xi = xr; xr = a;
+    } else {
+        const double c = cos32(i), sn = sin32(i);
+        const double a = fma(-xi, sn, xr * c);
+        xi = fma(xr, sn, xi * c);
+        xr = a;
+    }
+}
+
+template <int M>
+struct TileXI {
+    using Cfg = Fft2Cfg<M>;
+    static constexpr int T = Cfg::T, R = Cfg::R;
+    static_assert(2 * M / T == 32, "tile x kernels assume N/T = 32");
+    static constexpr int GT = kC * T, THREADS = 2 * GT;
+    static constexpr int NC = LaneTw<Cfg::R2>::NC;
+    static constexpr int MINB = (M >= 256) ? 1 : 2;
+    static constexpr int BOXR = M < 256 ? M : 256;
+    // [mbarriers: 128 B][row N: kC double2][X: 2 groups x M*kC][C: 2 groups x (M/2)*kC]
+    static constexpr size_t smem_bytes() { return 128 + sizeof(double2) * (size_t)(kC + 3 * M * kC); }
+};
+
+template <int M>
+__global__ void __launch_bounds__(TileXI<M>::THREADS, TileXI<M>::MINB)
+k_inv_x_t(const __grid_constant__ CUtensorMap tmB1, const double2* __restrict__ B1, double* __restrict__ phi,
+          const double* __restrict__ lane_g, const double2* __restrict__ Wg, long plane, long ntiles) {
+    using X_ = TileXI<M>;
+    using Cfg = typename X_::Cfg;
+    constexpr int R = X_::R, T = X_::T, GT = X_::GT, NC = X_::NC, NB2 = Cfg::NB2, N = 2 * M, H = R / 2;
+    extern __shared__ __align__(128) unsigned char smraw[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smraw);
+    double2* XN = reinterpret_cast<double2*>(smraw + 128);
+    double2* X = XN + kC;
+    double2* C = X + 2 * M * kC;
+    const int tid = threadIdx.x;
+    const int grp = tid / GT, gt = tid % GT, c = gt % kC, t = gt / kC;
+    double cc[NB2][NC], tn[NB2][NC];
+#pragma unroll
+    for (int m = 0; m < NB2; ++m)
+#pragma unroll
+        for (int i = 0; i < NC; ++i) {
+            cc[m][i] = lane_g[(t + T * m) * 2 * NC + i];
+            tn[m][i] = lane_g[(t + T * m) * 2 * NC + NC + i];
+        }
+    const double2 lam_n = Wg[2 * t];          // w_N^t
+    const double2 lam_k = Wg[2 * t + grp];    // w_2N^(2t+g)
+    if (tid == 0) { mbar_init(&full[0], 1); mbar_init(&full[1], 1); mbar_fence_init(); }
+    __syncthreads();
+    double2* Xg = X + grp * (M * kC);
+    auto issue = [&](long tile) {   // one thread of the group
+        const uint32_t bytes = (uint32_t)(M * kC * sizeof(double2)) + (grp == 0 ? (uint32_t)(kC * sizeof(double2)) : 0u);
+        mbar_arrive_expect_tx(&full[grp], bytes);
+#pragma unroll
+        for (int r0 = 0; r0 < M; r0 += X_::BOXR) tma_load_3d(Xg + r0 * kC, &tmB1, &full[grp], (int)(tile * kC * 2), grp, r0);
+        if (grp == 0) bulk_load(XN, B1 + (long)N * plane + tile * kC, kC * sizeof(double2), &full[0]);
+    };
+    auto prefetch = [&](long tile) {
+#pragma unroll
+        for (int r0 = 0; r0 < M; r0 += X_::BOXR) tma_prefetch_3d(&tmB1, (int)(tile * kC * 2), grp, r0);
+    };
+    long tile = blockIdx.x;
+    if (gt == 0 && tile < ntiles) issue(tile);
+    uint32_t parity = 0;
+    double2* Ec = Xg + c;
+    double2* Cmine = C + grp * (M / 2 * kC) + c;
+    double2* Ctheirs = C + (grp ^ 1) * (M / 2 * kC) + c;
+    for (; tile < ntiles; tile += gridDim.x) {
+        const bool more = tile + gridDim.x < ntiles;
+        if (gt == 0 && more) prefetch(tile + gridDim.x);
+        double zr[R], zi[R];
+        mbar_wait(&full[grp], parity);
+        parity ^= 1;
+        UntangleFwd<M>::run([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            const int j = t + T * i;
+            const double2 a = Ec[j * kC];
+            double2 bq;
+            if (grp) bq = Ec[(M - 1 - j) * kC];
+            else bq = (j == 0) ? XN[c] : Ec[(M - j) * kC];
+            const double br = bq.x, bi = -bq.y;
+            const double sr = a.x + br, si = a.y + bi;
+            double dr = a.x - br, di = a.y - bi;
+            cmul_conj(dr, di, lam_k);
+            cmul_w32c<i>(dr, di);
+            zr[i] = sr - di; zi[i] = si + dr;     // Z = (A + B) + i d
+        });
+        fft2_forward_tile<Cfg, kC>(zi, zr, t, Ec, 1 + grp, cc, tn);   // inverse: roles of re and im swapped
+        bar_sync(1 + grp, GT);   // exchange read back: X_g is free
+        if (gt == 0 && more) { fence_proxy_async(); issue(tile + gridDim.x); }
+        if (grp) {   // y_o[n] conj(w_N^n), n = t + T i
+            UntangleFwd<M>::run([&](auto ic) {
+                constexpr int i = decltype(ic)::value;
+                cmul_conj(zr[i], zi[i], lam_n);
+                cmul_w32c<i>(zr[i], zi[i]);
+            });
+        }
+        __syncthreads();         // C of the previous tile has been consumed
+#pragma unroll
+        for (int i = 0; i < H; ++i) {
+            Cmine[(t + T * i) * kC] = make_double2(grp ? zr[i] : zr[i + H], grp ? zi[i] : zi[i + H]);
+        }
+        __syncthreads();
+        double* out = phi + tile * kC + c;
+#pragma unroll
+        for (int i = 0; i < H; ++i) {
+            const double2 pv = Ctheirs[(t + T * i) * kC];
+            const int o = grp ? i + H : i;
+            const long n = t + T * o;
+            out[(2 * n) * plane] = (grp ? zr[i + H] : zr[i]) + pv.x;
+            out[(2 * n + 1) * plane] = (grp ? zi[i + H] : zi[i]) + pv.y;
+        }
+    }
+}
+
 // ================================================================================== K1: fwd_x_r2c
 // M = Nx/2.  Tile = (y, z-bundle of kW columns); rows are x.  LTAB = 2Nx = 4M.
 template <int M>
