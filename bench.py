@@ -345,13 +345,17 @@ def run_b200(args):
 def _ncu_traffic(kernel: str, wname: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
     committed `ncu --set full` summary under profiles/ (null until one exists for this workload)."""
-    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
     if not os.path.exists(path):
         return None
     try:
-        return json.load(open(path)).get(wname, {}).get(kernel)
+        for line in open(path):
+            f = line.strip().split(",")
+            if len(f) >= 3 and f[0] == wname and f[1] == kernel:
+                return float(f[2])
     except Exception:
         return None
+    return None
 
 
 def extras(args, peak):
