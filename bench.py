@@ -173,6 +173,37 @@ def run_reference(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------------
+# multi-GPU plumbing ("replicas only": no data-path collective; only the timing is reduced)
+# ------------------------------------------------------------------------------------------------
+def init_replicas(backend: str, device=None):
+    """Joins the torchrun rendezvous (RANK / WORLD_SIZE / MASTER_* from the environment) when
+    WORLD_SIZE > 1.  Returns (dist module or None, rank, world)."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    if world == 1:
+        return None, rank, world
+    import torch.distributed as dist
+    kw = {"device_id": device} if device is not None else {}
+    dist.init_process_group(backend, **kw)
+    return dist, rank, world
+
+
+def max_over_ranks(dist, value: float, device="cpu") -> float:
+    """The slowest rank's time: what every multi-GPU number is computed from."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replicas_value(world: int, ms_per_step_max: float) -> float:
+    """solves/s of the whole job: every rank completes one solve per step, in the slowest rank's time."""
+    return world * 1e3 / ms_per_step_max
+
+
 def workload_points(wname: str) -> int:
     return {"512": 512 ** 3, "256": 256 ** 3, "beam": 128 * 128 * 512, "64": 64 ** 3}[wname]
 
@@ -241,16 +272,11 @@ def run_b200(args):
     import torch
     from paper_2405_02603_b200 import binding, workloads as W
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
     torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dist, rank, world = init_replicas("nccl", torch.device("cuda", local))
     barrier = (lambda: dist.barrier()) if dist else None
 
     cfg_idx, builder, kw, wdesc = WORKLOADS[args.workload]
@@ -269,11 +295,8 @@ def run_b200(args):
 
     sampler = ClockSampler(local) if rank == 0 else None
     ms, clocks = time_solves(plan, rho, phi, args.steps, args.warmup, sampler, barrier)
-    if dist:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * 1e3 / ms
+    ms = max_over_ranks(dist, ms, "cuda")
+    value = replicas_value(world, ms)
 
     # per-kernel roofline (events on the launching stream, inside libfsp)
     model_total, model_k = plan.model_bytes()
@@ -305,10 +328,7 @@ def run_b200(args):
         plan.solve_host(rho_h, phi_h)       # synchronises the stream before returning
     torch.cuda.synchronize()
     t_e2e = (time.perf_counter() - t0) / ne
-    if dist:
-        t = torch.tensor([t_e2e], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        t_e2e = float(t.item())
+    t_e2e = max_over_ranks(dist, t_e2e, "cuda")
     e2e_ok = bool(torch.equal(phi_h.cuda(), phi))
     e2e = {"value": world / t_e2e, "unit": "solves/s", "h2d_bytes_per_step": 8 * V, "d2h_bytes_per_step": 8 * V,
            "ms_per_step": t_e2e * 1e3, "matches_device_solve": e2e_ok, "host_memory": "pinned"}
