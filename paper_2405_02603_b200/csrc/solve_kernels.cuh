@@ -463,21 +463,21 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
             cc[m][i] = lane_g[(t + T * m) * 2 * NC + i];
             tn[m][i] = lane_g[(t + T * m) * 2 * NC + NC + i];
         }
-    const long nwarps = (long)gridDim.x * WARPS;
+    const int nwarps = gridDim.x * WARPS;
     const int ny2 = 2 * Ny;
-    for (long grp = (long)blockIdx.x * WARPS + warp; grp < ngroups; grp += nwarps) {
-        const long s = grp * G + g;                       // position in the visiting order
-        const long kx = s / ny2;
-        const int r = (int)(s - kx * ny2);
+    for (int grp = blockIdx.x * WARPS + warp; grp < (int)ngroups; grp += nwarps) {
+        const int s = grp * G + g;                        // position in the visiting order
+        const int kx = s / ny2;
+        const int r = s - kx * ny2;
         const int ky = (r & 1) ? ny2 - ((r + 1) >> 1) : (r >> 1);
         const int qy = ky <= Ny ? ky : ny2 - ky;
-        double2* base = B2 + (kx * ny2 + ky) * M;
-        const double* grow = Gk + (kx * (Ny + 1) + qy) * Z::ROW + (b ? M / 2 + 1 : 0);
+        double2* base = B2 + ((long)kx * ny2 + ky) * M;
+        const double* grow = Gk + ((long)kx * (Ny + 1) + qy) * Z::ROW + (b ? M / 2 + 1 : 0);
         if constexpr (Z::GSTAGE) {
             // all lanes are past the previous pencil's reads of gst (the shuffles of the final combine)
             if (lane == 0) {
                 mbar_arrive_expect_tx(gbar, Z::ROW * 8);
-                bulk_load(gst, Gk + (kx * (Ny + 1) + qy) * Z::ROW, Z::ROW * 8, gbar);
+                bulk_load(gst, Gk + ((long)kx * (Ny + 1) + qy) * Z::ROW, Z::ROW * 8, gbar);
             }
         }
 
@@ -488,12 +488,12 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
             vr[i] = v.x; vi[i] = v.y;
         }
         {   // L2 prefetch of the next group's pencil(s): 16-byte elements, one 128-byte line per 8
-            const long s2 = s + nwarps * G;
-            if (s2 < ngroups * G) {
-                const long kx2 = s2 / ny2;
-                const int r2 = (int)(s2 - kx2 * ny2);
+            const int s2 = s + nwarps * G;
+            if (s2 < (int)ngroups * G) {
+                const int kx2 = s2 / ny2;
+                const int r2 = s2 - kx2 * ny2;
                 const int ky2 = (r2 & 1) ? ny2 - ((r2 + 1) >> 1) : (r2 >> 1);
-                const double2* nb = B2 + (kx2 * ny2 + ky2) * M;
+                const double2* nb = B2 + ((long)kx2 * ny2 + ky2) * M;
                 for (int e = (b * T + t) * 8; e < M; e += 2 * T * 8)
                     asm volatile("prefetch.global.L2 [%0];" ::"l"(nb + e));
             }
