@@ -35,7 +35,7 @@ ALGS = {"HE": 0, "VG": 1, "VG2": 2}
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", default="512", choices=sorted(WORKLOADS))
@@ -64,10 +64,14 @@ class ClockSampler:
         self.index, self.proc = index, None
 
     def start(self):
+        """Starts nvidia-smi and waits for its first sample, so that its start-up (driver queries that
+        can hold up kernel launches for milliseconds) is over before the timed region begins; every later
+        sample falls inside the timed region."""
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                 "-lms", "50"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                 "-lms", "25"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.first = self.proc.stdout.readline()
         except OSError:
             self.proc = None
 
@@ -82,7 +86,8 @@ class ClockSampler:
             out, _ = self.proc.communicate()
         sm, smax, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for line in out.strip().splitlines():
+        lines = out.strip().splitlines() or [getattr(self, "first", "")]   # the pre-region sample only if no other
+        for line in lines:
             f = [x.strip() for x in line.split(",")]
             if len(f) < 7:
                 continue

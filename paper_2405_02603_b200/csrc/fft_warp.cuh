@@ -99,26 +99,38 @@ template <int R2> struct LaneTw { static constexpr int NC = R2 >= 4 ? R2 / 2 : 1
 template <int r, int S>
 __device__ __forceinline__ void dft_lane(double* re, double* im, const double* __restrict__ cc,
                                          const double* __restrict__ tn) {
-    // in place: input x_i at re[S*brev_r(i)] (the caller loads it there), output Y_k at re[S*k]
+    // in place: input x_i at re[S*brev_r(i)] (the caller loads it there), output Y_k at re[S*k].
+    // Butterflies are emitted in batches of BT: first the 2*BT twiddle products, then the 4*BT sums, so
+    // that no FMA directly follows the one it depends on (one warp alone must keep the fp64 pipe fed).
+    constexpr int BT = (r / 2 < 4) ? r / 2 : 4;
 #pragma unroll
     for (int len = 2; len <= r; len *= 2) {
         const int half = len / 2;
         const int OFS = len >= 4 ? len / 4 : 0, Q = len >= 4 ? len / 4 : 1;
 #pragma unroll
-        for (int blk = 0; blk < r; blk += len) {
+        for (int b0 = 0; b0 < r / 2; b0 += BT) {
+            double ur[BT], ui[BT];
 #pragma unroll
-            for (int k = 0; k < half; ++k) {
-                const int p = S * (blk + k), q = S * (blk + k + half);
-                const double c = cc[OFS + (k % Q)], tg = tn[OFS + (k % Q)];
-                const double ar = re[p], ai = im[p], br = re[q], bi = im[q];
+            for (int j = 0; j < BT; ++j) {
+                const int bb = b0 + j, k = bb % half, blk = (bb / half) * len;
+                const int q = S * (blk + k + half);
+                const double tg = tn[OFS + (k % Q)];
                 // b (c - i s) = c [(br + bi tg) + i (bi - br tg)],  tg = s / c
-                const double ur = fma(bi, tg, br), ui = fma(-br, tg, bi);
+                ur[j] = fma(im[q], tg, re[q]);
+                ui[j] = fma(-re[q], tg, im[q]);
+            }
+#pragma unroll
+            for (int j = 0; j < BT; ++j) {
+                const int bb = b0 + j, k = bb % half, blk = (bb / half) * len;
+                const int p = S * (blk + k), q = S * (blk + k + half);
+                const double c = cc[OFS + (k % Q)];
+                const double ar = re[p], ai = im[p];
                 if (((k / Q) & 1) == 0) {
-                    re[q] = fma(-c, ur, ar); im[q] = fma(-c, ui, ai);
-                    re[p] = fma(c, ur, ar); im[p] = fma(c, ui, ai);
+                    re[q] = fma(-c, ur[j], ar); im[q] = fma(-c, ui[j], ai);
+                    re[p] = fma(c, ur[j], ar); im[p] = fma(c, ui[j], ai);
                 } else {  // twiddle times -i:  c (ui - i ur)
-                    re[q] = fma(-c, ui, ar); im[q] = fma(c, ur, ai);
-                    re[p] = fma(c, ui, ar); im[p] = fma(-c, ur, ai);
+                    re[q] = fma(-c, ui[j], ar); im[q] = fma(c, ur[j], ai);
+                    re[p] = fma(c, ui[j], ar); im[p] = fma(-c, ur[j], ai);
                 }
             }
         }
