@@ -149,11 +149,11 @@ __device__ __forceinline__ void fft2_forward_lc(double (&re)[Cfg::R], double (&i
                                                 const double (&cc)[Cfg::NB2][LaneTw<Cfg::R2>::NC],
                                                 const double (&tn)[Cfg::NB2][LaneTw<Cfg::R2>::NC]) {
     constexpr int R = Cfg::R, R1 = Cfg::R1, R2 = Cfg::R2, T = Cfg::T, NB1 = Cfg::NB1, NB2 = Cfg::NB2;
-#pragma unroll
-    for (int m = 0; m < NB1; ++m) dft_br<R1, NB1>(&re[m], &im[m]);
-    __syncwarp();  // earlier readers of buf are done
+    __syncwarp();  // earlier readers of buf are done (placed first so that the stores of one stage-1
+                   // butterfly can drain while the next one is computed)
 #pragma unroll
     for (int m = 0; m < NB1; ++m) {
+        dft_br<R1, NB1>(&re[m], &im[m]);
         double2* dst = buf + (t + T * m) * (R1 + 1);
 #pragma unroll
         for (int i = 0; i < R1; ++i)   // output i of butterfly m sits in register m + NB1*brev(i)

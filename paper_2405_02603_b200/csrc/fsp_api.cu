@@ -342,14 +342,16 @@ int do_fwd_x(fsp_plan* p, const double* rho) {
             p->tmRho_ptr = rho;
         }
         if (p->Nx == 512) return launch_fwd_x_t<256>(p);
-        return launch_fwd_x_t<128>(p);
+        if (p->Nx == 256) return launch_fwd_x_t<128>(p);
+        return launch_fwd_x_t<64>(p);
     }
     DISPATCH_X(launch_fwd_x, p->Nx / 2, p, rho)
 }
 int do_fwd_y(fsp_plan* p, int kx0, double2* B2, int np) {
     if (p->tile_y) {
         if (p->Ny == 512) return launch_fwd_y_t<512>(p, kx0, B2, np);
-        return launch_fwd_y_t<256>(p, kx0, B2, np);
+        if (p->Ny == 256) return launch_fwd_y_t<256>(p, kx0, B2, np);
+        return launch_fwd_y_t<128>(p, kx0, B2, np);
     }
     const double2* B1 = p->B1 + (size_t)kx0 * p->Ny * p->Nz;
     DISPATCH_YZ(launch_fwd_y, p->Ny, p, B1, B2, np)
@@ -395,7 +397,8 @@ int launch_inv_y_t(fsp_plan* p, double2* B1, int nplanes) {
 int do_inv_y(fsp_plan* p, const double2* B2, double2* B1, int np) {
     if (p->tile_y && B2 == p->B2) {
         if (p->Ny == 512) return launch_inv_y_t<512>(p, B1, np);
-        return launch_inv_y_t<256>(p, B1, np);
+        if (p->Ny == 256) return launch_inv_y_t<256>(p, B1, np);
+        return launch_inv_y_t<128>(p, B1, np);
     }
     DISPATCH_YZ(launch_inv_y, p->Ny, p, B2, B1, np)
 }
@@ -418,7 +421,8 @@ int launch_inv_x_t(fsp_plan* p, double* phi) {
 int do_inv_x(fsp_plan* p, double* phi) {
     if (p->tile_x) {
         if (p->Nx == 512) return launch_inv_x_t<256>(p, phi);
-        return launch_inv_x_t<128>(p, phi);
+        if (p->Nx == 256) return launch_inv_x_t<128>(p, phi);
+        return launch_inv_x_t<64>(p, phi);
     }
     DISPATCH_X(launch_inv_x, p->Nx / 2, p, phi)
 }
@@ -609,7 +613,7 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
     if (rc == FSP_OK && !p->z_warp) rc = dev_alloc(&p->Gh, ng, &p->bytes);
     if (rc == FSP_OK && p->z_warp) rc = dev_alloc(&p->Gk, (size_t)(Nx + 1) * (Ny + 1) * (Nz + 2), &p->bytes);
     if (rc == FSP_OK && p->z_warp) rc = make_z_lane_table(p);
-    p->tile_x = (Nx == 256 || Nx == 512) && ((long)Ny * Nz) % kC == 0;
+    p->tile_x = (Nx == 128 || Nx == 256 || Nx == 512) && ((long)Ny * Nz) % kC == 0;
     if (rc == FSP_OK && p->tile_x) rc = make_x_lane_table(p);
     if (rc == FSP_OK && p->tile_x) {
         const cuuint64_t plane = (cuuint64_t)Ny * Nz;
@@ -618,7 +622,7 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
         const cuuint32_t box[3] = {2 * kC, 1, (cuuint32_t)(Nx / 2 < 256 ? Nx / 2 : 256)};
         rc = make_tensor_map(&p->tmB1x, p->B1, 3, dims, strides, box);
     }
-    p->tile_y = (Ny == 256 || Ny == 512) && Nz >= kW;
+    p->tile_y = (Ny == 128 || Ny == 256 || Ny == 512) && Nz >= kW;
     if (rc == FSP_OK && p->tile_y) rc = make_y_lane_table(p);
     if (rc == FSP_OK && p->tile_y) {
         const cuuint64_t dims[3] = {(cuuint64_t)2 * Nz, (cuuint64_t)Ny, (cuuint64_t)(Nx + 1)};

@@ -123,7 +123,7 @@ struct TileY {
     static constexpr int GT = kW * T;             // threads per group
     static constexpr int THREADS = 2 * GT;
     static constexpr int NC = LaneTw<Cfg::R2>::NC;
-    static constexpr int MINB = (M >= 512) ? 1 : 2;
+    static constexpr int MINB = (M >= 512) ? 1 : (M >= 256 ? 2 : 4);
     static constexpr int BOXR = M < 256 ? M : 256;   // rows per TMA box (box dimensions are limited to 256)
     // [mbarriers: 128 B][X: M*kW][E: 2 groups x M*kW][wp: M]
     static constexpr size_t smem_bytes() { return 128 + sizeof(double2) * (size_t)(3 * M * kW + M); }
@@ -256,7 +256,7 @@ struct TileYI {
     static constexpr int T = Cfg::T, R = Cfg::R;
     static constexpr int GT = kW * T, THREADS = 2 * GT;
     static constexpr int NC = LaneTw<Cfg::R2>::NC;
-    static constexpr int MINB = (M >= 512) ? 1 : 2;
+    static constexpr int MINB = (M >= 512) ? 1 : (M >= 256 ? 2 : 4);
     static constexpr int BOXR = M < 256 ? M : 256;
     // [mbarriers: 128 B][X: 2 groups x M*kW][C: 2 groups x (M/2)*kW][wp: M]
     static constexpr size_t smem_bytes() { return 128 + sizeof(double2) * (size_t)(3 * M * kW + M); }
@@ -549,13 +549,14 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
 // Z[2j+1] (input times w_N^n); the untangling partner Z[N-k] has the parity of k, so it is found inside
 // the group: the group's exchange buffer is reused to look it up.  The twiddles w_2N^k and w_N^n factor
 // into a per-lane constant times a compile-time 32nd root of unity (k = (2t+g) + 2T i, n = t + T i,
-// N/T = 32), so no twiddle table is read.
+// N/T = 32 or 16), so no twiddle table is read.
 constexpr int kC = 16;
 template <int M>
 struct TileX {
     using Cfg = Fft2Cfg<M>;
     static constexpr int T = Cfg::T, R = Cfg::R;
-    static_assert(2 * M / T == 32, "tile x kernels assume N/T = 32");
+    static_assert(32 % (2 * M / T) == 0, "tile x kernels need N/T to divide 32");
+    static constexpr int WS = 32 / (2 * M / T);   // w_(N/T)^i = w_32^(WS i)
     static constexpr int GT = kC * T, THREADS = 2 * GT;
     static constexpr int NC = LaneTw<Cfg::R2>::NC;
     static constexpr int MINB = (M >= 256) ? 1 : 2;
@@ -639,7 +640,7 @@ k_fwd_x_t(const __grid_constant__ CUtensorMap tmRho, double2* __restrict__ B1, c
             UntangleFwd<M>::run([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
                 cmul(vr[i], vi[i], lam_n);
-                cmul_w32<i>(vr[i], vi[i]);
+                cmul_w32<i * X_::WS>(vr[i], vi[i]);
             });
         }
         fft2_forward_tile<Cfg, kC>(vr, vi, t, Ec, 1 + grp, cc, tn);
@@ -658,7 +659,7 @@ k_fwd_x_t(const __grid_constant__ CUtensorMap tmRho, double2* __restrict__ B1, c
             const double sr = ar + br, si = ai + bi;
             double dr = ar - br, di = ai - bi;
             cmul(dr, di, lam_k);
-            cmul_w32<i>(dr, di);
+            cmul_w32<i * X_::WS>(dr, di);
             const long k = 2 * j + grp;
             out[k * plane] = make_double2(sr + di, si - dr);
             if (i == 0 && grp == 0 && t == 0) out[(long)N * plane] = make_double2(2.0 * (ar - ai), 0.0);
@@ -690,7 +691,8 @@ template <int M>
 struct TileXI {
     using Cfg = Fft2Cfg<M>;
     static constexpr int T = Cfg::T, R = Cfg::R;
-    static_assert(2 * M / T == 32, "tile x kernels assume N/T = 32");
+    static_assert(32 % (2 * M / T) == 0, "tile x kernels need N/T to divide 32");
+    static constexpr int WS = 32 / (2 * M / T);   // w_(N/T)^i = w_32^(WS i)
     static constexpr int GT = kC * T, THREADS = 2 * GT;
     static constexpr int NC = LaneTw<Cfg::R2>::NC;
     static constexpr int MINB = (M >= 256) ? 1 : 2;
@@ -760,7 +762,7 @@ k_inv_x_t(const __grid_constant__ CUtensorMap tmB1, const double2* __restrict__ 
             const double sr = a.x + br, si = a.y + bi;
             double dr = a.x - br, di = a.y - bi;
             cmul_conj(dr, di, lam_k);
-            cmul_w32c<i>(dr, di);
+            cmul_w32c<i * X_::WS>(dr, di);
             zr[i] = sr - di; zi[i] = si + dr;     // Z = (A + B) + i d
         });
         fft2_forward_tile<Cfg, kC>(zi, zr, t, Ec, 1 + grp, cc, tn);   // inverse: roles of re and im swapped
@@ -770,7 +772,7 @@ k_inv_x_t(const __grid_constant__ CUtensorMap tmB1, const double2* __restrict__ 
             UntangleFwd<M>::run([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
                 cmul_conj(zr[i], zi[i], lam_n);
-                cmul_w32c<i>(zr[i], zi[i]);
+                cmul_w32c<i * X_::WS>(zr[i], zi[i]);
             });
         }
         __syncthreads();         // C of the previous tile has been consumed

@@ -68,6 +68,11 @@ __device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t b
 }
 
 // named barrier among nthreads threads (a multiple of 32) of the CTA; id 1..15 (0 is __syncthreads)
-__device__ __forceinline__ void bar_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+// (the id is an immediate for ids 1 and 2, the two groups of a tile kernel, so that ptxas counts the
+// barriers actually used instead of reserving all 16)
+__device__ __forceinline__ void bar_sync(int id, int nthreads) {
+    if (id == 1) asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
+    else asm volatile("bar.sync 2, %0;" ::"r"(nthreads) : "memory");
+}
 
 }  // namespace fsp
