@@ -11,6 +11,7 @@ from .oracle import (  # noqa: F401
     HOCKNEY,
     VICO,
     VICO_2,
+    VICO_SAFE,
     G0_DEFAULT,
     ALPHA_DEFAULT,
     OraclePlan,
@@ -21,6 +22,8 @@ from .oracle import (  # noqa: F401
     fft3d,
     green_spectrum,
     green_table,
+    green_table_vgm,
+    vg_safe_factors,
     num_threads,
     set_num_threads,
     solve_with_spectrum,

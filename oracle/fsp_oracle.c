@@ -18,6 +18,7 @@
  *   orc_green_table_he   PAPER.md:35,72-76  G = 1/(4 pi |x|), regularised at the origin (R5).
  *   orc_green_table_vg   PAPER.md:88-98     Eq. 3 on the 4N grid, inverse DFT, restricted.
  *   orc_green_table_vg2  PAPER.md:100-102,205  same values on the (2N+1)^3 grid, DCT-I.
+ *   orc_green_table_vgm / orc_vg_safe_factors   the same with per-axis oversampling m_d (8(f) N2, R17).
  *   orc_green_g2 /       PAPER.md:72-74  the 8-case mirror G2 on the doubled grid, and its DFT.
  *   orc_green_spectrum
  *   orc_solve            PAPER.md:67-82  steps 1-5: double, zero-pad, FFT, multiply, inverse FFT,
@@ -322,12 +323,19 @@ int orc_dct1(long n, long nout, const double* in, double* out, int method) {
  * DFT above becomes, axis by axis, the DCT-I of size 2N_d+1:
  *     T[d] = 1/prod_d(4 N_d h_d) * sum_k w_kx w_ky w_kz G_L(s_k) prod_d cos(pi k_d d_d/(2 N_d)),
  * kept for 0 <= d_d <= N_d.  Memory: (2Nx+1)(2Ny+1)(2Nz+1) reals (shrinking after each axis). */
-int orc_green_table_vg2(long Nx, long Ny, long Nz, const double h[3], double alpha, int method,
-                        double* T) {
-    if (Nx < 1 || Ny < 1 || Nz < 1 || !h || !T || !(h[0] > 0) || !(h[1] > 0) || !(h[2] > 0) ||
+/* General form with per-axis oversampling factors m[d] (even, >= 2): the frequency lattice is
+ * s_d = 2 pi k_d / (m_d N_d h_d), k_d in [0, m_d N_d / 2], and
+ *     T[d] = 1/prod_d(m_d N_d h_d) * sum_k w_kx w_ky w_kz G_L(s_k) prod_d cos(2 pi k_d d_d/(m_d N_d)),
+ * i.e. the DCT-I of size m_d N_d / 2 + 1 per axis.  m = (4,4,4) is the paper's choice. */
+int orc_green_table_vgm(long Nx, long Ny, long Nz, const double h[3], double alpha, int method,
+                        const long m[3], double* T) {
+    if (Nx < 1 || Ny < 1 || Nz < 1 || !h || !T || !m || !(h[0] > 0) || !(h[1] > 0) || !(h[2] > 0) ||
         !(alpha > 0))
         return ORC_EINVAL;
-    long Kx = 2 * Nx + 1, Ky = 2 * Ny + 1, Kz = 2 * Nz + 1;
+    for (int d = 0; d < 3; ++d)
+        if (m[d] < 2 || (m[d] & 1)) return ORC_EINVAL;
+    long nx = m[0] * Nx / 2, ny = m[1] * Ny / 2, nz = m[2] * Nz / 2; /* DCT-I sizes are n+1 */
+    long Kx = nx + 1, Ky = ny + 1, Kz = nz + 1;
     double L = orc_vg_window(Nx, Ny, Nz, h, alpha);
     double* f = (double*)malloc(sizeof(double) * (size_t)Kx * Ky * Kz);
     double* a = (double*)malloc(sizeof(double) * (size_t)Kx * Ky * (Nz + 1));
@@ -340,42 +348,61 @@ int orc_green_table_vg2(long Nx, long Ny, long Nz, const double h[3], double alp
     }
 #pragma omp parallel for schedule(static)
     for (long kx = 0; kx < Kx; ++kx) {
-        double sx = 2.0 * ORC_PI * kx / (4 * Nx * h[0]);
+        double sx = 2.0 * ORC_PI * kx / (m[0] * Nx * h[0]);
         for (long ky = 0; ky < Ky; ++ky) {
-            double sy = 2.0 * ORC_PI * ky / (4 * Ny * h[1]);
+            double sy = 2.0 * ORC_PI * ky / (m[1] * Ny * h[1]);
             for (long kz = 0; kz < Kz; ++kz) {
-                double sz = 2.0 * ORC_PI * kz / (4 * Nz * h[2]);
+                double sz = 2.0 * ORC_PI * kz / (m[2] * Nz * h[2]);
                 f[((size_t)kx * Ky + ky) * Kz + kz] = vg_GL(sx, sy, sz, L);
             }
         }
     }
-    long nmax = 2 * (Nx > Ny ? (Nx > Nz ? Nx : Nz) : (Ny > Nz ? Ny : Nz));
-    /* axis z: f[kx][ky][kz] -> a[kx][ky][dz] */
+    long nmax = nx > ny ? (nx > nz ? nx : nz) : (ny > nz ? ny : nz);
 #pragma omp parallel
     {
         double* work = (double*)malloc(sizeof(double) * 8 * (size_t)(nmax + 1));
+        /* axis z: f[kx][ky][kz] -> a[kx][ky][dz] */
 #pragma omp for schedule(static)
         for (long p = 0; p < Kx * Ky; ++p)
-            dct1_axis(2 * Nz, Nz + 1, f + (size_t)p * Kz, 1, a + (size_t)p * (Nz + 1), 1, method,
-                      work);
+            dct1_axis(nz, Nz + 1, f + (size_t)p * Kz, 1, a + (size_t)p * (Nz + 1), 1, method, work);
         /* axis y: a[kx][ky][dz] -> b[kx][dy][dz] */
 #pragma omp for collapse(2) schedule(static)
         for (long kx = 0; kx < Kx; ++kx)
             for (long dz = 0; dz <= Nz; ++dz)
-                dct1_axis(2 * Ny, Ny + 1, a + (size_t)kx * Ky * (Nz + 1) + dz, Nz + 1,
+                dct1_axis(ny, Ny + 1, a + (size_t)kx * Ky * (Nz + 1) + dz, Nz + 1,
                           b + (size_t)kx * (Ny + 1) * (Nz + 1) + dz, Nz + 1, method, work);
         /* axis x: b[kx][dy][dz] -> T[dx][dy][dz] */
 #pragma omp for schedule(static)
         for (long q = 0; q < (Ny + 1) * (Nz + 1); ++q)
-            dct1_axis(2 * Nx, Nx + 1, b + q, (Ny + 1) * (Nz + 1), T + q, (Ny + 1) * (Nz + 1),
-                      method, work);
+            dct1_axis(nx, Nx + 1, b + q, (Ny + 1) * (Nz + 1), T + q, (Ny + 1) * (Nz + 1), method, work);
         free(work);
     }
-    double scale = 1.0 / ((4.0 * Nx * h[0]) * (4.0 * Ny * h[1]) * (4.0 * Nz * h[2]));
+    double scale = 1.0 / (((double)m[0] * Nx * h[0]) * ((double)m[1] * Ny * h[1]) * ((double)m[2] * Nz * h[2]));
     for (long i = 0; i < (Nx + 1) * (Ny + 1) * (Nz + 1); ++i) T[i] *= scale;
     free(f);
     free(a);
     free(b);
+    return ORC_OK;
+}
+
+int orc_green_table_vg2(long Nx, long Ny, long Nz, const double h[3], double alpha, int method,
+                        double* T) {
+    const long m[3] = {4, 4, 4};
+    return orc_green_table_vgm(Nx, Ny, Nz, h, alpha, method, m, T);
+}
+
+/* Anisotropy-safe oversampling (reading R17; SURVEY 8(c) pt 12, 8(f) N2): the kernel
+ * truncated at radius L = alpha * diagonal is periodised with period m_d L_d along axis d, and
+ * displacements up to L_d are used, so no image overlaps iff m_d L_d >= L + L_d.  The factors are
+ * kept powers of two and never below the paper's 4:  m_d = 4, doubled while m_d < 1 + L / L_d. */
+int orc_vg_safe_factors(long Nx, long Ny, long Nz, const double h[3], double alpha, long m[3]) {
+    if (Nx < 1 || Ny < 1 || Nz < 1 || !h || !m || !(alpha > 0)) return ORC_EINVAL;
+    double L = orc_vg_window(Nx, Ny, Nz, h, alpha);
+    const long N[3] = {Nx, Ny, Nz};
+    for (int d = 0; d < 3; ++d) {
+        m[d] = 4;
+        while ((double)m[d] < 1.0 + L / (N[d] * h[d])) m[d] *= 2;
+    }
     return ORC_OK;
 }
 

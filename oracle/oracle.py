@@ -14,6 +14,7 @@ import threading
 import numpy as np
 
 HOCKNEY, VICO, VICO_2 = 0, 1, 2  # PAPER.md:199 solver names HOCKNEY / VICO / VICO_2
+VICO_SAFE = 3  # VICO_2 with per-axis oversampling m_d >= 1 + L/L_d (R17)
 G0_DEFAULT = 1.0 / (4.0 * math.pi)  # DESIGN.md reading R5
 ALPHA_DEFAULT = 1.1
 
@@ -56,6 +57,8 @@ def _load():
         lib.orc_green_table_he.argtypes = [L, L, L, _dp, D, _dp]
         lib.orc_green_table_vg.argtypes = [L, L, L, _dp, D, I, _dp]
         lib.orc_green_table_vg2.argtypes = [L, L, L, _dp, D, I, _dp]
+        lib.orc_green_table_vgm.argtypes = [L, L, L, _dp, D, I, _lp, _dp]
+        lib.orc_vg_safe_factors.argtypes = [L, L, L, _dp, D, _lp]
         lib.orc_green_spectrum.argtypes = [L, L, L, _dp, I, _dp]
         lib.orc_solve.argtypes = [L, L, L, _dp, _dp, I, _dp, _dp]
         lib.orc_direct_sum.argtypes = [L, L, L, _dp, _dp, _dp, L, _lp, _dp]
@@ -120,9 +123,31 @@ def vg_window(N, h, alpha: float = ALPHA_DEFAULT) -> float:
     return float(_load().orc_vg_window(N[0], N[1], N[2], _d(h), alpha))
 
 
+def vg_safe_factors(N, h, alpha: float = ALPHA_DEFAULT):
+    """Per-axis oversampling factors of VICO_SAFE: 4, doubled while m_d < 1 + L/L_d (R17)."""
+    h = _h3(h)
+    m = np.zeros(3, dtype=np.int64)
+    _check(_load().orc_vg_safe_factors(int(N[0]), int(N[1]), int(N[2]), _d(h), alpha, m.ctypes.data_as(_lp)),
+           "vg_safe_factors")
+    return tuple(int(v) for v in m)
+
+
+def green_table_vgm(N, h, m, alpha: float = ALPHA_DEFAULT, method: int = 0) -> np.ndarray:
+    """VG table from the lattice with per-axis oversampling factors m (even); m = (4,4,4) is VICO_2."""
+    Nx, Ny, Nz = (int(v) for v in N)
+    h = _h3(h)
+    mm = np.asarray(m, dtype=np.int64)
+    T = np.empty((Nx + 1, Ny + 1, Nz + 1), dtype=np.float64)
+    _check(_load().orc_green_table_vgm(Nx, Ny, Nz, _d(h), alpha, method, mm.ctypes.data_as(_lp), _d(T)),
+           "green_table_vgm")
+    return T
+
+
 def green_table(algorithm: int, N, h, g0: float = G0_DEFAULT, alpha: float = ALPHA_DEFAULT,
                 method: int = 0) -> np.ndarray:
-    """Real-space kernel table T of shape (Nx+1, Ny+1, Nz+1) for HOCKNEY / VICO / VICO_2."""
+    """Real-space kernel table T of shape (Nx+1, Ny+1, Nz+1) for HOCKNEY / VICO / VICO_2 / VICO_SAFE."""
+    if algorithm == VICO_SAFE:
+        return green_table_vgm(N, h, vg_safe_factors(N, h, alpha), alpha, method)
     Nx, Ny, Nz = (int(v) for v in N)
     h = _h3(h)
     T = np.empty((Nx + 1, Ny + 1, Nz + 1), dtype=np.float64)

@@ -308,3 +308,82 @@ def test_beam_like_gaussian_he_against_1d_integral():
     assert err < 5e-3
     vg = oracle.OraclePlan(w.N, w.h, oracle.VICO_2).precompute_green().solve(w.rho)
     assert np.isfinite(vg).all()
+
+
+# ------------------------------------------------- VICO_SAFE: per-axis oversampling
+def _iso_gaussian_in_long_box(N, sigma=0.05):
+    """Isotropic normalised Gaussian at the centre of the box [-1/2,1/2]^2 x [-2,2] (h equal on all axes)."""
+    lo, hi = (-0.5, -0.5, -2.0), (0.5, 0.5, 2.0)
+    rho = W.gaussian_density(N, lo, hi, (0.0, 0.0, 0.0), (sigma,) * 3)
+    return W.Workload("iso_gaussian_long_box", tuple(N), lo, hi, np.ascontiguousarray(rho),
+                      [(1.0, (0.0, 0.0, 0.0), (sigma,) * 3)])
+
+
+def test_vg_safe_factors_rule():
+    """m_d = 4, doubled while m_d < 1 + L/L_d: the paper's 4 on a cube (1 + 1.1 sqrt 3 = 2.9), 8 on the short
+    axes of the 1 x 1 x 4 box (1 + 4.67 = 5.67) and 4 on its long axis (1 + 1.17)."""
+    assert oracle.vg_safe_factors((16, 16, 16), (1 / 16,) * 3) == (4, 4, 4)
+    assert oracle.vg_safe_factors((32, 32, 128), (1 / 32,) * 3) == (8, 8, 4)
+    assert oracle.vg_safe_factors((16, 64, 16), (1 / 16, 1 / 16, 1 / 16)) == (8, 4, 8)
+
+
+def test_vg_safe_equals_vico2_on_a_cube_and_for_m_444():
+    N, h = (12, 16, 8), (0.07, 0.05, 0.11)
+    a = oracle.green_table_vgm(N, h, (4, 4, 4))
+    b = oracle.green_table(oracle.VICO_2, N, h)
+    assert np.array_equal(a, b)
+    c = oracle.green_table(oracle.VICO_SAFE, (16, 16, 16), (1 / 16,) * 3)
+    d = oracle.green_table(oracle.VICO_2, (16, 16, 16), (1 / 16,) * 3)
+    assert np.array_equal(c, d)
+
+
+def test_vg_table_is_insensitive_to_more_oversampling_once_safe():
+    """Once m_d L_d >= L + L_d no image of the truncated kernel reaches the table: raising m further (also
+    to a non power of two, through the O(n^2) cosine sum) only changes the quadrature of the band edge
+    |s_d| = pi/h_d (1e-4 of max T here, invisible to a band-limited rho), whereas the paper's literal 4 on
+    the long box puts O(1) images into the table (5e-2 of max T; reading R12)."""
+    N, h = (8, 8, 32), (1 / 8,) * 3
+    safe = oracle.green_table_vgm(N, h, (8, 8, 4))
+    more = oracle.green_table_vgm(N, h, (12, 10, 6), method=1)
+    lit = oracle.green_table_vgm(N, h, (4, 4, 4))
+    assert np.abs(safe - more).max() <= 5e-4 * np.abs(safe).max()
+    assert np.abs(safe - lit).max() > 1e-2 * np.abs(safe).max()
+
+
+def test_vg_safe_far_field_along_the_long_axis():
+    """T[d] -> 1/(4 pi r) at every displacement of the long box (to the ripple of the band limit, a few
+    1e-3 away from the table's edges), where the literal recipe has O(1) images of the truncated kernel."""
+    N, h = (16, 16, 64), (1 / 16,) * 3
+    T = oracle.green_table(oracle.VICO_SAFE, N, h)
+    lit = oracle.green_table(oracle.VICO_2, N, h)
+    for d in [(0, 0, 64), (3, 5, 40), (16, 0, 10), (5, 3, 62), (7, 11, 64), (2, 1, 33)]:
+        r = math.sqrt(sum((d[i] * h[i]) ** 2 for i in range(3)))
+        assert T[d] == pytest.approx(1.0 / (4 * math.pi * r), rel=3e-3)
+    for d in [(3, 5, 40), (2, 1, 33), (16, 0, 10)]:
+        r = math.sqrt(sum((d[i] * h[i]) ** 2 for i in range(3)))
+        assert abs(lit[d] * 4 * math.pi * r - 1.0) > 0.5
+
+
+def test_vg_safe_is_spectrally_accurate_in_the_long_box():
+    """Closed-form Gaussian potential in the 1 x 1 x 4 box: the literal recipe is off by
+    O(1) (SURVEY 8(c) pt 12: 6.0e-1), VICO_SAFE is spectrally accurate like VG on a cube (1e-9 at h = 1/32)."""
+    w = _iso_gaussian_in_long_box((32, 32, 128))
+    ex = gaussian_potential_iso(w)
+    safe = oracle.OraclePlan(w.N, w.h, oracle.VICO_SAFE).precompute_green().solve(w.rho)
+    lit = oracle.OraclePlan(w.N, w.h, oracle.VICO_2).precompute_green().solve(w.rho)
+    assert rel_l2(safe, ex) < 1e-8
+    assert rel_l2(lit, ex) > 1e-1
+
+
+def test_vg_safe_beam_like_gaussian_against_1d_integral():
+    """BASELINE.json config 4 at reduced size: VICO_SAFE against the anisotropic closed form; the box cuts
+    the Gaussian at 4 sigma_z, which floors any solver near 1e-5..1e-4."""
+    w = W.config4((32, 32, 128))
+    xs = W.cell_centres(w.N, w.lo, w.hi)
+    rng = np.random.default_rng(0)
+    pts_idx = np.stack([rng.integers(0, n, 200) for n in w.N], axis=1)
+    pts = np.stack([xs[d][pts_idx[:, d]] for d in range(3)], axis=1)
+    ex = gaussian_potential_aniso_points(w.gaussians[0][2], pts)
+    vg = oracle.OraclePlan(w.N, w.h, oracle.VICO_SAFE).precompute_green().solve(w.rho)
+    got = vg[pts_idx[:, 0], pts_idx[:, 1], pts_idx[:, 2]]
+    assert np.linalg.norm(got - ex) / np.linalg.norm(ex) < 3e-4
