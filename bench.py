@@ -29,7 +29,7 @@ WORKLOADS = {
     "beam": (3, "config4", {}, "configs[3]: 128x128x512 fp64, beam-like Gaussian"),
     "64": (1, "config2", {}, "configs[1]: 64^3 fp64, 4 seeded Gaussians (L2-resident, launch-bound)"),
 }
-ALGS = {"HE": 0, "VG": 1, "VG2": 2}
+ALGS = {"HE": 0, "VG": 1, "VG2": 2, "VGS": 3}
 
 
 def parse_args():
@@ -124,7 +124,7 @@ def oracle_time_solves(wname: str, alg: str, steps: int, warmup: int, budget_s: 
     """Times the oracle's solve (PAPER.md:67-82 steps 1-5, un-pruned, radix-2 FFT) as it stands on the
     host cores.  Returns (seconds per solve of the sample, sample workload, threads, description)."""
     import oracle
-    oalg = {"HE": oracle.HOCKNEY, "VG": oracle.VICO, "VG2": oracle.VICO_2}[alg]
+    oalg = {"HE": oracle.HOCKNEY, "VG": oracle.VICO, "VG2": oracle.VICO_2, "VGS": oracle.VICO_SAFE}[alg]
     # calibrate on 32^3, then take the largest edge whose (steps+warmup) solves fit the budget
     w = _sample_workload(wname, 32)
     pl = oracle.OraclePlan(w.N, w.h, oracle.HOCKNEY).precompute_green()
@@ -390,7 +390,7 @@ def extras(args, peak):
     import torch
     from paper_2405_02603_b200 import binding, workloads as W
     out = {}
-    todo = [("256", "HE"), ("beam", "HE"), (args.workload, "VG2" if args.alg == "HE" else "HE")]
+    todo = [("256", "HE"), ("beam", "HE"), ("beam", "VGS"), (args.workload, "VG2" if args.alg == "HE" else "HE")]
     for wname, alg in todo:
         if (wname, alg) == (args.workload, args.alg):
             continue

@@ -11,6 +11,7 @@
  *     FSP_VICO    : truncated-kernel spectrum Eq. 3, inverse FFT on the 4N grid, restricted
  *
  *     FSP_VICO_2  : same values from the (2N+1)^3 grid with a DCT-I
+ *     FSP_VICO_SAFE : FSP_VICO_2 with per-axis oversampling, safe on elongated boxes (see the enum)
  * (names as PAPER.md:199: HOCKNEY / VICO / VICO_2).
  *
  * Everything behind these calls runs in hand-written sm_100a CUDA kernels: no FFT library, no CPU
@@ -41,7 +42,18 @@ extern "C" {
 typedef struct fsp_plan fsp_plan; /* opaque, library-owned */
 
 /* algorithm */
-enum { FSP_HOCKNEY = 0, FSP_VICO = 1, FSP_VICO_2 = 2 };
+enum {
+    FSP_HOCKNEY = 0,
+    FSP_VICO = 1,
+    FSP_VICO_2 = 2,
+    /* FSP_VICO_2 with per-axis oversampling factors m_d instead of the paper's 4: m_d = 4,
+     * doubled while m_d < 1 + L / L_d, L = alpha * box diagonal, L_d = N_d h_d.  The kernel
+     * truncated at radius L is periodised with period m_d L_d and used up to displacement L_d, so its
+     * images stay out of the table iff m_d L_d >= L + L_d; with m = 4 that fails on boxes longer than
+     * about 2.7 times their shortest side (the paper's beam-dynamics use case).  Identical to
+     * FSP_VICO_2 whenever the rule gives (4,4,4), e.g. on every cube.  DESIGN.md reading R17. */
+    FSP_VICO_SAFE = 3
+};
 
 /* error codes */
 enum {
@@ -119,6 +131,10 @@ size_t fsp_precompute_peak_bytes(const fsp_plan* p);
 /* Algorithmic (minimal-traffic) HBM bytes of one solve: total, and per kernel
  * if per_kernel (host pointer to FSP_NUM_SOLVE_KERNELS doubles) is not NULL. */
 double fsp_model_bytes_per_solve(const fsp_plan* p, double* per_kernel);
+
+/* Oversampling factors (m_x, m_y, m_z) used by the last fsp_precompute_green of a VG algorithm
+ * (4,4,4 for FSP_VICO and FSP_VICO_2); m_out: host pointer to 3 ints. */
+int fsp_get_vg_factors(const fsp_plan* p, int* m_out);
 
 /* Copies the real-space table T, (Nx+1)(Ny+1)(Nz+1) doubles in C order, to host memory. */
 int fsp_get_green_table(const fsp_plan* p, double* T_host);

@@ -14,7 +14,7 @@ import os
 
 import numpy as np
 
-HOCKNEY, VICO, VICO_2 = 0, 1, 2                       # include/fsp.h
+HOCKNEY, VICO, VICO_2, VICO_SAFE = 0, 1, 2, 3           # include/fsp.h, PAPER.md:199 (+ DESIGN.md R17)
 PARAM_G0, PARAM_ALPHA, PARAM_CHUNK_PLANES = 0, 1, 2
 NUM_SOLVE_KERNELS = 5
 ERRORS = {0: "FSP_OK", -1: "FSP_ERR_INVALID_ARG", -2: "FSP_ERR_NOT_PRECOMPUTED",
@@ -37,6 +37,7 @@ SIGNATURES = {
     "fsp_plan_bytes": (_sz, [_vp]),
     "fsp_precompute_peak_bytes": (_sz, [_vp]),
     "fsp_model_bytes_per_solve": (_d, [_vp, _dp]),
+    "fsp_get_vg_factors": (_i, [_vp, _c.POINTER(_i)]),
     "fsp_get_green_table": (_i, [_vp, _dp]),
     "fsp_get_green_spectrum": (_i, [_vp, _dp]),
     "fsp_set_profiling": (_i, [_vp, _i]),
@@ -138,6 +139,12 @@ def model_bytes_per_solve(plan: int):
     return tot, [float(v) for v in per]
 
 
+def get_vg_factors(plan: int):
+    m = (_i * 3)()
+    _chk(lib().fsp_get_vg_factors(plan, m), "fsp_get_vg_factors")
+    return tuple(int(v) for v in m)
+
+
 def get_green_table(plan: int, N) -> np.ndarray:
     T = np.empty(tuple(n + 1 for n in N), dtype=np.float64)
     _chk(lib().fsp_get_green_table(plan, T.ctypes.data_as(_dp)), "fsp_get_green_table")
@@ -197,6 +204,9 @@ class Plan:
         """Host buffers (numpy arrays or pinned torch CPU tensors), copies inside the call."""
         solve_host(self.handle, rho_host, phi_host)
         return phi_host
+
+    def vg_factors(self):
+        return get_vg_factors(self.handle)
 
     def green_table(self) -> np.ndarray:
         return get_green_table(self.handle, self.N)

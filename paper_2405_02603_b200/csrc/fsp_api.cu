@@ -26,6 +26,7 @@ struct fsp_plan {
     cudaStream_t stream = nullptr;
     int device = 0;
     double g0 = 0.0, alpha = 1.1;
+    int vg_m[3] = {4, 4, 4};  // oversampling factors used by the last VG precompute
     // plan-owned device memory
     double2* B1 = nullptr;  // (Nx+1) * Ny * Nz
     double2* B2 = nullptr;  // (Nx+1) * 2Ny * Nz
@@ -504,8 +505,21 @@ int precompute_impl(fsp_plan* p) {
             k_restrict_vg<<<grid_for(tcount, blk), blk, 0, p->stream>>>(g, p->T, Nx, Ny, Nz, scale);
             CU(cudaGetLastError());
         } else {
-            // (2N+1)^3 real grid, DCT-I per axis with output pruned to N_d + 1
-            const long fd[3] = {2L * Nx + 1, 2L * Ny + 1, 2L * Nz + 1};
+            // (m_d N_d / 2 + 1) real grid per axis, DCT-I per axis with output pruned to N_d + 1
+            // (PAPER.md:100-102 with m = 4; FSP_VICO_SAFE: m_d = 4, doubled while m_d < 1 + L / L_d, R17)
+            int m[3] = {4, 4, 4};
+            if (p->algorithm == FSP_VICO_SAFE) {
+                const double Ld[3] = {Lx, Ly, Lz};
+                for (int d = 0; d < 3; ++d)
+                    while ((double)m[d] < 1.0 + L / Ld[d]) m[d] *= 2;
+            }
+            p->vg_m[0] = m[0]; p->vg_m[1] = m[1]; p->vg_m[2] = m[2];
+            const int nx = m[0] * Nx / 2, ny = m[1] * Ny / 2, nz = m[2] * Nz / 2;   // DCT-I sizes are n + 1
+            // the DCT kernel holds two arrays of 2n complex values in shared memory
+            if (sizeof(double2) * 4 * (size_t)(nx > ny ? (nx > nz ? nx : nz) : (ny > nz ? ny : nz)) > 227 * 1024)
+                return FSP_ERR_INVALID_ARG;
+            const double vscale = 1.0 / (((double)m[0] * Nx * hx) * ((double)m[1] * Ny * hy) * ((double)m[2] * Nz * hz));
+            const long fd[3] = {nx + 1L, ny + 1L, nz + 1L};
             const long ad[3] = {fd[0], fd[1], Nz + 1};
             const long bd[3] = {fd[0], Ny + 1, Nz + 1};
             double *f = nullptr, *a = nullptr, *b = nullptr;
@@ -518,11 +532,11 @@ int precompute_impl(fsp_plan* p) {
             rc = dev_alloc(&b, (size_t)bd[0] * bd[1] * bd[2], &peak);
             if (rc != FSP_OK) return rc;
             tmp.ptrs.push_back(b);
-            k_fill_gl_vg2<<<grid_for(fd[0] * fd[1] * fd[2], blk), blk, 0, p->stream>>>(f, Nx, Ny, Nz, hx, hy, hz, L);
+            k_fill_gl_vg2<<<grid_for(fd[0] * fd[1] * fd[2], blk), blk, 0, p->stream>>>(f, Nx, Ny, Nz, hx, hy, hz, L, m[0], m[1], m[2]);
             CU(cudaGetLastError());
-            if ((rc = dct1_axis(p, f, a, fd, ad, 2, 2 * Nz, Nz + 1, 1.0)) != FSP_OK) return rc;
-            if ((rc = dct1_axis(p, a, b, ad, bd, 1, 2 * Ny, Ny + 1, 1.0)) != FSP_OK) return rc;
-            if ((rc = dct1_axis(p, b, p->T, bd, tdims, 0, 2 * Nx, Nx + 1, scale)) != FSP_OK) return rc;
+            if ((rc = dct1_axis(p, f, a, fd, ad, 2, nz, Nz + 1, 1.0)) != FSP_OK) return rc;
+            if ((rc = dct1_axis(p, a, b, ad, bd, 1, ny, Ny + 1, 1.0)) != FSP_OK) return rc;
+            if ((rc = dct1_axis(p, b, p->T, bd, tdims, 0, nx, Nx + 1, vscale)) != FSP_OK) return rc;
         }
     }
     // Ghat octant = 3-D DCT-I of T (size N_d + 1 per axis)
@@ -586,7 +600,7 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
     if (!h || !(h[0] > 0.0) || !(h[1] > 0.0) || !(h[2] > 0.0)) return FSP_ERR_INVALID_ARG;
     if (!std::isfinite(h[0]) || !std::isfinite(h[1]) || !std::isfinite(h[2])) return FSP_ERR_INVALID_ARG;
     if (!pow2_in(Nx, 8, 512) || !pow2_in(Ny, 8, 1024) || !pow2_in(Nz, 8, 1024)) return FSP_ERR_INVALID_ARG;
-    if (algorithm != FSP_HOCKNEY && algorithm != FSP_VICO && algorithm != FSP_VICO_2) return FSP_ERR_INVALID_ARG;
+    if (algorithm != FSP_HOCKNEY && algorithm != FSP_VICO && algorithm != FSP_VICO_2 && algorithm != FSP_VICO_SAFE) return FSP_ERR_INVALID_ARG;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
         (void)cudaGetLastError();
@@ -772,6 +786,13 @@ double fsp_model_bytes_per_solve(const fsp_plan* p, double* per_kernel) {
         if (per_kernel) per_kernel[i] = k[i];
     }
     return tot;
+}
+
+int fsp_get_vg_factors(const fsp_plan* p, int* m_out) {
+    if (!p || !m_out) return FSP_ERR_INVALID_ARG;
+    if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
+    for (int d = 0; d < 3; ++d) m_out[d] = p->vg_m[d];
+    return FSP_OK;
 }
 
 int fsp_get_green_table(const fsp_plan* p, double* T_host) {

@@ -34,15 +34,17 @@ __global__ void k_fill_he(double* __restrict__ T, int Nx, int Ny, int Nz, double
     }
 }
 
-// VG2: f[kx][ky][kz] = G_L(2 pi k_d / (4 N_d h_d)), 0 <= k_d <= 2 N_d
+// VG2 / VG-safe: f[kx][ky][kz] = G_L(2 pi k_d / (m_d N_d h_d)), 0 <= k_d <= m_d N_d / 2
+// (m = 4 on every axis is the paper's lattice; R17 for the per-axis factors)
 __global__ void k_fill_gl_vg2(double* __restrict__ f, int Nx, int Ny, int Nz, double hx, double hy,
-                              double hz, double L) {
-    const long Kx = 2 * Nx + 1, Ky = 2 * Ny + 1, Kz = 2 * Nz + 1;
+                              double hz, double L, int mx, int my, int mz) {
+    const long Kx = (long)mx * Nx / 2 + 1, Ky = (long)my * Ny / 2 + 1, Kz = (long)mz * Nz / 2 + 1;
     const long total = Kx * Ky * Kz;
     const double PI2 = 6.28318530717958647692;
     for (long o = blockIdx.x * (long)blockDim.x + threadIdx.x; o < total; o += (long)gridDim.x * blockDim.x) {
         const long kz = o % Kz, ky = (o / Kz) % Ky, kx = o / (Kz * Ky);
-        f[o] = vg_GL(PI2 * kx / (4.0 * Nx * hx), PI2 * ky / (4.0 * Ny * hy), PI2 * kz / (4.0 * Nz * hz), L);
+        f[o] = vg_GL(PI2 * kx / ((double)mx * Nx * hx), PI2 * ky / ((double)my * Ny * hy),
+                     PI2 * kz / ((double)mz * Nz * hz), L);
     }
 }
 

@@ -211,3 +211,55 @@ def test_unaligned_rho_takes_the_plain_path():
         torch.cuda.synchronize()
     ref = oracle.OraclePlan(w.N, w.h, oracle.HOCKNEY).precompute_green().solve(w.rho)
     check(got.cpu().numpy(), ref)
+
+
+# ---- FSP_VICO_SAFE: per-axis oversampling of the VG precompute ----------------------
+SAFE_CASES = [((16, 16, 64), (1 / 16,) * 3), ((8, 32, 16), (0.1, 0.05, 0.2)), ((64, 16, 16), (0.02, 0.05, 0.04)),
+              ((16, 16, 16), (1 / 16,) * 3)]
+
+
+@pytest.mark.parametrize("N,h", SAFE_CASES)
+def test_vico_safe_table_spectrum_and_factors_parity(N, h):
+    with binding.Plan(N, h, binding.VICO_SAFE) as p:
+        p.precompute_green()
+        T, G, m = p.green_table(), p.green_spectrum(), p.vg_factors()
+    assert m == oracle.vg_safe_factors(N, h)
+    To = oracle.green_table(oracle.VICO_SAFE, N, h)
+    assert np.abs(T - To).max() <= 1e-13 * np.abs(To).max()
+    Go = oracle.green_spectrum(To).real[: N[0] + 1, : N[1] + 1, : N[2] + 1]
+    assert np.abs(G - Go).max() <= 1e-12 * np.abs(Go).max()
+
+
+def test_vico_safe_solve_parity_and_accuracy_in_a_long_box():
+    """Isotropic Gaussian in the 1 x 1 x 4 box at h = 1/32: parity with the oracle, spectral accuracy against
+    the closed form where the literal recipe (FSP_VICO_2) is off by O(1)."""
+    lo, hi, N = (-0.5, -0.5, -2.0), (0.5, 0.5, 2.0), (32, 32, 128)
+    rho = np.ascontiguousarray(W.gaussian_density(N, lo, hi, (0.0, 0.0, 0.0), (0.05,) * 3))
+    w = W.Workload("iso_gaussian_long_box", N, lo, hi, rho, [(1.0, (0.0, 0.0, 0.0), (0.05,) * 3)])
+    with binding.Plan(w.N, w.h, binding.VICO_SAFE) as p:
+        got = gpu_solve(p.precompute_green(), w.rho)
+        assert p.vg_factors() == (8, 8, 4)
+    ref = oracle.OraclePlan(w.N, w.h, oracle.VICO_SAFE).precompute_green().solve(w.rho)
+    check(got, ref)
+    ex = gaussian_potential_iso(w)
+    assert rel_l2(got, ex) < 1e-8
+    with binding.Plan(w.N, w.h, binding.VICO_2) as p:
+        lit = gpu_solve(p.precompute_green(), w.rho)
+    assert rel_l2(lit, ex) > 1e-1
+
+
+def test_vico_safe_full_size_beam_sampled():
+    """BASELINE.json config 4 (128 x 128 x 512) with FSP_VICO_SAFE: sampled outputs against Def. O1 with the
+    plan's table, and the table against the oracle's at sampled entries of a reduced replica is covered by
+    test_vico_safe_table_spectrum_and_factors_parity."""
+    w = W.config4()
+    with binding.Plan(w.N, w.h, binding.VICO_SAFE) as p:
+        p.precompute_green()
+        got = gpu_solve(p, w.rho)
+        T = p.green_table()
+        assert p.vg_factors() == (8, 8, 4)
+    idx = _spot_points(w.N, 500, seed=23)
+    ref = oracle.direct_sum(T, w.h, w.rho, idx)
+    g = got.reshape(-1)[idx]
+    assert np.linalg.norm(g - ref) / np.linalg.norm(ref) <= SPOT_L2_TOL
+    assert np.abs(g - ref).max() / np.abs(got).max() <= MAX_TOL
