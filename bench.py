@@ -411,7 +411,59 @@ def extras(args, peak):
                                      "frac_of_measured_peak": model_total / (ms * 1e-3) / 1e9 / peak,
                                      "precompute_green_s": t_pre, "rel_l2_vs_closed_form": _analytic_error(w, phi)}
         del rho, phi
+    for wname, steps in (("256", 20), ("512", 5)):
+        try:
+            torch.cuda.empty_cache()
+            out[f"cufft_unpruned_{wname}"] = cufft_comparison(wname, steps)
+        except Exception as e:   # a comparison line must never fail the bench
+            out[f"cufft_unpruned_{wname}"] = {"error": repr(e)[:200]}
+    torch.cuda.empty_cache()
     return out
+
+
+def cufft_comparison(wname, steps):
+    """Reported comparison only; the product never calls an FFT library: the un-pruned,
+    un-fused pipeline of PAPER.md:67-82 -- pad, rfftn, multiply, irfftn, crop -- on torch.fft (cuFFT), same
+    density, same timing loop.  Returns ms per solve and its agreement with the library's own solve."""
+    import numpy as np
+    import torch
+    from paper_2405_02603_b200 import binding, workloads as W
+    _, builder, kw, wdesc = WORKLOADS[wname]
+    w = getattr(W, builder)(**kw)
+    Nx, Ny, Nz = w.N
+    with binding.Plan(w.N, w.h, binding.HOCKNEY) as plan:
+        plan.precompute_green()
+        rho = torch.from_numpy(w.rho).cuda()
+        ours = plan.solve(rho).clone()
+        oct_ = torch.from_numpy(plan.green_spectrum()).cuda()            # (Nx+1, Ny+1, Nz+1), un-normalised
+    ix = torch.arange(2 * Nx, device="cuda"); ix = torch.minimum(ix, 2 * Nx - ix)
+    iy = torch.arange(2 * Ny, device="cuda"); iy = torch.minimum(iy, 2 * Ny - iy)
+    G = oct_[ix][:, iy].contiguous() * float(np.prod(w.h))              # (2Nx, 2Ny, Nz+1) real, h^3 folded in
+    del oct_
+
+    def solve():
+        pad = torch.zeros((2 * Nx, 2 * Ny, 2 * Nz), dtype=torch.float64, device="cuda")
+        pad[:Nx, :Ny, :Nz] = rho
+        spec = torch.fft.rfftn(pad)
+        del pad
+        spec *= G
+        full = torch.fft.irfftn(spec, s=(2 * Nx, 2 * Ny, 2 * Nz))
+        del spec
+        return full[:Nx, :Ny, :Nz]
+
+    for _ in range(3):
+        phi = solve()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        phi = solve()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    agree = float(torch.linalg.norm(phi - ours) / torch.linalg.norm(ours))
+    return {"workload": wdesc, "what": "torch.fft (cuFFT) pad + rfftn + multiply + irfftn + crop; comparison only",
+            "ms_per_solve": ms, "solves_per_s": 1e3 / ms, "steps": steps, "rel_l2_vs_libfsp": agree}
 
 
 if __name__ == "__main__":
