@@ -27,5 +27,6 @@ from .oracle import (  # noqa: F401
     num_threads,
     set_num_threads,
     solve_with_spectrum,
+    solve_field_with_spectrum,
     vg_window,
 )

@@ -23,6 +23,8 @@
  *   orc_green_spectrum
  *   orc_solve            PAPER.md:67-82  steps 1-5: double, zero-pad, FFT, multiply, inverse FFT,
  *                                        scale by hxhyhz, restrict.
+ *   orc_solve_field      PAPER.md:227-231 (Eq. A.1)  E = -grad phi, spectral gradient on the doubled
+ *                                        grid (8(f) N3, R18): steps 1-4, times -i k_d, inverse FFT, restrict.
  *
  * Pins (tests/test_oracle_*.py, all -m "not gpu"): numpy brute force on tiny grids, numpy.fft on
  * random vectors, the closed-form Gaussian potential with second-order (HE) and
@@ -475,6 +477,64 @@ int orc_solve(long Nx, long Ny, long Nz, const double h[3], const double* Ghat, 
             for (long k = 0; k < Nz; ++k)
                 phi[((size_t)i * Ny + j) * Nz + k] = scale * r2[2 * (((size_t)i * Dy + j) * Dz + k)];
     free(r2);
+    return ORC_OK;
+}
+
+/* Field output (Eq. A.1: E = -grad phi; reading R18):
+ * the gradient is taken spectrally on the doubled periodic grid, where the solver already is:
+ *   E_d = -hx hy hz F^-1{ i k_d F{rho2} x F{G2} } restricted,   k_d = 2 pi m'_d / (2 N_d h_d),
+ *   m' = m for m < N_d, m - 2 N_d for m > N_d, and 0 at the Nyquist index m = N_d (the derivative of
+ *   the real trigonometric interpolant).  phi is returned as in orc_solve.
+ * E: [3][Nx][Ny][Nz] (component-major, each component laid out like phi).  phi may be NULL. */
+int orc_solve_field(long Nx, long Ny, long Nz, const double h[3], const double* Ghat, int method,
+                    const double* rho, double* phi, double* E) {
+    if (Nx < 1 || Ny < 1 || Nz < 1 || !h || !Ghat || !rho || !E) return ORC_EINVAL;
+    long D[3] = {2 * Nx, 2 * Ny, 2 * Nz};
+    long Dx = D[0], Dy = D[1], Dz = D[2];
+    size_t total = (size_t)Dx * Dy * Dz, V = (size_t)Nx * Ny * Nz;
+    double* r2 = (double*)calloc(2 * total, sizeof(double));
+    double* w2 = (double*)malloc(2 * total * sizeof(double));
+    if (!r2 || !w2) { free(r2); free(w2); return ORC_ENOMEM; }
+    for (long i = 0; i < Nx; ++i)
+        for (long j = 0; j < Ny; ++j)
+            for (long k = 0; k < Nz; ++k)
+                r2[2 * (((size_t)i * Dy + j) * Dz + k)] = rho[((size_t)i * Ny + j) * Nz + k];
+    int rc = orc_fft3d(Dx, Dy, Dz, r2, -1, method);
+    if (rc != ORC_OK) { free(r2); free(w2); return rc; }
+#pragma omp parallel for schedule(static)
+    for (long o = 0; o < (long)total; ++o) {
+        double ar = r2[2 * o], ai = r2[2 * o + 1];
+        double br = Ghat[2 * o], bi = Ghat[2 * o + 1];
+        r2[2 * o] = ar * br - ai * bi;
+        r2[2 * o + 1] = ar * bi + ai * br;
+    }
+    double scale = h[0] * h[1] * h[2] / (double)total;
+    for (int d = -1; d < 3; ++d) {   /* d = -1: phi itself */
+        if (d < 0 && !phi) continue;
+#pragma omp parallel for schedule(static)
+        for (long i = 0; i < Dx; ++i)
+            for (long j = 0; j < Dy; ++j)
+                for (long k = 0; k < Dz; ++k) {
+                    size_t o = ((size_t)i * Dy + j) * Dz + k;
+                    double ar = r2[2 * o], ai = r2[2 * o + 1];
+                    if (d < 0) { w2[2 * o] = ar; w2[2 * o + 1] = ai; continue; }
+                    long m = d == 0 ? i : (d == 1 ? j : k), half = D[d] / 2;
+                    long mp = m < half ? m : (m == half ? 0 : m - D[d]);
+                    double kd = 2.0 * ORC_PI * (double)mp / ((double)D[d] * h[d]);
+                    /* -(i kd)(ar + i ai) = kd ai - i kd ar */
+                    w2[2 * o] = kd * ai;
+                    w2[2 * o + 1] = -kd * ar;
+                }
+        rc = orc_fft3d(Dx, Dy, Dz, w2, +1, method);
+        if (rc != ORC_OK) { free(r2); free(w2); return rc; }
+        double* out = d < 0 ? phi : E + (size_t)d * V;
+        for (long i = 0; i < Nx; ++i)
+            for (long j = 0; j < Ny; ++j)
+                for (long k = 0; k < Nz; ++k)
+                    out[((size_t)i * Ny + j) * Nz + k] = scale * w2[2 * (((size_t)i * Dy + j) * Dz + k)];
+    }
+    free(r2);
+    free(w2);
     return ORC_OK;
 }
 

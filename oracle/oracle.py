@@ -61,6 +61,7 @@ def _load():
         lib.orc_vg_safe_factors.argtypes = [L, L, L, _dp, D, _lp]
         lib.orc_green_spectrum.argtypes = [L, L, L, _dp, I, _dp]
         lib.orc_solve.argtypes = [L, L, L, _dp, _dp, I, _dp, _dp]
+        lib.orc_solve_field.argtypes = [L, L, L, _dp, _dp, I, _dp, _dp, _dp]
         lib.orc_direct_sum.argtypes = [L, L, L, _dp, _dp, _dp, L, _lp, _dp]
         _lib = lib
     return _lib
@@ -187,6 +188,21 @@ def solve_with_spectrum(Ghat: np.ndarray, h, rho: np.ndarray, method: int = 0) -
     return phi
 
 
+def solve_field_with_spectrum(Ghat: np.ndarray, h, rho: np.ndarray, method: int = 0):
+    """phi and E = -grad phi (Eq. A.1) by the spectral gradient on the doubled grid
+    (R18).  Returns (phi, E) with E of shape (3, Nx, Ny, Nz)."""
+    rho = np.ascontiguousarray(rho, dtype=np.float64)
+    Nx, Ny, Nz = rho.shape
+    Ghat = np.ascontiguousarray(Ghat, dtype=np.complex128)
+    assert Ghat.shape == (2 * Nx, 2 * Ny, 2 * Nz)
+    h = _h3(h)
+    phi = np.empty_like(rho)
+    E = np.empty((3,) + rho.shape, dtype=np.float64)
+    _check(_load().orc_solve_field(Nx, Ny, Nz, _d(h), _d(Ghat.view(np.float64)), method, _d(rho),
+                                   _d(phi), _d(E)), "solve_field")
+    return phi, E
+
+
 def direct_sum(T: np.ndarray, h, rho: np.ndarray, idx: np.ndarray | None = None) -> np.ndarray:
     """Def. O1: the plain O(V^2) discrete convolution, at all points or at flat indices ``idx``."""
     rho = np.ascontiguousarray(rho, dtype=np.float64)
@@ -235,6 +251,13 @@ class OraclePlan:
         if self.Ghat is None:
             self.Ghat = green_spectrum(self.T, self.method)
         return solve_with_spectrum(self.Ghat, self.h, rho, self.method)
+
+    def solve_field(self, rho: np.ndarray):
+        if self.T is None:
+            raise RuntimeError("solve_field before precompute_green")
+        if self.Ghat is None:
+            self.Ghat = green_spectrum(self.T, self.method)
+        return solve_field_with_spectrum(self.Ghat, self.h, rho, self.method)
 
     def direct_sum(self, rho: np.ndarray, idx=None) -> np.ndarray:
         return direct_sum(self.T, self.h, rho, idx)

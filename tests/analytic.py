@@ -54,3 +54,22 @@ def rel_l2(a: np.ndarray, b: np.ndarray) -> float:
 def rel_max(a: np.ndarray, b: np.ndarray) -> float:
     """Max-norm relative error max|a-b| / max|b| (reading R14)."""
     return float(np.abs(a - b).max() / np.abs(b).max())
+
+
+def gaussian_field_iso(w: W.Workload) -> np.ndarray:
+    """E = -grad phi of the closed form above (Eq. A.1), shape (3, Nx, Ny, Nz):
+        E(r) = (x / r) [ erf(r / (sqrt(2) s)) / r^2 - sqrt(2/pi) exp(-r^2 / (2 s^2)) / (s r) ] / (4 pi),  E(0) = 0.
+    """
+    xs = W.cell_centres(w.N, w.lo, w.hi)
+    E = np.zeros((3,) + tuple(w.N), dtype=np.float64)
+    for amp, c, sig in w.gaussians:
+        assert sig[0] == sig[1] == sig[2]
+        s = sig[0]
+        d = [xs[0][:, None, None] - c[0], xs[1][None, :, None] - c[1], xs[2][None, None, :] - c[2]]
+        r = np.sqrt(d[0] ** 2 + d[1] ** 2 + d[2] ** 2)
+        with np.errstate(divide="ignore", invalid="ignore"):
+            er = (erf(r / (math.sqrt(2.0) * s)) / r ** 2
+                  - math.sqrt(2.0 / math.pi) * np.exp(-r ** 2 / (2.0 * s * s)) / (s * r)) / (4.0 * math.pi)
+            for a in range(3):
+                E[a] += amp * np.where(r == 0.0, 0.0, er * d[a] / r)
+    return E

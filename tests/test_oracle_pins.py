@@ -13,7 +13,8 @@ import scipy.fft
 
 import oracle
 from paper_2405_02603_b200 import workloads as W
-from tests.analytic import gaussian_potential_aniso_points, gaussian_potential_iso, rel_l2, rel_max
+from tests.analytic import (gaussian_field_iso, gaussian_potential_aniso_points, gaussian_potential_iso, rel_l2,
+                            rel_max)
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
 PAPER = json.load(open(os.path.join(GOLD, "paper_invariants.json")))
@@ -387,3 +388,83 @@ def test_vg_safe_beam_like_gaussian_against_1d_integral():
     vg = oracle.OraclePlan(w.N, w.h, oracle.VICO_SAFE).precompute_green().solve(w.rho)
     got = vg[pts_idx[:, 0], pts_idx[:, 1], pts_idx[:, 2]]
     assert np.linalg.norm(got - ex) / np.linalg.norm(ex) < 3e-4
+
+
+# ---------------------------------------------------------------- field output E = -grad phi (8(f) N3, R18)
+def _cot_diff_matrix(L, h):
+    """Periodic spectral differentiation matrix of an even number L of points with spacing h (the textbook
+    closed form, e.g. Trefethen, Spectral Methods in MATLAB, ch. 3): D[i,j] = (pi / (L h)) (-1)^(i-j) cot(pi (i-j) / L),
+    D[i,i] = 0.  It differentiates the real trigonometric interpolant (Nyquist mode has zero derivative)."""
+    n = np.arange(L)[:, None] - np.arange(L)[None, :]
+    with np.errstate(divide="ignore", invalid="ignore"):
+        D = (math.pi / (L * h)) * np.where(n % 2 == 0, 1.0, -1.0) / np.tan(math.pi * n / L)
+    D[n == 0] = 0.0
+    return D
+
+
+def _brute_phi2(T, h, rho):
+    """The cyclic convolution of PAPER.md:80 on the whole doubled grid, written out in numpy (no FFT)."""
+    Nx, Ny, Nz = rho.shape
+    ix = [np.minimum(np.arange(2 * n), 2 * n - np.arange(2 * n)) for n in (Nx, Ny, Nz)]
+    G2 = T[np.ix_(*ix)]
+    phi2 = np.zeros((2 * Nx, 2 * Ny, 2 * Nz))
+    for a in range(Nx):
+        for b in range(Ny):
+            for c in range(Nz):
+                if rho[a, b, c] != 0.0:
+                    phi2 += rho[a, b, c] * np.roll(G2, (a, b, c), axis=(0, 1, 2))
+    return h[0] * h[1] * h[2] * phi2
+
+
+@pytest.mark.parametrize("N", [(4, 4, 4), (2, 8, 4), (4, 2, 8)])
+@pytest.mark.parametrize("alg", ["HE", "VG2", "random"])
+def test_field_equals_cot_matrix_derivative_of_brute_force_phi2(N, alg):
+    """No FFT on the reference side: phi2 by brute-force cyclic convolution, then the closed-form periodic
+    differentiation matrix along each axis.  Catches a wrong sign, a wrong k_d (axis swap, Nyquist), a wrong scale."""
+    w = W.random_density(N, seed=21)
+    if alg == "random":
+        T = np.random.default_rng(3).standard_normal(tuple(n + 1 for n in N))
+    else:
+        T = oracle.green_table(ALGS[alg], N, w.h)
+    phi, E = oracle.solve_field_with_spectrum(oracle.green_spectrum(T), w.h, w.rho)
+    phi2 = _brute_phi2(T, w.h, w.rho)
+    assert rel_max(phi, phi2[:N[0], :N[1], :N[2]]) < 1e-13
+    for d in range(3):
+        D = _cot_diff_matrix(2 * N[d], w.h[d])
+        ref = -np.moveaxis(np.tensordot(D, phi2, axes=([1], [d])), 0, d)[:N[0], :N[1], :N[2]]
+        assert rel_max(E[d], ref) < 1e-12, d
+
+
+def test_field_phi_identical_to_solve_and_linear():
+    N, h = (8, 16, 4), (0.1, 0.05, 0.2)
+    p = oracle.OraclePlan(N, h, oracle.HOCKNEY).precompute_green()
+    a, b = W.random_density(N, seed=1).rho, W.random_density(N, seed=2).rho
+    pa, Ea = p.solve_field(a)
+    pb, Eb = p.solve_field(b)
+    assert np.array_equal(pa, p.solve(a))
+    _, Ec = p.solve_field(2.0 * a - 3.0 * b)
+    assert rel_max(Ec, 2.0 * Ea - 3.0 * Eb) < 1e-13
+
+
+def test_field_is_antisymmetric_for_a_centred_gaussian():
+    w = W.config1(16)
+    _, E = oracle.OraclePlan(w.N, w.h, oracle.VICO_2).precompute_green().solve_field(w.rho)
+    assert np.abs(E[0] + E[0][::-1, :, :]).max() < 1e-12 * np.abs(E).max()
+    assert np.abs(E[1] + E[1][:, ::-1, :]).max() < 1e-12 * np.abs(E).max()
+    assert np.abs(E[2] + E[2][:, :, ::-1]).max() < 1e-12 * np.abs(E).max()
+    assert np.abs(E[0] - E[0][:, ::-1, :]).max() < 1e-12 * np.abs(E).max()
+    assert np.abs(E[0] - np.transpose(E[1], (1, 0, 2))).max() < 1e-12 * np.abs(E).max()
+
+
+def test_field_closed_form_he_second_order_vg_spectral():
+    """Closed-form Gaussian field (Eq. A.1 applied to PAPER.md:114).  HE: second order; VG: spectral, reaching
+    round-off at 64^3 -- the spectral gradient keeps the accuracy class of each solver (R18)."""
+    err = {}
+    for n in (16, 32, 64):
+        w = W.config1(n)
+        ref = gaussian_field_iso(w)
+        for name, alg in (("HE", oracle.HOCKNEY), ("VG", oracle.VICO_2)):
+            _, E = oracle.OraclePlan(w.N, w.h, alg).precompute_green().solve_field(w.rho)
+            err[name, n] = rel_l2(E, ref)
+    assert 3.3 < err["HE", 16] / err["HE", 32] < 4.6 and 3.3 < err["HE", 32] / err["HE", 64] < 4.6, err
+    assert err["VG", 16] < 3e-2 and err["VG", 32] < 2e-6 and err["VG", 64] < 1e-13, err
