@@ -117,6 +117,26 @@ int fsp_solve(fsp_plan* p, const double* rho_dev, double* phi_dev);
  */
 int fsp_solve_host(fsp_plan* p, const double* rho_host, double* phi_host);
 
+/*
+ * Field output -- PAPER.md:227-231, Eq. A.1: "the electric field E(x) is obtained from E = -grad phi".
+ * The paper does not say how the gradient is taken; here it is taken where the solver already is, in
+ * Fourier space on the doubled grid (reading R18):
+ *     E_d = -hx hy hz F^-1{ i k_d F{rho2} x F{G2} } restricted,  k_d = 2 pi m'_d / (2 N_d h_d),
+ * m' the signed mode number, zero at the Nyquist index m = N_d.  This keeps the accuracy class of the
+ * Green's function: second order for FSP_HOCKNEY, spectral for the Vico-Greengard algorithms.
+ *   rho_dev  device pointer, Nx*Ny*Nz doubles, read-only
+ *   phi_dev  device pointer, Nx*Ny*Nz doubles, or NULL if the potential is not wanted
+ *   E_dev    device pointer, 3*Nx*Ny*Nz doubles, component-major: E_dev[d*V + (ix*Ny+iy)*Nz+iz], d = x,y,z
+ * The two forward passes run once; each output runs the middle pass (with the factor -i k_d fused
+ * into the spectrum multiply) and the two inverse passes: 2 + 3*3 (+3) kernel launches.  The first
+ * call allocates one more plan-owned intermediate the size of the larger workspace array (counted by
+ * fsp_plan_bytes from then on).  FSP_PARAM_CHUNK_PLANES does not apply.  Asynchronous like fsp_solve.
+ */
+int fsp_solve_field(fsp_plan* p, const double* rho_dev, double* phi_dev, double* E_dev);
+
+/* The same from HOST buffers (phi_host may be NULL); synchronises the stream before returning. */
+int fsp_solve_field_host(fsp_plan* p, const double* rho_host, double* phi_host, double* E_host);
+
 /* Frees everything the plan owns (synchronises its stream first). */
 int fsp_destroy(fsp_plan* p);
 
@@ -131,6 +151,10 @@ size_t fsp_precompute_peak_bytes(const fsp_plan* p);
 /* Algorithmic (minimal-traffic) HBM bytes of one solve: total, and per kernel
  * if per_kernel (host pointer to FSP_NUM_SOLVE_KERNELS doubles) is not NULL. */
 double fsp_model_bytes_per_solve(const fsp_plan* p, double* per_kernel);
+
+/* Algorithmic HBM bytes of one fsp_solve_field: the two forward passes once, the middle pass and the
+ * two inverse passes once per output (3 components, + phi if with_phi != 0). */
+double fsp_model_bytes_per_field_solve(const fsp_plan* p, int with_phi);
 
 /* Oversampling factors (m_x, m_y, m_z) used by the last fsp_precompute_green of a VG algorithm
  * (4,4,4 for FSP_VICO and FSP_VICO_2); m_out: host pointer to 3 ints. */

@@ -28,5 +28,6 @@ from .oracle import (  # noqa: F401
     set_num_threads,
     solve_with_spectrum,
     solve_field_with_spectrum,
+    field_of_point_charges,
     vg_window,
 )

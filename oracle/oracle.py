@@ -203,6 +203,39 @@ def solve_field_with_spectrum(Ghat: np.ndarray, h, rho: np.ndarray, method: int 
     return phi, E
 
 
+def field_of_point_charges(T: np.ndarray, h, charges, points) -> np.ndarray:
+    """E = -grad phi (R18) of a few point charges, point by point, WITHOUT any FFT: usable at any mesh size.
+
+    With rho = sum_p q_p delta[y_p], phi2[x] = hx hy hz sum_p q_p G2[x - y_p] on the doubled periodic grid
+    (PAPER.md:72-80), and the spectral derivative along axis d of a periodic sequence of L = 2 N_d points is
+    the circular convolution with S[n] = (pi / (L h_d)) (-1)^n cot(pi n / L), S[0] = 0 (the derivative of the
+    real trigonometric interpolant).  So
+        E_d[x] = -hx hy hz sum_p q_p sum_{i'} S[x_d - y_pd - i'] G2[.., i', ..].
+    charges: list of ((ix, iy, iz), q);  points: (npts, 3) integer mesh indices.  Returns (npts, 3)."""
+    T = np.ascontiguousarray(T, dtype=np.float64)
+    N = tuple(n - 1 for n in T.shape)
+    h = _h3(h)
+    w = float(h[0] * h[1] * h[2])
+    points = np.asarray(points, dtype=np.int64)
+    out = np.zeros((len(points), 3), dtype=np.float64)
+    mir = [np.minimum(np.arange(2 * n), 2 * n - np.arange(2 * n)) for n in N]   # 8-case mirror, PAPER.md:74
+    for d in range(3):
+        L = 2 * N[d]
+        n = np.arange(L)
+        for (y, q) in charges:
+            for ip, x in enumerate(points):
+                disp = [int(x[a] - y[a]) % (2 * N[a]) for a in range(3)]
+                sel = [mir[a][disp[a]] for a in range(3)]
+                sel[d] = mir[d]                       # the whole line of G2 along axis d
+                line = T[sel[0], sel[1], sel[2]]      # G2[.., i', ..], i' = 0 .. L-1
+                m = (disp[d] - n) % L
+                with np.errstate(divide="ignore", invalid="ignore"):
+                    S = (np.pi / (L * h[d])) * np.where(m % 2 == 0, 1.0, -1.0) / np.tan(np.pi * m / L)
+                S[m == 0] = 0.0
+                out[ip, d] -= w * q * float(np.dot(S, line))
+    return out
+
+
 def direct_sum(T: np.ndarray, h, rho: np.ndarray, idx: np.ndarray | None = None) -> np.ndarray:
     """Def. O1: the plain O(V^2) discrete convolution, at all points or at flat indices ``idx``."""
     rho = np.ascontiguousarray(rho, dtype=np.float64)

@@ -33,6 +33,9 @@ SIGNATURES = {
     "fsp_precompute_green": (_i, [_vp]),
     "fsp_solve": (_i, [_vp, _vp, _vp]),
     "fsp_solve_host": (_i, [_vp, _vp, _vp]),
+    "fsp_solve_field": (_i, [_vp, _vp, _vp, _vp]),
+    "fsp_solve_field_host": (_i, [_vp, _vp, _vp, _vp]),
+    "fsp_model_bytes_per_field_solve": (_d, [_vp, _i]),
     "fsp_destroy": (_i, [_vp]),
     "fsp_plan_bytes": (_sz, [_vp]),
     "fsp_precompute_peak_bytes": (_sz, [_vp]),
@@ -121,6 +124,21 @@ def solve_host(plan: int, rho_host, phi_host) -> None:
     _chk(lib().fsp_solve_host(plan, _ptr(rho_host), _ptr(phi_host)), "fsp_solve_host")
 
 
+def solve_field(plan: int, rho_dev, phi_dev, E_dev) -> None:
+    """fsp_solve_field; phi_dev may be None."""
+    _chk(lib().fsp_solve_field(plan, _ptr(rho_dev), None if phi_dev is None else _ptr(phi_dev), _ptr(E_dev)),
+         "fsp_solve_field")
+
+
+def solve_field_host(plan: int, rho_host, phi_host, E_host) -> None:
+    _chk(lib().fsp_solve_field_host(plan, _ptr(rho_host), None if phi_host is None else _ptr(phi_host),
+                                    _ptr(E_host)), "fsp_solve_field_host")
+
+
+def model_bytes_per_field_solve(plan: int, with_phi: bool = True) -> float:
+    return float(lib().fsp_model_bytes_per_field_solve(plan, int(bool(with_phi))))
+
+
 def destroy(plan: int) -> None:
     _chk(lib().fsp_destroy(plan), "fsp_destroy")
 
@@ -199,6 +217,22 @@ class Plan:
         assert phi.is_cuda and phi.dtype == torch.float64 and phi.is_contiguous() and tuple(phi.shape) == self.N
         solve(self.handle, rho, phi)
         return phi
+
+    def solve_field(self, rho, phi=None, E=None, want_phi: bool = True):
+        """phi and E = -grad phi.  Returns (phi or None, E) with E of shape (3,) + N."""
+        import torch
+        assert rho.is_cuda and rho.dtype == torch.float64 and rho.is_contiguous() and tuple(rho.shape) == self.N
+        if phi is None and want_phi:
+            phi = torch.empty_like(rho)
+        if E is None:
+            E = torch.empty((3,) + self.N, dtype=torch.float64, device=rho.device)
+        assert E.is_cuda and E.dtype == torch.float64 and E.is_contiguous() and tuple(E.shape) == (3,) + self.N
+        solve_field(self.handle, rho, phi if want_phi else None, E)
+        return (phi if want_phi else None), E
+
+    def solve_field_host(self, rho_host, phi_host, E_host):
+        solve_field_host(self.handle, rho_host, phi_host, E_host)
+        return phi_host, E_host
 
     def solve_host(self, rho_host, phi_host):
         """Host buffers (numpy arrays or pinned torch CPU tensors), copies inside the call."""

@@ -42,13 +42,15 @@ struct fsp_plan {
     CUtensorMap tmB1x;      // B1 as [j][parity][2 Ny Nz doubles] (row = 2j + parity), box = 16 columns x 1 x <=256 (K5 input)
     CUtensorMap tmB1y;      // B1 as [kx][y][2 Nz doubles], box = 8 columns x <=256 rows (K2 input)
     CUtensorMap tmB2y;      // B2 as [kx][j][parity][2 Nz doubles], box = 8 columns x 1 parity x <=256 j (K4 input)
+    double2* B3 = nullptr;  // second B2-sized buffer, allocated by the first fsp_solve_field (derivative spectra)
+    CUtensorMap tmB3y;      // the same view of B3
     bool z_warp = false;    // K3 v2 (k_conv_z_w) is used
     int chunk_planes = 0;   // > 0: K2-K3-K4 run chunk_planes kx-planes at a time (L2-resident B2)
     int sm_count = 148;
     double* T = nullptr;    // (Nx+1)(Ny+1)(Nz+1)   real-space table
     double* Goct = nullptr; // (Nx+1)(Ny+1)(Nz+1)   un-normalised spectrum octant
     double2 *Wx = nullptr, *Wy = nullptr, *Wz = nullptr;  // exp(-2 pi i n / 2N_d), n < 2N_d
-    double *rho_stage = nullptr, *phi_stage = nullptr;
+    double *rho_stage = nullptr, *phi_stage = nullptr, *E_stage = nullptr;
     bool precomputed = false;
     size_t bytes = 0, peak_transient = 0;
     // profiling
@@ -244,32 +246,43 @@ int launch_inv_y(fsp_plan* p, const double2* B2, double2* B1, int nplanes) {
     k_inv_y<M><<<(unsigned)grid, G * kW * Cfg::T, smem, p->stream>>>(B2, B1, p->Wy, p->Nz, ntiles);
     return FSP_OK;
 }
-template <int M>
-int launch_conv_z(fsp_plan* p, double2* B2, const double* G, int nplanes) {
+// DER = false: in place on B2.  DER = true: B2 -> out with the factor -i k_d of `kap` (field output).
+template <int M, bool DER>
+int launch_conv_z_impl(fsp_plan* p, double2* B2, const double* G, int nplanes, double2* out, const DerK kap) {
     using Cfg = FftCfg<M>;
     constexpr int P = PencilGroups<Cfg>::P;
     const long npencils = (long)nplanes * (2 * p->Ny);
     const size_t smem = sizeof(double2) * (size_t)(2 * M + P * M);
-    CU(cudaFuncSetAttribute(k_conv_z<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_conv_z<M><<<(unsigned)((npencils + P - 1) / P), P * Cfg::T, smem, p->stream>>>(B2, G, p->Wz, npencils);
+    CU(cudaFuncSetAttribute(k_conv_z<M, DER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_conv_z<M, DER><<<(unsigned)((npencils + P - 1) / P), P * Cfg::T, smem, p->stream>>>(B2, G, p->Wz, npencils, out, p->Ny, kap);
     return FSP_OK;
 }
 template <int M>
-int launch_conv_z_w(fsp_plan* p, double2* B2, const double* G, int nplanes) {
+int launch_conv_z(fsp_plan* p, double2* B2, const double* G, int nplanes, double2* out, const DerK* kap) {
+    if (kap) return launch_conv_z_impl<M, true>(p, B2, G, nplanes, out, *kap);
+    return launch_conv_z_impl<M, false>(p, B2, G, nplanes, nullptr, DerK{0.0, 0.0, 0.0, 0});
+}
+template <int M, bool DER>
+int launch_conv_z_w_impl(fsp_plan* p, double2* B2, const double* G, int nplanes, double2* out, const DerK kap) {
     using Z = ConvZ<M>;
     const long ngroups = (long)nplanes * (2 * p->Ny) / Z::G;
     const size_t smem = Z::smem_bytes();
     static int occ = 0;  // CTAs per SM, queried once per transform length
     if (occ == 0) {
-        CU(cudaFuncSetAttribute(k_conv_z_w<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_conv_z_w<M>, Z::WARPS * 32, smem));
+        CU(cudaFuncSetAttribute(k_conv_z_w<M, DER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_conv_z_w<M, DER>, Z::WARPS * 32, smem));
         if (occ < 1) return FSP_ERR_CUDA;
     }
     long grid = (long)p->sm_count * occ;
     const long need = (ngroups + Z::WARPS - 1) / Z::WARPS;
     if (grid > need) grid = need;
-    k_conv_z_w<M><<<(unsigned)grid, Z::WARPS * 32, smem, p->stream>>>(B2, G, p->LTz, p->Wz, p->Ny, ngroups);
+    k_conv_z_w<M, DER><<<(unsigned)grid, Z::WARPS * 32, smem, p->stream>>>(B2, G, p->LTz, p->Wz, p->Ny, ngroups, out, kap);
     return FSP_OK;
+}
+template <int M>
+int launch_conv_z_w(fsp_plan* p, double2* B2, const double* G, int nplanes, double2* out, const DerK* kap) {
+    if (kap) return launch_conv_z_w_impl<M, true>(p, B2, G, nplanes, out, *kap);
+    return launch_conv_z_w_impl<M, false>(p, B2, G, nplanes, nullptr, DerK{0.0, 0.0, 0.0, 0});
 }
 template <int M>
 int launch_fwd_x(fsp_plan* p, const double* rho) {
@@ -368,18 +381,19 @@ int do_fwd_y(fsp_plan* p, int kx0, double2* B2, int np) {
         case 512: return fn<512>(__VA_ARGS__);           \
         default: return FSP_ERR_INVALID_ARG;             \
     }
-int do_conv_z_v1(fsp_plan* p, double2* B2, const double* G, int np) { DISPATCH_YZ(launch_conv_z, p->Nz, p, B2, G, np) }
-int do_conv_z_w(fsp_plan* p, double2* B2, const double* G, int np) { DISPATCH_W(launch_conv_z_w, p->Nz, p, B2, G, np) }
-// planes [kx0, kx0 + np) of the spectrum go with the np planes stored at B2
-int do_conv_z(fsp_plan* p, double2* B2, int kx0, int np) {
-    if (p->z_warp) return do_conv_z_w(p, B2, p->Gk + (size_t)kx0 * (p->Ny + 1) * (p->Nz + 2), np);
-    return do_conv_z_v1(p, B2, p->Gh + (size_t)kx0 * (2 * p->Ny) * (2 * p->Nz), np);
+int do_conv_z_v1(fsp_plan* p, double2* B2, const double* G, int np, double2* out, const DerK* kap) { DISPATCH_YZ(launch_conv_z, p->Nz, p, B2, G, np, out, kap) }
+int do_conv_z_w(fsp_plan* p, double2* B2, const double* G, int np, double2* out, const DerK* kap) { DISPATCH_W(launch_conv_z_w, p->Nz, p, B2, G, np, out, kap) }
+// planes [kx0, kx0 + np) of the spectrum go with the np planes stored at B2.
+// kap == nullptr: in place (phi); otherwise B2 -> out with the derivative factor (whole volume only, kx0 = 0).
+int do_conv_z(fsp_plan* p, double2* B2, int kx0, int np, double2* out = nullptr, const DerK* kap = nullptr) {
+    if (p->z_warp) return do_conv_z_w(p, B2, p->Gk + (size_t)kx0 * (p->Ny + 1) * (p->Nz + 2), np, out, kap);
+    return do_conv_z_v1(p, B2, p->Gh + (size_t)kx0 * (2 * p->Ny) * (2 * p->Nz), np, out, kap);
 }
 int make_z_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Nz, &p->LTz, &p->bytes) }
 int make_x_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Nx / 2, &p->LTx, &p->bytes) }
 int make_y_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Ny, &p->LTy, &p->bytes) }
 template <int M>
-int launch_inv_y_t(fsp_plan* p, double2* B1, int nplanes) {
+int launch_inv_y_t(fsp_plan* p, const CUtensorMap& tm, double2* B1, int nplanes) {
     using Y = TileYI<M>;
     const long ntiles = (long)nplanes * (p->Nz / kW);
     const size_t smem = Y::smem_bytes();
@@ -391,15 +405,16 @@ int launch_inv_y_t(fsp_plan* p, double2* B1, int nplanes) {
     }
     long grid = (long)p->sm_count * occ;
     if (grid > ntiles) grid = ntiles;
-    k_inv_y_t<M><<<(unsigned)grid, Y::THREADS, smem, p->stream>>>(p->tmB2y, B1, p->LTy, p->Wy, p->Nz, ntiles);
+    k_inv_y_t<M><<<(unsigned)grid, Y::THREADS, smem, p->stream>>>(tm, B1, p->LTy, p->Wy, p->Nz, ntiles);
     return FSP_OK;
 }
 // B2 must be the plan's own B2 (the tile kernel reads it through the plan's tensor map)
 int do_inv_y(fsp_plan* p, const double2* B2, double2* B1, int np) {
-    if (p->tile_y && B2 == p->B2) {
-        if (p->Ny == 512) return launch_inv_y_t<512>(p, B1, np);
-        if (p->Ny == 256) return launch_inv_y_t<256>(p, B1, np);
-        return launch_inv_y_t<128>(p, B1, np);
+    if (p->tile_y && (B2 == p->B2 || (p->B3 && B2 == p->B3))) {
+        const CUtensorMap& tm = B2 == p->B2 ? p->tmB2y : p->tmB3y;
+        if (p->Ny == 512) return launch_inv_y_t<512>(p, tm, B1, np);
+        if (p->Ny == 256) return launch_inv_y_t<256>(p, tm, B1, np);
+        return launch_inv_y_t<128>(p, tm, B1, np);
     }
     DISPATCH_YZ(launch_inv_y, p->Ny, p, B2, B1, np)
 }
@@ -565,7 +580,7 @@ int precompute_impl(fsp_plan* p) {
 }
 
 void free_plan_memory(fsp_plan* p) {
-    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->Gh); cudaFree(p->Gk); cudaFree(p->LTz); cudaFree(p->LTy); cudaFree(p->LTx); cudaFree(p->T); cudaFree(p->Goct);
+    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->B3); cudaFree(p->E_stage); cudaFree(p->Gh); cudaFree(p->Gk); cudaFree(p->LTz); cudaFree(p->LTy); cudaFree(p->LTx); cudaFree(p->T); cudaFree(p->Goct);
     cudaFree(p->Wx); cudaFree(p->Wy); cudaFree(p->Wz); cudaFree(p->rho_stage); cudaFree(p->phi_stage);
     for (cudaEvent_t e : p->events) cudaEventDestroy(e);
     p->events.clear();
@@ -754,6 +769,69 @@ int fsp_solve_host(fsp_plan* p, const double* rho_host, double* phi_host) {
     CU(cudaMemcpyAsync(phi_host, p->phi_stage, v * sizeof(double), cudaMemcpyDeviceToHost, p->stream));
     CU(cudaStreamSynchronize(p->stream));
     return FSP_OK;
+}
+
+int fsp_solve_field(fsp_plan* p, const double* rho_dev, double* phi_dev, double* E_dev) {
+    if (!p || !rho_dev || !E_dev || rho_dev == phi_dev || rho_dev == E_dev) return FSP_ERR_INVALID_ARG;
+    if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
+    const size_t n2 = (size_t)(p->Nx + 1) * 2 * p->Ny * p->Nz, V = (size_t)p->Nx * p->Ny * p->Nz;
+    int rc;
+    if (!p->B3) {   // first field solve of this plan: the buffer that receives the derivative spectra
+        if ((rc = dev_alloc(&p->B3, n2, &p->bytes)) != FSP_OK) return rc;
+        if (p->tile_y) {
+            const cuuint64_t dims[4] = {(cuuint64_t)2 * p->Nz, 2, (cuuint64_t)p->Ny, (cuuint64_t)(p->Nx + 1)};
+            const cuuint64_t strides[3] = {(cuuint64_t)p->Nz * 16, (cuuint64_t)2 * p->Nz * 16, (cuuint64_t)2 * p->Ny * p->Nz * 16};
+            const cuuint32_t box[4] = {2 * kW, 1, (cuuint32_t)(p->Ny < 256 ? p->Ny : 256), 1};
+            if ((rc = make_tensor_map(&p->tmB3y, p->B3, 4, dims, strides, box)) != FSP_OK) return rc;
+        }
+    }
+    const int planes = p->Nx + 1;
+    const double PI = 3.14159265358979323846;
+    // forward passes once: B2 = F_y F_x rho2
+    if ((rc = do_fwd_x(p, rho_dev)) != FSP_OK) return rc;
+    if ((rc = do_fwd_y(p, 0, p->B2, planes)) != FSP_OK) return rc;
+    // E_d: K3 with the factor -i k_d (B2 -> B3), then the inverse passes (R18)
+    for (int d = 0; d < 3; ++d) {
+        const int Nd = d == 0 ? p->Nx : (d == 1 ? p->Ny : p->Nz);
+        const double kd = 2.0 * PI / (2.0 * (double)Nd * p->h[d]);
+        const DerK kap{d == 0 ? kd : 0.0, d == 1 ? kd : 0.0, d == 2 ? kd : 0.0, p->Nx};
+        if ((rc = do_conv_z(p, p->B2, 0, planes, p->B3, &kap)) != FSP_OK) return rc;
+        if ((rc = do_inv_y(p, p->B3, p->B1, planes)) != FSP_OK) return rc;
+        if ((rc = do_inv_x(p, E_dev + (size_t)d * V)) != FSP_OK) return rc;
+    }
+    if (phi_dev) {   // phi last: its K3 runs in place and consumes the forward data
+        if ((rc = do_conv_z(p, p->B2, 0, planes)) != FSP_OK) return rc;
+        if ((rc = do_inv_y(p, p->B2, p->B1, planes)) != FSP_OK) return rc;
+        if ((rc = do_inv_x(p, phi_dev)) != FSP_OK) return rc;
+    }
+    CU(cudaGetLastError());
+    return FSP_OK;
+}
+
+int fsp_solve_field_host(fsp_plan* p, const double* rho_host, double* phi_host, double* E_host) {
+    if (!p || !rho_host || !E_host) return FSP_ERR_INVALID_ARG;
+    if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
+    const size_t v = (size_t)p->Nx * p->Ny * p->Nz;
+    int rc;
+    if (!p->rho_stage) {
+        if ((rc = dev_alloc(&p->rho_stage, v, &p->bytes)) != FSP_OK) return rc;
+        if ((rc = dev_alloc(&p->phi_stage, v, &p->bytes)) != FSP_OK) return rc;
+    }
+    if (!p->E_stage && (rc = dev_alloc(&p->E_stage, 3 * v, &p->bytes)) != FSP_OK) return rc;
+    CU(cudaMemcpyAsync(p->rho_stage, rho_host, v * sizeof(double), cudaMemcpyHostToDevice, p->stream));
+    if ((rc = fsp_solve_field(p, p->rho_stage, phi_host ? p->phi_stage : nullptr, p->E_stage)) != FSP_OK) return rc;
+    if (phi_host) CU(cudaMemcpyAsync(phi_host, p->phi_stage, v * sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaMemcpyAsync(E_host, p->E_stage, 3 * v * sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaStreamSynchronize(p->stream));
+    return FSP_OK;
+}
+
+double fsp_model_bytes_per_field_solve(const fsp_plan* p, int with_phi) {
+    if (!p) return 0.0;
+    double k[FSP_NUM_SOLVE_KERNELS];
+    fsp_model_bytes_per_solve(p, k);
+    const double nout = with_phi ? 4.0 : 3.0;
+    return k[0] + k[1] + nout * (k[2] + k[3] + k[4]);
 }
 
 int fsp_destroy(fsp_plan* p) {

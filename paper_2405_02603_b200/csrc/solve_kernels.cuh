@@ -39,6 +39,14 @@ __device__ __forceinline__ void cmul_conj(double& xr, double& xi, const double2 
     xr = a;
 }
 
+// DER (field output, R18): the spectrum is additionally multiplied by -i k_d
+// (k_d = kap.d * m', m' the signed mode number, zero at the Nyquist index; exactly one of kap.x/y/z is
+// non-zero) and the result goes to `out` instead of back into B2, so that the forward data in B2 serve
+// phi and all three components of E = -grad phi.
+struct DerK { double x, y, z; int Nx; };
+
+__device__ __forceinline__ double signed_mode(int m, int N) { return m < N ? (double)m : (m == N ? 0.0 : (double)(m - 2 * N)); }
+
 // copy the twiddle table exp(-2 pi i n/LTAB) into shared memory
 template <int LTAB>
 __device__ __forceinline__ void load_table(double2* __restrict__ Ws, const double2* __restrict__ Wg) {
@@ -352,10 +360,10 @@ k_inv_y_t(const __grid_constant__ CUtensorMap tmB2, double2* __restrict__ B1, co
 // Gh: [pencil][2][M] doubles, plane 0 = Ghat[2j] (even), plane 1 = Ghat[2j+1] (odd), scale folded in.
 template <class Cfg> struct PencilGroups { static constexpr int P = (Cfg::T >= 128) ? 1 : 128 / Cfg::T; };
 
-template <int M>
+template <int M, bool DER = false>
 __global__ void __launch_bounds__(PencilGroups<FftCfg<M>>::P* FftCfg<M>::T)
 k_conv_z(double2* __restrict__ B2, const double* __restrict__ Gh, const double2* __restrict__ Wg,
-         long npencils) {
+         long npencils, double2* __restrict__ out, int Ny, const DerK kap) {
     using Cfg = FftCfg<M>;
     constexpr int R = Cfg::R, T = Cfg::T, P = PencilGroups<Cfg>::P, LTAB = 2 * M;
     extern __shared__ double2 smem[];
@@ -368,6 +376,12 @@ k_conv_z(double2* __restrict__ B2, const double* __restrict__ Gh, const double2*
     const long pencil = (long)blockIdx.x * P + c;
     const bool valid = pencil < npencils;
     double2* base = B2 + (valid ? pencil : 0) * M;
+    double2* obase = DER ? out + (valid ? pencil : 0) * M : base;
+    double fp = 0.0;
+    if constexpr (DER) {
+        const int kx = (int)((valid ? pencil : 0) / (2 * Ny)), ky = (int)((valid ? pencil : 0) % (2 * Ny));
+        fp = kap.x * signed_mode(kx, kap.Nx) + kap.y * signed_mode(ky, Ny);
+    }
     const double* ge = Gh + (valid ? pencil : 0) * 2 * M;
     const double* go = ge + M;
 
@@ -385,7 +399,15 @@ k_conv_z(double2* __restrict__ B2, const double* __restrict__ Gh, const double2*
     for (int i = 0; i < R; ++i) { vr[i] = xr[i]; vi[i] = xi[i]; cmul(vr[i], vi[i], Ws[t + T * i]); }
     fft_forward<Cfg, 1, LTAB>(vr, vi, t, buf, Ws);
 #pragma unroll
-    for (int i = 0; i < R; ++i) { vr[i] *= gg[i]; vi[i] *= gg[i]; }
+    for (int i = 0; i < R; ++i) {
+        if constexpr (DER) {   // -i f Ghat X = f Ghat (X.im - i X.re)
+            const double cf = gg[i] * (fp + kap.z * signed_mode(2 * (t + T * i) + 1, M));
+            const double a = vr[i];
+            vr[i] = cf * vi[i]; vi[i] = -cf * a;
+        } else {
+            vr[i] *= gg[i]; vi[i] *= gg[i];
+        }
+    }
 #pragma unroll
     for (int i = 0; i < R; ++i) gg[i] = ge[t + T * i];
     fft_inverse<Cfg, 1, LTAB>(vr, vi, t, buf, Ws);
@@ -394,11 +416,19 @@ k_conv_z(double2* __restrict__ B2, const double* __restrict__ Gh, const double2*
     // even half-spectrum
     fft_forward<Cfg, 1, LTAB>(xr, xi, t, buf, Ws);
 #pragma unroll
-    for (int i = 0; i < R; ++i) { xr[i] *= gg[i]; xi[i] *= gg[i]; }
+    for (int i = 0; i < R; ++i) {
+        if constexpr (DER) {
+            const double cf = gg[i] * (fp + kap.z * signed_mode(2 * (t + T * i), M));
+            const double a = xr[i];
+            xr[i] = cf * xi[i]; xi[i] = -cf * a;
+        } else {
+            xr[i] *= gg[i]; xi[i] *= gg[i];
+        }
+    }
     fft_inverse<Cfg, 1, LTAB>(xr, xi, t, buf, Ws);
     if (valid) {
 #pragma unroll
-        for (int i = 0; i < R; ++i) base[t + T * i] = make_double2(xr[i] + vr[i], xi[i] + vi[i]);
+        for (int i = 0; i < R; ++i) obase[t + T * i] = make_double2(xr[i] + vr[i], xi[i] + vi[i]);
     }
 }
 
@@ -435,10 +465,10 @@ struct ConvZ {
     }
 };
 
-template <int M>
+template <int M, bool DER = false>
 __global__ void __launch_bounds__(ConvZ<M>::WARPS * 32, (M >= 512 ? 2 : 3))
 k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double* __restrict__ lane_g,
-           const double2* __restrict__ wp_g, int Ny, long ngroups) {
+           const double2* __restrict__ wp_g, int Ny, long ngroups, double2* __restrict__ out, const DerK kap) {
     using Z = ConvZ<M>;
     using Cfg = typename Z::Cfg;
     constexpr int R = Z::R, T = Z::T, G = Z::G, WARPS = Z::WARPS, H = R / 2, NC = Z::NC, NB2 = Cfg::NB2;
@@ -472,6 +502,9 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
         const int ky = (r & 1) ? ny2 - ((r + 1) >> 1) : (r >> 1);
         const int qy = ky <= Ny ? ky : ny2 - ky;
         double2* base = B2 + ((long)kx * ny2 + ky) * M;
+        double2* obase = DER ? out + ((long)kx * ny2 + ky) * M : base;
+        double fp = 0.0;   // pencil-constant part of the derivative factor
+        if constexpr (DER) fp = kap.x * signed_mode(kx, kap.Nx) + kap.y * signed_mode(ky, Ny);
         const double* grow = Gk + ((long)kx * (Ny + 1) + qy) * Z::ROW + (b ? M / 2 + 1 : 0);
         if constexpr (Z::GSTAGE) {
             // all lanes are past the previous pencil's reads of gst (the shuffles of the final combine)
@@ -519,7 +552,13 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
                     const int j = t + T * i;
                     const int m = b ? (j < M - 1 - j ? j : M - 1 - j) : (j < M - j ? j : M - j);
                     const double gk = Z::GSTAGE ? gsrc[m] : __ldg(gsrc + m);
-                    vr[i] *= gk; vi[i] *= -gk;
+                    if constexpr (DER) {   // conj(-i f Ghat X) = f Ghat (X.im + i X.re)
+                        const double cf = gk * (fp + kap.z * signed_mode(2 * j + b, M));
+                        const double a = vr[i];
+                        vr[i] = cf * vi[i]; vi[i] = cf * a;
+                    } else {
+                        vr[i] *= gk; vi[i] *= -gk;
+                    }
                 }
             }
         }
@@ -537,7 +576,7 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
             const double2 w = wp[t + T * o];
             const double zr = fma(-w.y, qi, fma(w.x, qr, ar));
             const double zi = fma(w.y, qr, fma(w.x, qi, ai));
-            base[t + T * o] = make_double2(zr, -zi);
+            obase[t + T * o] = make_double2(zr, -zi);
         }
     }
 }

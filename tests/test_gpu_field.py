@@ -1,0 +1,152 @@
+"""-m gpu: field output E = -grad phi (R18) of the CUDA path,
+through the C ABI (fsp_solve_field), against the CPU oracle (orc_solve_field) element by element; at the
+full benchmark sizes against the FFT-free point-by-point reference (oracle.field_of_point_charges).
+Tolerances as for phi: relative L2 <= 1e-12, max-norm relative <= 1e-10."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2405_02603_b200 import binding, workloads as W
+from tests.analytic import gaussian_field_iso, rel_l2, rel_max
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+L2_TOL, MAX_TOL = 1e-12, 1e-10
+ALGS = {"HE": (binding.HOCKNEY, oracle.HOCKNEY), "VG2": (binding.VICO_2, oracle.VICO_2)}
+
+
+def gpu_field(plan, rho_np, want_phi=True):
+    rho = torch.from_numpy(rho_np).cuda()
+    phi, E = plan.solve_field(rho, want_phi=want_phi)
+    torch.cuda.synchronize()
+    return (phi.cpu().numpy() if want_phi else None), E.cpu().numpy()
+
+
+def check(got, ref):
+    assert np.isfinite(got).all()
+    assert rel_l2(got, ref) <= L2_TOL, f"rel L2 {rel_l2(got, ref):.3e}"
+    assert rel_max(got, ref) <= MAX_TOL, f"max rel {rel_max(got, ref):.3e}"
+
+
+@pytest.mark.parametrize("alg", ["HE", "VG2"])
+def test_config1_field_16(alg):
+    w = W.config1(16)
+    with binding.Plan(w.N, w.h, ALGS[alg][0]) as p:
+        phi, E = gpu_field(p.precompute_green(), w.rho)
+    phi_o, E_o = oracle.OraclePlan(w.N, w.h, ALGS[alg][1]).precompute_green().solve_field(w.rho)
+    check(phi, phi_o)
+    check(E, E_o)
+    for d in range(3):
+        check(E[d], E_o[d])
+
+
+@pytest.mark.parametrize("alg", ["HE", "VG2"])
+def test_config2_field_64_and_closed_form(alg):
+    """64^3, four signed Gaussians: parity, and accuracy against the superposed closed-form field."""
+    w = W.config2(64, 1)
+    with binding.Plan(w.N, w.h, ALGS[alg][0]) as p:
+        phi, E = gpu_field(p.precompute_green(), w.rho)
+    phi_o, E_o = oracle.OraclePlan(w.N, w.h, ALGS[alg][1]).precompute_green().solve_field(w.rho)
+    check(phi, phi_o)
+    check(E, E_o)
+    err = rel_l2(E, gaussian_field_iso(w))
+    assert err < (5e-2 if alg == "HE" else 2e-4), err   # VG: the box cuts the Gaussians' tails
+
+
+def test_centred_gaussian_field_reaches_round_off_with_vg_at_64():
+    w = W.config1(64)
+    with binding.Plan(w.N, w.h, binding.VICO_2) as p:
+        _, E = gpu_field(p.precompute_green(), w.rho, want_phi=False)
+    assert rel_l2(E, gaussian_field_iso(w)) < 1e-13
+
+
+@pytest.mark.parametrize("N", [(8, 8, 8), (16, 32, 128), (128, 16, 32), (64, 8, 256), (8, 256, 8), (256, 8, 8),
+                               (8, 8, 512), (8, 512, 8), (512, 8, 8), (8, 8, 1024), (8, 1024, 8), (128, 128, 16),
+                               (256, 256, 8), (16, 128, 64)])
+def test_field_random_density_every_fft_length(N):
+    """Dense random rho, anisotropic spacing: every kernel generation and transform length on every axis, so
+    that a wrong mode number on any path (signed index, Nyquist, even/odd branch) shows."""
+    w = W.random_density(N, seed=5)
+    with binding.Plan(w.N, w.h, binding.HOCKNEY) as p:
+        p.precompute_green()
+        phi, E = gpu_field(p, w.rho)
+        phi_plain = p.solve(torch.from_numpy(w.rho).cuda()).cpu().numpy()
+    assert np.array_equal(phi, phi_plain)   # the same kernels on the same data
+    phi_o, E_o = oracle.OraclePlan(w.N, w.h, oracle.HOCKNEY).precompute_green().solve_field(w.rho)
+    check(phi, phi_o)
+    check(E, E_o)
+    for d in range(3):
+        check(E[d], E_o[d])
+
+
+def test_field_without_phi_and_host_variant():
+    w = W.random_density((16, 8, 32), seed=8)
+    with binding.Plan(w.N, w.h, binding.VICO_2) as p:
+        p.precompute_green()
+        phi, E = gpu_field(p, w.rho)
+        none, E2 = gpu_field(p, w.rho, want_phi=False)
+        assert none is None and np.array_equal(E, E2)
+        phi_h, E_h = np.empty_like(w.rho), np.empty((3,) + w.N)
+        p.solve_field_host(np.ascontiguousarray(w.rho), phi_h, E_h)
+        assert np.array_equal(phi_h, phi) and np.array_equal(E_h, E)
+        E_h2 = np.empty((3,) + w.N)
+        p.solve_field_host(np.ascontiguousarray(w.rho), None, E_h2)
+        assert np.array_equal(E_h2, E)
+
+
+def test_field_argument_errors():
+    with binding.Plan((8, 8, 8), (0.1,) * 3, binding.HOCKNEY) as p:
+        rho = torch.zeros((8, 8, 8), dtype=torch.float64, device="cuda")
+        E = torch.zeros((3, 8, 8, 8), dtype=torch.float64, device="cuda")
+        with pytest.raises(binding.FspError) as e:
+            binding.solve_field(p.handle, rho, None, E)
+        assert e.value.code == -2
+        p.precompute_green()
+        with pytest.raises(binding.FspError) as e:
+            binding.solve_field(p.handle, rho, None, 0)
+        assert e.value.code == -1
+
+
+@pytest.mark.parametrize("name", ["256", "beam", "512"])
+def test_full_size_field_of_point_charges(name):
+    """BASELINE.json configs 3-5 in the launch configuration bench.py times: a handful of seeded point charges,
+    E at 150 sampled mesh points against the FFT-free definition (oracle.field_of_point_charges) evaluated on
+    the oracle's own table near the charges' lines -- here the GPU's exported table, whose parity with the
+    oracle's is tests/test_gpu_parity.py's table test."""
+    N = {"256": (256, 256, 256), "beam": (128, 128, 512), "512": (512, 512, 512)}[name]
+    lo, hi = ((-0.5, -0.5, -0.5), (0.5, 0.5, 0.5)) if name != "beam" else ((-0.5, -0.5, -2.0), (0.5, 0.5, 2.0))
+    h = tuple((hi[d] - lo[d]) / N[d] for d in range(3))
+    rng = np.random.default_rng(17)
+    charges = [(tuple(int(rng.integers(0, N[d])) for d in range(3)), float(rng.uniform(0.5, 1.5) * rng.choice([-1, 1])))
+               for _ in range(4)]
+    charges.append(((0, N[1] - 1, N[2] // 2), 1.0))
+    pts = np.stack([rng.integers(0, N[d], size=150) for d in range(3)], axis=1)
+    pts[0] = (0, 0, 0)
+    pts[1] = (N[0] - 1, N[1] - 1, N[2] - 1)
+    pts[2] = charges[0][0]
+    k = 3   # near field: a few cells around every charge (clipped to the mesh)
+    for y, _ in charges:
+        for off in ((1, 0, 0), (0, -2, 1), (-1, 1, -3), (2, 2, 2), (0, 0, -1), (-3, 0, 2)):
+            pts[k] = [min(max(y[d] + off[d], 0), N[d] - 1) for d in range(3)]
+            k += 1
+    rho = torch.zeros(N, dtype=torch.float64, device="cuda")
+    for y, q in charges:
+        rho[y] = q
+    with binding.Plan(N, h, binding.HOCKNEY) as p:
+        p.precompute_green()
+        T = p.green_table()
+        _, E = p.solve_field(rho, want_phi=False)
+        torch.cuda.synchronize()
+        ip = torch.from_numpy(pts).cuda()
+        got = E[:, ip[:, 0], ip[:, 1], ip[:, 2]].T.cpu().numpy()
+        scale = float(E.abs().max())
+    del E, rho
+    torch.cuda.empty_cache()
+    ref = oracle.field_of_point_charges(T, h, charges, pts)
+    assert np.abs(got - ref).max() <= MAX_TOL * scale, np.abs(got - ref).max() / scale
+    # the field of point charges spans many decades (far-field samples ~1e-4 of the maximum): round-off scales
+    # with the field maximum (R14), so the L2 bound is on the rms error relative to it
+    assert np.linalg.norm(got - ref) / np.sqrt(got.size) <= L2_TOL * scale
+    far = np.abs(ref) > 1e-3 * scale
+    assert far.sum() > 10 and np.abs(got - ref)[far].max() <= 1e-9 * np.abs(ref)[far].min()

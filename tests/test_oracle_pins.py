@@ -468,3 +468,18 @@ def test_field_closed_form_he_second_order_vg_spectral():
             err[name, n] = rel_l2(E, ref)
     assert 3.3 < err["HE", 16] / err["HE", 32] < 4.6 and 3.3 < err["HE", 32] / err["HE", 64] < 4.6, err
     assert err["VG", 16] < 3e-2 and err["VG", 32] < 2e-6 and err["VG", 64] < 1e-13, err
+
+
+def test_field_of_point_charges_matches_fft_path():
+    """The FFT-free point-by-point field (used for full-size GPU parity) against orc_solve_field."""
+    N, h = (8, 4, 16), (0.1, 0.2, 0.05)
+    T = oracle.green_table(oracle.HOCKNEY, N, h)
+    charges = [((1, 2, 3), 1.5), ((7, 0, 15), -0.75), ((4, 3, 8), 2.0)]
+    rho = np.zeros(N)
+    for y, q in charges:
+        rho[y] = q
+    _, E = oracle.solve_field_with_spectrum(oracle.green_spectrum(T), h, rho)
+    pts = np.array([(0, 0, 0), (7, 3, 15), (1, 2, 3), (4, 1, 9), (6, 2, 0)])
+    got = oracle.field_of_point_charges(T, h, charges, pts)
+    ref = np.stack([E[:, p[0], p[1], p[2]] for p in pts])
+    assert np.abs(got - ref).max() < 1e-12 * np.abs(E).max()
