@@ -127,8 +127,9 @@ int fsp_solve_host(fsp_plan* p, const double* rho_host, double* phi_host);
  *   rho_dev  device pointer, Nx*Ny*Nz doubles, read-only
  *   phi_dev  device pointer, Nx*Ny*Nz doubles, or NULL if the potential is not wanted
  *   E_dev    device pointer, 3*Nx*Ny*Nz doubles, component-major: E_dev[d*V + (ix*Ny+iy)*Nz+iz], d = x,y,z
- * The two forward passes run once; each output runs the middle pass (with the factor -i k_d fused
- * into the spectrum multiply) and the two inverse passes: 2 + 3*3 (+3) kernel launches.  The first
+ * The factor -i k_d is fused into the pass that transforms axis d (the spectrum multiply of the middle
+ * pass for z, the input of the inverse y pass, the input of the inverse x pass), and everything before
+ * that pass is shared: 2 forward + 2 middle + 3 inverse-y + 3 (+1 for phi) inverse-x launches.  The first
  * call allocates one more plan-owned intermediate the size of the larger workspace array (counted by
  * fsp_plan_bytes from then on).  FSP_PARAM_CHUNK_PLANES does not apply.  Asynchronous like fsp_solve.
  */
@@ -152,8 +153,8 @@ size_t fsp_precompute_peak_bytes(const fsp_plan* p);
  * if per_kernel (host pointer to FSP_NUM_SOLVE_KERNELS doubles) is not NULL. */
 double fsp_model_bytes_per_solve(const fsp_plan* p, double* per_kernel);
 
-/* Algorithmic HBM bytes of one fsp_solve_field: the two forward passes once, the middle pass and the
- * two inverse passes once per output (3 components, + phi if with_phi != 0). */
+/* Algorithmic HBM bytes of one fsp_solve_field: K1 + K2 + 2 K3 + 3 K4 + (3 or 4) K5 in the per-kernel
+ * figures of fsp_model_bytes_per_solve (4 K5 if with_phi != 0). */
 double fsp_model_bytes_per_field_solve(const fsp_plan* p, int with_phi);
 
 /* Oversampling factors (m_x, m_y, m_z) used by the last fsp_precompute_green of a VG algorithm

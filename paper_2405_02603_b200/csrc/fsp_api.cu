@@ -229,22 +229,27 @@ int launch_fwd_y(fsp_plan* p, const double2* B1, double2* B2, int nplanes) {
     k_fwd_y<M><<<(unsigned)grid, G * kW * Cfg::T, smem, p->stream>>>(B1, B2, p->Wy, p->Nz, ntiles);
     return FSP_OK;
 }
-template <int M>
-int launch_inv_y(fsp_plan* p, const double2* B2, double2* B1, int nplanes) {
+template <int M, bool DER>
+int launch_inv_y_impl(fsp_plan* p, const double2* B2, double2* B1, int nplanes, double kder) {
     using Cfg = FftCfg<M>;
     constexpr int G = TileGroups<Cfg>::G;
     const long ntiles = (long)nplanes * (p->Nz / kW);
     const size_t smem = sizeof(double2) * (size_t)(2 * M + G * M * kW);
     static int occ = 0;
     if (occ == 0) {
-        CU(cudaFuncSetAttribute(k_inv_y<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_inv_y<M>, G * kW * Cfg::T, smem));
+        CU(cudaFuncSetAttribute(k_inv_y<M, DER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_inv_y<M, DER>, G * kW * Cfg::T, smem));
         if (occ < 1) return FSP_ERR_CUDA;
     }
     long grid = (ntiles + G - 1) / G;
     if (grid > (long)p->sm_count * occ) grid = (long)p->sm_count * occ;
-    k_inv_y<M><<<(unsigned)grid, G * kW * Cfg::T, smem, p->stream>>>(B2, B1, p->Wy, p->Nz, ntiles);
+    k_inv_y<M, DER><<<(unsigned)grid, G * kW * Cfg::T, smem, p->stream>>>(B2, B1, p->Wy, p->Nz, ntiles, kder);
     return FSP_OK;
+}
+// kder != 0: the E_y variant (input rows times -i kder m'(ky))
+template <int M>
+int launch_inv_y(fsp_plan* p, const double2* B2, double2* B1, int nplanes, double kder) {
+    return kder != 0.0 ? launch_inv_y_impl<M, true>(p, B2, B1, nplanes, kder) : launch_inv_y_impl<M, false>(p, B2, B1, nplanes, 0.0);
 }
 // DER = false: in place on B2.  DER = true: B2 -> out with the factor -i k_d of `kap` (field output).
 template <int M, bool DER>
@@ -294,15 +299,20 @@ int launch_fwd_x(fsp_plan* p, const double* rho) {
     k_fwd_x_r2c<M><<<(unsigned)((ntiles + G - 1) / G), G * kW * Cfg::T, smem, p->stream>>>(rho, p->B1, p->Wx, p->Ny, p->Nz, ntiles);
     return FSP_OK;
 }
-template <int M>
-int launch_inv_x(fsp_plan* p, double* phi) {
+template <int M, bool DER>
+int launch_inv_x_impl(fsp_plan* p, double* phi, double kder) {
     using Cfg = FftCfg<M>;
     constexpr int G = TileGroups<Cfg>::G;
     const long ntiles = (long)p->Ny * (p->Nz / kW);
     const size_t smem = sizeof(double2) * (size_t)(4 * M + G * M * kW);
-    CU(cudaFuncSetAttribute(k_inv_x_c2r<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_inv_x_c2r<M><<<(unsigned)((ntiles + G - 1) / G), G * kW * Cfg::T, smem, p->stream>>>(p->B1, phi, p->Wx, p->Ny, p->Nz, ntiles);
+    CU(cudaFuncSetAttribute(k_inv_x_c2r<M, DER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_inv_x_c2r<M, DER><<<(unsigned)((ntiles + G - 1) / G), G * kW * Cfg::T, smem, p->stream>>>(p->B1, phi, p->Wx, p->Ny, p->Nz, ntiles, kder);
     return FSP_OK;
+}
+// kder != 0: the E_x variant (X[k] times -i kder k)
+template <int M>
+int launch_inv_x(fsp_plan* p, double* phi, double kder) {
+    return kder != 0.0 ? launch_inv_x_impl<M, true>(p, phi, kder) : launch_inv_x_impl<M, false>(p, phi, 0.0);
 }
 
 #define DISPATCH_YZ(fn, M, ...)                          \
@@ -392,55 +402,63 @@ int do_conv_z(fsp_plan* p, double2* B2, int kx0, int np, double2* out = nullptr,
 int make_z_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Nz, &p->LTz, &p->bytes) }
 int make_x_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Nx / 2, &p->LTx, &p->bytes) }
 int make_y_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Ny, &p->LTy, &p->bytes) }
-template <int M>
-int launch_inv_y_t(fsp_plan* p, const CUtensorMap& tm, double2* B1, int nplanes) {
+template <int M, bool DER>
+int launch_inv_y_t_impl(fsp_plan* p, const CUtensorMap& tm, double2* B1, int nplanes, double kder) {
     using Y = TileYI<M>;
     const long ntiles = (long)nplanes * (p->Nz / kW);
     const size_t smem = Y::smem_bytes();
     static int occ = 0;
     if (occ == 0) {
-        CU(cudaFuncSetAttribute(k_inv_y_t<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_inv_y_t<M>, Y::THREADS, smem));
+        CU(cudaFuncSetAttribute(k_inv_y_t<M, DER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_inv_y_t<M, DER>, Y::THREADS, smem));
         if (occ < 1) return FSP_ERR_CUDA;
     }
     long grid = (long)p->sm_count * occ;
     if (grid > ntiles) grid = ntiles;
-    k_inv_y_t<M><<<(unsigned)grid, Y::THREADS, smem, p->stream>>>(tm, B1, p->LTy, p->Wy, p->Nz, ntiles);
+    k_inv_y_t<M, DER><<<(unsigned)grid, Y::THREADS, smem, p->stream>>>(tm, B1, p->LTy, p->Wy, p->Nz, ntiles, kder);
     return FSP_OK;
 }
+template <int M>
+int launch_inv_y_t(fsp_plan* p, const CUtensorMap& tm, double2* B1, int nplanes, double kder) {
+    return kder != 0.0 ? launch_inv_y_t_impl<M, true>(p, tm, B1, nplanes, kder) : launch_inv_y_t_impl<M, false>(p, tm, B1, nplanes, 0.0);
+}
 // B2 must be the plan's own B2 (the tile kernel reads it through the plan's tensor map)
-int do_inv_y(fsp_plan* p, const double2* B2, double2* B1, int np) {
+int do_inv_y(fsp_plan* p, const double2* B2, double2* B1, int np, double kder = 0.0) {
     if (p->tile_y && (B2 == p->B2 || (p->B3 && B2 == p->B3))) {
         const CUtensorMap& tm = B2 == p->B2 ? p->tmB2y : p->tmB3y;
-        if (p->Ny == 512) return launch_inv_y_t<512>(p, tm, B1, np);
-        if (p->Ny == 256) return launch_inv_y_t<256>(p, tm, B1, np);
-        return launch_inv_y_t<128>(p, tm, B1, np);
+        if (p->Ny == 512) return launch_inv_y_t<512>(p, tm, B1, np, kder);
+        if (p->Ny == 256) return launch_inv_y_t<256>(p, tm, B1, np, kder);
+        return launch_inv_y_t<128>(p, tm, B1, np, kder);
     }
-    DISPATCH_YZ(launch_inv_y, p->Ny, p, B2, B1, np)
+    DISPATCH_YZ(launch_inv_y, p->Ny, p, B2, B1, np, kder)
 }
-template <int M>
-int launch_inv_x_t(fsp_plan* p, double* phi) {
+template <int M, bool DER>
+int launch_inv_x_t_impl(fsp_plan* p, double* phi, double kder) {
     using X_ = TileXI<M>;
     const long plane = (long)p->Ny * p->Nz, ntiles = plane / kC;
     const size_t smem = X_::smem_bytes();
     static int occ = 0;
     if (occ == 0) {
-        CU(cudaFuncSetAttribute(k_inv_x_t<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_inv_x_t<M>, X_::THREADS, smem));
+        CU(cudaFuncSetAttribute(k_inv_x_t<M, DER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_inv_x_t<M, DER>, X_::THREADS, smem));
         if (occ < 1) return FSP_ERR_CUDA;
     }
     long grid = (long)p->sm_count * occ;
     if (grid > ntiles) grid = ntiles;
-    k_inv_x_t<M><<<(unsigned)grid, X_::THREADS, smem, p->stream>>>(p->tmB1x, p->B1, phi, p->LTx, p->Wx, plane, ntiles);
+    k_inv_x_t<M, DER><<<(unsigned)grid, X_::THREADS, smem, p->stream>>>(p->tmB1x, p->B1, phi, p->LTx, p->Wx, plane, ntiles, kder);
     return FSP_OK;
 }
-int do_inv_x(fsp_plan* p, double* phi) {
+template <int M>
+int launch_inv_x_t(fsp_plan* p, double* phi, double kder) {
+    return kder != 0.0 ? launch_inv_x_t_impl<M, true>(p, phi, kder) : launch_inv_x_t_impl<M, false>(p, phi, 0.0);
+}
+int do_inv_x(fsp_plan* p, double* phi, double kder = 0.0) {
     if (p->tile_x) {
-        if (p->Nx == 512) return launch_inv_x_t<256>(p, phi);
-        if (p->Nx == 256) return launch_inv_x_t<128>(p, phi);
-        return launch_inv_x_t<64>(p, phi);
+        if (p->Nx == 512) return launch_inv_x_t<256>(p, phi, kder);
+        if (p->Nx == 256) return launch_inv_x_t<128>(p, phi, kder);
+        return launch_inv_x_t<64>(p, phi, kder);
     }
-    DISPATCH_X(launch_inv_x, p->Nx / 2, p, phi)
+    DISPATCH_X(launch_inv_x, p->Nx / 2, p, phi, kder)
 }
 
 unsigned grid_for(long total, int block) {
@@ -790,20 +808,24 @@ int fsp_solve_field(fsp_plan* p, const double* rho_dev, double* phi_dev, double*
     // forward passes once: B2 = F_y F_x rho2
     if ((rc = do_fwd_x(p, rho_dev)) != FSP_OK) return rc;
     if ((rc = do_fwd_y(p, 0, p->B2, planes)) != FSP_OK) return rc;
-    // E_d: K3 with the factor -i k_d (B2 -> B3), then the inverse passes (R18)
-    for (int d = 0; d < 3; ++d) {
-        const int Nd = d == 0 ? p->Nx : (d == 1 ? p->Ny : p->Nz);
-        const double kd = 2.0 * PI / (2.0 * (double)Nd * p->h[d]);
-        const DerK kap{d == 0 ? kd : 0.0, d == 1 ? kd : 0.0, d == 2 ? kd : 0.0, p->Nx};
-        if ((rc = do_conv_z(p, p->B2, 0, planes, p->B3, &kap)) != FSP_OK) return rc;
-        if ((rc = do_inv_y(p, p->B3, p->B1, planes)) != FSP_OK) return rc;
-        if ((rc = do_inv_x(p, E_dev + (size_t)d * V)) != FSP_OK) return rc;
-    }
-    if (phi_dev) {   // phi last: its K3 runs in place and consumes the forward data
-        if ((rc = do_conv_z(p, p->B2, 0, planes)) != FSP_OK) return rc;
-        if ((rc = do_inv_y(p, p->B2, p->B1, planes)) != FSP_OK) return rc;
-        if ((rc = do_inv_x(p, phi_dev)) != FSP_OK) return rc;
-    }
+    // The factor -i k_d (R18) commutes with the inverse passes along the other axes, so it is
+    // applied in the pass that transforms ITS axis and everything before that pass is shared:
+    const double kx = 2.0 * PI / (2.0 * (double)p->Nx * p->h[0]);
+    const double ky = 2.0 * PI / (2.0 * (double)p->Ny * p->h[1]);
+    const double kz = 2.0 * PI / (2.0 * (double)p->Nz * p->h[2]);
+    // E_z: K3 with the factor fused into the spectrum multiply (B2 -> B3), K4, K5
+    const DerK kap{0.0, 0.0, kz, p->Nx};
+    if ((rc = do_conv_z(p, p->B2, 0, planes, p->B3, &kap)) != FSP_OK) return rc;
+    if ((rc = do_inv_y(p, p->B3, p->B1, planes)) != FSP_OK) return rc;
+    if ((rc = do_inv_x(p, E_dev + 2 * V)) != FSP_OK) return rc;
+    // phi and E_x: plain K3 (in place), K4, then K5 twice on the same B1 (plain, and with -i kx on its input)
+    if ((rc = do_conv_z(p, p->B2, 0, planes)) != FSP_OK) return rc;
+    if ((rc = do_inv_y(p, p->B2, p->B1, planes)) != FSP_OK) return rc;
+    if (phi_dev && (rc = do_inv_x(p, phi_dev)) != FSP_OK) return rc;
+    if ((rc = do_inv_x(p, E_dev, kx)) != FSP_OK) return rc;
+    // E_y: K4 with -i ky on its input rows (B2 still holds the output of the plain K3), K5
+    if ((rc = do_inv_y(p, p->B2, p->B1, planes, ky)) != FSP_OK) return rc;
+    if ((rc = do_inv_x(p, E_dev + V)) != FSP_OK) return rc;
     CU(cudaGetLastError());
     return FSP_OK;
 }
@@ -830,8 +852,7 @@ double fsp_model_bytes_per_field_solve(const fsp_plan* p, int with_phi) {
     if (!p) return 0.0;
     double k[FSP_NUM_SOLVE_KERNELS];
     fsp_model_bytes_per_solve(p, k);
-    const double nout = with_phi ? 4.0 : 3.0;
-    return k[0] + k[1] + nout * (k[2] + k[3] + k[4]);
+    return k[0] + k[1] + 2.0 * k[2] + 3.0 * k[3] + (with_phi ? 4.0 : 3.0) * k[4];
 }
 
 int fsp_destroy(fsp_plan* p) {

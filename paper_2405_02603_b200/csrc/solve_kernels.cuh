@@ -45,6 +45,9 @@ __device__ __forceinline__ void cmul_conj(double& xr, double& xi, const double2 
 // phi and all three components of E = -grad phi.
 struct DerK { double x, y, z; int Nx; };
 
+// x <- (-i c) x
+__device__ __forceinline__ void mul_minus_i(double& xr, double& xi, const double c) { const double a = xr; xr = c * xi; xi = -c * a; }
+
 __device__ __forceinline__ double signed_mode(int m, int N) { return m < N ? (double)m : (m == N ? 0.0 : (double)(m - 2 * N)); }
 
 // copy the twiddle table exp(-2 pi i n/LTAB) into shared memory
@@ -198,10 +201,11 @@ k_fwd_y_t(const __grid_constant__ CUtensorMap tmB1, double2* __restrict__ B2, co
 }
 
 // ====================================================================================== K4: inv_y
-template <int M>
+// DER: input row ky is multiplied by -i kder m'(ky) first (E_y of the field output, see DerK)
+template <int M, bool DER = false>
 __global__ void __launch_bounds__(TileGroups<FftCfg<M>>::G* kW* FftCfg<M>::T)
 k_inv_y(const double2* __restrict__ B2, double2* __restrict__ B1, const double2* __restrict__ Wg,
-        int Nz, long ntiles) {
+        int Nz, long ntiles, const double kder) {
     using Cfg = FftCfg<M>;
     constexpr int R = Cfg::R, T = Cfg::T, G = TileGroups<Cfg>::G, LTAB = 2 * M;
     extern __shared__ double2 smem[];
@@ -229,6 +233,10 @@ k_inv_y(const double2* __restrict__ B2, double2* __restrict__ B1, const double2*
             double2 a = valid ? in[row * Nz] : make_double2(0.0, 0.0);
             double2 b = valid ? in[(row + 1) * Nz] : make_double2(0.0, 0.0);
             er[i] = a.x; ei[i] = a.y; qr[i] = b.x; qi[i] = b.y;
+            if constexpr (DER) {
+                mul_minus_i(er[i], ei[i], kder * signed_mode((int)row, M));
+                mul_minus_i(qr[i], qi[i], kder * signed_mode((int)row + 1, M));
+            }
         }
         {
             const long tn = tile + (long)gridDim.x * G;
@@ -270,10 +278,10 @@ struct TileYI {
     static constexpr size_t smem_bytes() { return 128 + sizeof(double2) * (size_t)(3 * M * kW + M); }
 };
 
-template <int M>
+template <int M, bool DER = false>
 __global__ void __launch_bounds__(TileYI<M>::THREADS, TileYI<M>::MINB)
 k_inv_y_t(const __grid_constant__ CUtensorMap tmB2, double2* __restrict__ B1, const double* __restrict__ lane_g,
-          const double2* __restrict__ wp_g, int Nz, long ntiles) {
+          const double2* __restrict__ wp_g, int Nz, long ntiles, const double kder) {
     using Y = TileYI<M>;
     using Cfg = typename Y::Cfg;
     constexpr int R = Y::R, T = Y::T, GT = Y::GT, NC = Y::NC, NB2 = Cfg::NB2, H = R / 2;
@@ -326,6 +334,7 @@ k_inv_y_t(const __grid_constant__ CUtensorMap tmB2, double2* __restrict__ B1, co
         for (int i = 0; i < R; ++i) {
             const double2 v = Ec[(t + T * i) * kW];
             vr[i] = v.x; vi[i] = v.y;
+            if constexpr (DER) mul_minus_i(vr[i], vi[i], kder * signed_mode(2 * (t + T * i) + grp, M));
         }
         // inverse transform = forward transform with the roles of re and im swapped; the first barrier
         // inside also separates the reads of X_g above from its reuse as exchange buffer
@@ -740,10 +749,11 @@ struct TileXI {
     static constexpr size_t smem_bytes() { return 128 + sizeof(double2) * (size_t)(kC + 3 * M * kC); }
 };
 
-template <int M>
+// DER: X[k] is multiplied by -i kder k first (zero at the Nyquist index k = Nx): E_x of the field output
+template <int M, bool DER = false>
 __global__ void __launch_bounds__(TileXI<M>::THREADS, TileXI<M>::MINB)
 k_inv_x_t(const __grid_constant__ CUtensorMap tmB1, const double2* __restrict__ B1, double* __restrict__ phi,
-          const double* __restrict__ lane_g, const double2* __restrict__ Wg, long plane, long ntiles) {
+          const double* __restrict__ lane_g, const double2* __restrict__ Wg, long plane, long ntiles, const double kder) {
     using X_ = TileXI<M>;
     using Cfg = typename X_::Cfg;
     constexpr int R = X_::R, T = X_::T, GT = X_::GT, NC = X_::NC, NB2 = Cfg::NB2, N = 2 * M, H = R / 2;
@@ -793,10 +803,15 @@ k_inv_x_t(const __grid_constant__ CUtensorMap tmB1, const double2* __restrict__ 
         UntangleFwd<M>::run([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             const int j = t + T * i;
-            const double2 a = Ec[j * kC];
+            double2 a = Ec[j * kC];
             double2 bq;
             if (grp) bq = Ec[(M - 1 - j) * kC];
             else bq = (j == 0) ? XN[c] : Ec[(M - j) * kC];
+            if constexpr (DER) {
+                const int k = 2 * j + grp;
+                mul_minus_i(a.x, a.y, kder * (double)k);
+                mul_minus_i(bq.x, bq.y, k == 0 ? 0.0 : kder * (double)(N - k));
+            }
             const double br = bq.x, bi = -bq.y;
             const double sr = a.x + br, si = a.y + bi;
             double dr = a.x - br, di = a.y - bi;
@@ -903,10 +918,10 @@ k_fwd_x_r2c(const double* __restrict__ rho, double2* __restrict__ B1, const doub
 }
 
 // ================================================================================== K5: inv_x_c2r
-template <int M>
+template <int M, bool DER = false>
 __global__ void __launch_bounds__(TileGroups<FftCfg<M>>::G* kW* FftCfg<M>::T)
 k_inv_x_c2r(const double2* __restrict__ B1, double* __restrict__ phi, const double2* __restrict__ Wg,
-            int Ny, int Nz, long ntiles) {
+            int Ny, int Nz, long ntiles, const double kder) {
     using Cfg = FftCfg<M>;
     constexpr int R = Cfg::R, T = Cfg::T, G = TileGroups<Cfg>::G, LTAB = 4 * M, N = 2 * M;
     extern __shared__ double2 smem[];
@@ -933,8 +948,12 @@ k_inv_x_c2r(const double2* __restrict__ B1, double* __restrict__ phi, const doub
 #pragma unroll
         for (int o = 0; o < 2; ++o) {
             const int k = 2 * (t + T * i) + o;
-            const double2 a = valid ? in[(long)k * plane] : make_double2(0.0, 0.0);
-            const double2 bq = valid ? in[(long)(N - k) * plane] : make_double2(0.0, 0.0);
+            double2 a = valid ? in[(long)k * plane] : make_double2(0.0, 0.0);
+            double2 bq = valid ? in[(long)(N - k) * plane] : make_double2(0.0, 0.0);
+            if constexpr (DER) {
+                mul_minus_i(a.x, a.y, kder * (double)k);
+                mul_minus_i(bq.x, bq.y, k == 0 ? 0.0 : kder * (double)(N - k));
+            }
             const double br = bq.x, bi = -bq.y;
             const double sr = a.x + br, si = a.y + bi;
             double dr = a.x - br, di = a.y - bi;
