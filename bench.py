@@ -411,6 +411,35 @@ def extras(args, peak):
                                      "frac_of_measured_peak": model_total / (ms * 1e-3) / 1e9 / peak,
                                      "precompute_green_s": t_pre, "rel_l2_vs_closed_form": _analytic_error(w, phi)}
         del rho, phi
+    # field output: phi and E = -grad phi in one call, against 4 separate solves' worth of work
+    for wname in ("256", args.workload):
+        _, builder, kw, wdesc = WORKLOADS[wname]
+        w = getattr(W, builder)(**kw)
+        V = int(np.prod(w.N))
+        torch.cuda.empty_cache()
+        with binding.Plan(w.N, w.h, binding.VICO_2) as plan:
+            plan.precompute_green()
+            rho = torch.from_numpy(w.rho).cuda()
+            phi = torch.empty_like(rho)
+            E = torch.empty((3,) + tuple(w.N), dtype=torch.float64, device="cuda")
+            steps = 50 if V <= 256 ** 3 else max(5, args.steps // 4)
+            for _ in range(5):
+                plan.solve_field(rho, phi, E)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(steps):
+                plan.solve_field(rho, phi, E)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / steps
+            model = binding.model_bytes_per_field_solve(plan.handle, True)
+            out[f"field_{wname}_VG2"] = {"workload": wdesc, "what": "fsp_solve_field: phi + E (3 components), 11 launches",
+                                         "ms_per_field_solve": ms, "field_solves_per_s": 1e3 / ms, "steps": steps,
+                                         "model_gbs": model / (ms * 1e-3) / 1e9,
+                                         "frac_of_measured_peak": model / (ms * 1e-3) / 1e9 / peak,
+                                         "plan_bytes": plan.bytes}
+        del rho, phi, E
     for wname, steps in (("256", 20), ("512", 5)):
         try:
             torch.cuda.empty_cache()
