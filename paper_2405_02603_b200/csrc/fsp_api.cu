@@ -475,6 +475,26 @@ int dct1_axis(fsp_plan* p, const double* in, double* out, const long in_dims[3],
     const int o1 = (axis + 1) % 3, o2 = (axis + 2) % 3;
     const long n1 = in_dims[o1], n2 = in_dims[o2];
     const int Lf = 2 * n;
+    {   // tile kernel: C pencils per CTA along the contiguous dimension (z; y when the transform axis is z)
+        const int bdim = axis == 2 ? 1 : 2, adim = axis == 2 ? 0 : (axis == 0 ? 1 : 0);
+        const long nA = in_dims[adim], nB = in_dims[bdim];
+        auto tile_smem = [&](int C) { return sizeof(double2) * ((size_t)n + (size_t)C * Lf); };
+        const long args_in[3] = {is[adim], is[bdim], is[axis]}, args_out[3] = {os[adim], os[bdim], os[axis]};
+        if (tile_smem(8) <= 72 * 1024) {   // at least 3 CTAs per SM: the stages are latency-bound
+            CU(cudaFuncSetAttribute(k_dct1_tile<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_smem(8)));
+            k_dct1_tile<8><<<(unsigned)(nA * ((nB + 7) / 8)), 512, tile_smem(8), p->stream>>>(
+                in, out, n, nout, nB, args_in[0], args_in[1], args_in[2], args_out[0], args_out[1], args_out[2], scale);
+            CU(cudaGetLastError());
+            return FSP_OK;
+        }
+        if (tile_smem(4) <= 200 * 1024) {
+            CU(cudaFuncSetAttribute(k_dct1_tile<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_smem(4)));
+            k_dct1_tile<4><<<(unsigned)(nA * ((nB + 3) / 4)), tile_smem(4) <= 76 * 1024 ? 256 : 1024, tile_smem(4), p->stream>>>(
+                in, out, n, nout, nB, args_in[0], args_in[1], args_in[2], args_out[0], args_out[1], args_out[2], scale);
+            CU(cudaGetLastError());
+            return FSP_OK;
+        }
+    }
     const size_t smem = sizeof(double2) * 2 * (size_t)Lf;
     CU(cudaFuncSetAttribute(k_dct1_pencils, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int threads = Lf / 2 < 256 ? (Lf / 2 < 32 ? 32 : Lf / 2) : 256;

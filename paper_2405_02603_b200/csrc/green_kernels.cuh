@@ -119,6 +119,72 @@ __global__ void k_dct1_pencils(const double* __restrict__ in, double* __restrict
     for (int d = threadIdx.x; d < nout; d += blockDim.x) dst[(long)d * sa_out] = scale * r[d].x;
 }
 
+// The same DCT-I for a TILE of C adjacent pencils per CTA (C even): pencils (a, b0 .. b0+C-1) of an
+// nA x nB pencil grid; element k of pencil (a, b) at in[a*sA + b*sB + k*sK].  Two things make it several
+// times faster than k_dct1_pencils: (1) two real-even pencils are packed as the real and imaginary part of
+// ONE complex sequence -- both transforms are real, so they come out as Re and Im of the result; (2) the
+// tile is chosen along the contiguous dimension, so that global accesses are full sectors; the twiddles
+// come from a shared-memory table filled once per CTA.  Shared memory: [tw: Lf/2][a: C/2*Lf][b: C/2*Lf].
+template <int C>
+__global__ void k_dct1_tile(const double* __restrict__ in, double* __restrict__ out, int n, int nout,
+                            long nB, long sA_in, long sB_in, long sK_in, long sA_out, long sB_out,
+                            long sK_out, double scale) {
+    extern __shared__ double2 sm[];
+    const int Lf = 2 * n, half = n, S = C / 2;
+    double2* tw = sm;
+    double2* a = sm + half;
+    double2* b = a + (long)S * Lf;
+    const long tilesB = (nB + C - 1) / C;
+    const long ia = blockIdx.x / tilesB, b0 = (blockIdx.x % tilesB) * C;
+    const int nc = (int)(nB - b0 < C ? nB - b0 : C);   // pencils of this tile
+    const double* src = in + ia * sA_in + b0 * sB_in;
+    double* dst = out + ia * sA_out + b0 * sB_out;
+    for (int k = threadIdx.x; k < half; k += blockDim.x) {
+        double sn, cs;
+        sincospi((double)k / (double)half, &sn, &cs);   // exp(+2 pi i k / Lf)
+        tw[k] = make_double2(cs, sn);
+    }
+    double* af = reinterpret_cast<double*>(a);
+    // load with the even extension: position m and Lf - m both hold input k
+    const int total = (n + 1) * C;
+    for (int e = threadIdx.x; e < total; e += blockDim.x) {
+        int k, c;
+        if (sK_in == 1) { k = e % (n + 1); c = e / (n + 1); }   // contiguous transform axis: k fastest
+        else { c = e % C; k = e / C; }                          // strided axis: pencils fastest
+        const double v = c < nc ? src[(long)c * sB_in + (long)k * sK_in] : 0.0;
+        const long sq = (long)(c >> 1) * Lf;
+        af[2 * (sq + k) + (c & 1)] = v;
+        if (k > 0 && k < n) af[2 * (sq + Lf - k) + (c & 1)] = v;
+    }
+    // radix-2 Stockham, all S sequences together
+    for (int Ns = 1; Ns < Lf; Ns <<= 1) {
+        __syncthreads();
+        const int tstep = half / Ns;
+        for (int e = threadIdx.x; e < S * half; e += blockDim.x) {
+            const int q = e / half, j = e - q * half;
+            const int k = j & (Ns - 1);
+            const double2 w = tw[k * tstep];
+            const double2* aq = a + (long)q * Lf;
+            double2* bq = b + (long)q * Lf;
+            const double2 u = aq[j], v0 = aq[j + half];
+            const double2 v = make_double2(v0.x * w.x - v0.y * w.y, v0.x * w.y + v0.y * w.x);
+            const int j0 = ((j - k) << 1) + k;
+            bq[j0] = make_double2(u.x + v.x, u.y + v.y);
+            bq[j0 + Ns] = make_double2(u.x - v.x, u.y - v.y);
+        }
+        double2* t2 = a; a = b; b = t2;
+    }
+    __syncthreads();
+    const double* rf = reinterpret_cast<const double*>(a);
+    const int ototal = nout * C;
+    for (int e = threadIdx.x; e < ototal; e += blockDim.x) {
+        int d, c;
+        if (sK_out == 1) { d = e % nout; c = e / nout; }
+        else { c = e % C; d = e / C; }
+        if (c < nc) dst[(long)c * sB_out + (long)d * sK_out] = scale * rf[2 * ((long)(c >> 1) * Lf + d) + (c & 1)];
+    }
+}
+
 // VG: T[d] = scale * Re g[dx][dy][dz], d <= N, from the (4N)^3 complex grid
 __global__ void k_restrict_vg(const double2* __restrict__ g, double* __restrict__ T, int Nx, int Ny,
                               int Nz, double scale) {
