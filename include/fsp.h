@@ -92,6 +92,15 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
 int fsp_plan_set_param(fsp_plan* p, int which, double value);
 
 /*
+ * New mesh spacings for an existing plan (same Nx, Ny, Nz) -- PAPER.md:98: the Green's function is
+ * reused "as long as the mesh spacing does not change"; when the domain follows the bunch it does
+ * change, and only the precompute has to be redone: workspace, tables and tensor maps are kept.
+ * Invalidates the spectrum: fsp_solve returns FSP_ERR_NOT_PRECOMPUTED until fsp_precompute_green
+ * has been called again.  h: host pointer to 3 doubles, all > 0.
+ */
+int fsp_plan_set_spacing(fsp_plan* p, const double* h);
+
+/*
  * precompute_green(plan) -- PAPER.md:72-76 (HE), :88-98 (VG), :100-102 (VG modified); "calculated
  * ... in only one pre-computation step ... reused every time step".
  * Fills the plan-owned real-space table T[dx][dy][dz] (0 <= d_d <= N_d, the kernel at displacement

@@ -30,6 +30,7 @@ _vp, _dp, _i, _d, _sz = _c.c_void_p, _c.POINTER(_c.c_double), _c.c_int, _c.c_dou
 SIGNATURES = {
     "fsp_plan_create": (_i, [_c.POINTER(_vp), _i, _i, _i, _dp, _i, _vp]),
     "fsp_plan_set_param": (_i, [_vp, _i, _d]),
+    "fsp_plan_set_spacing": (_i, [_vp, _dp]),
     "fsp_precompute_green": (_i, [_vp]),
     "fsp_solve": (_i, [_vp, _vp, _vp]),
     "fsp_solve_host": (_i, [_vp, _vp, _vp]),
@@ -110,6 +111,11 @@ def plan_create(Nx: int, Ny: int, Nz: int, h, algorithm: int, cuda_stream: int =
 
 def plan_set_param(plan: int, which: int, value: float) -> None:
     _chk(lib().fsp_plan_set_param(plan, which, value), "fsp_plan_set_param")
+
+
+def plan_set_spacing(plan: int, h) -> None:
+    hh = (ctypes.c_double * 3)(*[float(v) for v in np.broadcast_to(np.asarray(h, dtype=np.float64), (3,))])
+    _chk(lib().fsp_plan_set_spacing(plan, hh), "fsp_plan_set_spacing")
 
 
 def precompute_green(plan: int) -> None:
@@ -206,6 +212,12 @@ class Plan:
 
     def precompute_green(self):
         precompute_green(self.handle)
+        return self
+
+    def set_spacing(self, h):
+        """New spacings for the same mesh; precompute_green must be called again."""
+        plan_set_spacing(self.handle, h)
+        self.h = tuple(float(v) for v in np.broadcast_to(np.asarray(h, dtype=np.float64), (3,)))
         return self
 
     def solve(self, rho, phi=None):

@@ -733,6 +733,15 @@ int fsp_plan_set_param(fsp_plan* p, int which, double value) {
     return FSP_ERR_INVALID_ARG;
 }
 
+int fsp_plan_set_spacing(fsp_plan* p, const double* h) {
+    if (!p || !h) return FSP_ERR_INVALID_ARG;
+    for (int d = 0; d < 3; ++d)
+        if (!(h[d] > 0.0) || !std::isfinite(h[d])) return FSP_ERR_INVALID_ARG;
+    p->h[0] = h[0]; p->h[1] = h[1]; p->h[2] = h[2];
+    p->precomputed = false;   // the table and the spectrum belong to the old spacing
+    return FSP_OK;
+}
+
 int fsp_precompute_green(fsp_plan* p) {
     if (!p) return FSP_ERR_INVALID_ARG;
     p->precomputed = false;

@@ -556,11 +556,15 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
                     gpar ^= 1;
                     gsrc = gst + (b ? M / 2 + 1 : 0);
                 }
+                // row index min(j, M-b-j), j = t + T i: j for the first half of the registers, M-b-j for the
+                // second (T R = M), i.e. compile-time offsets from two lane pointers
+                const double* gA = gsrc + t;
+                const double* gB = gsrc + (M - b - t);
 #pragma unroll
                 for (int i = 0; i < R; ++i) {
                     const int j = t + T * i;
-                    const int m = b ? (j < M - 1 - j ? j : M - 1 - j) : (j < M - j ? j : M - j);
-                    const double gk = Z::GSTAGE ? gsrc[m] : __ldg(gsrc + m);
+                    const double gk = Z::GSTAGE ? (i < R / 2 ? gA[T * i] : gB[-T * i])
+                                                : (i < R / 2 ? __ldg(gA + T * i) : __ldg(gB - T * i));
                     if constexpr (DER) {   // conj(-i f Ghat X) = f Ghat (X.im + i X.re)
                         const double cf = gk * (fp + kap.z * signed_mode(2 * j + b, M));
                         const double a = vr[i];
@@ -582,7 +586,9 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
             const int o = b ? i + H : i;
             const double ar = b ? pr : vr[i], ai = b ? pi : vi[i];            // v_e[n]
             const double qr = b ? vr[i + H] : pr, qi = b ? vi[i + H] : pi;    // v_o[n]
-            const double2 w = wp[t + T * o];
+            // w^(n + M/2) = -i w^n: both branches read the same table entry (one broadcast access)
+            const double2 w0 = wp[t + T * i];
+            const double2 w = b ? make_double2(w0.y, -w0.x) : w0;
             const double zr = fma(-w.y, qi, fma(w.x, qr, ar));
             const double zi = fma(w.y, qr, fma(w.x, qi, ai));
             obase[t + T * o] = make_double2(zr, -zi);

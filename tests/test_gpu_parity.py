@@ -264,3 +264,24 @@ def test_vico_safe_full_size_beam_sampled():
     g = got.reshape(-1)[idx]
     assert np.linalg.norm(g - ref) / np.linalg.norm(ref) <= SPOT_L2_TOL
     assert np.abs(g - ref).max() / np.abs(got).max() <= MAX_TOL
+
+
+def test_set_spacing_invalidates_and_matches_a_fresh_plan():
+    """a change of mesh spacing needs the Green's function again, nothing else."""
+    w = W.random_density((16, 32, 8), seed=9)
+    h2 = (0.07, 0.02, 0.11)
+    rho = torch.from_numpy(w.rho).cuda()
+    with binding.Plan(w.N, w.h, binding.VICO_2) as p:
+        p.precompute_green()
+        p.solve(rho)
+        p.set_spacing(h2)
+        with pytest.raises(binding.FspError) as e:
+            p.solve(rho)
+        assert e.value.code == -2
+        got = p.precompute_green().solve(rho).cpu().numpy()
+        with pytest.raises(binding.FspError):
+            binding.plan_set_spacing(p.handle, (0.1, -1.0, 0.1))
+    with binding.Plan(w.N, h2, binding.VICO_2) as q:
+        fresh = q.precompute_green().solve(rho).cpu().numpy()
+    assert np.array_equal(got, fresh)
+    check(got, oracle.OraclePlan(w.N, h2, oracle.VICO_2).precompute_green().solve(w.rho))
