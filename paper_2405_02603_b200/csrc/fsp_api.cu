@@ -336,6 +336,7 @@ int launch_inv_x(fsp_plan* p, double* phi, double kder) {
         case 64: return fn<64>(__VA_ARGS__);             \
         case 128: return fn<128>(__VA_ARGS__);           \
         case 256: return fn<256>(__VA_ARGS__);           \
+        case 512: return fn<512>(__VA_ARGS__);           \
         default: return FSP_ERR_INVALID_ARG;             \
     }
 
@@ -652,7 +653,7 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
     *out = nullptr;
     if (!h || !(h[0] > 0.0) || !(h[1] > 0.0) || !(h[2] > 0.0)) return FSP_ERR_INVALID_ARG;
     if (!std::isfinite(h[0]) || !std::isfinite(h[1]) || !std::isfinite(h[2])) return FSP_ERR_INVALID_ARG;
-    if (!pow2_in(Nx, 8, 512) || !pow2_in(Ny, 8, 1024) || !pow2_in(Nz, 8, 1024)) return FSP_ERR_INVALID_ARG;
+    if (!pow2_in(Nx, 8, 1024) || !pow2_in(Ny, 8, 1024) || !pow2_in(Nz, 8, 1024)) return FSP_ERR_INVALID_ARG;
     if (algorithm != FSP_HOCKNEY && algorithm != FSP_VICO && algorithm != FSP_VICO_2 && algorithm != FSP_VICO_SAFE) return FSP_ERR_INVALID_ARG;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
