@@ -127,6 +127,18 @@ int fsp_solve(fsp_plan* p, const double* rho_dev, double* phi_dev);
 int fsp_solve_host(fsp_plan* p, const double* rho_host, double* phi_host);
 
 /*
+ * n solves from HOST buffers as a pipeline: while solve i runs, rho of solve i+1 is copied in and phi of
+ * solve i-1 is copied out, on two copy streams of the plan and two pairs of plan-owned staging buffers
+ * (PCIe is full duplex, and the copies take about three times as long as the five kernels).  Every
+ * solve still has its input copied host->device and its result copied device->host inside the call; the
+ * results are identical to n calls of fsp_solve_host.  For independent densities (bunches, time slices
+ * already on the host); pointers may repeat.  Needs pinned host memory to overlap.  Synchronises all
+ * three streams before returning.
+ *   rho_hosts, phi_hosts  host arrays of n host pointers, each to Nx*Ny*Nz doubles
+ */
+int fsp_solve_host_batch(fsp_plan* p, int n, const double* const* rho_hosts, double* const* phi_hosts);
+
+/*
  * Field output -- PAPER.md:227-231, Eq. A.1: "the electric field E(x) is obtained from E = -grad phi".
  * The paper does not say how the gradient is taken; here it is taken where the solver already is, in
  * Fourier space on the doubled grid (reading R18):

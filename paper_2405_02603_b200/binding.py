@@ -34,6 +34,7 @@ SIGNATURES = {
     "fsp_precompute_green": (_i, [_vp]),
     "fsp_solve": (_i, [_vp, _vp, _vp]),
     "fsp_solve_host": (_i, [_vp, _vp, _vp]),
+    "fsp_solve_host_batch": (_i, [_vp, _i, _c.POINTER(_vp), _c.POINTER(_vp)]),
     "fsp_solve_field": (_i, [_vp, _vp, _vp, _vp]),
     "fsp_solve_field_host": (_i, [_vp, _vp, _vp, _vp]),
     "fsp_model_bytes_per_field_solve": (_d, [_vp, _i]),
@@ -128,6 +129,15 @@ def solve(plan: int, rho_dev, phi_dev) -> None:
 
 def solve_host(plan: int, rho_host, phi_host) -> None:
     _chk(lib().fsp_solve_host(plan, _ptr(rho_host), _ptr(phi_host)), "fsp_solve_host")
+
+
+def solve_host_batch(plan: int, rho_hosts, phi_hosts) -> None:
+    """fsp_solve_host_batch: sequences of host buffers (numpy arrays or pinned torch CPU tensors)."""
+    n = len(rho_hosts)
+    assert len(phi_hosts) == n
+    ra = (ctypes.c_void_p * max(n, 1))(*[_ptr(x) for x in rho_hosts])
+    pa = (ctypes.c_void_p * max(n, 1))(*[_ptr(x) for x in phi_hosts])
+    _chk(lib().fsp_solve_host_batch(plan, n, ra, pa), "fsp_solve_host_batch")
 
 
 def solve_field(plan: int, rho_dev, phi_dev, E_dev) -> None:
@@ -250,6 +260,11 @@ class Plan:
         """Host buffers (numpy arrays or pinned torch CPU tensors), copies inside the call."""
         solve_host(self.handle, rho_host, phi_host)
         return phi_host
+
+    def solve_host_batch(self, rho_hosts, phi_hosts):
+        """n pipelined solves from host buffers (copy-in, solve and copy-out of neighbouring solves overlap)."""
+        solve_host_batch(self.handle, rho_hosts, phi_hosts)
+        return phi_hosts
 
     def vg_factors(self):
         return get_vg_factors(self.handle)

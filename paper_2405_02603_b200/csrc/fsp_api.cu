@@ -51,6 +51,10 @@ struct fsp_plan {
     double* Goct = nullptr; // (Nx+1)(Ny+1)(Nz+1)   un-normalised spectrum octant
     double2 *Wx = nullptr, *Wy = nullptr, *Wz = nullptr;  // exp(-2 pi i n / 2N_d), n < 2N_d
     double *rho_stage = nullptr, *phi_stage = nullptr, *E_stage = nullptr;
+    // fsp_solve_host_batch: second pair of staging buffers, copy streams, hand-off events (created on first use)
+    double *rho_stage2 = nullptr, *phi_stage2 = nullptr;
+    cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+    cudaEvent_t ev_h2d[2] = {nullptr, nullptr}, ev_solve[2] = {nullptr, nullptr}, ev_d2h[2] = {nullptr, nullptr};
     bool precomputed = false;
     size_t bytes = 0, peak_transient = 0;
     // profiling
@@ -619,10 +623,17 @@ int precompute_impl(fsp_plan* p) {
 }
 
 void free_plan_memory(fsp_plan* p) {
-    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->B3); cudaFree(p->E_stage); cudaFree(p->Gh); cudaFree(p->Gk); cudaFree(p->LTz); cudaFree(p->LTy); cudaFree(p->LTx); cudaFree(p->T); cudaFree(p->Goct);
+    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->B3); cudaFree(p->E_stage); cudaFree(p->rho_stage2); cudaFree(p->phi_stage2); cudaFree(p->Gh); cudaFree(p->Gk); cudaFree(p->LTz); cudaFree(p->LTy); cudaFree(p->LTx); cudaFree(p->T); cudaFree(p->Goct);
     cudaFree(p->Wx); cudaFree(p->Wy); cudaFree(p->Wz); cudaFree(p->rho_stage); cudaFree(p->phi_stage);
     for (cudaEvent_t e : p->events) cudaEventDestroy(e);
     p->events.clear();
+    for (int i = 0; i < 2; ++i) {
+        if (p->ev_h2d[i]) cudaEventDestroy(p->ev_h2d[i]);
+        if (p->ev_solve[i]) cudaEventDestroy(p->ev_solve[i]);
+        if (p->ev_d2h[i]) cudaEventDestroy(p->ev_d2h[i]);
+    }
+    if (p->s_h2d) cudaStreamDestroy(p->s_h2d);
+    if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
 }
 
 }  // namespace
@@ -815,6 +826,57 @@ int fsp_solve_host(fsp_plan* p, const double* rho_host, double* phi_host) {
     int rc = fsp_solve(p, p->rho_stage, p->phi_stage);
     if (rc != FSP_OK) return rc;
     CU(cudaMemcpyAsync(phi_host, p->phi_stage, v * sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaStreamSynchronize(p->stream));
+    return FSP_OK;
+}
+
+int fsp_solve_host_batch(fsp_plan* p, int n, const double* const* rho_hosts, double* const* phi_hosts) {
+    if (!p || n < 0 || (n > 0 && (!rho_hosts || !phi_hosts))) return FSP_ERR_INVALID_ARG;
+    for (int i = 0; i < n; ++i)
+        if (!rho_hosts[i] || !phi_hosts[i]) return FSP_ERR_INVALID_ARG;
+    if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
+    if (n == 0) return FSP_OK;
+    const size_t v = (size_t)p->Nx * p->Ny * p->Nz;
+    int rc;
+    if (!p->rho_stage) {
+        if ((rc = dev_alloc(&p->rho_stage, v, &p->bytes)) != FSP_OK) return rc;
+        if ((rc = dev_alloc(&p->phi_stage, v, &p->bytes)) != FSP_OK) return rc;
+    }
+    if (!p->rho_stage2) {
+        if ((rc = dev_alloc(&p->rho_stage2, v, &p->bytes)) != FSP_OK) return rc;
+        if ((rc = dev_alloc(&p->phi_stage2, v, &p->bytes)) != FSP_OK) return rc;
+        CU(cudaStreamCreateWithFlags(&p->s_h2d, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithFlags(&p->s_d2h, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            CU(cudaEventCreateWithFlags(&p->ev_h2d[i], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&p->ev_solve[i], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&p->ev_d2h[i], cudaEventDisableTiming));
+        }
+    }
+    double* rs[2] = {p->rho_stage, p->rho_stage2};
+    double* ps[2] = {p->phi_stage, p->phi_stage2};
+    // earlier work on the plan's stream may still use the staging buffers
+    CU(cudaEventRecord(p->ev_solve[0], p->stream));
+    CU(cudaStreamWaitEvent(p->s_h2d, p->ev_solve[0], 0));
+    CU(cudaStreamWaitEvent(p->s_d2h, p->ev_solve[0], 0));
+    for (int i = 0; i < n; ++i) {
+        const int s = i & 1;
+        // copy-in of solve i: its staging buffer is free once solve i-2 has run
+        if (i >= 2) CU(cudaStreamWaitEvent(p->s_h2d, p->ev_solve[s], 0));
+        CU(cudaMemcpyAsync(rs[s], rho_hosts[i], v * sizeof(double), cudaMemcpyHostToDevice, p->s_h2d));
+        CU(cudaEventRecord(p->ev_h2d[s], p->s_h2d));
+        // solve i: needs its input, and its output buffer back from the copy-out of solve i-2
+        CU(cudaStreamWaitEvent(p->stream, p->ev_h2d[s], 0));
+        if (i >= 2) CU(cudaStreamWaitEvent(p->stream, p->ev_d2h[s], 0));
+        if ((rc = fsp_solve(p, rs[s], ps[s])) != FSP_OK) return rc;
+        CU(cudaEventRecord(p->ev_solve[s], p->stream));
+        // copy-out of solve i
+        CU(cudaStreamWaitEvent(p->s_d2h, p->ev_solve[s], 0));
+        CU(cudaMemcpyAsync(phi_hosts[i], ps[s], v * sizeof(double), cudaMemcpyDeviceToHost, p->s_d2h));
+        CU(cudaEventRecord(p->ev_d2h[s], p->s_d2h));
+    }
+    CU(cudaStreamSynchronize(p->s_d2h));
+    CU(cudaStreamSynchronize(p->s_h2d));
     CU(cudaStreamSynchronize(p->stream));
     return FSP_OK;
 }

@@ -285,3 +285,28 @@ def test_set_spacing_invalidates_and_matches_a_fresh_plan():
         fresh = q.precompute_green().solve(rho).cpu().numpy()
     assert np.array_equal(got, fresh)
     check(got, oracle.OraclePlan(w.N, h2, oracle.VICO_2).precompute_green().solve(w.rho))
+
+
+def test_solve_host_batch_equals_solve_host():
+    """fsp_solve_host_batch (copies of neighbouring solves overlapped) gives the results of n single calls."""
+    N, h = (32, 16, 64), (0.05, 0.1, 0.02)
+    rhos = [torch.from_numpy(W.random_density(N, seed=s).rho).pin_memory() for s in range(5)]
+    with binding.Plan(N, h, binding.HOCKNEY) as p:
+        p.precompute_green()
+        single = []
+        for r in rhos:
+            out = torch.empty_like(r).pin_memory()
+            p.solve_host(r, out)
+            single.append(out.clone())
+        outs = [torch.empty_like(r).pin_memory() for r in rhos]
+        p.solve_host_batch(rhos, outs)
+        for a, b in zip(outs, single):
+            assert torch.equal(a, b)
+        p.solve_host_batch([], [])
+        ring = [torch.empty_like(rhos[0]).pin_memory() for _ in range(2)]   # repeated output pointers
+        p.solve_host_batch(rhos, [ring[i % 2] for i in range(5)])
+        assert torch.equal(ring[0], single[4]) and torch.equal(ring[1], single[3])
+        out = np.empty(N)   # pageable numpy buffers work too (copies then do not overlap)
+        p.solve_host_batch([rhos[2].numpy()], [out])
+        assert np.array_equal(out, single[2].numpy())
+    check(single[0].numpy(), oracle.OraclePlan(N, h, oracle.HOCKNEY).precompute_green().solve(rhos[0].numpy()))
