@@ -18,8 +18,13 @@
  * fallback.  One GPU, one plan = one mesh; fp64 throughout.  eps0 = 1: the caller divides by eps0.
  *
  * Conventions
- *   - Mesh Nx x Ny x Nz, spacings h[0..2] = hx, hy, hz.  Each N_d must be a power of
- *     two with 8 <= N_d <= 1024 (the paper's sizes are all powers of two).
+ *   - Mesh Nx x Ny x Nz, spacings h[0..2] = hx, hy, hz, 2 <= N_d <= 1024.  The transforms
+ *     are power-of-two (the paper's sizes all are): a mesh with another N_d is embedded
+ *     in the next power-of-two mesh N'_d >= max(N_d, 8) (zero density outside, result cropped; DESIGN.md
+ *     R19).  The cyclic convolution is exact for any period >= 2 N_d - 1, so FSP_HOCKNEY gives the paper's
+ *     result for the caller's mesh; the Vico-Greengard table is that of the enclosing box N'_d h_d
+ *     (a larger truncation radius L, same free-space kernel); the spectral gradient of fsp_solve_field
+ *     has period 2 N'_d h_d.  Cost and memory are those of the N' mesh.
  *   - rho, phi: dense fp64 arrays of shape (Nx, Ny, Nz) in C order, index (ix*Ny + iy)*Nz + iz,
  *     iz fastest.  The sample position inside a cell does not matter (translation invariance).
  *   - "dev" pointers are CUDA device pointers on the device that was current at plan creation;
@@ -58,7 +63,7 @@ enum {
 /* error codes */
 enum {
     FSP_OK = 0,
-    FSP_ERR_INVALID_ARG = -1,     /* null pointer, N not a power of two in [8,1024], h <= 0, bad enum */
+    FSP_ERR_INVALID_ARG = -1,     /* null pointer, N_d outside [2,1024], h <= 0, bad enum             */
     FSP_ERR_NOT_PRECOMPUTED = -2, /* fsp_solve / getters before fsp_precompute_green                 */
     FSP_ERR_OUT_OF_MEMORY = -3,   /* device allocation failed (e.g. FSP_VICO at 512^3: (4N)^3 grid)  */
     FSP_ERR_CUDA = -4,            /* a CUDA runtime call or kernel launch failed                     */
@@ -186,7 +191,8 @@ int fsp_get_vg_factors(const fsp_plan* p, int* m_out);
 int fsp_get_green_table(const fsp_plan* p, double* T_host);
 
 /* Copies the unique octant of the un-normalised spectrum F{G2}[kx][ky][kz], 0 <= k_d <= N_d,
- * (Nx+1)(Ny+1)(Nz+1) doubles in C order (F{G2} is real and even), to host memory. */
+ * (Nx+1)(Ny+1)(Nz+1) doubles in C order (F{G2} is real and even), to host memory.  Power-of-two meshes
+ * only: on an embedded mesh the spectrum belongs to the transform mesh (FSP_ERR_INVALID_ARG). */
 int fsp_get_green_spectrum(const fsp_plan* p, double* Ghat_host);
 
 /*

@@ -20,7 +20,10 @@ using namespace fsp;
 #define FSP_VERSION_NUM 100
 
 struct fsp_plan {
-    int Nx = 0, Ny = 0, Nz = 0;
+    int Nx = 0, Ny = 0, Nz = 0;   // transform mesh: each a power of two (the caller's mesh when that is one)
+    int Ux = 0, Uy = 0, Uz = 0;   // the caller's mesh; U_d <= N_d
+    bool padded = false;          // U != N: rho is embedded in / phi cropped from the transform mesh (R19)
+    double *rho_pad = nullptr, *phi_pad = nullptr;   // Nx*Ny*Nz each, only when padded
     double h[3] = {0, 0, 0};
     int algorithm = 0;
     cudaStream_t stream = nullptr;
@@ -466,11 +469,39 @@ int do_inv_x(fsp_plan* p, double* phi, double kder = 0.0) {
     DISPATCH_X(launch_inv_x, p->Nx / 2, p, phi, kder)
 }
 
+// embed (dir = 0: small -> big) or crop (dir = 1: big -> small) a Ux x Uy x Uz block at the origin of an
+// Nx x Ny x Nz array (non-power-of-two meshes, R19); the rest of the big array stays zero
+__global__ void k_embed_crop(double* __restrict__ big, double* __restrict__ small_, int Uy, int Uz, int Ny, int Nz,
+                             long total, int dir) {
+    for (long o = blockIdx.x * (long)blockDim.x + threadIdx.x; o < total; o += (long)gridDim.x * blockDim.x) {
+        const int z = (int)(o % Uz), y = (int)((o / Uz) % Uy);
+        const long x = o / ((long)Uz * Uy);
+        const long q = (x * Ny + y) * Nz + z;
+        if (dir == 0) big[q] = small_[o];
+        else small_[o] = big[q];
+    }
+}
+
 unsigned grid_for(long total, int block) {
     long g = (total + block - 1) / block;
     const long cap = 148L * 32;
     return (unsigned)(g < cap ? (g > 0 ? g : 1) : cap);
 }
+
+size_t user_volume(const fsp_plan* p) { return (size_t)p->Ux * p->Uy * p->Uz; }
+int embed_rho(fsp_plan* p, const double* rho_user) {   // rho_pad <- rho (its zero part was set at plan creation)
+    const long tot = (long)user_volume(p);
+    k_embed_crop<<<grid_for(tot, 256), 256, 0, p->stream>>>(p->rho_pad, const_cast<double*>(rho_user), p->Uy, p->Uz, p->Ny, p->Nz, tot, 0);
+    CU(cudaGetLastError());
+    return FSP_OK;
+}
+int crop_out(fsp_plan* p, double* dst_user) {          // dst <- phi_pad restricted to the caller's mesh
+    const long tot = (long)user_volume(p);
+    k_embed_crop<<<grid_for(tot, 256), 256, 0, p->stream>>>(p->phi_pad, dst_user, p->Uy, p->Uz, p->Ny, p->Nz, tot, 1);
+    CU(cudaGetLastError());
+    return FSP_OK;
+}
+int next_pow2_min8(int n) { int q = 8; while (q < n) q *= 2; return q; }
 
 // batched DCT-I along one axis of a real 3-D array (C order), output pruned to nout along that axis
 int dct1_axis(fsp_plan* p, const double* in, double* out, const long in_dims[3], const long out_dims[3],
@@ -623,7 +654,7 @@ int precompute_impl(fsp_plan* p) {
 }
 
 void free_plan_memory(fsp_plan* p) {
-    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->B3); cudaFree(p->E_stage); cudaFree(p->rho_stage2); cudaFree(p->phi_stage2); cudaFree(p->Gh); cudaFree(p->Gk); cudaFree(p->LTz); cudaFree(p->LTy); cudaFree(p->LTx); cudaFree(p->T); cudaFree(p->Goct);
+    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->B3); cudaFree(p->rho_pad); cudaFree(p->phi_pad); cudaFree(p->E_stage); cudaFree(p->rho_stage2); cudaFree(p->phi_stage2); cudaFree(p->Gh); cudaFree(p->Gk); cudaFree(p->LTz); cudaFree(p->LTy); cudaFree(p->LTx); cudaFree(p->T); cudaFree(p->Goct);
     cudaFree(p->Wx); cudaFree(p->Wy); cudaFree(p->Wz); cudaFree(p->rho_stage); cudaFree(p->phi_stage);
     for (cudaEvent_t e : p->events) cudaEventDestroy(e);
     p->events.clear();
@@ -664,7 +695,10 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
     *out = nullptr;
     if (!h || !(h[0] > 0.0) || !(h[1] > 0.0) || !(h[2] > 0.0)) return FSP_ERR_INVALID_ARG;
     if (!std::isfinite(h[0]) || !std::isfinite(h[1]) || !std::isfinite(h[2])) return FSP_ERR_INVALID_ARG;
-    if (!pow2_in(Nx, 8, 1024) || !pow2_in(Ny, 8, 1024) || !pow2_in(Nz, 8, 1024)) return FSP_ERR_INVALID_ARG;
+    if (Nx < 2 || Ny < 2 || Nz < 2 || Nx > 1024 || Ny > 1024 || Nz > 1024) return FSP_ERR_INVALID_ARG;
+    const int Ux = Nx, Uy = Ny, Uz = Nz;
+    // the transforms are power-of-two: any other mesh is embedded in the next one (R19)
+    Nx = next_pow2_min8(Ux); Ny = next_pow2_min8(Uy); Nz = next_pow2_min8(Uz);
     if (algorithm != FSP_HOCKNEY && algorithm != FSP_VICO && algorithm != FSP_VICO_2 && algorithm != FSP_VICO_SAFE) return FSP_ERR_INVALID_ARG;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
@@ -674,6 +708,8 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
     fsp_plan* p = new (std::nothrow) fsp_plan();
     if (!p) return FSP_ERR_OUT_OF_MEMORY;
     p->Nx = Nx; p->Ny = Ny; p->Nz = Nz;
+    p->Ux = Ux; p->Uy = Uy; p->Uz = Uz;
+    p->padded = Ux != Nx || Uy != Ny || Uz != Nz;
     p->h[0] = h[0]; p->h[1] = h[1]; p->h[2] = h[2];
     p->algorithm = algorithm;
     p->stream = static_cast<cudaStream_t>(cuda_stream);
@@ -685,6 +721,9 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
     if (rc == FSP_OK && prop.major != 10) rc = FSP_ERR_NO_DEVICE;  // the library holds sm_100a code only
     const size_t n1 = (size_t)(Nx + 1) * Ny * Nz, n2 = (size_t)(Nx + 1) * 2 * Ny * Nz;
     const size_t ng = (size_t)(Nx + 1) * 2 * Ny * 2 * Nz, nt = (size_t)(Nx + 1) * (Ny + 1) * (Nz + 1);
+    if (rc == FSP_OK && p->padded) rc = dev_alloc(&p->rho_pad, (size_t)Nx * Ny * Nz, &p->bytes);
+    if (rc == FSP_OK && p->padded) rc = dev_alloc(&p->phi_pad, (size_t)Nx * Ny * Nz, &p->bytes);
+    if (rc == FSP_OK && p->padded && cudaMemset(p->rho_pad, 0, sizeof(double) * (size_t)Nx * Ny * Nz) != cudaSuccess) rc = FSP_ERR_CUDA;
     if (rc == FSP_OK) rc = dev_alloc(&p->B1, n1, &p->bytes);
     if (rc == FSP_OK) rc = dev_alloc(&p->B2, n2, &p->bytes);
     p->z_warp = Nz <= 512;
@@ -770,6 +809,14 @@ int fsp_precompute_green(fsp_plan* p) {
 int fsp_solve(fsp_plan* p, const double* rho_dev, double* phi_dev) {
     if (!p || !rho_dev || !phi_dev || rho_dev == phi_dev) return FSP_ERR_INVALID_ARG;
     if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
+    double* phi_user = nullptr;
+    if (p->padded) {   // embed, solve on the transform mesh, crop
+        int rce = embed_rho(p, rho_dev);
+        if (rce != FSP_OK) return rce;
+        rho_dev = p->rho_pad;
+        phi_user = phi_dev;
+        phi_dev = p->phi_pad;
+    }
     cudaEvent_t* ev = nullptr;
     if (p->profiling) {
         if (p->events_used + 6 > p->events.size()) {
@@ -807,6 +854,7 @@ int fsp_solve(fsp_plan* p, const double* rho_dev, double* phi_dev) {
     if (ev) CU(cudaEventRecord(ev[4], p->stream));
     }
     if ((rc = do_inv_x(p, phi_dev)) != FSP_OK) return rc;
+    if (phi_user && (rc = crop_out(p, phi_user)) != FSP_OK) return rc;
     if (ev) CU(cudaEventRecord(ev[5], p->stream));
     CU(cudaGetLastError());
     return FSP_OK;
@@ -815,7 +863,7 @@ int fsp_solve(fsp_plan* p, const double* rho_dev, double* phi_dev) {
 int fsp_solve_host(fsp_plan* p, const double* rho_host, double* phi_host) {
     if (!p || !rho_host || !phi_host) return FSP_ERR_INVALID_ARG;
     if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
-    const size_t v = (size_t)p->Nx * p->Ny * p->Nz;
+    const size_t v = user_volume(p);
     if (!p->rho_stage) {
         int rc = dev_alloc(&p->rho_stage, v, &p->bytes);
         if (rc != FSP_OK) return rc;
@@ -836,7 +884,7 @@ int fsp_solve_host_batch(fsp_plan* p, int n, const double* const* rho_hosts, dou
         if (!rho_hosts[i] || !phi_hosts[i]) return FSP_ERR_INVALID_ARG;
     if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
     if (n == 0) return FSP_OK;
-    const size_t v = (size_t)p->Nx * p->Ny * p->Nz;
+    const size_t v = user_volume(p);
     int rc;
     if (!p->rho_stage) {
         if ((rc = dev_alloc(&p->rho_stage, v, &p->bytes)) != FSP_OK) return rc;
@@ -884,8 +932,18 @@ int fsp_solve_host_batch(fsp_plan* p, int n, const double* const* rho_hosts, dou
 int fsp_solve_field(fsp_plan* p, const double* rho_dev, double* phi_dev, double* E_dev) {
     if (!p || !rho_dev || !E_dev || rho_dev == phi_dev || rho_dev == E_dev) return FSP_ERR_INVALID_ARG;
     if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
-    const size_t n2 = (size_t)(p->Nx + 1) * 2 * p->Ny * p->Nz, V = (size_t)p->Nx * p->Ny * p->Nz;
+    const size_t n2 = (size_t)(p->Nx + 1) * 2 * p->Ny * p->Nz, V = user_volume(p);
     int rc;
+    if (p->padded) {
+        if ((rc = embed_rho(p, rho_dev)) != FSP_OK) return rc;
+        rho_dev = p->rho_pad;
+    }
+    // last pass of one output: straight into the caller's array, or through phi_pad and a crop (R19)
+    auto out_x = [&](double* dst, double kder) -> int {
+        if (!p->padded) return do_inv_x(p, dst, kder);
+        int r = do_inv_x(p, p->phi_pad, kder);
+        return r != FSP_OK ? r : crop_out(p, dst);
+    };
     if (!p->B3) {   // first field solve of this plan: the buffer that receives the derivative spectra
         if ((rc = dev_alloc(&p->B3, n2, &p->bytes)) != FSP_OK) return rc;
         if (p->tile_y) {
@@ -909,15 +967,15 @@ int fsp_solve_field(fsp_plan* p, const double* rho_dev, double* phi_dev, double*
     const DerK kap{0.0, 0.0, kz, p->Nx};
     if ((rc = do_conv_z(p, p->B2, 0, planes, p->B3, &kap)) != FSP_OK) return rc;
     if ((rc = do_inv_y(p, p->B3, p->B1, planes)) != FSP_OK) return rc;
-    if ((rc = do_inv_x(p, E_dev + 2 * V)) != FSP_OK) return rc;
+    if ((rc = out_x(E_dev + 2 * V, 0.0)) != FSP_OK) return rc;
     // phi and E_x: plain K3 (in place), K4, then K5 twice on the same B1 (plain, and with -i kx on its input)
     if ((rc = do_conv_z(p, p->B2, 0, planes)) != FSP_OK) return rc;
     if ((rc = do_inv_y(p, p->B2, p->B1, planes)) != FSP_OK) return rc;
-    if (phi_dev && (rc = do_inv_x(p, phi_dev)) != FSP_OK) return rc;
-    if ((rc = do_inv_x(p, E_dev, kx)) != FSP_OK) return rc;
+    if (phi_dev && (rc = out_x(phi_dev, 0.0)) != FSP_OK) return rc;
+    if ((rc = out_x(E_dev, kx)) != FSP_OK) return rc;
     // E_y: K4 with -i ky on its input rows (B2 still holds the output of the plain K3), K5
     if ((rc = do_inv_y(p, p->B2, p->B1, planes, ky)) != FSP_OK) return rc;
-    if ((rc = do_inv_x(p, E_dev + V)) != FSP_OK) return rc;
+    if ((rc = out_x(E_dev + V, 0.0)) != FSP_OK) return rc;
     CU(cudaGetLastError());
     return FSP_OK;
 }
@@ -925,7 +983,7 @@ int fsp_solve_field(fsp_plan* p, const double* rho_dev, double* phi_dev, double*
 int fsp_solve_field_host(fsp_plan* p, const double* rho_host, double* phi_host, double* E_host) {
     if (!p || !rho_host || !E_host) return FSP_ERR_INVALID_ARG;
     if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
-    const size_t v = (size_t)p->Nx * p->Ny * p->Nz;
+    const size_t v = user_volume(p);
     int rc;
     if (!p->rho_stage) {
         if ((rc = dev_alloc(&p->rho_stage, v, &p->bytes)) != FSP_OK) return rc;
@@ -991,12 +1049,22 @@ int fsp_get_green_table(const fsp_plan* p, double* T_host) {
     if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
     const size_t nt = (size_t)(p->Nx + 1) * (p->Ny + 1) * (p->Nz + 1);
     CU(cudaStreamSynchronize(p->stream));
+    if (p->padded) {   // the caller's block (Ux+1)(Uy+1)(Uz+1) of the table of the transform mesh
+        std::vector<double> full(nt);
+        CU(cudaMemcpy(full.data(), p->T, nt * sizeof(double), cudaMemcpyDeviceToHost));
+        for (int i = 0; i <= p->Ux; ++i)
+            for (int j = 0; j <= p->Uy; ++j)
+                for (int k = 0; k <= p->Uz; ++k)
+                    T_host[((size_t)i * (p->Uy + 1) + j) * (p->Uz + 1) + k] = full[((size_t)i * (p->Ny + 1) + j) * (p->Nz + 1) + k];
+        return FSP_OK;
+    }
     CU(cudaMemcpy(T_host, p->T, nt * sizeof(double), cudaMemcpyDeviceToHost));
     return FSP_OK;
 }
 
 int fsp_get_green_spectrum(const fsp_plan* p, double* Ghat_host) {
     if (!p || !Ghat_host) return FSP_ERR_INVALID_ARG;
+    if (p->padded) return FSP_ERR_INVALID_ARG;   // the spectrum lives on the transform mesh, not the caller's
     if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
     const size_t nt = (size_t)(p->Nx + 1) * (p->Ny + 1) * (p->Nz + 1);
     CU(cudaStreamSynchronize(p->stream));

@@ -41,8 +41,9 @@ def test_static_queries_and_error_strings(libpath):
 
 
 @pytest.mark.parametrize("args", [
-    (12, 16, 16, (0.1, 0.1, 0.1), 0),      # not a power of two
-    (16, 16, 4, (0.1, 0.1, 0.1), 0),       # too small
+    (1, 16, 16, (0.1, 0.1, 0.1), 0),       # too small (any 2 <= N_d <= 1024 is accepted, R19)
+    (16, 16, 0, (0.1, 0.1, 0.1), 0),
+    (16, 1025, 16, (0.1, 0.1, 0.1), 0),    # too large
     (16, 2048, 16, (0.1, 0.1, 0.1), 0),    # too large
     (16, 16, 16, (0.1, -0.1, 0.1), 0),     # h <= 0
     (16, 16, 16, (0.1, 0.1, float("nan")), 0),

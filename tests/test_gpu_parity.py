@@ -310,3 +310,84 @@ def test_solve_host_batch_equals_solve_host():
         p.solve_host_batch([rhos[2].numpy()], [out])
         assert np.array_equal(out, single[2].numpy())
     check(single[0].numpy(), oracle.OraclePlan(N, h, oracle.HOCKNEY).precompute_green().solve(rhos[0].numpy()))
+
+
+@pytest.mark.parametrize("N", [(8, 8, 8), (256, 128, 16)])
+def test_degenerate_densities(N):
+    """Empty (all-zero) density -> exactly zero potential and field; a constant density and a single charge in
+    the last corner (the longest wrap-around distance of the doubled grid) against the oracle; exact scaling by
+    a power of two."""
+    h = (0.1, 0.2, 0.05)
+    op = oracle.OraclePlan(N, h, oracle.HOCKNEY).precompute_green()
+    with binding.Plan(N, h, binding.HOCKNEY) as p:
+        p.precompute_green()
+        zero = torch.zeros(N, dtype=torch.float64, device="cuda")
+        assert float(p.solve(zero).abs().max()) == 0.0
+        _, E = p.solve_field(zero, want_phi=False)
+        assert float(E.abs().max()) == 0.0
+        const = np.full(N, 3.5)
+        check(gpu_solve(p, const), op.solve(const))
+        corner = np.zeros(N)
+        corner[-1, -1, -1] = -2.0
+        got = gpu_solve(p, corner)
+        check(got, op.solve(corner))
+        assert np.array_equal(gpu_solve(p, corner * 2.0 ** 40), got * 2.0 ** 40)
+
+
+# ---------------------------------------------------------------- any mesh size (SURVEY 8(f) N4, DESIGN.md R19)
+def _ref_on_enclosing_box(alg, N, h, rho):
+    """R19: the transforms run on the next power-of-two mesh N' >= max(N, 8).  The convolution on the caller's
+    mesh needs the table at displacements below N only, so the reference is the paper's steps 1-5 on the 2N grid
+    (oracle O2, direct DFT for these lengths) with the table of the enclosing box -- for HE the very same table."""
+    Np = tuple(max(8, 1 << (n - 1).bit_length()) for n in N)
+    T = oracle.green_table(alg, Np, h)[: N[0] + 1, : N[1] + 1, : N[2] + 1].copy()
+    return T, oracle.solve_with_spectrum(oracle.green_spectrum(T), h, rho)
+
+
+@pytest.mark.parametrize("alg", ["HE", "VG2"])
+@pytest.mark.parametrize("N", [(12, 20, 9), (3, 5, 2), (24, 17, 33), (40, 96, 72), (100, 8, 130)])
+def test_any_mesh_size_against_the_oracle(alg, N):
+    w = W.random_density(N, seed=13)
+    with binding.Plan(w.N, w.h, ALGS[alg][0]) as p:
+        p.precompute_green()
+        got = gpu_solve(p, w.rho)
+        T = p.green_table()
+        rho = torch.from_numpy(w.rho).cuda()
+        phi2 = p.solve(rho).cpu().numpy()          # repeatable: the zero part of the embedding stays zero
+        host = np.empty(N)
+        p.solve_host(np.ascontiguousarray(w.rho), host)
+        with pytest.raises(binding.FspError):
+            p.green_spectrum()
+    To, ref = _ref_on_enclosing_box(ALGS[alg][1], N, w.h, w.rho)
+    assert T.shape == To.shape and np.abs(T - To).max() <= 1e-13 * np.abs(To).max()
+    check(got, ref)
+    assert np.array_equal(got, phi2) and np.array_equal(got, host)
+    if alg == "HE":   # identical to the plan made for exactly this mesh by the plain definition
+        idx = np.random.default_rng(1).integers(0, int(np.prod(N)), size=40)
+        o1 = oracle.direct_sum(oracle.green_table(oracle.HOCKNEY, N, w.h), w.h, w.rho, idx)
+        assert np.abs(got.ravel()[idx] - o1).max() <= MAX_TOL * np.abs(ref).max()
+
+
+def test_any_mesh_size_field_and_accuracy():
+    """96^3 Gaussian (not a power of two): VG reaches round-off against the closed form, field included."""
+    from tests.analytic import gaussian_field_iso
+    w = W.config1(96)
+    with binding.Plan(w.N, w.h, binding.VICO_2) as p:
+        p.precompute_green()
+        rho = torch.from_numpy(w.rho).cuda()
+        phi, E = p.solve_field(rho)
+        torch.cuda.synchronize()
+        phi, E = phi.cpu().numpy(), E.cpu().numpy()
+    assert rel_l2(phi, gaussian_potential_iso(w)) < 1e-13
+    assert rel_l2(E, gaussian_field_iso(w)) < 1e-12
+    w2 = W.random_density((20, 12, 36), seed=3)
+    with binding.Plan(w2.N, w2.h, binding.HOCKNEY) as p:
+        p.precompute_green()
+        _, E2 = p.solve_field(torch.from_numpy(w2.rho).cuda(), want_phi=False)
+        E2 = E2.cpu().numpy()
+    # the spectral gradient lives on the transform mesh (period 2 N' h): reference = oracle on the embedded density
+    Np = (32, 16, 64)
+    emb = np.zeros(Np)
+    emb[:20, :12, :36] = w2.rho
+    _, Eo = oracle.OraclePlan(Np, w2.h, oracle.HOCKNEY).precompute_green().solve_field(emb)
+    check(E2, Eo[:, :20, :12, :36])
