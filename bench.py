@@ -418,6 +418,7 @@ def extras(args, peak):
         w = getattr(W, builder)(**kw)
         V = int(np.prod(w.N))
         with binding.Plan(w.N, w.h, ALGS[alg]) as plan:
+            plan.precompute_green(); torch.cuda.synchronize()   # untimed: allocator churn left by the previous leg
             t0 = time.perf_counter(); plan.precompute_green(); torch.cuda.synchronize()
             t_pre = time.perf_counter() - t0
             rho = torch.from_numpy(w.rho).cuda()

@@ -29,7 +29,7 @@ struct Fft2CfgT {
     static constexpr int NB1 = R / R1_, NB2 = R / R2_;
     static constexpr int BUF = M_ + M_ / R1_;  // padded exchange buffer, in double2 elements
     static_assert(R1_ * R2_ == M_, "radices must multiply to M");
-    static_assert(T >= 1 && T <= 16, "a lane group must fit half a warp");
+    static_assert(T >= 1 && T <= 32, "a lane group must fit a warp");
 };
 template <int M> struct Fft2Cfg;
 template <> struct Fft2Cfg<8> : Fft2CfgT<8, 4, 2> {};
@@ -39,6 +39,7 @@ template <> struct Fft2Cfg<64> : Fft2CfgT<64, 8, 8> {};
 template <> struct Fft2Cfg<128> : Fft2CfgT<128, 16, 8> {};
 template <> struct Fft2Cfg<256> : Fft2CfgT<256, 16, 16> {};
 template <> struct Fft2Cfg<512> : Fft2CfgT<512, 16, 32> {};
+template <> struct Fft2Cfg<1024> : Fft2CfgT<1024, 32, 32> {};   // one branch per warp (k_conv_z_p)
 
 // padded address of position p (one pad element after every R1 positions)
 template <int R1>

@@ -275,7 +275,27 @@ int launch_conv_z(fsp_plan* p, double2* B2, const double* G, int nplanes, double
     return launch_conv_z_impl<M, false>(p, B2, G, nplanes, nullptr, DerK{0.0, 0.0, 0.0, 0});
 }
 template <int M, bool DER>
+int launch_conv_z_p_impl(fsp_plan* p, double2* B2, const double* G, int nplanes, double2* out, const DerK kap) {
+    using Z = ConvZP<M>;
+    const long nsteps = (long)nplanes * (2 * p->Ny) / Z::G;   // pair steps: G pencils each
+    const size_t smem = Z::smem_bytes();
+    static int occ = 0;
+    if (occ == 0) {
+        CU(cudaFuncSetAttribute(k_conv_z_p<M, DER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_conv_z_p<M, DER>, Z::WARPS * 32, smem));
+        if (occ < 1) return FSP_ERR_CUDA;
+    }
+    long grid = (long)p->sm_count * occ;
+    const long need = (nsteps + Z::PAIRS - 1) / Z::PAIRS;
+    if (grid > need) grid = need;
+    k_conv_z_p<M, DER><<<(unsigned)grid, Z::WARPS * 32, smem, p->stream>>>(B2, G, p->LTz, p->Wz, p->Ny, nsteps, out, kap);
+    return FSP_OK;
+}
+template <int M, bool DER>
 int launch_conv_z_w_impl(fsp_plan* p, double2* B2, const double* G, int nplanes, double2* out, const DerK kap) {
+    // Nz >= 256: warp pairs (k_conv_z_p); below: both branches in one warp (k_conv_z_w)
+    if constexpr (M >= 256) return launch_conv_z_p_impl<M, DER>(p, B2, G, nplanes, out, kap);
+    else {
     using Z = ConvZ<M>;
     const long ngroups = (long)nplanes * (2 * p->Ny) / Z::G;
     const size_t smem = Z::smem_bytes();
@@ -290,6 +310,7 @@ int launch_conv_z_w_impl(fsp_plan* p, double2* B2, const double* G, int nplanes,
     if (grid > need) grid = need;
     k_conv_z_w<M, DER><<<(unsigned)grid, Z::WARPS * 32, smem, p->stream>>>(B2, G, p->LTz, p->Wz, p->Ny, ngroups, out, kap);
     return FSP_OK;
+    }
 }
 template <int M>
 int launch_conv_z_w(fsp_plan* p, double2* B2, const double* G, int nplanes, double2* out, const DerK* kap) {
@@ -397,6 +418,7 @@ int do_fwd_y(fsp_plan* p, int kx0, double2* B2, int np) {
         case 128: return fn<128>(__VA_ARGS__);           \
         case 256: return fn<256>(__VA_ARGS__);           \
         case 512: return fn<512>(__VA_ARGS__);           \
+        case 1024: return fn<1024>(__VA_ARGS__);         \
         default: return FSP_ERR_INVALID_ARG;             \
     }
 int do_conv_z_v1(fsp_plan* p, double2* B2, const double* G, int np, double2* out, const DerK* kap) { DISPATCH_YZ(launch_conv_z, p->Nz, p, B2, G, np, out, kap) }
@@ -726,7 +748,7 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
     if (rc == FSP_OK && p->padded && cudaMemset(p->rho_pad, 0, sizeof(double) * (size_t)Nx * Ny * Nz) != cudaSuccess) rc = FSP_ERR_CUDA;
     if (rc == FSP_OK) rc = dev_alloc(&p->B1, n1, &p->bytes);
     if (rc == FSP_OK) rc = dev_alloc(&p->B2, n2, &p->bytes);
-    p->z_warp = Nz <= 512;
+    p->z_warp = true;   // every Nz has a warp-level K3 (Nz = 1024: warp pairs, k_conv_z_p)
     p->sm_count = prop.multiProcessorCount > 0 ? prop.multiProcessorCount : 148;
     if (rc == FSP_OK && !p->z_warp) rc = dev_alloc(&p->Gh, ng, &p->bytes);
     if (rc == FSP_OK && p->z_warp) rc = dev_alloc(&p->Gk, (size_t)(Nx + 1) * (Ny + 1) * (Nz + 2), &p->bytes);

@@ -596,6 +596,151 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
     }
 }
 
+// ========================================================================= K3 (v2, pairs): conv_z_p
+// A pencil is handled by a PAIR of warps: warp 2q runs the even half-spectrum branch, warp 2q+1 the odd one,
+// each for G = 32/T pencils at a time (T lanes per pencil: Nz = 1024 -> T = 32, one pencil per pair step;
+// Nz = 512, 256 -> T = 16, two).  Compared with k_conv_z_w (both branches in the two halves of ONE warp)
+// nothing is executed under a branch predicate: the pre-twiddle of the odd branch costs issue slots in the
+// odd warps only, and the final sum needs no per-lane selects.  Everything else is the same: one copy of the
+// transform code run twice, lane-constant stage-2 twiddles, octant spectrum with the row(s) staged by bulk
+// async copies per pair step, the visiting order that lets two pencils share a spectrum row in L2.  The
+// final sum y[n] = conj(v_e[n] + w^n v_o[n]) exchanges half of each branch's values through the (then free)
+// exchange buffers, with a named barrier over the pair; each warp stores half of each pencil.
+template <int M>
+struct ConvZP {
+    using Cfg = Fft2Cfg<M>;
+    static constexpr int T = Cfg::T, R = Cfg::R;
+    static constexpr int G = 32 / T;                       // pencils per warp
+    static constexpr int PAIRS = (M <= 256) ? 6 : 4, WARPS = 2 * PAIRS;
+    static constexpr int MINB = 1;
+    static constexpr int ROW = M + 2;
+    static constexpr int NC = LaneTw<Cfg::R2>::NC;
+    // [wp: M double2][exchange: WARPS*G*BUF double2][G rows: PAIRS*G*ROW doubles][mbarriers: PAIRS]
+    static constexpr size_t smem_bytes() {
+        return sizeof(double2) * (size_t)(M + WARPS * G * Cfg::BUF) + sizeof(double) * (size_t)(PAIRS * G * ROW) + 8 * PAIRS;
+    }
+};
+
+template <int M, bool DER = false>
+__global__ void __launch_bounds__(ConvZP<M>::WARPS * 32, ConvZP<M>::MINB)
+k_conv_z_p(double2* __restrict__ B2, const double* __restrict__ Gk, const double* __restrict__ lane_g,
+           const double2* __restrict__ wp_g, int Ny, long nsteps, double2* __restrict__ out, const DerK kap) {
+    using Z = ConvZP<M>;
+    using Cfg = typename Z::Cfg;
+    constexpr int R = Z::R, T = Z::T, G = Z::G, PAIRS = Z::PAIRS, WARPS = Z::WARPS, H = R / 2, NC = Z::NC, NB2 = Cfg::NB2;
+    extern __shared__ double2 smem[];
+    double2* wp = smem;          // M: w_2M^n, n < M
+    for (int n = threadIdx.x; n < M; n += blockDim.x) wp[n] = wp_g[n];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, q = warp >> 1, b = warp & 1;
+    const int g = lane / T, t = lane % T;
+    double2* buf = smem + M + (warp * G + g) * Cfg::BUF;
+    double2* pbuf = smem + M + ((warp ^ 1) * G + g) * Cfg::BUF;          // the partner's buffer
+    double* gall = reinterpret_cast<double*>(smem + M + WARPS * G * Cfg::BUF);
+    double* gst = gall + (q * G + g) * Z::ROW;
+    uint64_t* gbar = reinterpret_cast<uint64_t*>(gall + PAIRS * G * Z::ROW) + q;
+    if (b == 0 && lane == 0) { mbar_init(gbar, 1); mbar_fence_init(); }
+    __syncthreads();
+    uint32_t gpar = 0;
+    double cc[NB2][NC], tn[NB2][NC];
+#pragma unroll
+    for (int m = 0; m < NB2; ++m)
+#pragma unroll
+        for (int i = 0; i < NC; ++i) {
+            cc[m][i] = lane_g[(t + T * m) * 2 * NC + i];
+            tn[m][i] = lane_g[(t + T * m) * 2 * NC + NC + i];
+        }
+    const int npairs = gridDim.x * PAIRS;
+    const int ny2 = 2 * Ny;
+    auto locate = [&](int s_, int& kx_, int& ky_) {   // position in the visiting order -> (kx, ky)
+        kx_ = s_ / ny2;
+        const int r_ = s_ - kx_ * ny2;
+        ky_ = (r_ & 1) ? ny2 - ((r_ + 1) >> 1) : (r_ >> 1);
+    };
+    for (int step = blockIdx.x * PAIRS + q; step < (int)nsteps; step += npairs) {
+        int kx, ky;
+        locate(step * G + g, kx, ky);
+        const int qy = ky <= Ny ? ky : ny2 - ky;
+        double2* base = B2 + ((long)kx * ny2 + ky) * M;
+        double2* obase = DER ? out + ((long)kx * ny2 + ky) * M : base;
+        double fp = 0.0;
+        if constexpr (DER) fp = kap.x * signed_mode(kx, kap.Nx) + kap.y * signed_mode(ky, Ny);
+        // both warps are past the previous step's reads of the staged rows (the pair barrier ending the combine)
+        if (b == 0 && lane == 0) {
+            mbar_arrive_expect_tx(gbar, G * Z::ROW * 8);
+#pragma unroll
+            for (int gg = 0; gg < G; ++gg) {
+                int kx2, ky2;
+                locate(step * G + gg, kx2, ky2);
+                const int qy2 = ky2 <= Ny ? ky2 : ny2 - ky2;
+                bulk_load(gall + (q * G + gg) * Z::ROW, Gk + ((long)kx2 * (Ny + 1) + qy2) * Z::ROW, Z::ROW * 8, gbar);
+            }
+        }
+        (void)qy;
+        double vr[R], vi[R];
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            const double2 v = base[t + T * i];
+            vr[i] = v.x; vi[i] = v.y;
+        }
+        {   // L2 prefetch of the pair's next pencils, half of the lines from each warp
+            const int s2 = (step + npairs) * G + g;
+            if (step + npairs < (int)nsteps) {
+                int kx2, ky2;
+                locate(s2, kx2, ky2);
+                const double2* nb = B2 + ((long)kx2 * ny2 + ky2) * M;
+                for (int e = (b * T + t) * 8; e < M; e += 2 * T * 8)
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(nb + e));
+            }
+        }
+        if (b) {
+#pragma unroll
+            for (int i = 0; i < R; ++i) cmul(vr[i], vi[i], wp[t + T * i]);
+        }
+#pragma unroll 1
+        for (int pass = 0; pass < 2; ++pass) {
+            fft2_forward_lc<Cfg>(vr, vi, t, buf, cc, tn);
+            if (pass == 0) {
+                mbar_wait(gbar, gpar);
+                gpar ^= 1;
+                const double* gsrc = gst + (b ? M / 2 + 1 : 0);
+                const double* gA = gsrc + t;
+                const double* gB = gsrc + (M - b - t);
+#pragma unroll
+                for (int i = 0; i < R; ++i) {
+                    const double gk = i < R / 2 ? gA[T * i] : gB[-T * i];   // row index min(j, M-b-j), j = t + T i
+                    if constexpr (DER) {
+                        const double cf = gk * (fp + kap.z * signed_mode(2 * (t + T * i) + b, M));
+                        const double a = vr[i];
+                        vr[i] = cf * vi[i]; vi[i] = cf * a;
+                    } else {
+                        vr[i] *= gk; vi[i] *= -gk;
+                    }
+                }
+            }
+        }
+        // v = FFT(conj(Ghat X)) on each branch; y[n] = conj(v_e[n] + w^n v_o[n]).  The odd warp paid for the
+        // pre-twiddle (4 fp64 instructions per point), so the even warp forms the whole sum (4 per point) and
+        // stores the pencil: the two warps of a pair carry the same fp64 load.
+        if (b) {
+            __syncwarp();   // this warp's exchange reads are complete: buf becomes the outbox
+#pragma unroll
+            for (int i = 0; i < R; ++i) buf[t + T * i] = make_double2(vr[i], vi[i]);
+        }
+        bar_sync(1 + q, 64);
+        if (!b) {
+#pragma unroll
+            for (int i = 0; i < R; ++i) {
+                const double2 pv = pbuf[t + T * i];   // v_o[n], n = t + T i
+                const double2 w = wp[t + T * i];
+                const double zr = fma(-w.y, pv.y, fma(w.x, pv.x, vr[i]));
+                const double zi = fma(w.y, pv.x, fma(w.x, pv.y, vi[i]));
+                obase[t + T * i] = make_double2(zr, -zi);
+            }
+        }
+        bar_sync(1 + q, 64);   // the even warp has read the outbox (and both are done with the staged rows)
+    }
+}
+
 // ================================================================================ K1 (v2): fwd_x_r2c_t
 // Tile kernel for the real-to-complex pass along x (M = Nx/2 complex points z[n] = rho[2n] + i rho[2n+1]).
 // Tile = all Nx rows of kC = 16 adjacent columns of the flattened (y, z) plane (one 128-byte line of

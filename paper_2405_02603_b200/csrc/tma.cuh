@@ -72,7 +72,11 @@ __device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t b
 // barriers actually used instead of reserving all 16)
 __device__ __forceinline__ void bar_sync(int id, int nthreads) {
     if (id == 1) asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
-    else asm volatile("bar.sync 2, %0;" ::"r"(nthreads) : "memory");
+    else if (id == 2) asm volatile("bar.sync 2, %0;" ::"r"(nthreads) : "memory");
+    else if (id == 3) asm volatile("bar.sync 3, %0;" ::"r"(nthreads) : "memory");
+    else if (id == 4) asm volatile("bar.sync 4, %0;" ::"r"(nthreads) : "memory");
+    else if (id == 5) asm volatile("bar.sync 5, %0;" ::"r"(nthreads) : "memory");
+    else asm volatile("bar.sync 6, %0;" ::"r"(nthreads) : "memory");
 }
 
 }  // namespace fsp
