@@ -33,8 +33,7 @@ struct fsp_plan {
     // plan-owned device memory
     double2* B1 = nullptr;  // (Nx+1) * Ny * Nz
     double2* B2 = nullptr;  // (Nx+1) * 2Ny * Nz
-    double* Gh = nullptr;   // (Nx+1) * 2Ny * 2Nz   spectrum, full K3-v1 layout (only when Nz = 1024)
-    double* Gk = nullptr;   // (Nx+1)(Ny+1)(Nz+2)   spectrum octant in K3-v2 layout, scale folded in
+    double* Gk = nullptr;   // (Nx+1)(Ny+1)(Nz+2)   spectrum octant in K3's layout, scale folded in
     double* LTz = nullptr;  // lane-constant stage-2 twiddles of the z transform (fft_warp.cuh dft_lane)
     double* LTy = nullptr;  // the same for the y transform (tile kernels)
     bool tile_y = false;    // K2/K4 tile kernels (TMA-staged) are used
@@ -47,7 +46,6 @@ struct fsp_plan {
     CUtensorMap tmB2y;      // B2 as [kx][j][parity][2 Nz doubles], box = 8 columns x 1 parity x <=256 j (K4 input)
     double2* B3 = nullptr;  // second B2-sized buffer, allocated by the first fsp_solve_field (derivative spectra)
     CUtensorMap tmB3y;      // the same view of B3
-    bool z_warp = false;    // K3 v2 (k_conv_z_w) is used
     int chunk_planes = 0;   // > 0: K2-K3-K4 run chunk_planes kx-planes at a time (L2-resident B2)
     int sm_count = 148;
     double* T = nullptr;    // (Nx+1)(Ny+1)(Nz+1)   real-space table
@@ -260,21 +258,6 @@ int launch_inv_y(fsp_plan* p, const double2* B2, double2* B1, int nplanes, doubl
 }
 // DER = false: in place on B2.  DER = true: B2 -> out with the factor -i k_d of `kap` (field output).
 template <int M, bool DER>
-int launch_conv_z_impl(fsp_plan* p, double2* B2, const double* G, int nplanes, double2* out, const DerK kap) {
-    using Cfg = FftCfg<M>;
-    constexpr int P = PencilGroups<Cfg>::P;
-    const long npencils = (long)nplanes * (2 * p->Ny);
-    const size_t smem = sizeof(double2) * (size_t)(2 * M + P * M);
-    CU(cudaFuncSetAttribute(k_conv_z<M, DER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_conv_z<M, DER><<<(unsigned)((npencils + P - 1) / P), P * Cfg::T, smem, p->stream>>>(B2, G, p->Wz, npencils, out, p->Ny, kap);
-    return FSP_OK;
-}
-template <int M>
-int launch_conv_z(fsp_plan* p, double2* B2, const double* G, int nplanes, double2* out, const DerK* kap) {
-    if (kap) return launch_conv_z_impl<M, true>(p, B2, G, nplanes, out, *kap);
-    return launch_conv_z_impl<M, false>(p, B2, G, nplanes, nullptr, DerK{0.0, 0.0, 0.0, 0});
-}
-template <int M, bool DER>
 int launch_conv_z_p_impl(fsp_plan* p, double2* B2, const double* G, int nplanes, double2* out, const DerK kap) {
     using Z = ConvZP<M>;
     const long nsteps = (long)nplanes * (2 * p->Ny) / Z::G;   // pair steps: G pencils each
@@ -421,13 +404,11 @@ int do_fwd_y(fsp_plan* p, int kx0, double2* B2, int np) {
         case 1024: return fn<1024>(__VA_ARGS__);         \
         default: return FSP_ERR_INVALID_ARG;             \
     }
-int do_conv_z_v1(fsp_plan* p, double2* B2, const double* G, int np, double2* out, const DerK* kap) { DISPATCH_YZ(launch_conv_z, p->Nz, p, B2, G, np, out, kap) }
 int do_conv_z_w(fsp_plan* p, double2* B2, const double* G, int np, double2* out, const DerK* kap) { DISPATCH_W(launch_conv_z_w, p->Nz, p, B2, G, np, out, kap) }
 // planes [kx0, kx0 + np) of the spectrum go with the np planes stored at B2.
 // kap == nullptr: in place (phi); otherwise B2 -> out with the derivative factor (whole volume only, kx0 = 0).
 int do_conv_z(fsp_plan* p, double2* B2, int kx0, int np, double2* out = nullptr, const DerK* kap = nullptr) {
-    if (p->z_warp) return do_conv_z_w(p, B2, p->Gk + (size_t)kx0 * (p->Ny + 1) * (p->Nz + 2), np, out, kap);
-    return do_conv_z_v1(p, B2, p->Gh + (size_t)kx0 * (2 * p->Ny) * (2 * p->Nz), np, out, kap);
+    return do_conv_z_w(p, B2, p->Gk + (size_t)kx0 * (p->Ny + 1) * (p->Nz + 2), np, out, kap);
 }
 int make_z_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Nz, &p->LTz, &p->bytes) }
 int make_x_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Nx / 2, &p->LTx, &p->bytes) }
@@ -662,12 +643,9 @@ int precompute_impl(fsp_plan* p) {
     }
     // scale: hx hy hz / (8 Nx Ny Nz) (inverse DFT) / 2 (K1 produces 2X)
     const double gscale = hx * hy * hz / (8.0 * (double)Nx * (double)Ny * (double)Nz) * 0.5;
-    if (p->z_warp) {
+    {
         const long gk_total = (long)(Nx + 1) * (Ny + 1) * (Nz + 2);
         k_layout_spectrum_oct<<<grid_for(gk_total, blk), blk, 0, p->stream>>>(p->Goct, p->Gk, Nx, Ny, Nz, gscale);
-    } else {
-        const long gh_total = (long)(Nx + 1) * (2 * Ny) * (2 * Nz);
-        k_layout_spectrum<<<grid_for(gh_total, blk), blk, 0, p->stream>>>(p->Goct, p->Gh, Nx, Ny, Nz, gscale);
     }
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(p->stream));
@@ -676,7 +654,7 @@ int precompute_impl(fsp_plan* p) {
 }
 
 void free_plan_memory(fsp_plan* p) {
-    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->B3); cudaFree(p->rho_pad); cudaFree(p->phi_pad); cudaFree(p->E_stage); cudaFree(p->rho_stage2); cudaFree(p->phi_stage2); cudaFree(p->Gh); cudaFree(p->Gk); cudaFree(p->LTz); cudaFree(p->LTy); cudaFree(p->LTx); cudaFree(p->T); cudaFree(p->Goct);
+    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->B3); cudaFree(p->rho_pad); cudaFree(p->phi_pad); cudaFree(p->E_stage); cudaFree(p->rho_stage2); cudaFree(p->phi_stage2); cudaFree(p->Gk); cudaFree(p->LTz); cudaFree(p->LTy); cudaFree(p->LTx); cudaFree(p->T); cudaFree(p->Goct);
     cudaFree(p->Wx); cudaFree(p->Wy); cudaFree(p->Wz); cudaFree(p->rho_stage); cudaFree(p->phi_stage);
     for (cudaEvent_t e : p->events) cudaEventDestroy(e);
     p->events.clear();
@@ -742,17 +720,15 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
     if (cudaGetDevice(&p->device) != cudaSuccess || cudaGetDeviceProperties(&prop, p->device) != cudaSuccess) rc = FSP_ERR_NO_DEVICE;
     if (rc == FSP_OK && prop.major != 10) rc = FSP_ERR_NO_DEVICE;  // the library holds sm_100a code only
     const size_t n1 = (size_t)(Nx + 1) * Ny * Nz, n2 = (size_t)(Nx + 1) * 2 * Ny * Nz;
-    const size_t ng = (size_t)(Nx + 1) * 2 * Ny * 2 * Nz, nt = (size_t)(Nx + 1) * (Ny + 1) * (Nz + 1);
+    const size_t nt = (size_t)(Nx + 1) * (Ny + 1) * (Nz + 1);
     if (rc == FSP_OK && p->padded) rc = dev_alloc(&p->rho_pad, (size_t)Nx * Ny * Nz, &p->bytes);
     if (rc == FSP_OK && p->padded) rc = dev_alloc(&p->phi_pad, (size_t)Nx * Ny * Nz, &p->bytes);
     if (rc == FSP_OK && p->padded && cudaMemset(p->rho_pad, 0, sizeof(double) * (size_t)Nx * Ny * Nz) != cudaSuccess) rc = FSP_ERR_CUDA;
     if (rc == FSP_OK) rc = dev_alloc(&p->B1, n1, &p->bytes);
     if (rc == FSP_OK) rc = dev_alloc(&p->B2, n2, &p->bytes);
-    p->z_warp = true;   // every Nz has a warp-level K3 (Nz = 1024: warp pairs, k_conv_z_p)
     p->sm_count = prop.multiProcessorCount > 0 ? prop.multiProcessorCount : 148;
-    if (rc == FSP_OK && !p->z_warp) rc = dev_alloc(&p->Gh, ng, &p->bytes);
-    if (rc == FSP_OK && p->z_warp) rc = dev_alloc(&p->Gk, (size_t)(Nx + 1) * (Ny + 1) * (Nz + 2), &p->bytes);
-    if (rc == FSP_OK && p->z_warp) rc = make_z_lane_table(p);
+    if (rc == FSP_OK) rc = dev_alloc(&p->Gk, (size_t)(Nx + 1) * (Ny + 1) * (Nz + 2), &p->bytes);
+    if (rc == FSP_OK) rc = make_z_lane_table(p);
     p->tile_x = (Nx == 128 || Nx == 256 || Nx == 512) && ((long)Ny * Nz) % kC == 0;
     if (rc == FSP_OK && p->tile_x) rc = make_x_lane_table(p);
     if (rc == FSP_OK && p->tile_x) {
@@ -1046,9 +1022,9 @@ double fsp_model_bytes_per_solve(const fsp_plan* p, double* per_kernel) {
     double k[FSP_NUM_SOLVE_KERNELS];
     k[0] = 8.0 * V + 16.0 * H;                      // K1: read rho, write B1
     k[1] = 16.0 * H + 32.0 * H;                     // K2: read B1, write B2
-    // K3: read+write B2, read Ghat (real): the unique octant once (v2), or 2Nz values per pencil (v1)
+    // K3: read+write B2, read the unique octant of Ghat (real) once
     k[2] = 32.0 * H + 32.0 * H +
-           (p->z_warp ? 8.0 * (double)(p->Nx + 1) * (p->Ny + 1) * (p->Nz + 2) : 8.0 * 4.0 * H);
+           8.0 * (double)(p->Nx + 1) * (p->Ny + 1) * (p->Nz + 2);
     k[3] = 32.0 * H + 16.0 * H;                     // K4
     k[4] = 16.0 * H + 8.0 * V;                      // K5
     double tot = 0.0;

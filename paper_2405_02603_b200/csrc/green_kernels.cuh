@@ -196,24 +196,7 @@ __global__ void k_restrict_vg(const double2* __restrict__ g, double* __restrict_
     }
 }
 
-// Spectrum layout for K3: Gh[(kx*2Ny + ky)][parity][j] = scale * Goct[kx][min(ky,2Ny-ky)][min(kz,2Nz-kz)],
-// kz = 2j + parity  (F{G2} is even under k -> 2N-k).
-__global__ void k_layout_spectrum(const double* __restrict__ Goct, double* __restrict__ Gh, int Nx,
-                                  int Ny, int Nz, double scale) {
-    const long total = (long)(Nx + 1) * (2 * Ny) * (2 * Nz);
-    for (long o = blockIdx.x * (long)blockDim.x + threadIdx.x; o < total; o += (long)gridDim.x * blockDim.x) {
-        const int j = (int)(o % Nz);
-        const int par = (int)((o / Nz) & 1);
-        const long pen = o / (2 * Nz);
-        const int ky = (int)(pen % (2 * Ny));
-        const long kx = pen / (2 * Ny);
-        const int kz = 2 * j + par;
-        const int qy = ky <= Ny ? ky : 2 * Ny - ky, qz = kz <= Nz ? kz : 2 * Nz - kz;
-        Gh[o] = scale * Goct[(kx * (Ny + 1) + qy) * (Nz + 1) + qz];
-    }
-}
-
-// Spectrum layout for K3 v2 (k_conv_z_w): the unique octant only, rows de-interleaved by parity of kz:
+// Spectrum layout for K3 (k_conv_z_p, k_conv_z_w): the unique octant only, rows de-interleaved by parity of kz:
 //   Gk[(kx*(Ny+1) + qy)*(Nz+2) + m]              = scale * Goct[kx][qy][2m],    m <= Nz/2   (E)
 //   Gk[(kx*(Ny+1) + qy)*(Nz+2) + Nz/2 + 1 + m]   = scale * Goct[kx][qy][2m+1],  m <  Nz/2   (O)
 __global__ void k_layout_spectrum_oct(const double* __restrict__ Goct, double* __restrict__ Gk, int Nx,

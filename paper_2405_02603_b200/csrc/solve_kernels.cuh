@@ -364,83 +364,6 @@ k_inv_y_t(const __grid_constant__ CUtensorMap tmB2, double2* __restrict__ B1, co
     }
 }
 
-// ===================================================================================== K3: conv_z
-// Contiguous pencils of M = Nz complex; T threads per pencil (t fastest), P pencils per CTA.
-// Gh: [pencil][2][M] doubles, plane 0 = Ghat[2j] (even), plane 1 = Ghat[2j+1] (odd), scale folded in.
-template <class Cfg> struct PencilGroups { static constexpr int P = (Cfg::T >= 128) ? 1 : 128 / Cfg::T; };
-
-template <int M, bool DER = false>
-__global__ void __launch_bounds__(PencilGroups<FftCfg<M>>::P* FftCfg<M>::T)
-k_conv_z(double2* __restrict__ B2, const double* __restrict__ Gh, const double2* __restrict__ Wg,
-         long npencils, double2* __restrict__ out, int Ny, const DerK kap) {
-    using Cfg = FftCfg<M>;
-    constexpr int R = Cfg::R, T = Cfg::T, P = PencilGroups<Cfg>::P, LTAB = 2 * M;
-    extern __shared__ double2 smem[];
-    double2* Ws = smem;
-    double2* xb = smem + LTAB;  // P * M
-    load_table<LTAB>(Ws, Wg);
-    const int tid = threadIdx.x;
-    const int t = tid % T, c = tid / T;
-    double2* buf = xb + c * M;
-    const long pencil = (long)blockIdx.x * P + c;
-    const bool valid = pencil < npencils;
-    double2* base = B2 + (valid ? pencil : 0) * M;
-    double2* obase = DER ? out + (valid ? pencil : 0) * M : base;
-    double fp = 0.0;
-    if constexpr (DER) {
-        const int kx = (int)((valid ? pencil : 0) / (2 * Ny)), ky = (int)((valid ? pencil : 0) % (2 * Ny));
-        fp = kap.x * signed_mode(kx, kap.Nx) + kap.y * signed_mode(ky, Ny);
-    }
-    const double* ge = Gh + (valid ? pencil : 0) * 2 * M;
-    const double* go = ge + M;
-
-    double xr[R], xi[R], vr[R], vi[R], gg[R];
-#pragma unroll
-    for (int i = 0; i < R; ++i) {
-        double2 v = valid ? base[t + T * i] : make_double2(0.0, 0.0);
-        xr[i] = v.x; xi[i] = v.y;
-    }
-#pragma unroll
-    for (int i = 0; i < R; ++i) gg[i] = go[t + T * i];
-    __syncthreads();
-    // odd half-spectrum: y_o = conj(w^n) IFFT( Go * FFT(x w^n) )
-#pragma unroll
-    for (int i = 0; i < R; ++i) { vr[i] = xr[i]; vi[i] = xi[i]; cmul(vr[i], vi[i], Ws[t + T * i]); }
-    fft_forward<Cfg, 1, LTAB>(vr, vi, t, buf, Ws);
-#pragma unroll
-    for (int i = 0; i < R; ++i) {
-        if constexpr (DER) {   // -i f Ghat X = f Ghat (X.im - i X.re)
-            const double cf = gg[i] * (fp + kap.z * signed_mode(2 * (t + T * i) + 1, M));
-            const double a = vr[i];
-            vr[i] = cf * vi[i]; vi[i] = -cf * a;
-        } else {
-            vr[i] *= gg[i]; vi[i] *= gg[i];
-        }
-    }
-#pragma unroll
-    for (int i = 0; i < R; ++i) gg[i] = ge[t + T * i];
-    fft_inverse<Cfg, 1, LTAB>(vr, vi, t, buf, Ws);
-#pragma unroll
-    for (int i = 0; i < R; ++i) cmul_conj(vr[i], vi[i], Ws[t + T * i]);
-    // even half-spectrum
-    fft_forward<Cfg, 1, LTAB>(xr, xi, t, buf, Ws);
-#pragma unroll
-    for (int i = 0; i < R; ++i) {
-        if constexpr (DER) {
-            const double cf = gg[i] * (fp + kap.z * signed_mode(2 * (t + T * i), M));
-            const double a = xr[i];
-            xr[i] = cf * xi[i]; xi[i] = -cf * a;
-        } else {
-            xr[i] *= gg[i]; xi[i] *= gg[i];
-        }
-    }
-    fft_inverse<Cfg, 1, LTAB>(xr, xi, t, buf, Ws);
-    if (valid) {
-#pragma unroll
-        for (int i = 0; i < R; ++i) obase[t + T * i] = make_double2(xr[i] + vr[i], xi[i] + vi[i]);
-    }
-}
-
 // ============================================================================== K3 (v2): conv_z_w
 // One pencil per group of 2T lanes of a warp: lanes with b = 0 run the even
 // half-spectrum branch, lanes with b = 1 the odd one, each a two-stage single-exchange FFT of
