@@ -490,8 +490,7 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
                                                 : (i < R / 2 ? __ldg(gA + T * i) : __ldg(gB - T * i));
                     if constexpr (DER) {   // conj(-i f Ghat X) = f Ghat (X.im + i X.re)
                         const double cf = gk * (fp + kap.z * signed_mode(2 * j + b, M));
-                        const double a = vr[i];
-                        vr[i] = cf * vi[i]; vi[i] = cf * a;
+                        vr[i] *= cf; vi[i] *= -cf;   // the factor -i is applied to the final sum
                     } else {
                         vr[i] *= gk; vi[i] *= -gk;
                     }
@@ -514,7 +513,7 @@ k_conv_z_w(double2* __restrict__ B2, const double* __restrict__ Gk, const double
             const double2 w = b ? make_double2(w0.y, -w0.x) : w0;
             const double zr = fma(-w.y, qi, fma(w.x, qr, ar));
             const double zi = fma(w.y, qr, fma(w.x, qi, ai));
-            obase[t + T * o] = make_double2(zr, -zi);
+            obase[t + T * o] = DER ? make_double2(-zi, -zr) : make_double2(zr, -zi);   // DER: -i y
         }
     }
 }
@@ -628,13 +627,19 @@ k_conv_z_p(double2* __restrict__ B2, const double* __restrict__ Gk, const double
                 const double* gsrc = gst + (b ? M / 2 + 1 : 0);
                 const double* gA = gsrc + t;
                 const double* gB = gsrc + (M - b - t);
+                const double fz0 = fp + kap.z * (double)(2 * t + b);   // DER only
+                const bool nyq = (2 * t + b) == 0;                      // register R/2 of this lane is kz = M
 #pragma unroll
                 for (int i = 0; i < R; ++i) {
                     const double gk = i < R / 2 ? gA[T * i] : gB[-T * i];   // row index min(j, M-b-j), j = t + T i
                     if constexpr (DER) {
-                        const double cf = gk * (fp + kap.z * signed_mode(2 * (t + T * i) + b, M));
-                        const double a = vr[i];
-                        vr[i] = cf * vi[i]; vi[i] = cf * a;
+                        // signed mode of kz = 2 (t + T i) + b: kz for the first half of the registers, kz - 2M for
+                        // the second (T R = M), zero at the Nyquist index kz = M: a lane constant plus a
+                        // compile-time offset, no integer arithmetic per point
+                        // (the factor -i itself is applied to the final sum: F^-1 is linear)
+                        double cf = gk * fma(kap.z, (double)(i < R / 2 ? 2 * T * i : 2 * T * i - 2 * M), fz0);
+                        if (i == R / 2) cf = nyq ? gk * fp : cf;
+                        vr[i] *= cf; vi[i] *= -cf;
                     } else {
                         vr[i] *= gk; vi[i] *= -gk;
                     }
@@ -657,7 +662,7 @@ k_conv_z_p(double2* __restrict__ B2, const double* __restrict__ Gk, const double
                 const double2 w = wp[t + T * i];
                 const double zr = fma(-w.y, pv.y, fma(w.x, pv.x, vr[i]));
                 const double zi = fma(w.y, pv.x, fma(w.x, pv.y, vi[i]));
-                obase[t + T * i] = make_double2(zr, -zi);
+                obase[t + T * i] = DER ? make_double2(-zi, -zr) : make_double2(zr, -zi);   // DER: -i y
             }
         }
         bar_sync(1 + q, 64);   // the even warp has read the outbox (and both are done with the staged rows)
@@ -848,6 +853,7 @@ k_inv_x_t(const __grid_constant__ CUtensorMap tmB1, const double2* __restrict__ 
         }
     const double2 lam_n = Wg[2 * t];          // w_N^t
     const double2 lam_k = Wg[2 * t + grp];    // w_2N^(2t+g)
+    const double kd0 = kder * (double)(2 * t + grp);   // DER only
     if (tid == 0) { mbar_init(&full[0], 1); mbar_init(&full[1], 1); mbar_fence_init(); }
     __syncthreads();
     double2* Xg = X + grp * (M * kC);
@@ -881,10 +887,10 @@ k_inv_x_t(const __grid_constant__ CUtensorMap tmB1, const double2* __restrict__ 
             double2 bq;
             if (grp) bq = Ec[(M - 1 - j) * kC];
             else bq = (j == 0) ? XN[c] : Ec[(M - j) * kC];
-            if constexpr (DER) {
-                const int k = 2 * j + grp;
-                mul_minus_i(a.x, a.y, kder * (double)k);
-                mul_minus_i(bq.x, bq.y, k == 0 ? 0.0 : kder * (double)(N - k));
+            if constexpr (DER) {   // k = (2t + grp) + 2T i: a lane constant plus a compile-time multiple
+                const double ck = fma(kder * (double)(2 * T), (double)i, kd0);
+                mul_minus_i(a.x, a.y, ck);
+                mul_minus_i(bq.x, bq.y, (i == 0 && kd0 == 0.0) ? 0.0 : kder * (double)N - ck);   // N - k; row N is the Nyquist row
             }
             const double br = bq.x, bi = -bq.y;
             const double sr = a.x + br, si = a.y + bi;
