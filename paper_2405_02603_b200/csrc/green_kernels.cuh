@@ -156,8 +156,36 @@ __global__ void k_dct1_tile(const double* __restrict__ in, double* __restrict__ 
         af[2 * (sq + k) + (c & 1)] = v;
         if (k > 0 && k < n) af[2 * (sq + Lf - k) + (c & 1)] = v;
     }
-    // radix-2 Stockham, all S sequences together
-    for (int Ns = 1; Ns < Lf; Ns <<= 1) {
+    // Stockham autosort, all S sequences together: radix-4 stages (half the exchanges and barriers of radix 2),
+    // then one radix-2 stage if log2(Lf) is odd.  Sign +: exp(+2 pi i ..); the input is real-even, so the sign
+    // does not matter for the result.
+    int Ns = 1;
+    const int quarter = Lf >> 2;
+    for (; Ns * 4 <= Lf; Ns <<= 2) {
+        __syncthreads();
+        const int tstep = quarter / Ns;   // w1 = exp(2 pi i k / (4 Ns)) = tw[k * Lf / (4 Ns)]
+        for (int e = threadIdx.x; e < S * quarter; e += blockDim.x) {
+            const int q = e / quarter, j = e - q * quarter;
+            const int k = j & (Ns - 1);
+            const double2 w1 = tw[k * tstep], w2 = tw[2 * k * tstep];
+            const double2 w3 = make_double2(w1.x * w2.x - w1.y * w2.y, w1.x * w2.y + w1.y * w2.x);
+            const double2* aq = a + (long)q * Lf;
+            double2* bq = b + (long)q * Lf;
+            const double2 x0 = aq[j], y1 = aq[j + quarter], y2 = aq[j + 2 * quarter], y3 = aq[j + 3 * quarter];
+            const double2 x1 = make_double2(y1.x * w1.x - y1.y * w1.y, y1.x * w1.y + y1.y * w1.x);
+            const double2 x2 = make_double2(y2.x * w2.x - y2.y * w2.y, y2.x * w2.y + y2.y * w2.x);
+            const double2 x3 = make_double2(y3.x * w3.x - y3.y * w3.y, y3.x * w3.y + y3.y * w3.x);
+            const double2 s02 = make_double2(x0.x + x2.x, x0.y + x2.y), d02 = make_double2(x0.x - x2.x, x0.y - x2.y);
+            const double2 s13 = make_double2(x1.x + x3.x, x1.y + x3.y), d13 = make_double2(x1.x - x3.x, x1.y - x3.y);
+            const int j0 = ((j - k) << 2) + k;
+            bq[j0] = make_double2(s02.x + s13.x, s02.y + s13.y);
+            bq[j0 + Ns] = make_double2(d02.x - d13.y, d02.y + d13.x);          // + i (x1 - x3)
+            bq[j0 + 2 * Ns] = make_double2(s02.x - s13.x, s02.y - s13.y);
+            bq[j0 + 3 * Ns] = make_double2(d02.x + d13.y, d02.y - d13.x);      // - i (x1 - x3)
+        }
+        double2* t2 = a; a = b; b = t2;
+    }
+    for (; Ns < Lf; Ns <<= 1) {
         __syncthreads();
         const int tstep = half / Ns;
         for (int e = threadIdx.x; e < S * half; e += blockDim.x) {
