@@ -391,3 +391,23 @@ def test_any_mesh_size_field_and_accuracy():
     emb[:20, :12, :36] = w2.rho
     _, Eo = oracle.OraclePlan(Np, w2.h, oracle.HOCKNEY).precompute_green().solve_field(emb)
     check(E2, Eo[:, :20, :12, :36])
+
+
+@pytest.mark.parametrize("N", [(256, 256, 256), (128, 128, 512), (64, 64, 1024)])
+def test_repeated_solves_are_bitwise_identical_at_bench_sizes(N):
+    """A race in the pair kernel's hand-over (named barriers, staged spectrum rows) or in the tile kernels'
+    buffer recycling would show as run-to-run differences: five solves of dense random data, bit for bit."""
+    h = tuple(1.0 / n for n in N)
+    with binding.Plan(N, h, binding.HOCKNEY) as p:
+        p.precompute_green()
+        g = torch.Generator(device="cuda").manual_seed(5)
+        rho = torch.rand(N, dtype=torch.float64, device="cuda", generator=g) - 0.5
+        first = p.solve(rho).clone()
+        keep = rho.clone()
+        for _ in range(4):
+            assert torch.equal(p.solve(rho), first)
+        assert torch.equal(rho, keep) and bool(torch.isfinite(first).all())
+        _, E1 = p.solve_field(rho, want_phi=False)
+        E1 = E1.clone()
+        _, E2 = p.solve_field(rho, want_phi=False)
+        assert torch.equal(E1, E2)
