@@ -394,6 +394,18 @@ def run_b200(args):
         pts = ws.N[0] * ws.N[1] * ws.N[2] / dt
         line["cpu_baseline"] = {"value": pts / V, "unit": "solves/s", "cores": threads, "kind": "oracle",
                                 "sample": desc, "grid_points_per_s": pts}
+        try:   # single-thread time beside the all-cores one (one 64^3 solve, same code)
+            import oracle
+            w1 = _sample_workload(args.workload, 64)
+            p1 = oracle.OraclePlan(w1.N, w1.h, oracle.HOCKNEY).precompute_green()
+            oracle.set_num_threads(1)
+            p1.solve(w1.rho)
+            t0 = time.perf_counter(); p1.solve(w1.rho); t1 = time.perf_counter() - t0
+            oracle.set_num_threads(threads)
+            line["cpu_baseline"]["single_thread"] = {"value": (64 ** 3 / t1) / V, "unit": "solves/s", "cores": 1,
+                                                     "sample": "one 64^3 solve, grid-points/s scaled to the workload's V"}
+        except Exception as ex:
+            line["cpu_baseline"]["single_thread"] = {"error": repr(ex)[:120]}
     if rank == 0:
         print(json.dumps(line))
     if dist:
