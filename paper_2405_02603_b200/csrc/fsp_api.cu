@@ -66,8 +66,6 @@ struct fsp_plan {
 
 namespace {
 
-bool pow2_in(int n, int lo, int hi) { return n >= lo && n <= hi && (n & (n - 1)) == 0; }
-
 int map_cuda(cudaError_t e) {
     if (e == cudaSuccess) return FSP_OK;
     if (e == cudaErrorMemoryAllocation) return FSP_ERR_OUT_OF_MEMORY;

@@ -549,7 +549,7 @@ k_conv_z_p(double2* __restrict__ B2, const double* __restrict__ Gk, const double
            const double2* __restrict__ wp_g, int Ny, long nsteps, double2* __restrict__ out, const DerK kap) {
     using Z = ConvZP<M>;
     using Cfg = typename Z::Cfg;
-    constexpr int R = Z::R, T = Z::T, G = Z::G, PAIRS = Z::PAIRS, WARPS = Z::WARPS, H = R / 2, NC = Z::NC, NB2 = Cfg::NB2;
+    constexpr int R = Z::R, T = Z::T, G = Z::G, PAIRS = Z::PAIRS, WARPS = Z::WARPS, NC = Z::NC, NB2 = Cfg::NB2;
     extern __shared__ double2 smem[];
     double2* wp = smem;          // M: w_2M^n, n < M
     for (int n = threadIdx.x; n < M; n += blockDim.x) wp[n] = wp_g[n];
