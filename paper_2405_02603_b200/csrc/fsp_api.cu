@@ -202,7 +202,7 @@ int make_tensor_map(CUtensorMap* tm, void* base, int rank, const cuuint64_t* dim
 template <int M>
 int launch_fwd_y_t(fsp_plan* p, int kx0, double2* B2, int nplanes) {
     using Y = TileY<M>;
-    const long ntiles = (long)nplanes * (p->Nz / kW);
+    const long ntiles = (long)nplanes * (p->Nz / Y::KW);
     const size_t smem = Y::smem_bytes();
     static int occ = 0;
     if (occ == 0) {
@@ -383,6 +383,7 @@ int do_fwd_x(fsp_plan* p, const double* rho) {
 }
 int do_fwd_y(fsp_plan* p, int kx0, double2* B2, int np) {
     if (p->tile_y) {
+        if (p->Ny == 1024) return launch_fwd_y_t<1024>(p, kx0, B2, np);
         if (p->Ny == 512) return launch_fwd_y_t<512>(p, kx0, B2, np);
         if (p->Ny == 256) return launch_fwd_y_t<256>(p, kx0, B2, np);
         return launch_fwd_y_t<128>(p, kx0, B2, np);
@@ -414,7 +415,7 @@ int make_y_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Ny, &p->LTy, 
 template <int M, bool DER>
 int launch_inv_y_t_impl(fsp_plan* p, const CUtensorMap& tm, double2* B1, int nplanes, double kder) {
     using Y = TileYI<M>;
-    const long ntiles = (long)nplanes * (p->Nz / kW);
+    const long ntiles = (long)nplanes * (p->Nz / Y::KW);
     const size_t smem = Y::smem_bytes();
     static int occ = 0;
     if (occ == 0) {
@@ -435,6 +436,7 @@ int launch_inv_y_t(fsp_plan* p, const CUtensorMap& tm, double2* B1, int nplanes,
 int do_inv_y(fsp_plan* p, const double2* B2, double2* B1, int np, double kder = 0.0) {
     if (p->tile_y && (B2 == p->B2 || (p->B3 && B2 == p->B3))) {
         const CUtensorMap& tm = B2 == p->B2 ? p->tmB2y : p->tmB3y;
+        if (p->Ny == 1024) return launch_inv_y_t<1024>(p, tm, B1, np, kder);
         if (p->Ny == 512) return launch_inv_y_t<512>(p, tm, B1, np, kder);
         if (p->Ny == 256) return launch_inv_y_t<256>(p, tm, B1, np, kder);
         return launch_inv_y_t<128>(p, tm, B1, np, kder);
@@ -736,18 +738,19 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
         const cuuint32_t box[3] = {2 * kC, 1, (cuuint32_t)(Nx / 2 < 256 ? Nx / 2 : 256)};
         rc = make_tensor_map(&p->tmB1x, p->B1, 3, dims, strides, box);
     }
-    p->tile_y = (Ny == 128 || Ny == 256 || Ny == 512) && Nz >= kW;
+    p->tile_y = (Ny == 128 || Ny == 256 || Ny == 512 || Ny == 1024) && Nz >= kW;
+    const cuuint32_t kwy = Ny == 1024 ? 4 : kW;   // TileY<M>::KW: columns per tile of the y tile kernels
     if (rc == FSP_OK && p->tile_y) rc = make_y_lane_table(p);
     if (rc == FSP_OK && p->tile_y) {
         const cuuint64_t dims[3] = {(cuuint64_t)2 * Nz, (cuuint64_t)Ny, (cuuint64_t)(Nx + 1)};
         const cuuint64_t strides[2] = {(cuuint64_t)Nz * 16, (cuuint64_t)Ny * Nz * 16};
-        const cuuint32_t box[3] = {2 * kW, (cuuint32_t)(Ny < 256 ? Ny : 256), 1};
+        const cuuint32_t box[3] = {2 * kwy, (cuuint32_t)(Ny < 256 ? Ny : 256), 1};
         rc = make_tensor_map(&p->tmB1y, p->B1, 3, dims, strides, box);
     }
     if (rc == FSP_OK && p->tile_y) {
         const cuuint64_t dims[4] = {(cuuint64_t)2 * Nz, 2, (cuuint64_t)Ny, (cuuint64_t)(Nx + 1)};
         const cuuint64_t strides[3] = {(cuuint64_t)Nz * 16, (cuuint64_t)2 * Nz * 16, (cuuint64_t)2 * Ny * Nz * 16};
-        const cuuint32_t box[4] = {2 * kW, 1, (cuuint32_t)(Ny < 256 ? Ny : 256), 1};
+        const cuuint32_t box[4] = {2 * kwy, 1, (cuuint32_t)(Ny < 256 ? Ny : 256), 1};
         rc = make_tensor_map(&p->tmB2y, p->B2, 4, dims, strides, box);
     }
     if (rc == FSP_OK) rc = dev_alloc(&p->T, nt, &p->bytes);
@@ -945,7 +948,7 @@ int fsp_solve_field(fsp_plan* p, const double* rho_dev, double* phi_dev, double*
         if (p->tile_y) {
             const cuuint64_t dims[4] = {(cuuint64_t)2 * p->Nz, 2, (cuuint64_t)p->Ny, (cuuint64_t)(p->Nx + 1)};
             const cuuint64_t strides[3] = {(cuuint64_t)p->Nz * 16, (cuuint64_t)2 * p->Nz * 16, (cuuint64_t)2 * p->Ny * p->Nz * 16};
-            const cuuint32_t box[4] = {2 * kW, 1, (cuuint32_t)(p->Ny < 256 ? p->Ny : 256), 1};
+            const cuuint32_t box[4] = {2 * (cuuint32_t)(p->Ny == 1024 ? 4 : kW), 1, (cuuint32_t)(p->Ny < 256 ? p->Ny : 256), 1};
             if ((rc = make_tensor_map(&p->tmB3y, p->B3, 4, dims, strides, box)) != FSP_OK) return rc;
         }
     }

@@ -131,13 +131,14 @@ template <int M>
 struct TileY {
     using Cfg = Fft2Cfg<M>;
     static constexpr int T = Cfg::T, R = Cfg::R;
-    static constexpr int GT = kW * T;             // threads per group
+    static constexpr int KW = (M >= 1024) ? 4 : kW;   // columns per tile: 1024 rows x 8 columns would not fit shared memory
+    static constexpr int GT = KW * T;             // threads per group
     static constexpr int THREADS = 2 * GT;
     static constexpr int NC = LaneTw<Cfg::R2>::NC;
     static constexpr int MINB = (M >= 512) ? 1 : (M >= 256 ? 2 : 4);
     static constexpr int BOXR = M < 256 ? M : 256;   // rows per TMA box (box dimensions are limited to 256)
     // [mbarriers: 128 B][X: M*kW][E: 2 groups x M*kW][wp: M]
-    static constexpr size_t smem_bytes() { return 128 + sizeof(double2) * (size_t)(3 * M * kW + M); }
+    static constexpr size_t smem_bytes() { return 128 + sizeof(double2) * (size_t)(3 * M * KW + M); }
 };
 
 template <int M>
@@ -146,14 +147,14 @@ k_fwd_y_t(const __grid_constant__ CUtensorMap tmB1, double2* __restrict__ B2, co
           const double2* __restrict__ wp_g, int Nz, int kx0, long ntiles) {
     using Y = TileY<M>;
     using Cfg = typename Y::Cfg;
-    constexpr int R = Y::R, T = Y::T, GT = Y::GT, NC = Y::NC, NB2 = Cfg::NB2;
+    constexpr int R = Y::R, T = Y::T, GT = Y::GT, NC = Y::NC, NB2 = Cfg::NB2, KW = Y::KW;
     extern __shared__ __align__(128) unsigned char smraw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smraw);
     double2* X = reinterpret_cast<double2*>(smraw + 128);
-    double2* E = X + M * kW;
-    double2* wp = E + 2 * M * kW;
+    double2* E = X + M * KW;
+    double2* wp = E + 2 * M * KW;
     const int tid = threadIdx.x;
-    const int grp = tid / GT, gt = tid % GT, c = gt % kW, t = gt / kW;
+    const int grp = tid / GT, gt = tid % GT, c = gt % KW, t = gt / KW;
     for (int n = tid; n < M; n += Y::THREADS) wp[n] = wp_g[n];
     double cc[NB2][NC], tn[NB2][NC];
 #pragma unroll
@@ -165,17 +166,17 @@ k_fwd_y_t(const __grid_constant__ CUtensorMap tmB1, double2* __restrict__ B2, co
         }
     if (tid == 0) { mbar_init(full, 1); mbar_fence_init(); }
     __syncthreads();
-    const int nzb = Nz / kW;
+    const int nzb = Nz / KW;
     auto issue = [&](long tile) {   // one thread: arm the barrier, then one TMA per box of rows
         const int kx = (int)(tile / nzb), zb = (int)(tile % nzb);
-        mbar_arrive_expect_tx(full, (uint32_t)(M * kW * sizeof(double2)));
+        mbar_arrive_expect_tx(full, (uint32_t)(M * KW * sizeof(double2)));
 #pragma unroll
-        for (int r0 = 0; r0 < M; r0 += Y::BOXR) tma_load_3d(X + r0 * kW, &tmB1, full, zb * kW * 2, r0, kx0 + kx);
+        for (int r0 = 0; r0 < M; r0 += Y::BOXR) tma_load_3d(X + r0 * KW, &tmB1, full, zb * KW * 2, r0, kx0 + kx);
     };
     long tile = blockIdx.x;
     if (tid == 0 && tile < ntiles) issue(tile);
     uint32_t parity = 0;
-    double2* Ec = E + grp * (M * kW) + c;
+    double2* Ec = E + grp * (M * KW) + c;
     for (; tile < ntiles; tile += gridDim.x) {
         const long kx = tile / nzb;
         const int zb = (int)(tile % nzb);
@@ -184,7 +185,7 @@ k_fwd_y_t(const __grid_constant__ CUtensorMap tmB1, double2* __restrict__ B2, co
         parity ^= 1;
 #pragma unroll
         for (int i = 0; i < R; ++i) {
-            const double2 v = X[(t + T * i) * kW + c];
+            const double2 v = X[(t + T * i) * KW + c];
             vr[i] = v.x; vi[i] = v.y;
         }
         __syncthreads();   // every thread holds its part of the tile: X may be refilled
@@ -193,8 +194,8 @@ k_fwd_y_t(const __grid_constant__ CUtensorMap tmB1, double2* __restrict__ B2, co
 #pragma unroll
             for (int i = 0; i < R; ++i) cmul(vr[i], vi[i], wp[t + T * i]);
         }
-        fft2_forward_tile<Cfg, kW>(vr, vi, t, Ec, 1 + grp, cc, tn);
-        double2* out = B2 + ((kx * 2 * M + grp) * (long)Nz + zb * kW + c);
+        fft2_forward_tile<Cfg, KW>(vr, vi, t, Ec, 1 + grp, cc, tn);
+        double2* out = B2 + ((kx * 2 * M + grp) * (long)Nz + zb * KW + c);
 #pragma unroll
         for (int i = 0; i < R; ++i) out[(long)(2 * (t + T * i)) * Nz] = make_double2(vr[i], vi[i]);
     }
@@ -270,12 +271,13 @@ template <int M>
 struct TileYI {
     using Cfg = Fft2Cfg<M>;
     static constexpr int T = Cfg::T, R = Cfg::R;
-    static constexpr int GT = kW * T, THREADS = 2 * GT;
+    static constexpr int KW = (M >= 1024) ? 4 : kW;
+    static constexpr int GT = KW * T, THREADS = 2 * GT;
     static constexpr int NC = LaneTw<Cfg::R2>::NC;
     static constexpr int MINB = (M >= 512) ? 1 : (M >= 256 ? 2 : 4);
     static constexpr int BOXR = M < 256 ? M : 256;
     // [mbarriers: 128 B][X: 2 groups x M*kW][C: 2 groups x (M/2)*kW][wp: M]
-    static constexpr size_t smem_bytes() { return 128 + sizeof(double2) * (size_t)(3 * M * kW + M); }
+    static constexpr size_t smem_bytes() { return 128 + sizeof(double2) * (size_t)(3 * M * KW + M); }
 };
 
 template <int M, bool DER = false>
@@ -284,14 +286,14 @@ k_inv_y_t(const __grid_constant__ CUtensorMap tmB2, double2* __restrict__ B1, co
           const double2* __restrict__ wp_g, int Nz, long ntiles, const double kder) {
     using Y = TileYI<M>;
     using Cfg = typename Y::Cfg;
-    constexpr int R = Y::R, T = Y::T, GT = Y::GT, NC = Y::NC, NB2 = Cfg::NB2, H = R / 2;
+    constexpr int R = Y::R, T = Y::T, GT = Y::GT, NC = Y::NC, NB2 = Cfg::NB2, H = R / 2, KW = Y::KW;
     extern __shared__ __align__(128) unsigned char smraw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smraw);   // full[0], full[1]
     double2* X = reinterpret_cast<double2*>(smraw + 128);
-    double2* C = X + 2 * M * kW;
-    double2* wp = C + M * kW;
+    double2* C = X + 2 * M * KW;
+    double2* wp = C + M * KW;
     const int tid = threadIdx.x;
-    const int grp = tid / GT, gt = tid % GT, c = gt % kW, t = gt / kW;
+    const int grp = tid / GT, gt = tid % GT, c = gt % KW, t = gt / KW;
     for (int n = tid; n < M; n += Y::THREADS) wp[n] = wp_g[n];
     double cc[NB2][NC], tn[NB2][NC];
 #pragma unroll
@@ -303,25 +305,25 @@ k_inv_y_t(const __grid_constant__ CUtensorMap tmB2, double2* __restrict__ B1, co
         }
     if (tid == 0) { mbar_init(&full[0], 1); mbar_init(&full[1], 1); mbar_fence_init(); }
     __syncthreads();
-    const int nzb = Nz / kW;
-    double2* Xg = X + grp * (M * kW);
+    const int nzb = Nz / KW;
+    double2* Xg = X + grp * (M * KW);
     auto issue = [&](long tile) {   // one thread of the group: this group's rows of the tile
         const int kx = (int)(tile / nzb), zb = (int)(tile % nzb);
-        mbar_arrive_expect_tx(&full[grp], (uint32_t)(M * kW * sizeof(double2)));
+        mbar_arrive_expect_tx(&full[grp], (uint32_t)(M * KW * sizeof(double2)));
 #pragma unroll
-        for (int r0 = 0; r0 < M; r0 += Y::BOXR) tma_load_4d(Xg + r0 * kW, &tmB2, &full[grp], zb * kW * 2, grp, r0, kx);
+        for (int r0 = 0; r0 < M; r0 += Y::BOXR) tma_load_4d(Xg + r0 * KW, &tmB2, &full[grp], zb * KW * 2, grp, r0, kx);
     };
     auto prefetch = [&](long tile) {
         const int kx = (int)(tile / nzb), zb = (int)(tile % nzb);
 #pragma unroll
-        for (int r0 = 0; r0 < M; r0 += Y::BOXR) tma_prefetch_4d(&tmB2, zb * kW * 2, grp, r0, kx);
+        for (int r0 = 0; r0 < M; r0 += Y::BOXR) tma_prefetch_4d(&tmB2, zb * KW * 2, grp, r0, kx);
     };
     long tile = blockIdx.x;
     if (gt == 0 && tile < ntiles) issue(tile);
     uint32_t parity = 0;
     double2* Ec = Xg + c;
-    double2* Cmine = C + grp * (M / 2 * kW) + c;          // what this group gives away
-    double2* Ctheirs = C + (grp ^ 1) * (M / 2 * kW) + c;  // what it receives
+    double2* Cmine = C + grp * (M / 2 * KW) + c;          // what this group gives away
+    double2* Ctheirs = C + (grp ^ 1) * (M / 2 * KW) + c;  // what it receives
     for (; tile < ntiles; tile += gridDim.x) {
         const long kx = tile / nzb;
         const int zb = (int)(tile % nzb);
@@ -332,26 +334,26 @@ k_inv_y_t(const __grid_constant__ CUtensorMap tmB2, double2* __restrict__ B1, co
         parity ^= 1;
 #pragma unroll
         for (int i = 0; i < R; ++i) {
-            const double2 v = Ec[(t + T * i) * kW];
+            const double2 v = Ec[(t + T * i) * KW];
             vr[i] = v.x; vi[i] = v.y;
             if constexpr (DER) mul_minus_i(vr[i], vi[i], kder * signed_mode(2 * (t + T * i) + grp, M));
         }
         // inverse transform = forward transform with the roles of re and im swapped; the first barrier
         // inside also separates the reads of X_g above from its reuse as exchange buffer
-        fft2_forward_tile<Cfg, kW>(vi, vr, t, Ec, 1 + grp, cc, tn);
+        fft2_forward_tile<Cfg, KW>(vi, vr, t, Ec, 1 + grp, cc, tn);
         bar_sync(1 + grp, GT);   // exchange read back by the whole group: X_g is free
         if (gt == 0 && more) { fence_proxy_async(); issue(tile + gridDim.x); }
         __syncthreads();         // C of the previous tile has been consumed by both groups
 #pragma unroll
         for (int i = 0; i < H; ++i) {
             const int s = grp ? i : i + H;    // group 1 gives away y_o[n], i < H; group 0 gives y_e[n], i >= H
-            Cmine[(t + T * i) * kW] = make_double2(vr[s], vi[s]);
+            Cmine[(t + T * i) * KW] = make_double2(vr[s], vi[s]);
         }
         __syncthreads();
-        double2* out = B1 + ((kx * M) * (long)Nz + zb * kW + c);
+        double2* out = B1 + ((kx * M) * (long)Nz + zb * KW + c);
 #pragma unroll
         for (int i = 0; i < H; ++i) {
-            const double2 pv = Ctheirs[(t + T * i) * kW];
+            const double2 pv = Ctheirs[(t + T * i) * KW];
             const int o = grp ? i + H : i;
             const double er = grp ? pv.x : vr[i], ei = grp ? pv.y : vi[i];                 // y_e[n]
             const double qr = grp ? vr[i + H] : pv.x, qi = grp ? vi[i + H] : pv.y;         // y_o[n]
