@@ -42,6 +42,36 @@ __device__ __forceinline__ double cos32(int k) {
 }
 __device__ __forceinline__ double sin32(int k) { return cos32(k - 8); }  // sin(x) = cos(x - pi/2)
 
+// w_64^k = cos(pi k/32) - i sin(pi k/32) (the x tile kernels at Nx = 1024; even k reproduce cos32 bit for bit)
+__device__ __forceinline__ double cos64(int k) {
+    k &= 63;
+    if (k > 32) k = 64 - k;            // cos is even
+    const bool neg = k > 16;           // cos(pi - x) = -cos x
+    if (neg) k = 32 - k;
+    double v = 0.0;
+    switch (k) {
+        case 0: v = 1.0; break;
+        case 1: v = 0.995184726672196886245; break;
+        case 2: v = 0.980785280403230449126; break;
+        case 3: v = 0.956940335732208864936; break;
+        case 4: v = 0.923879532511286756128; break;
+        case 5: v = 0.881921264348355029713; break;
+        case 6: v = 0.831469612302545237079; break;
+        case 7: v = 0.773010453362736960811; break;
+        case 8: v = 0.707106781186547524401; break;
+        case 9: v = 0.634393284163645498215; break;
+        case 10: v = 0.555570233019602224743; break;
+        case 11: v = 0.471396736825997648556; break;
+        case 12: v = 0.382683432365089771728; break;
+        case 13: v = 0.290284677254462367636; break;
+        case 14: v = 0.195090322016128267848; break;
+        case 15: v = 0.0980171403295606019942; break;
+        default: v = 0.0; break;       // k = 16
+    }
+    return neg ? -v : v;
+}
+__device__ __forceinline__ double sin64(int k) { return cos64(k - 16); }
+
 // ---- r-point DFT, in place, on elements re[0], re[S], re[2S], ... (natural order in and out) ---
 template <int r, int S>
 __device__ __forceinline__ void dft_inplace(double* re, double* im) {

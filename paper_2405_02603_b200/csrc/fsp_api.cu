@@ -352,7 +352,7 @@ int launch_inv_x(fsp_plan* p, double* phi, double kder) {
 template <int M>
 int launch_fwd_x_t(fsp_plan* p) {
     using X_ = TileX<M>;
-    const long plane = (long)p->Ny * p->Nz, ntiles = plane / kC;
+    const long plane = (long)p->Ny * p->Nz, ntiles = plane / X_::KC;
     const size_t smem = X_::smem_bytes();
     static int occ = 0;
     if (occ == 0) {
@@ -370,11 +370,12 @@ int do_fwd_x(fsp_plan* p, const double* rho) {
         if (rho != p->tmRho_ptr) {   // the caller owns rho: encode the map for this address (host only, ~1 us)
             const cuuint64_t dims[2] = {(cuuint64_t)p->Ny * p->Nz, (cuuint64_t)p->Nx};
             const cuuint64_t strides[1] = {(cuuint64_t)p->Ny * p->Nz * 8};
-            const cuuint32_t box[2] = {kC, (cuuint32_t)(p->Nx < 256 ? p->Nx : 256)};
+            const cuuint32_t box[2] = {(cuuint32_t)(p->Nx == 1024 ? 8 : kC), (cuuint32_t)(p->Nx < 256 ? p->Nx : 256)};   // TileX<M>::KC columns
             int rc = make_tensor_map(&p->tmRho, const_cast<double*>(rho), 2, dims, strides, box);
             if (rc != FSP_OK) return rc;
             p->tmRho_ptr = rho;
         }
+        if (p->Nx == 1024) return launch_fwd_x_t<512>(p);
         if (p->Nx == 512) return launch_fwd_x_t<256>(p);
         if (p->Nx == 256) return launch_fwd_x_t<128>(p);
         return launch_fwd_x_t<64>(p);
@@ -446,7 +447,7 @@ int do_inv_y(fsp_plan* p, const double2* B2, double2* B1, int np, double kder = 
 template <int M, bool DER>
 int launch_inv_x_t_impl(fsp_plan* p, double* phi, double kder) {
     using X_ = TileXI<M>;
-    const long plane = (long)p->Ny * p->Nz, ntiles = plane / kC;
+    const long plane = (long)p->Ny * p->Nz, ntiles = plane / X_::KC;
     const size_t smem = X_::smem_bytes();
     static int occ = 0;
     if (occ == 0) {
@@ -464,7 +465,9 @@ int launch_inv_x_t(fsp_plan* p, double* phi, double kder) {
     return kder != 0.0 ? launch_inv_x_t_impl<M, true>(p, phi, kder) : launch_inv_x_t_impl<M, false>(p, phi, 0.0);
 }
 int do_inv_x(fsp_plan* p, double* phi, double kder = 0.0) {
-    if (p->tile_x) {
+    // Nx = 1024: 8-column tiles would write phi in half lines (measured 11.9 ms against 9.5 ms for the
+    // first-generation kernel at 1024^3), so K5 stays on the first-generation kernel there (K1 does not: 7.9 vs 12.6)
+    if (p->tile_x && p->Nx != 1024) {
         if (p->Nx == 512) return launch_inv_x_t<256>(p, phi, kder);
         if (p->Nx == 256) return launch_inv_x_t<128>(p, phi, kder);
         return launch_inv_x_t<64>(p, phi, kder);
@@ -729,13 +732,13 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
     p->sm_count = prop.multiProcessorCount > 0 ? prop.multiProcessorCount : 148;
     if (rc == FSP_OK) rc = dev_alloc(&p->Gk, (size_t)(Nx + 1) * (Ny + 1) * (Nz + 2), &p->bytes);
     if (rc == FSP_OK) rc = make_z_lane_table(p);
-    p->tile_x = (Nx == 128 || Nx == 256 || Nx == 512) && ((long)Ny * Nz) % kC == 0;
+    p->tile_x = (Nx == 128 || Nx == 256 || Nx == 512 || Nx == 1024) && ((long)Ny * Nz) % kC == 0;
     if (rc == FSP_OK && p->tile_x) rc = make_x_lane_table(p);
     if (rc == FSP_OK && p->tile_x) {
         const cuuint64_t plane = (cuuint64_t)Ny * Nz;
         const cuuint64_t dims[3] = {2 * plane, 2, (cuuint64_t)(Nx / 2)};
         const cuuint64_t strides[2] = {plane * 16, 2 * plane * 16};
-        const cuuint32_t box[3] = {2 * kC, 1, (cuuint32_t)(Nx / 2 < 256 ? Nx / 2 : 256)};
+        const cuuint32_t box[3] = {2 * (cuuint32_t)(Nx == 1024 ? 8 : kC), 1, (cuuint32_t)(Nx / 2 < 256 ? Nx / 2 : 256)};   // TileXI<M>::KC columns
         rc = make_tensor_map(&p->tmB1x, p->B1, 3, dims, strides, box);
     }
     p->tile_y = (Ny == 128 || Ny == 256 || Ny == 512 || Ny == 1024) && Nz >= kW;

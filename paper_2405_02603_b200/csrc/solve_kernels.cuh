@@ -684,13 +684,15 @@ template <int M>
 struct TileX {
     using Cfg = Fft2Cfg<M>;
     static constexpr int T = Cfg::T, R = Cfg::R;
-    static_assert(32 % (2 * M / T) == 0, "tile x kernels need N/T to divide 32");
-    static constexpr int WS = 32 / (2 * M / T);   // w_(N/T)^i = w_32^(WS i)
-    static constexpr int GT = kC * T, THREADS = 2 * GT;
+    static constexpr int ROOT = 2 * M / T;        // N/T: the compile-time roots are w_ROOT^i
+    static_assert(64 % ROOT == 0, "tile x kernels need N/T to divide 64");
+    static constexpr int WS = ROOT <= 32 ? 32 / ROOT : 1;   // w_ROOT^i = w_32^(WS i), or w_64^i when ROOT = 64
+    static constexpr int KC = (M >= 512) ? 8 : kC;   // columns per tile (Nx = 1024: 8, registers and shared memory)
+    static constexpr int GT = KC * T, THREADS = 2 * GT;
     static constexpr int NC = LaneTw<Cfg::R2>::NC;
     static constexpr int MINB = (M >= 256) ? 1 : 2;
     // [mbarriers: 128 B][X: 2M rows x kC doubles = M*kC double2][E: 2 groups x M*kC double2]
-    static constexpr size_t smem_bytes() { return 128 + sizeof(double2) * (size_t)(3 * M * kC); }
+    static constexpr size_t smem_bytes() { return 128 + sizeof(double2) * (size_t)(3 * M * KC); }
 };
 
 // x * w_32^i (compile-time i)
@@ -703,6 +705,32 @@ __device__ __forceinline__ void cmul_w32(double& xr, double& xi) {
         const double c = cos32(i), sn = sin32(i);
         const double a = fma(xi, sn, xr * c);
         xi = fma(-xr, sn, xi * c);
+        xr = a;
+    }
+}
+
+// x * w_64^i (compile-time i)
+template <int i>
+__device__ __forceinline__ void cmul_w64(double& xr, double& xi) {
+    if constexpr ((i & 63) == 0) {
+    } else if constexpr ((i & 63) == 16) {   // -i
+        const double a = xi; xi = -xr; xr = a;
+    } else {
+        const double c = cos64(i), sn = sin64(i);
+        const double a = fma(xi, sn, xr * c);
+        xi = fma(-xr, sn, xi * c);
+        xr = a;
+    }
+}
+template <int i>
+__device__ __forceinline__ void cmul_w64c(double& xr, double& xi) {   // x * conj(w_64^i)
+    if constexpr ((i & 63) == 0) {
+    } else if constexpr ((i & 63) == 16) {   // +i
+        const double a = -xi; xi = xr; xr = a;
+    } else {
+        const double c = cos64(i), sn = sin64(i);
+        const double a = fma(-xi, sn, xr * c);
+        xi = fma(xr, sn, xi * c);
         xr = a;
     }
 }
@@ -724,14 +752,14 @@ k_fwd_x_t(const __grid_constant__ CUtensorMap tmRho, double2* __restrict__ B1, c
           const double2* __restrict__ Wg, long plane, long ntiles) {
     using X_ = TileX<M>;
     using Cfg = typename X_::Cfg;
-    constexpr int R = X_::R, T = X_::T, GT = X_::GT, NC = X_::NC, NB2 = Cfg::NB2, N = 2 * M;
+    constexpr int R = X_::R, T = X_::T, GT = X_::GT, NC = X_::NC, NB2 = Cfg::NB2, N = 2 * M, KC = X_::KC;
     constexpr int BOXR = N < 256 ? N : 256;
     extern __shared__ __align__(128) unsigned char smraw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smraw);
     double* Xd = reinterpret_cast<double*>(smraw + 128);
-    double2* E = reinterpret_cast<double2*>(smraw + 128) + M * kC;
+    double2* E = reinterpret_cast<double2*>(smraw + 128) + M * KC;
     const int tid = threadIdx.x;
-    const int grp = tid / GT, gt = tid % GT, c = gt % kC, t = gt / kC;
+    const int grp = tid / GT, gt = tid % GT, c = gt % KC, t = gt / KC;
     double cc[NB2][NC], tn[NB2][NC];
 #pragma unroll
     for (int m = 0; m < NB2; ++m)
@@ -745,14 +773,14 @@ k_fwd_x_t(const __grid_constant__ CUtensorMap tmRho, double2* __restrict__ B1, c
     if (tid == 0) { mbar_init(full, 1); mbar_fence_init(); }
     __syncthreads();
     auto issue = [&](long tile) {
-        mbar_arrive_expect_tx(full, (uint32_t)(N * kC * sizeof(double)));
+        mbar_arrive_expect_tx(full, (uint32_t)(N * KC * sizeof(double)));
 #pragma unroll
-        for (int r0 = 0; r0 < N; r0 += BOXR) tma_load_2d(Xd + r0 * kC, &tmRho, full, (int)(tile * kC), r0);
+        for (int r0 = 0; r0 < N; r0 += BOXR) tma_load_2d(Xd + r0 * KC, &tmRho, full, (int)(tile * KC), r0);
     };
     long tile = blockIdx.x;
     if (tid == 0 && tile < ntiles) issue(tile);
     uint32_t parity = 0;
-    double2* Ec = E + grp * (M * kC) + c;
+    double2* Ec = E + grp * (M * KC) + c;
     for (; tile < ntiles; tile += gridDim.x) {
         double vr[R], vi[R];
         mbar_wait(full, parity);
@@ -760,8 +788,8 @@ k_fwd_x_t(const __grid_constant__ CUtensorMap tmRho, double2* __restrict__ B1, c
 #pragma unroll
         for (int i = 0; i < R; ++i) {
             const int n = t + T * i;
-            vr[i] = Xd[(2 * n) * kC + c];
-            vi[i] = Xd[(2 * n + 1) * kC + c];
+            vr[i] = Xd[(2 * n) * KC + c];
+            vi[i] = Xd[(2 * n + 1) * KC + c];
         }
         __syncthreads();   // X may be refilled
         if (tid == 0 && tile + gridDim.x < ntiles) issue(tile + gridDim.x);
@@ -769,26 +797,26 @@ k_fwd_x_t(const __grid_constant__ CUtensorMap tmRho, double2* __restrict__ B1, c
             UntangleFwd<M>::run([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
                 cmul(vr[i], vi[i], lam_n);
-                cmul_w32<i * X_::WS>(vr[i], vi[i]);
+                if constexpr (X_::ROOT <= 32) cmul_w32<i * X_::WS>(vr[i], vi[i]); else cmul_w64<i>(vr[i], vi[i]);
             });
         }
-        fft2_forward_tile<Cfg, kC>(vr, vi, t, Ec, 1 + grp, cc, tn);
+        fft2_forward_tile<Cfg, KC>(vr, vi, t, Ec, 1 + grp, cc, tn);
         // untangle: X'[k] = (A + B) - i w_2N^k (A - B), A = Z[k], B = conj(Z[N-k]), k = 2j + g, j = t + T i
         bar_sync(1 + grp, GT);   // exchange buffer read back by the whole group
 #pragma unroll
-        for (int i = 0; i < R; ++i) Ec[(t + T * i) * kC] = make_double2(vr[i], vi[i]);
+        for (int i = 0; i < R; ++i) Ec[(t + T * i) * KC] = make_double2(vr[i], vi[i]);
         bar_sync(1 + grp, GT);
-        double2* out = B1 + tile * kC + c;
+        double2* out = B1 + tile * KC + c;
         UntangleFwd<M>::run([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             const int j = t + T * i;
             const int jp = grp ? M - 1 - j : (M - j) & (M - 1);
-            const double2 bq = Ec[jp * kC];
+            const double2 bq = Ec[jp * KC];
             const double ar = vr[i], ai = vi[i], br = bq.x, bi = -bq.y;
             const double sr = ar + br, si = ai + bi;
             double dr = ar - br, di = ai - bi;
             cmul(dr, di, lam_k);
-            cmul_w32<i * X_::WS>(dr, di);
+            if constexpr (X_::ROOT <= 32) cmul_w32<i * X_::WS>(dr, di); else cmul_w64<i>(dr, di);
             const long k = 2 * j + grp;
             out[k * plane] = make_double2(sr + di, si - dr);
             if (i == 0 && grp == 0 && t == 0) out[(long)N * plane] = make_double2(2.0 * (ar - ai), 0.0);
@@ -820,14 +848,16 @@ template <int M>
 struct TileXI {
     using Cfg = Fft2Cfg<M>;
     static constexpr int T = Cfg::T, R = Cfg::R;
-    static_assert(32 % (2 * M / T) == 0, "tile x kernels need N/T to divide 32");
-    static constexpr int WS = 32 / (2 * M / T);   // w_(N/T)^i = w_32^(WS i)
-    static constexpr int GT = kC * T, THREADS = 2 * GT;
+    static constexpr int ROOT = 2 * M / T;
+    static_assert(64 % ROOT == 0, "tile x kernels need N/T to divide 64");
+    static constexpr int WS = ROOT <= 32 ? 32 / ROOT : 1;   // w_ROOT^i = w_32^(WS i), or w_64^i when ROOT = 64
+    static constexpr int KC = (M >= 512) ? 8 : kC;
+    static constexpr int GT = KC * T, THREADS = 2 * GT;
     static constexpr int NC = LaneTw<Cfg::R2>::NC;
     static constexpr int MINB = (M >= 256) ? 1 : 2;
     static constexpr int BOXR = M < 256 ? M : 256;
-    // [mbarriers: 128 B][row N: kC double2][X: 2 groups x M*kC][C: 2 groups x (M/2)*kC]
-    static constexpr size_t smem_bytes() { return 128 + sizeof(double2) * (size_t)(kC + 3 * M * kC); }
+    // [mbarriers: 128 B][row N: KC double2][X: 2 groups x M*KC][C: 2 groups x (M/2)*KC]
+    static constexpr size_t smem_bytes() { return 128 + sizeof(double2) * (size_t)(KC + 3 * M * KC); }
 };
 
 // DER: X[k] is multiplied by -i kder k first (zero at the Nyquist index k = Nx): E_x of the field output
@@ -837,14 +867,14 @@ k_inv_x_t(const __grid_constant__ CUtensorMap tmB1, const double2* __restrict__ 
           const double* __restrict__ lane_g, const double2* __restrict__ Wg, long plane, long ntiles, const double kder) {
     using X_ = TileXI<M>;
     using Cfg = typename X_::Cfg;
-    constexpr int R = X_::R, T = X_::T, GT = X_::GT, NC = X_::NC, NB2 = Cfg::NB2, N = 2 * M, H = R / 2;
+    constexpr int R = X_::R, T = X_::T, GT = X_::GT, NC = X_::NC, NB2 = Cfg::NB2, N = 2 * M, H = R / 2, KC = X_::KC;
     extern __shared__ __align__(128) unsigned char smraw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smraw);
     double2* XN = reinterpret_cast<double2*>(smraw + 128);
-    double2* X = XN + kC;
-    double2* C = X + 2 * M * kC;
+    double2* X = XN + KC;
+    double2* C = X + 2 * M * KC;
     const int tid = threadIdx.x;
-    const int grp = tid / GT, gt = tid % GT, c = gt % kC, t = gt / kC;
+    const int grp = tid / GT, gt = tid % GT, c = gt % KC, t = gt / KC;
     double cc[NB2][NC], tn[NB2][NC];
 #pragma unroll
     for (int m = 0; m < NB2; ++m)
@@ -858,24 +888,24 @@ k_inv_x_t(const __grid_constant__ CUtensorMap tmB1, const double2* __restrict__ 
     const double kd0 = kder * (double)(2 * t + grp);   // DER only
     if (tid == 0) { mbar_init(&full[0], 1); mbar_init(&full[1], 1); mbar_fence_init(); }
     __syncthreads();
-    double2* Xg = X + grp * (M * kC);
+    double2* Xg = X + grp * (M * KC);
     auto issue = [&](long tile) {   // one thread of the group
-        const uint32_t bytes = (uint32_t)(M * kC * sizeof(double2)) + (grp == 0 ? (uint32_t)(kC * sizeof(double2)) : 0u);
+        const uint32_t bytes = (uint32_t)(M * KC * sizeof(double2)) + (grp == 0 ? (uint32_t)(KC * sizeof(double2)) : 0u);
         mbar_arrive_expect_tx(&full[grp], bytes);
 #pragma unroll
-        for (int r0 = 0; r0 < M; r0 += X_::BOXR) tma_load_3d(Xg + r0 * kC, &tmB1, &full[grp], (int)(tile * kC * 2), grp, r0);
-        if (grp == 0) bulk_load(XN, B1 + (long)N * plane + tile * kC, kC * sizeof(double2), &full[0]);
+        for (int r0 = 0; r0 < M; r0 += X_::BOXR) tma_load_3d(Xg + r0 * KC, &tmB1, &full[grp], (int)(tile * KC * 2), grp, r0);
+        if (grp == 0) bulk_load(XN, B1 + (long)N * plane + tile * KC, KC * sizeof(double2), &full[0]);
     };
     auto prefetch = [&](long tile) {
 #pragma unroll
-        for (int r0 = 0; r0 < M; r0 += X_::BOXR) tma_prefetch_3d(&tmB1, (int)(tile * kC * 2), grp, r0);
+        for (int r0 = 0; r0 < M; r0 += X_::BOXR) tma_prefetch_3d(&tmB1, (int)(tile * KC * 2), grp, r0);
     };
     long tile = blockIdx.x;
     if (gt == 0 && tile < ntiles) issue(tile);
     uint32_t parity = 0;
     double2* Ec = Xg + c;
-    double2* Cmine = C + grp * (M / 2 * kC) + c;
-    double2* Ctheirs = C + (grp ^ 1) * (M / 2 * kC) + c;
+    double2* Cmine = C + grp * (M / 2 * KC) + c;
+    double2* Ctheirs = C + (grp ^ 1) * (M / 2 * KC) + c;
     for (; tile < ntiles; tile += gridDim.x) {
         const bool more = tile + gridDim.x < ntiles;
         if (gt == 0 && more) prefetch(tile + gridDim.x);
@@ -885,10 +915,10 @@ k_inv_x_t(const __grid_constant__ CUtensorMap tmB1, const double2* __restrict__ 
         UntangleFwd<M>::run([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             const int j = t + T * i;
-            double2 a = Ec[j * kC];
+            double2 a = Ec[j * KC];
             double2 bq;
-            if (grp) bq = Ec[(M - 1 - j) * kC];
-            else bq = (j == 0) ? XN[c] : Ec[(M - j) * kC];
+            if (grp) bq = Ec[(M - 1 - j) * KC];
+            else bq = (j == 0) ? XN[c] : Ec[(M - j) * KC];
             if constexpr (DER) {   // k = (2t + grp) + 2T i: a lane constant plus a compile-time multiple
                 const double ck = fma(kder * (double)(2 * T), (double)i, kd0);
                 mul_minus_i(a.x, a.y, ck);
@@ -898,29 +928,29 @@ k_inv_x_t(const __grid_constant__ CUtensorMap tmB1, const double2* __restrict__ 
             const double sr = a.x + br, si = a.y + bi;
             double dr = a.x - br, di = a.y - bi;
             cmul_conj(dr, di, lam_k);
-            cmul_w32c<i * X_::WS>(dr, di);
+            if constexpr (X_::ROOT <= 32) cmul_w32c<i * X_::WS>(dr, di); else cmul_w64c<i>(dr, di);
             zr[i] = sr - di; zi[i] = si + dr;     // Z = (A + B) + i d
         });
-        fft2_forward_tile<Cfg, kC>(zi, zr, t, Ec, 1 + grp, cc, tn);   // inverse: roles of re and im swapped
+        fft2_forward_tile<Cfg, KC>(zi, zr, t, Ec, 1 + grp, cc, tn);   // inverse: roles of re and im swapped
         bar_sync(1 + grp, GT);   // exchange read back: X_g is free
         if (gt == 0 && more) { fence_proxy_async(); issue(tile + gridDim.x); }
         if (grp) {   // y_o[n] conj(w_N^n), n = t + T i
             UntangleFwd<M>::run([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
                 cmul_conj(zr[i], zi[i], lam_n);
-                cmul_w32c<i * X_::WS>(zr[i], zi[i]);
+                if constexpr (X_::ROOT <= 32) cmul_w32c<i * X_::WS>(zr[i], zi[i]); else cmul_w64c<i>(zr[i], zi[i]);
             });
         }
         __syncthreads();         // C of the previous tile has been consumed
 #pragma unroll
         for (int i = 0; i < H; ++i) {
-            Cmine[(t + T * i) * kC] = make_double2(grp ? zr[i] : zr[i + H], grp ? zi[i] : zi[i + H]);
+            Cmine[(t + T * i) * KC] = make_double2(grp ? zr[i] : zr[i + H], grp ? zi[i] : zi[i + H]);
         }
         __syncthreads();
-        double* out = phi + tile * kC + c;
+        double* out = phi + tile * KC + c;
 #pragma unroll
         for (int i = 0; i < H; ++i) {
-            const double2 pv = Ctheirs[(t + T * i) * kC];
+            const double2 pv = Ctheirs[(t + T * i) * KC];
             const int o = grp ? i + H : i;
             const long n = t + T * o;
             out[(2 * n) * plane] = (grp ? zr[i + H] : zr[i]) + pv.x;
