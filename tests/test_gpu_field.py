@@ -62,7 +62,7 @@ def test_centred_gaussian_field_reaches_round_off_with_vg_at_64():
 
 
 @pytest.mark.parametrize("N", [(8, 8, 8), (16, 32, 128), (128, 16, 32), (64, 8, 256), (8, 256, 8), (256, 8, 8),
-                               (8, 8, 512), (8, 512, 8), (512, 8, 8), (8, 8, 1024), (8, 1024, 8), (1024, 8, 8), (128, 128, 16),
+                               (8, 8, 512), (8, 512, 8), (512, 8, 8), (8, 8, 1024), (8, 1024, 8), (16, 1024, 32), (1024, 8, 8), (128, 128, 16),
                                (256, 256, 8), (16, 128, 64)])
 def test_field_random_density_every_fft_length(N):
     """Dense random rho, anisotropic spacing: every kernel generation and transform length on every axis, so

@@ -66,7 +66,7 @@ def test_config2_multigauss_64(alg, seed):
 
 @pytest.mark.parametrize("N", [(8, 8, 8), (16, 8, 8), (8, 16, 8), (8, 8, 16), (32, 64, 16), (16, 32, 128), (128, 16, 32),
                                (64, 8, 256), (8, 256, 8), (256, 8, 8), (8, 8, 512), (8, 512, 8), (512, 8, 8), (8, 8, 1024),
-                               (8, 1024, 8), (1024, 8, 8), (1024, 16, 32), (8, 128, 8), (128, 128, 16), (16, 128, 64), (128, 8, 16), (256, 256, 8), (512, 16, 8),
+                               (8, 1024, 8), (16, 1024, 64), (1024, 8, 8), (1024, 16, 32), (8, 128, 8), (128, 128, 16), (16, 128, 64), (128, 8, 16), (256, 256, 8), (512, 16, 8),
                                (16, 512, 24 // 3)])
 def test_random_density_every_fft_length(N):
     """Dense random rho (no zero tail to hide an indexing error), anisotropic spacing, every
