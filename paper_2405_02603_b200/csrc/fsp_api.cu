@@ -17,7 +17,7 @@
 
 using namespace fsp;
 
-#define FSP_VERSION_NUM 100
+#define FSP_VERSION_NUM 110
 
 struct fsp_plan {
     int Nx = 0, Ny = 0, Nz = 0;   // transform mesh: each a power of two (the caller's mesh when that is one)
