@@ -23,6 +23,7 @@ from .oracle import (  # noqa: F401
     green_spectrum,
     green_table,
     green_table_vgm,
+    green_table_vg_entries,
     vg_safe_factors,
     num_threads,
     set_num_threads,

@@ -12,7 +12,9 @@
  *
  *   orc_direct_sum*      PAPER.md:35   "discretizing G and rho on the computational mesh, and
  *                                        approximating the integral as a sum" (+ weight hxhyhz of
- *                                        PAPER.md:80).  THE plain definition (Def. O1).
+ *                                        PAPER.md:80).  THE plain definition (Def. O1); long double sums.
+ *   orc_green_table_vg_entries  PAPER.md:100-102  single entries of the VG table by the explicit triple
+ *                                        cosine sum (no transform): the reference for tables at full size.
  *   orc_fft_radix2 /     PAPER.md:37   the Fourier transform F; textbook iterative radix-2
  *   orc_dft_direct                      Cooley-Tukey and the O(n^2) definition of the DFT.
  *   orc_green_table_he   PAPER.md:35,72-76  G = 1/(4 pi |x|), regularised at the origin (R5).
@@ -541,30 +543,93 @@ int orc_solve_field(long Nx, long Ny, long Nz, const double h[3], const double* 
 /* Def. O1 (PAPER.md:35 with the weight of PAPER.md:80), the plain discrete convolution:
  *   phi[i,j,k] = hx hy hz sum_{i',j',k'} T[|i-i'|,|j-j'|,|k-k'|] rho[i',j',k'].
  * Evaluated only at the npts output points listed in idx (flat C-order indices); idx == NULL
- * means all Nx Ny Nz points.  O(npts * V). */
+ * means all Nx Ny Nz points.  O(npts * V).
+ * The V products are added in plain order in `long double` (x87 80-bit, 64-bit mantissa): the sum of
+ * V ~ 1e8 terms then carries a rounding error of ~ sqrt(V) 2^-64 ~ 5e-16 instead of sqrt(V) 2^-53 ~ 1e-12,
+ * so that the reference is good to the 1e-12 the GPU path is held to at the full sizes (BASELINE.json
+ * north_star tolerance); only the final value is rounded to fp64. */
 int orc_direct_sum(long Nx, long Ny, long Nz, const double h[3], const double* T, const double* rho,
                    long npts, const long* idx, double* out) {
     if (Nx < 1 || Ny < 1 || Nz < 1 || !h || !T || !rho || !out) return ORC_EINVAL;
     long V = Nx * Ny * Nz;
     if (!idx) npts = V;
-    double w = h[0] * h[1] * h[2];
+    long double w = (long double)h[0] * (long double)h[1] * (long double)h[2];
 #pragma omp parallel for schedule(dynamic, 1)
     for (long p = 0; p < npts; ++p) {
         long f = idx ? idx[p] : p;
         long i = f / (Ny * Nz), j = (f / Nz) % Ny, k = f % Nz;
-        double acc = 0.0;
+        long double acc = 0.0L;
         for (long a = 0; a < Nx; ++a) {
             long dx = labs(i - a);
             for (long b = 0; b < Ny; ++b) {
                 long dy = labs(j - b);
                 const double* Trow = T + (dx * (Ny + 1) + dy) * (Nz + 1);
                 const double* rrow = rho + ((size_t)a * Ny + b) * Nz;
-                double s = 0.0;
-                for (long c = 0; c < Nz; ++c) s += Trow[labs(k - c)] * rrow[c];
-                acc += s;
+                for (long c = 0; c < Nz; ++c) acc += (long double)Trow[labs(k - c)] * (long double)rrow[c];
             }
         }
-        out[p] = w * acc;
+        out[p] = (double)(w * acc);
     }
     return ORC_OK;
+}
+
+/* One entry of the Vico-Greengard table by the explicit triple cosine sum (G_L is real
+ * and even, so the inverse DFT of PAPER.md:94-98 on the m_d N_d lattice "reduces to a discrete cosine
+ * transform"; type 1), written out term by term with no transform at all:
+ *     T[d] = 1/prod_d(m_d N_d h_d) * sum_{kx=0..nx} sum_{ky=0..ny} sum_{kz=0..nz}
+ *                w_kx w_ky w_kz G_L(s_k) cos(pi kx dx/nx) cos(pi ky dy/ny) cos(pi kz dz/nz),
+ *     n_d = m_d N_d / 2,  s_d = 2 pi k_d / (m_d N_d h_d),  w_0 = w_n = 1, w_k = 2 otherwise,
+ * for the npts entries d[p] = (dx, dy, dz) listed in d (3 longs each).  m = (4,4,4) is the paper's lattice
+ * (VICO / VICO_2), other even m the anisotropy-safe one (R17).  O(npts * nx ny nz): usable for a handful of
+ * entries at any mesh size (the 512^3 table needs a 1025^3 lattice, 1.1e9 terms per entry), which is what the
+ * full-size GPU table checks use.  The cosines are taken at arguments reduced mod 2n; sums in long double. */
+int orc_green_table_vg_entries(long Nx, long Ny, long Nz, const double h[3], double alpha, const long m[3],
+                               long npts, const long* d, double* out) {
+    if (Nx < 1 || Ny < 1 || Nz < 1 || !h || !m || !d || !out || npts < 0 || !(h[0] > 0) || !(h[1] > 0) ||
+        !(h[2] > 0) || !(alpha > 0))
+        return ORC_EINVAL;
+    for (int a = 0; a < 3; ++a)
+        if (m[a] < 2 || (m[a] & 1)) return ORC_EINVAL;
+    const long n[3] = {m[0] * Nx / 2, m[1] * Ny / 2, m[2] * Nz / 2};
+    const double L = orc_vg_window(Nx, Ny, Nz, h, alpha);
+    const double period[3] = {(double)m[0] * Nx * h[0], (double)m[1] * Ny * h[1], (double)m[2] * Nz * h[2]};
+    int err = 0;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (long p = 0; p < npts; ++p) {
+        /* weighted cosine factors of this entry along each axis */
+        double* c[3] = {NULL, NULL, NULL};
+        int bad = 0;
+        for (int a = 0; a < 3; ++a) {
+            c[a] = (double*)malloc(sizeof(double) * (size_t)(n[a] + 1));
+            if (!c[a]) { bad = 1; break; }
+            for (long k = 0; k <= n[a]; ++k) {
+                long kd = (long)(((int64_t)k * (int64_t)d[3 * p + a]) % (int64_t)(2 * n[a]));
+                double wk = (k == 0 || k == n[a]) ? 1.0 : 2.0;
+                c[a][k] = wk * cos(ORC_PI * (double)kd / (double)n[a]);
+            }
+        }
+        if (bad) {
+#pragma omp atomic write
+            err = 1;
+        } else {
+            long double acc = 0.0L;
+            for (long kx = 0; kx <= n[0]; ++kx) {
+                double sx = 2.0 * ORC_PI * kx / period[0];
+                long double ax = 0.0L;
+                for (long ky = 0; ky <= n[1]; ++ky) {
+                    double sy = 2.0 * ORC_PI * ky / period[1];
+                    long double ay = 0.0L;
+                    for (long kz = 0; kz <= n[2]; ++kz) {
+                        double sz = 2.0 * ORC_PI * kz / period[2];
+                        ay += (long double)(vg_GL(sx, sy, sz, L) * c[2][kz]);
+                    }
+                    ax += ay * c[1][ky];
+                }
+                acc += ax * c[0][kx];
+            }
+            out[p] = (double)(acc / ((long double)period[0] * period[1] * period[2]));
+        }
+        for (int a = 0; a < 3; ++a) free(c[a]);
+    }
+    return err ? ORC_ENOMEM : ORC_OK;
 }

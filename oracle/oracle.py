@@ -1,7 +1,8 @@
 """ctypes marshalling for ``fsp_oracle.c`` (TEST INFRASTRUCTURE -- see ``oracle/__init__.py``).
 
-No arithmetic of the method is done in this file: every function checks shapes, hands contiguous
-numpy fp64 arrays to the C oracle and returns the result.
+Every function but one checks shapes, hands contiguous numpy fp64 arrays to the C oracle and returns the
+result.  The exception is ``field_of_point_charges``: an FFT-free, point-by-point numpy evaluation of the field
+of a few point charges (oracle-side arithmetic, pinned in tests/test_oracle_pins.py against orc_solve_field).
 """
 from __future__ import annotations
 
@@ -63,6 +64,7 @@ def _load():
         lib.orc_solve.argtypes = [L, L, L, _dp, _dp, I, _dp, _dp]
         lib.orc_solve_field.argtypes = [L, L, L, _dp, _dp, I, _dp, _dp, _dp]
         lib.orc_direct_sum.argtypes = [L, L, L, _dp, _dp, _dp, L, _lp, _dp]
+        lib.orc_green_table_vg_entries.argtypes = [L, L, L, _dp, D, _lp, L, _lp, _dp]
         _lib = lib
     return _lib
 
@@ -142,6 +144,21 @@ def green_table_vgm(N, h, m, alpha: float = ALPHA_DEFAULT, method: int = 0) -> n
     _check(_load().orc_green_table_vgm(Nx, Ny, Nz, _d(h), alpha, method, mm.ctypes.data_as(_lp), _d(T)),
            "green_table_vgm")
     return T
+
+
+def green_table_vg_entries(N, h, m, entries, alpha: float = ALPHA_DEFAULT) -> np.ndarray:
+    """Entries T[dx, dy, dz] of the VG table (oversampling factors m, (4,4,4) = the paper's) by the explicit
+    triple cosine sum of PAPER.md:100-102, one entry at a time, no transform.  entries: (npts, 3) integers."""
+    Nx, Ny, Nz = (int(v) for v in N)
+    h = _h3(h)
+    mm = np.ascontiguousarray(m, dtype=np.int64)
+    d = np.ascontiguousarray(entries, dtype=np.int64).reshape(-1, 3)
+    assert ctypes.sizeof(ctypes.c_long) == 8
+    assert (d >= 0).all() and (d <= np.array([Nx, Ny, Nz])).all()
+    out = np.empty(d.shape[0], dtype=np.float64)
+    _check(_load().orc_green_table_vg_entries(Nx, Ny, Nz, _d(h), alpha, mm.ctypes.data_as(_lp), d.shape[0],
+                                              d.ctypes.data_as(_lp), _d(out)), "green_table_vg_entries")
+    return out
 
 
 def green_table(algorithm: int, N, h, g0: float = G0_DEFAULT, alpha: float = ALPHA_DEFAULT,

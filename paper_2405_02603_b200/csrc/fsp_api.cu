@@ -546,17 +546,54 @@ int dct1_axis(fsp_plan* p, const double* in, double* out, const long in_dims[3],
     return FSP_OK;
 }
 
-int fft_axis(fsp_plan* p, double2* data, const long dims[3], int axis, int sign) {
+// tile geometry shared by the plain-VG passes: C pencils adjacent along the contiguous dimension (z; y when the
+// transform axis is z), nA x nB pencil grid, strides {sA, sB, sK} of a C-order array with dimensions dims
+struct AxisTiling { long nA, nB, sA, sB, sK; };
+AxisTiling axis_tiling(const long dims[3], int axis) {
     const long st[3] = {dims[1] * dims[2], dims[2], 1};
-    const int o1 = (axis + 1) % 3, o2 = (axis + 2) % 3;
-    const int Lf = (int)dims[axis];
-    const size_t smem = sizeof(double2) * 2 * (size_t)Lf;
-    CU(cudaFuncSetAttribute(k_fft_pencils, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    int threads = Lf / 2 < 256 ? (Lf / 2 < 32 ? 32 : Lf / 2) : 256;
-    k_fft_pencils<<<(unsigned)(dims[o1] * dims[o2]), threads, smem, p->stream>>>(data, Lf, st[axis], dims[o2],
-                                                                                st[o1], st[o2], sign);
+    const int bdim = axis == 2 ? 1 : 2, adim = axis == 2 ? 0 : (axis == 0 ? 1 : 0);
+    return AxisTiling{dims[adim], dims[bdim], st[adim], st[bdim], st[axis]};
+}
+
+template <int C>
+int launch_ifft_tile(fsp_plan* p, double2* data, int Lf, long nA, long nB, long sA, long sB, long sK, size_t smem) {
+    CU(cudaFuncSetAttribute(k_ifft_tile<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_ifft_tile<C><<<(unsigned)(nA * ((nB + C - 1) / C)), smem <= 72 * 1024 ? 512 : 1024, smem, p->stream>>>(data, Lf, nB, sA, sB, sK);
     CU(cudaGetLastError());
     return FSP_OK;
+}
+// in-place unscaled inverse DFT along `axis` of the complex array data[dims], for the pencils whose index along the
+// tiled dimension is below nB_used
+int ifft_axis(fsp_plan* p, double2* data, const long dims[3], int axis, long nA_used, long nB_used) {
+    const AxisTiling t = axis_tiling(dims, axis);
+    const int Lf = (int)dims[axis];
+    auto smem = [&](int C) { return sizeof(double2) * ((size_t)Lf / 2 + 2 * (size_t)C * Lf); };
+    const size_t cap = 200 * 1024;
+    if (smem(8) <= 72 * 1024) return launch_ifft_tile<8>(p, data, Lf, nA_used, nB_used, t.sA, t.sB, t.sK, smem(8));
+    if (smem(4) <= cap) return launch_ifft_tile<4>(p, data, Lf, nA_used, nB_used, t.sA, t.sB, t.sK, smem(4));
+    if (smem(2) <= cap) return launch_ifft_tile<2>(p, data, Lf, nA_used, nB_used, t.sA, t.sB, t.sK, smem(2));
+    if (smem(1) <= cap) return launch_ifft_tile<1>(p, data, Lf, nA_used, nB_used, t.sA, t.sB, t.sK, smem(1));
+    return FSP_ERR_INVALID_ARG;
+}
+template <int C>
+int launch_c2r_tile(fsp_plan* p, const double2* in, double* out, int Lf, int nout, long nA, long nB, const AxisTiling& ti,
+                    const AxisTiling& to, double scale, size_t smem) {
+    CU(cudaFuncSetAttribute(k_c2r_tile<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_c2r_tile<C><<<(unsigned)(nA * ((nB + C - 1) / C)), smem <= 72 * 1024 ? 512 : 1024, smem, p->stream>>>(
+        in, out, Lf, nout, nB, ti.sA, ti.sB, ti.sK, to.sA, to.sB, to.sK, scale);
+    CU(cudaGetLastError());
+    return FSP_OK;
+}
+// C2R along `axis` (half spectrum Lf/2 + 1 in, nout reals out), pencils (a < nA_used, b < nB_used)
+int c2r_axis(fsp_plan* p, const double2* in, double* out, const long in_dims[3], const long out_dims[3], int axis, int Lf,
+             int nout, long nA_used, long nB_used, double scale) {
+    const AxisTiling ti = axis_tiling(in_dims, axis), to = axis_tiling(out_dims, axis);
+    auto smem = [&](int C) { return sizeof(double2) * ((size_t)Lf / 2 + (size_t)C * Lf); };
+    const size_t cap = 200 * 1024;
+    if (smem(8) <= 72 * 1024) return launch_c2r_tile<8>(p, in, out, Lf, nout, nA_used, nB_used, ti, to, scale, smem(8));
+    if (smem(4) <= cap) return launch_c2r_tile<4>(p, in, out, Lf, nout, nA_used, nB_used, ti, to, scale, smem(4));
+    if (smem(2) <= cap) return launch_c2r_tile<2>(p, in, out, Lf, nout, nA_used, nB_used, ti, to, scale, smem(2));
+    return FSP_ERR_INVALID_ARG;
 }
 
 struct ScopedFree {
@@ -584,21 +621,20 @@ int precompute_impl(fsp_plan* p) {
         const double L = p->alpha * std::sqrt(Lx * Lx + Ly * Ly + Lz * Lz);
         const double scale = 1.0 / ((4.0 * Nx * hx) * (4.0 * Ny * hy) * (4.0 * Nz * hz));
         if (p->algorithm == FSP_VICO) {
-            // (4N)^3 complex grid: fill, unscaled inverse DFT axis by axis, restrict
-            const long gd[3] = {4L * Nx, 4L * Ny, 4L * Nz};
+            // (4N)^3 lattice of G_L, real, stored as its C2R half spectrum (2Nx+1) x 4Ny x 4Nz complex: fill, unscaled
+            // inverse DFT along z (all pencils), along y (columns dz <= Nz only), C2R along x for dy <= Ny, dz <= Nz
+            // straight into T (the restriction of PAPER.md:98)
+            const long gd[3] = {2L * Nx + 1, 4L * Ny, 4L * Nz};
             const size_t gcount = (size_t)gd[0] * gd[1] * gd[2];
             double2* g = nullptr;
             int rc = dev_alloc(&g, gcount, &peak);
             if (rc != FSP_OK) return rc;
             tmp.ptrs.push_back(g);
-            k_fill_gl_vg<<<grid_for((long)gcount, blk), blk, 0, p->stream>>>(g, Nx, Ny, Nz, hx, hy, hz, L);
+            k_fill_gl_vg_half<<<grid_for((long)gcount, blk), blk, 0, p->stream>>>(g, Nx, Ny, Nz, hx, hy, hz, L);
             CU(cudaGetLastError());
-            for (int axis = 2; axis >= 0; --axis) {
-                rc = fft_axis(p, g, gd, axis, +1);
-                if (rc != FSP_OK) return rc;
-            }
-            k_restrict_vg<<<grid_for(tcount, blk), blk, 0, p->stream>>>(g, p->T, Nx, Ny, Nz, scale);
-            CU(cudaGetLastError());
+            if ((rc = ifft_axis(p, g, gd, 2, gd[0], gd[1])) != FSP_OK) return rc;
+            if ((rc = ifft_axis(p, g, gd, 1, gd[0], Nz + 1)) != FSP_OK) return rc;
+            if ((rc = c2r_axis(p, g, p->T, gd, tdims, 0, 4 * Nx, Nx + 1, Ny + 1, Nz + 1, scale)) != FSP_OK) return rc;
         } else {
             // (m_d N_d / 2 + 1) real grid per axis, DCT-I per axis with output pruned to N_d + 1
             // (PAPER.md:100-102 with m = 4; FSP_VICO_SAFE: m_d = 4, doubled while m_d < 1 + L / L_d, R17)

@@ -1,7 +1,8 @@
 // green_kernels.cuh -- Green's-function precompute (done once per plan).
 //
 //   HE:  T[d] = 1/(4 pi |d h|), T[0] = g0.
-//   VG:      G_L (Eq. 3) on the (4N)^3 lattice, inverse DFT, restricted to d <= N.
+//   VG:      G_L (Eq. 3) on the (4N)^3 lattice (stored as its C2R half spectrum), inverse DFT,
+//                              restricted to d <= N.
 //   VG2:    G_L on the (2N+1)^3 lattice, DCT-I per axis, restricted to d <= N.
 //   all: Ghat = F{G2} of the 8-case mirror = 3-D DCT-I of T (G2 is real and even).
 //
@@ -48,16 +49,18 @@ __global__ void k_fill_gl_vg2(double* __restrict__ f, int Nx, int Ny, int Nz, do
     }
 }
 
-// VG: g[ix][iy][iz] complex on the (4N)^3 lattice, DFT frequency order k in {0..2N-1, -2N..-1}
-__global__ void k_fill_gl_vg(double2* __restrict__ g, int Nx, int Ny, int Nz, double hx, double hy,
-                             double hz, double L) {
-    const long Mx = 4 * Nx, My = 4 * Ny, Mz = 4 * Nz;
-    const long total = Mx * My * Mz;
+// VG (plain): the (4N)^3 lattice of G_L is real, so its inverse DFT is a C2R transform and only
+// the half spectrum kx in [0, 2Nx] is stored: g[kx][iy][iz] complex, (2Nx+1) x 4Ny x 4Nz, ky and kz in DFT
+// frequency order {0..2N-1, -2N..-1} (513 x 1024 x 1024 complex = 8.6 GB at 256^3).
+__global__ void k_fill_gl_vg_half(double2* __restrict__ g, int Nx, int Ny, int Nz, double hx, double hy,
+                                  double hz, double L) {
+    const long Kx = 2L * Nx + 1, My = 4L * Ny, Mz = 4L * Nz;
+    const long total = Kx * My * Mz;
     const double PI2 = 6.28318530717958647692;
     for (long o = blockIdx.x * (long)blockDim.x + threadIdx.x; o < total; o += (long)gridDim.x * blockDim.x) {
-        const long iz = o % Mz, iy = (o / Mz) % My, ix = o / (Mz * My);
-        const long kx = ix < 2 * Nx ? ix : ix - Mx, ky = iy < 2 * Ny ? iy : iy - My, kz = iz < 2 * Nz ? iz : iz - Mz;
-        g[o] = make_double2(vg_GL(PI2 * kx / (Mx * hx), PI2 * ky / (My * hy), PI2 * kz / (Mz * hz), L), 0.0);
+        const long iz = o % Mz, iy = (o / Mz) % My, kx = o / (Mz * My);
+        const long ky = iy < 2 * Ny ? iy : iy - My, kz = iz < 2 * Nz ? iz : iz - Mz;
+        g[o] = make_double2(vg_GL(PI2 * kx / (4.0 * Nx * hx), PI2 * ky / (My * hy), PI2 * kz / (Mz * hz), L), 0.0);
     }
 }
 
@@ -84,20 +87,6 @@ __device__ __forceinline__ double2* smem_fft_radix2(double2* a, double2* b, int 
     return a;
 }
 
-// In-place complex FFT of pencils: element i of pencil (i1, i2) at data[i1*s1 + i2*s2 + i*sa].
-// grid.x = n1 * n2 pencils.
-__global__ void k_fft_pencils(double2* __restrict__ data, int Lf, long sa, long n2, long s1, long s2,
-                              int sign) {
-    extern __shared__ double2 sm[];
-    double2* a = sm;
-    double2* b = sm + Lf;
-    const long p = blockIdx.x;
-    double2* base = data + (p / n2) * s1 + (p % n2) * s2;
-    for (int i = threadIdx.x; i < Lf; i += blockDim.x) a[i] = base[(long)i * sa];
-    double2* r = smem_fft_radix2(a, b, Lf, sign);
-    for (int i = threadIdx.x; i < Lf; i += blockDim.x) base[(long)i * sa] = r[i];
-}
-
 // Un-normalised DCT-I (REDFT00) of pencils: n+1 real inputs -> first nout outputs,
 //   out[d] = sum_k w_k in[k] cos(pi k d / n),  w_0 = w_n = 1, else 2,
 // evaluated as the length-2n DFT of the even extension.
@@ -119,46 +108,12 @@ __global__ void k_dct1_pencils(const double* __restrict__ in, double* __restrict
     for (int d = threadIdx.x; d < nout; d += blockDim.x) dst[(long)d * sa_out] = scale * r[d].x;
 }
 
-// The same DCT-I for a TILE of C adjacent pencils per CTA (C even): pencils (a, b0 .. b0+C-1) of an
-// nA x nB pencil grid; element k of pencil (a, b) at in[a*sA + b*sB + k*sK].  Two things make it several
-// times faster than k_dct1_pencils: (1) two real-even pencils are packed as the real and imaginary part of
-// ONE complex sequence -- both transforms are real, so they come out as Re and Im of the result; (2) the
-// tile is chosen along the contiguous dimension, so that global accesses are full sectors; the twiddles
-// come from a shared-memory table filled once per CTA.  Shared memory: [tw: Lf/2][a: C/2*Lf][b: C/2*Lf].
-template <int C>
-__global__ void k_dct1_tile(const double* __restrict__ in, double* __restrict__ out, int n, int nout,
-                            long nB, long sA_in, long sB_in, long sK_in, long sA_out, long sB_out,
-                            long sK_out, double scale) {
-    extern __shared__ double2 sm[];
-    const int Lf = 2 * n, half = n, S = C / 2;
-    double2* tw = sm;
-    double2* a = sm + half;
-    double2* b = a + (long)S * Lf;
-    const long tilesB = (nB + C - 1) / C;
-    const long ia = blockIdx.x / tilesB, b0 = (blockIdx.x % tilesB) * C;
-    const int nc = (int)(nB - b0 < C ? nB - b0 : C);   // pencils of this tile
-    const double* src = in + ia * sA_in + b0 * sB_in;
-    double* dst = out + ia * sA_out + b0 * sB_out;
-    for (int k = threadIdx.x; k < half; k += blockDim.x) {
-        double sn, cs;
-        sincospi((double)k / (double)half, &sn, &cs);   // exp(+2 pi i k / Lf)
-        tw[k] = make_double2(cs, sn);
-    }
-    double* af = reinterpret_cast<double*>(a);
-    // load with the even extension: position m and Lf - m both hold input k
-    const int total = (n + 1) * C;
-    for (int e = threadIdx.x; e < total; e += blockDim.x) {
-        int k, c;
-        if (sK_in == 1) { k = e % (n + 1); c = e / (n + 1); }   // contiguous transform axis: k fastest
-        else { c = e % C; k = e / C; }                          // strided axis: pencils fastest
-        const double v = c < nc ? src[(long)c * sB_in + (long)k * sK_in] : 0.0;
-        const long sq = (long)(c >> 1) * Lf;
-        af[2 * (sq + k) + (c & 1)] = v;
-        if (k > 0 && k < n) af[2 * (sq + Lf - k) + (c & 1)] = v;
-    }
-    // Stockham autosort, all S sequences together: radix-4 stages (half the exchanges and barriers of radix 2),
-    // then one radix-2 stage if log2(Lf) is odd.  Sign +: exp(+2 pi i ..); the input is real-even, so the sign
-    // does not matter for the result.
+// Stockham autosort FFT of S sequences of Lf complex points held in shared memory (sequence q at a + q*Lf), all
+// threads of the CTA: radix-4 stages (half the exchanges and barriers of radix 2), then one radix-2 stage if
+// log2(Lf) is odd.  Sign +: exp(+2 pi i ..), i.e. the unscaled inverse DFT.  tw[k] = exp(+2 pi i k / Lf), k < Lf/2.
+// a and b ping-pong; returns the buffer that holds the natural-order result (a barrier has been passed).
+__device__ __forceinline__ double2* smem_stockham(double2* a, double2* b, const double2* __restrict__ tw, int S, int Lf) {
+    const int half = Lf >> 1;
     int Ns = 1;
     const int quarter = Lf >> 2;
     for (; Ns * 4 <= Lf; Ns <<= 2) {
@@ -203,6 +158,47 @@ __global__ void k_dct1_tile(const double* __restrict__ in, double* __restrict__ 
         double2* t2 = a; a = b; b = t2;
     }
     __syncthreads();
+    return a;
+}
+
+// The same DCT-I for a TILE of C adjacent pencils per CTA (C even): pencils (a, b0 .. b0+C-1) of an
+// nA x nB pencil grid; element k of pencil (a, b) at in[a*sA + b*sB + k*sK].  Two things make it several
+// times faster than k_dct1_pencils: (1) two real-even pencils are packed as the real and imaginary part of
+// ONE complex sequence -- both transforms are real, so they come out as Re and Im of the result; (2) the
+// tile is chosen along the contiguous dimension, so that global accesses are full sectors; the twiddles
+// come from a shared-memory table filled once per CTA.  Shared memory: [tw: Lf/2][a: C/2*Lf][b: C/2*Lf].
+template <int C>
+__global__ void k_dct1_tile(const double* __restrict__ in, double* __restrict__ out, int n, int nout,
+                            long nB, long sA_in, long sB_in, long sK_in, long sA_out, long sB_out,
+                            long sK_out, double scale) {
+    extern __shared__ double2 sm[];
+    const int Lf = 2 * n, half = n, S = C / 2;
+    double2* tw = sm;
+    double2* a = sm + half;
+    double2* b = a + (long)S * Lf;
+    const long tilesB = (nB + C - 1) / C;
+    const long ia = blockIdx.x / tilesB, b0 = (blockIdx.x % tilesB) * C;
+    const int nc = (int)(nB - b0 < C ? nB - b0 : C);   // pencils of this tile
+    const double* src = in + ia * sA_in + b0 * sB_in;
+    double* dst = out + ia * sA_out + b0 * sB_out;
+    for (int k = threadIdx.x; k < half; k += blockDim.x) {
+        double sn, cs;
+        sincospi((double)k / (double)half, &sn, &cs);   // exp(+2 pi i k / Lf)
+        tw[k] = make_double2(cs, sn);
+    }
+    double* af = reinterpret_cast<double*>(a);
+    // load with the even extension: position m and Lf - m both hold input k
+    const int total = (n + 1) * C;
+    for (int e = threadIdx.x; e < total; e += blockDim.x) {
+        int k, c;
+        if (sK_in == 1) { k = e % (n + 1); c = e / (n + 1); }   // contiguous transform axis: k fastest
+        else { c = e % C; k = e / C; }                          // strided axis: pencils fastest
+        const double v = c < nc ? src[(long)c * sB_in + (long)k * sK_in] : 0.0;
+        const long sq = (long)(c >> 1) * Lf;
+        af[2 * (sq + k) + (c & 1)] = v;
+        if (k > 0 && k < n) af[2 * (sq + Lf - k) + (c & 1)] = v;
+    }
+    a = smem_stockham(a, b, tw, S, Lf);
     const double* rf = reinterpret_cast<const double*>(a);
     const int ototal = nout * C;
     for (int e = threadIdx.x; e < ototal; e += blockDim.x) {
@@ -213,14 +209,85 @@ __global__ void k_dct1_tile(const double* __restrict__ in, double* __restrict__ 
     }
 }
 
-// VG: T[d] = scale * Re g[dx][dy][dz], d <= N, from the (4N)^3 complex grid
-__global__ void k_restrict_vg(const double2* __restrict__ g, double* __restrict__ T, int Nx, int Ny,
-                              int Nz, double scale) {
-    const long total = (long)(Nx + 1) * (Ny + 1) * (Nz + 1);
-    const long My = 4 * Ny, Mz = 4 * Nz;
-    for (long o = blockIdx.x * (long)blockDim.x + threadIdx.x; o < total; o += (long)gridDim.x * blockDim.x) {
-        const long dz = o % (Nz + 1), dy = (o / (Nz + 1)) % (Ny + 1), dx = o / ((long)(Nz + 1) * (Ny + 1));
-        T[o] = scale * g[(dx * My + dy) * Mz + dz].x;
+// Unscaled inverse complex DFT (sign +) of length Lf along one axis for a TILE of C adjacent pencils per CTA, in
+// place or out of place (plain VG, y and z axes of the half-spectrum lattice).  Same tiling as k_dct1_tile: the C
+// pencils are adjacent along the contiguous dimension, so the strided axes are read and written in full sectors
+// (C x 16 bytes per row); element k of pencil (a, b) at data[a*sA + b*sB + k*sK].  Only pencils b < nB are
+// transformed (the later passes need the columns d <= N only).  Shared memory: [tw: Lf/2][a: C*Lf][b: C*Lf].
+template <int C>
+__global__ void k_ifft_tile(double2* __restrict__ data, int Lf, long nB, long sA, long sB, long sK) {
+    extern __shared__ double2 sm[];
+    const int half = Lf >> 1;
+    double2* tw = sm;
+    double2* a = sm + half;
+    double2* b = a + (long)C * Lf;
+    const long tilesB = (nB + C - 1) / C;
+    const long ia = blockIdx.x / tilesB, b0 = (blockIdx.x % tilesB) * C;
+    const int nc = (int)(nB - b0 < C ? nB - b0 : C);
+    double2* base = data + ia * sA + b0 * sB;
+    for (int k = threadIdx.x; k < half; k += blockDim.x) {
+        double sn, cs;
+        sincospi((double)k / (double)half, &sn, &cs);   // exp(+2 pi i k / Lf)
+        tw[k] = make_double2(cs, sn);
+    }
+    const int total = Lf * C;
+    for (int e = threadIdx.x; e < total; e += blockDim.x) {
+        int k, c;
+        if (sK == 1) { k = e % Lf; c = e / Lf; }
+        else { c = e % C; k = e / C; }
+        a[(long)c * Lf + k] = c < nc ? base[(long)c * sB + (long)k * sK] : make_double2(0.0, 0.0);
+    }
+    a = smem_stockham(a, b, tw, C, Lf);
+    for (int e = threadIdx.x; e < total; e += blockDim.x) {
+        int k, c;
+        if (sK == 1) { k = e % Lf; c = e / Lf; }
+        else { c = e % C; k = e / C; }
+        if (c < nc) base[(long)c * sB + (long)k * sK] = a[(long)c * Lf + k];
+    }
+}
+
+// C2R along one axis for a tile of C adjacent pencils (C even): the input holds the half spectrum X[k], k <= Lf/2,
+// of a REAL sequence of length Lf (X[Lf-k] = conj X[k]); outputs x[n] = sum_k X[k] exp(+2 pi i k n / Lf), n < nout,
+// times `scale`.  Two real transforms per complex FFT: pencils 2q and 2q+1 are packed as Z = A + i B (with the
+// Hermitian extension Z[Lf-k] = conj A[k] + i conj B[k]), and come out as Re z and Im z.  Last pass of the plain VG
+// precompute: in = the lattice after its y and z passes, out = the table T (restriction to n <= N).
+template <int C>
+__global__ void k_c2r_tile(const double2* __restrict__ in, double* __restrict__ out, int Lf, int nout, long nB,
+                           long sA_in, long sB_in, long sK_in, long sA_out, long sB_out, long sK_out, double scale) {
+    extern __shared__ double2 sm[];
+    const int half = Lf >> 1, S = C / 2;
+    double2* tw = sm;
+    double2* a = sm + half;
+    double2* b = a + (long)S * Lf;
+    const long tilesB = (nB + C - 1) / C;
+    const long ia = blockIdx.x / tilesB, b0 = (blockIdx.x % tilesB) * C;
+    const int nc = (int)(nB - b0 < C ? nB - b0 : C);
+    const double2* src = in + ia * sA_in + b0 * sB_in;
+    double* dst = out + ia * sA_out + b0 * sB_out;
+    for (int k = threadIdx.x; k < half; k += blockDim.x) {
+        double sn, cs;
+        sincospi((double)k / (double)half, &sn, &cs);
+        tw[k] = make_double2(cs, sn);
+    }
+    const int total = (half + 1) * S;
+    for (int e = threadIdx.x; e < total; e += blockDim.x) {
+        int k, q;
+        if (sK_in == 1) { k = e % (half + 1); q = e / (half + 1); }
+        else { q = e % S; k = e / S; }
+        const int c0 = 2 * q, c1 = 2 * q + 1;
+        const double2 A = c0 < nc ? src[(long)c0 * sB_in + (long)k * sK_in] : make_double2(0.0, 0.0);
+        const double2 B = c1 < nc ? src[(long)c1 * sB_in + (long)k * sK_in] : make_double2(0.0, 0.0);
+        a[(long)q * Lf + k] = make_double2(A.x - B.y, A.y + B.x);                       // A + i B
+        if (k > 0 && k < half) a[(long)q * Lf + Lf - k] = make_double2(A.x + B.y, B.x - A.y);   // conj A + i conj B
+    }
+    a = smem_stockham(a, b, tw, S, Lf);
+    const double* rf = reinterpret_cast<const double*>(a);
+    const int ototal = nout * C;
+    for (int e = threadIdx.x; e < ototal; e += blockDim.x) {
+        int d, c;
+        if (sK_out == 1) { d = e % nout; c = e / nout; }
+        else { c = e % C; d = e / C; }
+        if (c < nc) dst[(long)c * sB_out + (long)d * sK_out] = scale * rf[2 * ((long)(c >> 1) * Lf + d) + (c & 1)];
     }
 }
 

@@ -143,12 +143,12 @@ def test_g0_and_alpha_parameters():
 
 
 # ---- full-size configurations, in the launch configuration bench.py times ---------------------------
-# The oracle's FFT path (O2) at 256^3 / 512^3 needs a (2N)^3 complex array and minutes of host time, so
-# these sizes are checked on SAMPLED outputs against the plain definition O1 (the triple sum),
-# which the oracle evaluates one point at a time.  O1 adds V ~ 1e7..1e8 products in fp64 in plain order:
-# its own rounding error is ~ sqrt(V) 2^-53 ~ 1e-12, hence 1e-11 on the sampled relative L2 here (the
-# full-field comparisons above keep 1e-12); the max-norm tolerance stays BASELINE.json's 1e-10.
-SPOT_L2_TOL = 1e-11
+# 512^3 is out of reach of the oracle's FFT path (O2 needs a 1024^3 complex array twice), so the full sizes are
+# checked here on SAMPLED outputs against the plain definition O1 (the triple sum), which the oracle
+# evaluates one point at a time, adding its V ~ 1e7..1e8 products in long double (rounding error ~ sqrt(V) 2^-64),
+# so BASELINE.json's 1e-12 / 1e-10 apply unchanged.  Configs 3 and 4 are also compared in full with O2 in
+# tests/test_gpu_parity_fullsize.py.
+SPOT_L2_TOL = L2_TOL
 
 
 def _spot_points(N, n, seed):

@@ -74,6 +74,37 @@ def test_direct_sum_matches_numpy_brute_force():
     assert np.abs(oracle.direct_sum(T, w.h, w.rho, idx) - ref.ravel()[idx]).max() < 1e-14 * np.abs(ref).max()
 
 
+def test_direct_sum_is_correctly_rounded_against_exact_summation():
+    """orc_direct_sum adds its V products in long double so that it stays good to ~1e-15 where V ~ 1e8 (the
+    full-size spot checks hold the GPU to 1e-12 against it).  Reference: the same sum in exact rational arithmetic
+    (Python fractions), on a mesh where that is affordable, with values spanning 12 orders of magnitude and random
+    signs (cancellation).  The result must be the exact sum to within the final rounding to fp64 plus 2e-19 of the
+    sum of absolute values (a 64-bit-mantissa accumulation of 1680 terms)."""
+    from fractions import Fraction
+    N = (6, 7, 40)
+    rng = np.random.default_rng(41)
+    rho = rng.standard_normal(N) * 10.0 ** rng.uniform(-6, 6, size=N)
+    T = rng.standard_normal(tuple(n + 1 for n in N)) * 10.0 ** rng.uniform(-6, 6, size=tuple(n + 1 for n in N))
+    h = (0.3, 0.7, 0.11)
+    idx = np.array([0, 5, 333, 1679, 901], dtype=np.int64)
+    got = oracle.direct_sum(T, h, rho, idx)
+    ii, jj, kk = np.arange(N[0]), np.arange(N[1]), np.arange(N[2])
+    worst_plain = 0.0
+    for p, f in enumerate(idx):
+        i, j, k = np.unravel_index(f, N)
+        Tw = T[np.abs(i - ii)[:, None, None], np.abs(j - jj)[None, :, None], np.abs(k - kk)[None, None, :]]
+        exact = sum((Fraction(float(a)) * Fraction(float(b)) for a, b in zip(Tw.ravel(), rho.ravel())), Fraction(0))
+        exact *= Fraction(h[0]) * Fraction(h[1]) * Fraction(h[2])
+        scale = float(sum(abs(Fraction(float(a)) * Fraction(float(b))) for a, b in zip(Tw.ravel(), rho.ravel()))
+                      * Fraction(h[0]) * Fraction(h[1]) * Fraction(h[2]))
+        assert abs(Fraction(float(got[p])) - exact) <= Fraction(2e-19) * Fraction(scale) + abs(exact) * Fraction(2.3e-16)
+        plain = 0.0
+        for a, b in zip(Tw.ravel(), rho.ravel()):
+            plain += a * b
+        worst_plain = max(worst_plain, abs(plain * h[0] * h[1] * h[2] - float(exact)) / scale)
+    assert worst_plain > 1e-18   # the fp64 plain-order sum is measurably worse on this input
+
+
 @pytest.mark.parametrize("N", [(4, 4, 4), (8, 8, 8), (2, 8, 4), (4, 2, 16)])
 @pytest.mark.parametrize("alg", ["HE", "VG", "VG2", "random"])
 def test_fft_path_equals_plain_convolution(N, alg):
@@ -181,6 +212,38 @@ def test_vg_table_matches_numpy_irfftn_of_eq3():
     ref = G4[: N[0] + 1, : N[1] + 1, : N[2] + 1]
     T = oracle.green_table(oracle.VICO, N, h, alpha=alpha)
     assert np.abs(T - ref).max() < 1e-13 * np.abs(ref).max()
+
+
+@pytest.mark.parametrize("N,h,m", [((4, 4, 4), (0.25,) * 3, (4, 4, 4)), ((3, 6, 5), (0.1, 0.07, 0.2), (4, 4, 4)),
+                                   ((4, 2, 8), (0.1, 0.3, 0.05), (4, 8, 2)), ((8, 8, 8), (0.125,) * 3, (4, 4, 4))])
+def test_vg_table_entries_by_explicit_cosine_sum(N, h, m):
+    """orc_green_table_vg_entries (the reference for full-size GPU tables) against (1) the triple cosine sum of
+    PAPER.md:100-102 written here in numpy with scipy's DCT-I (type 1, un-normalised), (2) the table the oracle's
+    transform route gives, and (3) for m = (4,4,4) the plain 4N inverse DFT of PAPER.md:94-98 (numpy ifftn)."""
+    alpha = 1.1
+    n = [m[d] * N[d] // 2 for d in range(3)]
+    L = alpha * math.sqrt(sum((N[d] * h[d]) ** 2 for d in range(3)))
+    s = [2.0 * np.pi * np.arange(n[d] + 1) / (m[d] * N[d] * h[d]) for d in range(3)]
+    S = np.sqrt(s[0][:, None, None] ** 2 + s[1][None, :, None] ** 2 + s[2][None, None, :] ** 2)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        GL = np.where(S == 0.0, 0.5 * L * L, 2.0 * (np.sin(0.5 * L * S) / S) ** 2)
+    ref = scipy.fft.dctn(GL, type=1) / np.prod([m[d] * N[d] * h[d] for d in range(3)])
+    ref = ref[: N[0] + 1, : N[1] + 1, : N[2] + 1]
+    ent = np.array([(0, 0, 0), (N[0], N[1], N[2]), (1, 0, 0), (0, 1, 0), (0, 0, 1), (N[0], 0, 1), (1, N[1], N[2] - 1),
+                    (N[0] // 2, N[1] // 2, N[2] // 2)])
+    got = oracle.green_table_vg_entries(N, h, m, ent, alpha)
+    want = ref[ent[:, 0], ent[:, 1], ent[:, 2]]
+    assert np.abs(got - want).max() <= 1e-13 * np.abs(ref).max()
+    To = oracle.green_table_vgm(N, h, m, alpha)
+    assert np.abs(got - To[ent[:, 0], ent[:, 1], ent[:, 2]]).max() <= 1e-13 * np.abs(To).max()
+    if m == (4, 4, 4):
+        k = [np.fft.fftfreq(4 * N[d], d=1.0 / (4 * N[d])) for d in range(3)]
+        sx, sy, sz = (2.0 * np.pi * k[d] / (4 * N[d] * h[d]) for d in range(3))
+        S4 = np.sqrt(sx[:, None, None] ** 2 + sy[None, :, None] ** 2 + sz[None, None, :] ** 2)
+        with np.errstate(divide="ignore", invalid="ignore"):
+            G4 = np.where(S4 == 0.0, 0.5 * L * L, 2.0 * (np.sin(0.5 * L * S4) / S4) ** 2)
+        T4 = np.fft.ifftn(G4).real * G4.size / np.prod([4 * N[d] * h[d] for d in range(3)])
+        assert np.abs(got - T4[ent[:, 0], ent[:, 1], ent[:, 2]]).max() <= 1e-13 * np.abs(T4).max()
 
 
 def test_vg_far_field_and_origin_constant():
@@ -309,6 +372,31 @@ def test_beam_like_gaussian_he_against_1d_integral():
     assert err < 5e-3
     vg = oracle.OraclePlan(w.N, w.h, oracle.VICO_2).precompute_green().solve(w.rho)
     assert np.isfinite(vg).all()
+
+
+def test_uniform_sphere_vg_is_only_second_order():
+    """PAPER.md:118-129 (Eq. 5) and :137: for the non-smooth source (a uniform sphere of radius 1 centred in a box
+    of side 2.4) "the Vico-Greengard solver is only as good as the Hockney-Eastwood solver": second order, not
+    spectral.  With Delta phi = -rho, rho = 1 inside (the factor 4 pi G and the sign of Eq. 5 drop out of a relative
+    error, SURVEY 8(c) pt 17): phi = (3 - r^2)/6 for r <= 1, 1/(3r) outside.  The survey's numpy study gives
+    HE / VG = 3.1e-2 / 2.5e-2 (16^3), 1.8e-3 / 2.2e-3 (32^3), 1.5e-3 / 1.8e-3 (64^3): erratic but never spectral."""
+    err = {}
+    for n in (16, 32, 64):
+        N, lo, hi = (n, n, n), (0.0,) * 3, (2.4,) * 3
+        xs = W.cell_centres(N, lo, hi)
+        r = np.sqrt((xs[0][:, None, None] - 1.2) ** 2 + (xs[1][None, :, None] - 1.2) ** 2 + (xs[2][None, None, :] - 1.2) ** 2)
+        rho = np.where(r <= 1.0, 1.0, 0.0)
+        ex = np.where(r <= 1.0, (3.0 - r ** 2) / 6.0, 1.0 / (3.0 * np.maximum(r, 1e-300)))
+        h = (2.4 / n,) * 3
+        for alg in ("HE", "VG2"):
+            phi = oracle.OraclePlan(N, h, ALGS[alg]).precompute_green().solve(rho)
+            err[alg, n] = rel_l2(phi, ex)
+    for n, (he, vg) in {16: (3.1e-2, 2.5e-2), 32: (1.8e-3, 2.2e-3), 64: (1.5e-3, 1.8e-3)}.items():
+        assert err["HE", n] == pytest.approx(he, rel=0.1) and err["VG2", n] == pytest.approx(vg, rel=0.1)
+    for n in (16, 32, 64):
+        assert 0.5 < err["VG2", n] / err["HE", n] < 2.0          # VG no better than HE on this source
+    assert err["VG2", 64] > 1e-4                                  # nowhere near spectral (smooth source: 3.6e-16)
+    assert err["VG2", 16] / err["VG2", 64] > 10.0 and err["HE", 16] / err["HE", 64] > 10.0   # ~ second order overall
 
 
 # ------------------------------------------------- VICO_SAFE: per-axis oversampling (SURVEY 8(f) N2, R17)
