@@ -73,9 +73,16 @@ enum {
 /* parameters settable before fsp_precompute_green */
 enum {
     FSP_PARAM_G0 = 0,    /* HE value at the origin, default +1/(4 pi)  (R5) */
-    FSP_PARAM_ALPHA = 1, /* VG window factor, default 1.1               */
-    FSP_PARAM_CHUNK_PLANES = 2 /* kx-planes per pass of the y-z-y middle (0 = all at once); takes
+    FSP_PARAM_ALPHA = 1, /* VG window factor, default 1.1; must be > 1 (L = alpha x diagonal
+                            has to exceed the largest displacement), else FSP_ERR_INVALID_ARG       */
+    FSP_PARAM_CHUNK_PLANES = 2, /* kx-planes per pass of the y-z-y middle (0 = all at once); takes
                                   effect at the next fsp_solve; does not change results             */
+    FSP_PARAM_K3_VARIANT = 3 /* kernel of the z pass at Nz = 256, 512 (kept for A/B measurements): 0 (default) =
+                                the whole zero-padded pencil in one lane group (k_conv_z_f); 1 = two half-
+                                length branches in a warp pair (k_conv_z_p); 2 (Nz = 512) = the pair scheme
+                                with 32 lanes per branch (k_conv_z_s).  Invalidates the spectrum (its row
+                                layout follows the kernel): call fsp_precompute_green again.  Results agree
+                                to rounding, all within the tolerances of DESIGN.md                  */
 };
 
 /* number of kernels one fsp_solve launches (the five passes of DESIGN.md "The path") */

@@ -15,13 +15,13 @@ import os
 import numpy as np
 
 HOCKNEY, VICO, VICO_2, VICO_SAFE = 0, 1, 2, 3           # include/fsp.h, PAPER.md:199 (+ DESIGN.md R17)
-PARAM_G0, PARAM_ALPHA, PARAM_CHUNK_PLANES = 0, 1, 2
+PARAM_G0, PARAM_ALPHA, PARAM_CHUNK_PLANES, PARAM_K3_VARIANT = 0, 1, 2, 3
 NUM_SOLVE_KERNELS = 5
 ERRORS = {0: "FSP_OK", -1: "FSP_ERR_INVALID_ARG", -2: "FSP_ERR_NOT_PRECOMPUTED",
           -3: "FSP_ERR_OUT_OF_MEMORY", -4: "FSP_ERR_CUDA", -5: "FSP_ERR_NO_DEVICE"}
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libfsp.so")
+LIB_PATH = os.environ.get("FSP_LIB", os.path.join(_HERE, "libfsp.so"))
 _lib = None
 
 # every symbol include/fsp.h declares, with its ctypes signature

@@ -129,10 +129,12 @@ __host__ __device__ constexpr int brev(int v, int r) {
     return o;
 }
 
-template <int r, int S>
+// LO..HI: the radix-2 levels (butterfly spans len = LO, 2 LO, .., HI) that are executed; the full transform is
+// LO = 2, HI = r.  Splitting off the first level lets a caller prune it (fft2_padded_pass).
+template <int r, int S, int LO = 2, int HI = r>
 __device__ __forceinline__ void dft_br(double* re, double* im) {
 #pragma unroll
-    for (int len = 2; len <= r; len *= 2) {
+    for (int len = LO; len <= HI; len *= 2) {
         const int half = len / 2;
 #pragma unroll
         for (int blk = 0; blk < r; blk += len) {

@@ -35,6 +35,10 @@ struct fsp_plan {
     double2* B2 = nullptr;  // (Nx+1) * 2Ny * Nz
     double* Gk = nullptr;   // (Nx+1)(Ny+1)(Nz+2)   spectrum octant in K3's layout, scale folded in
     double* LTz = nullptr;  // lane-constant stage-2 twiddles of the z transform (fft_warp.cuh dft_lane)
+    double* LTzs = nullptr; // Nz = 512: constants of the 32-lane transform (k_conv_z_s): stage 2 [32][16], shuffled level [2][16]
+    double* LTzf = nullptr; // Nz = 256, 512: stage-2 constants of the padded transform of 2 Nz points (k_conv_z_f)
+    int k3_variant = 0;     // FSP_PARAM_K3_VARIANT
+    bool gk_natural = false; // Gk rows in natural order (k_conv_z_f) instead of [E | O] (decided by the last precompute)
     double* LTy = nullptr;  // the same for the y transform (tile kernels)
     bool tile_y = false;    // K2/K4 tile kernels (TMA-staged) are used
     double* LTx = nullptr;  // lane-constant twiddles of the x transform (length Nx/2)
@@ -167,6 +171,27 @@ int make_lane_table(double** dst, int M, int R1, size_t* acc) {
 template <int M>
 int lane_table_for(double** dst, size_t* acc) { return make_lane_table(dst, M, Fft2Cfg<M>::R1, acc); }
 
+// constants of fft512s_forward (fft_warp.cuh): the stage-2 table of make_lane_table for 512 = 32 x 16, followed by
+// (cos[8] | tan[8]) of w_32^(m + 8 h), m < 8, for h = 0 and h = 1 (the radix-2 level shared by lane pairs)
+int make_lane_table_512s(double** dst, size_t* acc) {
+    const int M = 512, R1 = 32, R2 = 16, NC = 8;
+    std::vector<double> hst((size_t)R1 * 2 * NC + 32, 0.0);
+    for (int j = 0; j < R1; ++j)
+        for (int r = 2; r <= R2; r *= 2) {
+            const int ofs = r >= 4 ? r / 4 : 0, q = r >= 4 ? r / 4 : 1;
+            for (int k = 0; k < q; ++k)
+                cos_tan((long)j * R2 + (long)k * M, (long)r * M, &hst[(size_t)j * 2 * NC + ofs + k],
+                        &hst[(size_t)j * 2 * NC + NC + ofs + k]);
+        }
+    for (int h = 0; h < 2; ++h)
+        for (int m = 0; m < 8; ++m)
+            cos_tan(m + 8 * h, 32, &hst[(size_t)R1 * 2 * NC + h * 16 + m], &hst[(size_t)R1 * 2 * NC + h * 16 + 8 + m]);
+    int rc = dev_alloc(dst, hst.size(), acc);
+    if (rc != FSP_OK) return rc;
+    CU(cudaMemcpy(*dst, hst.data(), sizeof(double) * hst.size(), cudaMemcpyHostToDevice));
+    return FSP_OK;
+}
+
 // ---- TMA tensor maps ---------------------------------------------------------------------------------
 // cuTensorMapEncodeTiled is fetched through the runtime so that libfsp.so does not link libcuda directly.
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -272,9 +297,47 @@ int launch_conv_z_p_impl(fsp_plan* p, double2* B2, const double* G, int nplanes,
     k_conv_z_p<M, DER><<<(unsigned)grid, Z::WARPS * 32, smem, p->stream>>>(B2, G, p->LTz, p->Wz, p->Ny, nsteps, out, kap);
     return FSP_OK;
 }
+template <bool DER>
+int launch_conv_z_s_impl(fsp_plan* p, double2* B2, const double* G, int nplanes, double2* out, const DerK kap) {
+    using Z = ConvZS;
+    const long nsteps = (long)nplanes * (2 * p->Ny);   // pair steps: one pencil each
+    const size_t smem = Z::smem_bytes();
+    static int occ = 0;
+    if (occ == 0) {
+        CU(cudaFuncSetAttribute(k_conv_z_s<DER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_conv_z_s<DER>, Z::WARPS * 32, smem));
+        if (occ < 1) return FSP_ERR_CUDA;
+    }
+    long grid = (long)p->sm_count * occ;
+    const long need = (nsteps + Z::PAIRS - 1) / Z::PAIRS;
+    if (grid > need) grid = need;
+    k_conv_z_s<DER><<<(unsigned)grid, Z::WARPS * 32, smem, p->stream>>>(B2, G, p->LTzs, p->Wz, p->Ny, nsteps, out, kap);
+    return FSP_OK;
+}
+template <int M2, bool DER>
+int launch_conv_z_f_impl(fsp_plan* p, double2* B2, const double* G, int nplanes, double2* out, const DerK kap) {
+    using Z = ConvZF<M2>;
+    const long ngroups = (long)nplanes * (2 * p->Ny) / Z::G;
+    const size_t smem = Z::smem_bytes();
+    static int occ = 0;
+    if (occ == 0) {
+        CU(cudaFuncSetAttribute(k_conv_z_f<M2, DER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_conv_z_f<M2, DER>, Z::WARPS * 32, smem));
+        if (occ < 1) return FSP_ERR_CUDA;
+    }
+    long grid = (long)p->sm_count * occ;
+    const long need = (ngroups + Z::WARPS - 1) / Z::WARPS;
+    if (grid > need) grid = need;
+    k_conv_z_f<M2, DER><<<(unsigned)grid, Z::WARPS * 32, smem, p->stream>>>(B2, G, p->LTzf, p->Ny, ngroups, out, kap);
+    return FSP_OK;
+}
 template <int M, bool DER>
 int launch_conv_z_w_impl(fsp_plan* p, double2* B2, const double* G, int nplanes, double2* out, const DerK kap) {
-    // Nz >= 256: warp pairs (k_conv_z_p); below: both branches in one warp (k_conv_z_w)
+    // Nz = 256, 512: the whole padded pencil in one lane group (k_conv_z_f); FSP_PARAM_K3_VARIANT = 1 and Nz = 1024:
+    // warp pairs (k_conv_z_p); variant 2 at Nz = 512: warp pairs with 32 lanes per branch (k_conv_z_s);
+    // below 256: both branches in one warp (k_conv_z_w)
+    if constexpr (M == 512 || M == 256) { if (p->gk_natural) return launch_conv_z_f_impl<2 * M, DER>(p, B2, G, nplanes, out, kap); }
+    if constexpr (M == 512) { if (p->k3_variant == 2) return launch_conv_z_s_impl<DER>(p, B2, G, nplanes, out, kap); }
     if constexpr (M >= 256) return launch_conv_z_p_impl<M, DER>(p, B2, G, nplanes, out, kap);
     else {
     using Z = ConvZ<M>;
@@ -684,7 +747,9 @@ int precompute_impl(fsp_plan* p) {
     const double gscale = hx * hy * hz / (8.0 * (double)Nx * (double)Ny * (double)Nz) * 0.5;
     {
         const long gk_total = (long)(Nx + 1) * (Ny + 1) * (Nz + 2);
-        k_layout_spectrum_oct<<<grid_for(gk_total, blk), blk, 0, p->stream>>>(p->Goct, p->Gk, Nx, Ny, Nz, gscale);
+        p->gk_natural = (Nz == 256 || Nz == 512) && p->k3_variant == 0;
+        if (p->gk_natural) k_layout_spectrum_nat<<<grid_for(gk_total, blk), blk, 0, p->stream>>>(p->Goct, p->Gk, Nx, Ny, Nz, gscale);
+        else k_layout_spectrum_oct<<<grid_for(gk_total, blk), blk, 0, p->stream>>>(p->Goct, p->Gk, Nx, Ny, Nz, gscale);
     }
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(p->stream));
@@ -693,7 +758,7 @@ int precompute_impl(fsp_plan* p) {
 }
 
 void free_plan_memory(fsp_plan* p) {
-    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->B3); cudaFree(p->rho_pad); cudaFree(p->phi_pad); cudaFree(p->E_stage); cudaFree(p->rho_stage2); cudaFree(p->phi_stage2); cudaFree(p->Gk); cudaFree(p->LTz); cudaFree(p->LTy); cudaFree(p->LTx); cudaFree(p->T); cudaFree(p->Goct);
+    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->B3); cudaFree(p->rho_pad); cudaFree(p->phi_pad); cudaFree(p->E_stage); cudaFree(p->rho_stage2); cudaFree(p->phi_stage2); cudaFree(p->Gk); cudaFree(p->LTz); cudaFree(p->LTzs); cudaFree(p->LTzf); cudaFree(p->LTy); cudaFree(p->LTx); cudaFree(p->T); cudaFree(p->Goct);
     cudaFree(p->Wx); cudaFree(p->Wy); cudaFree(p->Wz); cudaFree(p->rho_stage); cudaFree(p->phi_stage);
     for (cudaEvent_t e : p->events) cudaEventDestroy(e);
     p->events.clear();
@@ -768,6 +833,9 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
     p->sm_count = prop.multiProcessorCount > 0 ? prop.multiProcessorCount : 148;
     if (rc == FSP_OK) rc = dev_alloc(&p->Gk, (size_t)(Nx + 1) * (Ny + 1) * (Nz + 2), &p->bytes);
     if (rc == FSP_OK) rc = make_z_lane_table(p);
+    if (rc == FSP_OK && Nz == 512) rc = make_lane_table_512s(&p->LTzs, &p->bytes);
+    if (rc == FSP_OK && Nz == 512) rc = lane_table_for<1024>(&p->LTzf, &p->bytes);
+    if (rc == FSP_OK && Nz == 256) rc = lane_table_for<512>(&p->LTzf, &p->bytes);
     p->tile_x = (Nx == 128 || Nx == 256 || Nx == 512 || Nx == 1024) && ((long)Ny * Nz) % kC == 0;
     if (rc == FSP_OK && p->tile_x) rc = make_x_lane_table(p);
     if (rc == FSP_OK && p->tile_x) {
@@ -814,8 +882,14 @@ int fsp_plan_set_param(fsp_plan* p, int which, double value) {
         p->chunk_planes = (int)value;
         return FSP_OK;
     }
+    if (which == FSP_PARAM_K3_VARIANT) {
+        if (value != 0.0 && value != 1.0 && value != 2.0) return FSP_ERR_INVALID_ARG;
+        p->k3_variant = (int)value;
+        p->precomputed = false;   // the layout of the spectrum rows depends on the kernel
+        return FSP_OK;
+    }
     if (which == FSP_PARAM_ALPHA) {
-        if (!(value > 0.0)) return FSP_ERR_INVALID_ARG;
+        if (!(value > 1.0)) return FSP_ERR_INVALID_ARG;   // the window must exceed the domain diagonal
         p->alpha = value;
         return FSP_OK;
     }

@@ -308,4 +308,17 @@ __global__ void k_layout_spectrum_oct(const double* __restrict__ Goct, double* _
     }
 }
 
+// Spectrum layout for k_conv_z_f: the unique octant, rows in natural order with one pad element:
+//   Gk[(kx*(Ny+1) + qy)*(Nz+2) + kz] = scale * Goct[kx][qy][kz],  kz <= Nz
+__global__ void k_layout_spectrum_nat(const double* __restrict__ Goct, double* __restrict__ Gk, int Nx,
+                                      int Ny, int Nz, double scale) {
+    const long row = Nz + 2;
+    const long total = (long)(Nx + 1) * (Ny + 1) * row;
+    for (long o = blockIdx.x * (long)blockDim.x + threadIdx.x; o < total; o += (long)gridDim.x * blockDim.x) {
+        const int c = (int)(o % row);
+        const long pr = o / row;
+        Gk[o] = c <= Nz ? scale * Goct[pr * (Nz + 1) + c] : 0.0;
+    }
+}
+
 }  // namespace fsp

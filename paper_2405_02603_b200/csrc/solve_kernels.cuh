@@ -671,6 +671,261 @@ k_conv_z_p(double2* __restrict__ B2, const double* __restrict__ Gk, const double
     }
 }
 
+// ====================================================================== K3 (v4, Nz = 256, 512): conv_z_f
+// One lane group transforms the WHOLE zero-padded pencil of M2 = 2 Nz points (1024 = 32 x 32 over a warp at
+// Nz = 512; 512 = 16 x 32 over a half-warp, two pencils per warp, at Nz = 256) with fft2_padded_pass: forward with
+// the zero half pruned inside stage 1, times Ghat, inverse with the discarded half pruned inside stage 2.  Against
+// the branch-pair kernels (k_conv_z_p, k_conv_z_w: two half-length transforms per direction) the pencil is read
+// once, there is no pre-twiddle x[n] w^n, no final sum y_e + conj(w^n) y_o, no twiddle table and no hand-over
+// between warps: 704 instead of 992 L1/shared-memory wavefronts per pencil, the same fp64 work.
+// Spectrum rows: the unique octant in natural order (k_layout_spectrum_nat), Ghat[kz] = row[min(kz, M2 - kz)]: every
+// read is a lane pointer plus a compile-time offset.  Rows are staged by bulk async copies (one mbarrier per warp);
+// visiting order as in k_conv_z_w (two pencils sharing a row run back to back).  Persistent warps, no CTA barrier.
+template <int M2>
+struct ConvZF {
+    using Cfg = Fft2Cfg<M2>;
+    static constexpr int M = M2 / 2;                       // Nz
+    static constexpr int T = Cfg::T, R = Cfg::R;
+    static constexpr int G = 32 / T;                       // pencils per warp
+#ifndef FSP_ZF_WARPS
+#define FSP_ZF_WARPS 8
+#endif
+    static constexpr int WARPS = FSP_ZF_WARPS;             // 8 warps at <= 255 registers (warps are allocated in fours:
+                                                           // the next step, 12, leaves 168 registers and spills)
+    static constexpr int ROW = M + 2;                      // doubles per spectrum row: Ghat[0..M], one pad
+    static constexpr int NC = LaneTw<Cfg::R2>::NC;
+    // [exchange: WARPS*G*BUF double2][G rows: WARPS*G*ROW doubles][mbarriers: WARPS]
+    static constexpr size_t smem_bytes() {
+        return sizeof(double2) * (size_t)(WARPS * G * Cfg::BUF) + sizeof(double) * (size_t)(WARPS * G * ROW) + 8 * WARPS;
+    }
+};
+
+template <int M2, bool DER = false>
+__global__ void __launch_bounds__(ConvZF<M2>::WARPS * 32, 1)
+k_conv_z_f(double2* __restrict__ B2, const double* __restrict__ Gk, const double* __restrict__ lane_g, int Ny,
+           long ngroups, double2* __restrict__ out, const DerK kap) {
+    using Z = ConvZF<M2>;
+    using Cfg = typename Z::Cfg;
+    constexpr int M = Z::M, R = Z::R, T = Z::T, G = Z::G, WARPS = Z::WARPS, NC = Z::NC, H = R / 2;
+    extern __shared__ double2 smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int g = lane / T, t = lane % T;
+    double2* buf = smem + (warp * G + g) * Cfg::BUF;
+    double* gall = reinterpret_cast<double*>(smem + WARPS * G * Cfg::BUF);
+    double* gst = gall + (warp * G + g) * Z::ROW;
+    uint64_t* gbar = reinterpret_cast<uint64_t*>(gall + WARPS * G * Z::ROW) + warp;
+    if (lane == 0) { mbar_init(gbar, 1); mbar_fence_init(); }
+    __syncwarp();
+    uint32_t gpar = 0;
+    double cc[NC], tn[NC];   // stage-2 twiddles of this lane's butterfly j = t, in registers for the whole kernel
+#pragma unroll
+    for (int i = 0; i < NC; ++i) {
+        cc[i] = lane_g[t * 2 * NC + i];
+        tn[i] = lane_g[t * 2 * NC + NC + i];
+    }
+    // Ghat[kz], kz = t + T i: the row entry min(kz, M2 - kz); rows are in natural order (k_layout_spectrum_nat), so a
+    // lane group reads T consecutive doubles per instruction (no bank conflicts)
+    const double* gA = gst + t;
+    const double* gB = gst + (M2 - t);
+    const int nwarps = gridDim.x * WARPS;
+    const int ny2 = 2 * Ny;
+    auto locate = [&](int s_, int& kx_, int& ky_) {   // position in the visiting order -> (kx, ky)
+        kx_ = s_ / ny2;
+        const int r_ = s_ - kx_ * ny2;
+        ky_ = (r_ & 1) ? ny2 - ((r_ + 1) >> 1) : (r_ >> 1);
+    };
+    for (int grp = blockIdx.x * WARPS + warp; grp < (int)ngroups; grp += nwarps) {
+        int kx, ky;
+        locate(grp * G + g, kx, ky);
+        double2* base = B2 + ((long)kx * ny2 + ky) * M;
+        double2* obase = DER ? out + ((long)kx * ny2 + ky) * M : base;
+        double fp = 0.0;   // pencil-constant part of the derivative factor
+        if constexpr (DER) fp = kap.x * signed_mode(kx, kap.Nx) + kap.y * signed_mode(ky, Ny);
+        // every lane is past the previous group's reads of the staged rows (the __syncwarp()s of its second pass)
+        if (lane == 0) {
+            mbar_arrive_expect_tx(gbar, G * Z::ROW * 8);
+#pragma unroll
+            for (int gg = 0; gg < G; ++gg) {
+                int kx2, ky2;
+                locate(grp * G + gg, kx2, ky2);
+                const int qy2 = ky2 <= Ny ? ky2 : ny2 - ky2;
+                bulk_load(gall + (warp * G + gg) * Z::ROW, Gk + ((long)kx2 * (Ny + 1) + qy2) * Z::ROW, Z::ROW * 8, gbar);
+            }
+        }
+        double vr[R], vi[R];
+#pragma unroll
+        for (int i = 0; i < H; ++i) {   // the non-zero half of the padded pencil, and the first radix-2 level of the
+            const double2 v = base[t + T * i];   // forward pass: (x_i, 0) -> (x_i, x_i)
+            vr[i] = v.x; vi[i] = v.y;
+            vr[i + H] = v.x; vi[i + H] = v.y;
+        }
+        if (grp + nwarps < (int)ngroups) {   // L2 prefetch of this lane group's next pencil: M * 16 / 128 lines
+            int kx2, ky2;
+            locate((grp + nwarps) * G + g, kx2, ky2);
+            const double2* nb = B2 + ((long)kx2 * ny2 + ky2) * M;
+#pragma unroll
+            for (int e = 0; e < M / 8; e += T) asm volatile("prefetch.global.L2 [%0];" ::"l"(nb + (e + t) * 8));
+        }
+#pragma unroll 1
+        for (int pass = 0; pass < 2; ++pass) {
+            fft2_padded_pass<Cfg>(vr, vi, t, buf, cc, tn, pass);
+            if (pass == 0) {   // Y = conj(Ghat X)
+                mbar_wait(gbar, gpar);
+                gpar ^= 1;
+                const double fz0 = fp + kap.z * (double)t;   // DER only
+#pragma unroll
+                for (int i = 0; i < R; ++i) {
+                    const double gk = i < H ? gA[T * i] : gB[-T * i];
+                    if constexpr (DER) {
+                        // signed mode of kz = t + T i: kz below M, kz - M2 above, zero at the Nyquist index kz = M
+                        // (t = 0, i = R/2); the factor -i itself is applied to the final result (F^-1 is linear)
+                        double cf = gk * fma(kap.z, (double)(i < H ? T * i : T * i - M2), fz0);
+                        if (i == H) cf = t == 0 ? gk * fp : cf;
+                        vr[i] *= cf; vi[i] *= -cf;
+                    } else {
+                        vr[i] *= gk; vi[i] *= -gk;
+                    }
+                }
+            }
+        }
+        // v = FFT(conj(Ghat X)) = conj(y): the kept half
+#pragma unroll
+        for (int i = 0; i < H; ++i)
+            obase[t + T * i] = DER ? make_double2(-vi[i], -vr[i]) : make_double2(vr[i], -vi[i]);   // DER: -i y
+    }
+}
+
+// ====================================================================== K3 (v3, Nz = 512): conv_z_s
+// The pair scheme of k_conv_z_p with the 32-lane transform of fft_warp.cuh (fft512s_forward): a warp holds ONE
+// pencil branch with 16 points per lane, so the kernel needs half the registers (<= 128) and an SM runs 16 warps
+// (8 pairs) instead of 8: with four warps per scheduler the fp64 phases of some warps overlap the shared-memory
+// phases of the others (k_conv_z_p at 254 registers: fp64 pipe 59 %, 2 warps per scheduler).  Everything else as
+// in k_conv_z_p: one copy of the transform run twice (IFFT(Y) = conj(FFT(conj(Y)))), octant spectrum rows staged by
+// bulk async copies, the visiting order that lets two pencils share a row in L2, hand-over of v_o through the odd
+// warp's exchange buffer under a pair barrier.
+struct ConvZS {
+    using F = Fft512S;
+    static constexpr int M = 512, T = 32, R = 16;
+    static constexpr int PAIRS = 8, WARPS = 2 * PAIRS;
+    static constexpr int ROW = M + 2;
+    // [wp: M double2][exchange: WARPS*BUF double2][G rows: PAIRS*ROW doubles][mbarriers: PAIRS]
+    static constexpr size_t smem_bytes() {
+        return sizeof(double2) * (size_t)(M + WARPS * F::BUF) + sizeof(double) * (size_t)(PAIRS * ROW) + 8 * PAIRS;
+    }
+};
+
+template <bool DER = false>
+__global__ void __launch_bounds__(ConvZS::WARPS * 32, 1)
+k_conv_z_s(double2* __restrict__ B2, const double* __restrict__ Gk, const double* __restrict__ lane_g,
+           const double2* __restrict__ wp_g, int Ny, long nsteps, double2* __restrict__ out, const DerK kap) {
+    using Z = ConvZS;
+    using F = Fft512S;
+    constexpr int M = Z::M, R = Z::R, T = Z::T, PAIRS = Z::PAIRS, WARPS = Z::WARPS, NC = F::NC;
+    extern __shared__ double2 smem[];
+    double2* wp = smem;          // M: w_2M^n, n < M
+    for (int n = threadIdx.x; n < M; n += blockDim.x) wp[n] = wp_g[n];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, q = warp >> 1, b = warp & 1;
+    const int t = lane;
+    double2* buf = smem + M + warp * F::BUF;
+    double2* pbuf = smem + M + (warp ^ 1) * F::BUF;          // the partner's buffer
+    double* gall = reinterpret_cast<double*>(smem + M + WARPS * F::BUF);
+    double* gst = gall + q * Z::ROW;
+    uint64_t* gbar = reinterpret_cast<uint64_t*>(gall + PAIRS * Z::ROW) + q;
+    if (b == 0 && lane == 0) { mbar_init(gbar, 1); mbar_fence_init(); }
+    __syncthreads();
+    uint32_t gpar = 0;
+    double cc[NC], tn[NC], xc[8], xt[8];
+#pragma unroll
+    for (int i = 0; i < NC; ++i) {
+        cc[i] = lane_g[t * 2 * NC + i];
+        tn[i] = lane_g[t * 2 * NC + NC + i];
+    }
+#pragma unroll
+    for (int m = 0; m < 8; ++m) {
+        xc[m] = lane_g[32 * 2 * NC + (lane >> 4) * 16 + m];
+        xt[m] = lane_g[32 * 2 * NC + (lane >> 4) * 16 + 8 + m];
+    }
+    const int npairs = gridDim.x * PAIRS;
+    const int ny2 = 2 * Ny;
+    auto locate = [&](int s_, int& kx_, int& ky_) {   // position in the visiting order -> (kx, ky)
+        kx_ = s_ / ny2;
+        const int r_ = s_ - kx_ * ny2;
+        ky_ = (r_ & 1) ? ny2 - ((r_ + 1) >> 1) : (r_ >> 1);
+    };
+    for (int step = blockIdx.x * PAIRS + q; step < (int)nsteps; step += npairs) {
+        int kx, ky;
+        locate(step, kx, ky);
+        const int qy = ky <= Ny ? ky : ny2 - ky;
+        double2* base = B2 + ((long)kx * ny2 + ky) * M;
+        double2* obase = DER ? out + ((long)kx * ny2 + ky) * M : base;
+        double fp = 0.0;
+        if constexpr (DER) fp = kap.x * signed_mode(kx, kap.Nx) + kap.y * signed_mode(ky, Ny);
+        // both warps are past the previous step's reads of the staged row (the pair barrier ending the combine)
+        if (b == 0 && lane == 0) {
+            mbar_arrive_expect_tx(gbar, Z::ROW * 8);
+            bulk_load(gst, Gk + ((long)kx * (Ny + 1) + qy) * Z::ROW, Z::ROW * 8, gbar);
+        }
+        double vr[R], vi[R];
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            const double2 v = base[t + T * i];
+            vr[i] = v.x; vi[i] = v.y;
+        }
+        if (step + npairs < (int)nsteps) {   // L2 prefetch of the pair's next pencil, half of the lines from each warp
+            int kx2, ky2;
+            locate(step + npairs, kx2, ky2);
+            const double2* nb = B2 + ((long)kx2 * ny2 + ky2) * M;
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(nb + (b * 32 + lane) * 8));   // 64 lines of 128 bytes
+        }
+        if (b) {
+#pragma unroll
+            for (int i = 0; i < R; ++i) cmul(vr[i], vi[i], wp[t + T * i]);
+        }
+#pragma unroll 1
+        for (int pass = 0; pass < 2; ++pass) {
+            fft512s_forward(vr, vi, lane, buf, cc, tn, xc, xt);
+            if (pass == 0) {
+                mbar_wait(gbar, gpar);
+                gpar ^= 1;
+                const double* gsrc = gst + (b ? M / 2 + 1 : 0);
+                const double* gA = gsrc + t;
+                const double* gB = gsrc + (M - b - t);
+                const double fz0 = fp + kap.z * (double)(2 * t + b);   // DER only
+                const bool nyq = (2 * t + b) == 0;                      // register R/2 of this lane is kz = M
+#pragma unroll
+                for (int i = 0; i < R; ++i) {
+                    const double gk = i < R / 2 ? gA[T * i] : gB[-T * i];   // row index min(j, M-b-j), j = t + T i
+                    if constexpr (DER) {
+                        double cf = gk * fma(kap.z, (double)(i < R / 2 ? 2 * T * i : 2 * T * i - 2 * M), fz0);
+                        if (i == R / 2) cf = nyq ? gk * fp : cf;
+                        vr[i] *= cf; vi[i] *= -cf;
+                    } else {
+                        vr[i] *= gk; vi[i] *= -gk;
+                    }
+                }
+            }
+        }
+        // v = FFT(conj(Ghat X)) on each branch; y[n] = conj(v_e[n] + w^n v_o[n]), formed by the even warp
+        if (b) {
+            __syncwarp();   // this warp's exchange reads are complete: buf becomes the outbox
+#pragma unroll
+            for (int i = 0; i < R; ++i) buf[t + T * i] = make_double2(vr[i], vi[i]);
+        }
+        bar_sync(1 + q, 64);
+        if (!b) {
+#pragma unroll
+            for (int i = 0; i < R; ++i) {
+                const double2 pv = pbuf[t + T * i];   // v_o[n], n = t + T i
+                const double2 w = wp[t + T * i];
+                const double zr = fma(-w.y, pv.y, fma(w.x, pv.x, vr[i]));
+                const double zi = fma(w.y, pv.x, fma(w.x, pv.y, vi[i]));
+                obase[t + T * i] = DER ? make_double2(-zi, -zr) : make_double2(zr, -zi);   // DER: -i y
+            }
+        }
+        bar_sync(1 + q, 64);   // the even warp has read the outbox (and both are done with the staged row)
+    }
+}
+
 // ================================================================================ K1 (v2): fwd_x_r2c_t
 // Tile kernel for the real-to-complex pass along x (M = Nx/2 complex points z[n] = rho[2n] + i rho[2n+1]).
 // Tile = all Nx rows of kC = 16 adjacent columns of the flattened (y, z) plane (one 128-byte line of

@@ -76,7 +76,9 @@ __device__ __forceinline__ void bar_sync(int id, int nthreads) {
     else if (id == 3) asm volatile("bar.sync 3, %0;" ::"r"(nthreads) : "memory");
     else if (id == 4) asm volatile("bar.sync 4, %0;" ::"r"(nthreads) : "memory");
     else if (id == 5) asm volatile("bar.sync 5, %0;" ::"r"(nthreads) : "memory");
-    else asm volatile("bar.sync 6, %0;" ::"r"(nthreads) : "memory");
+    else if (id == 6) asm volatile("bar.sync 6, %0;" ::"r"(nthreads) : "memory");
+    else if (id == 7) asm volatile("bar.sync 7, %0;" ::"r"(nthreads) : "memory");
+    else asm volatile("bar.sync 8, %0;" ::"r"(nthreads) : "memory");
 }
 
 }  // namespace fsp

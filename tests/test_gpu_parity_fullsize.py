@@ -85,6 +85,27 @@ def test_full_field_of_the_field_output_where_loops_iterate(N):
         check(E[d], E_o[d])
 
 
+@pytest.mark.parametrize("N,variant", [((32, 32, 512), 1), ((32, 32, 512), 2), ((64, 32, 256), 1), ((16, 64, 512), 0)])
+def test_z_pass_kernel_variants_full_field(N, variant):
+    """FSP_PARAM_K3_VARIANT: the branch-pair kernels of the z pass (k_conv_z_p, k_conv_z_s) stay selectable for A/B
+    measurements; each against the oracle, phi and the field (the DER variants), where the persistent loops iterate."""
+    w = W.random_density(N, seed=sum(N) + 3)
+    with binding.Plan(w.N, w.h, binding.VICO_2) as p:
+        binding.plan_set_param(p.handle, binding.PARAM_K3_VARIANT, variant)
+        with pytest.raises(binding.FspError):
+            binding.plan_set_param(p.handle, binding.PARAM_K3_VARIANT, 3)
+        p.precompute_green()
+        phi, E = p.solve_field(torch.from_numpy(w.rho).cuda())
+        phi2 = p.solve(torch.from_numpy(w.rho).cuda())
+        torch.cuda.synchronize()
+        assert torch.equal(phi, phi2)
+        phi, E = phi.cpu().numpy(), E.cpu().numpy()
+    phi_o, E_o = oracle.OraclePlan(w.N, w.h, oracle.VICO_2).precompute_green().solve_field(w.rho)
+    check(phi, phi_o)
+    for d in range(3):
+        check(E[d], E_o[d])
+
+
 # ---- (b) BASELINE configs 3 and 4, full field against O2 with the oracle's own table -------------------------
 @pytest.mark.parametrize("alg", ["HE", "VG2"])
 def test_config3_256_full_field_against_the_oracle(alg):
