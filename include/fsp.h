@@ -27,8 +27,13 @@
  *     has period 2 N'_d h_d.  Cost and memory are those of the N' mesh.
  *   - rho, phi: dense fp64 arrays of shape (Nx, Ny, Nz) in C order, index (ix*Ny + iy)*Nz + iz,
  *     iz fastest.  The sample position inside a cell does not matter (translation invariance).
- *   - "dev" pointers are CUDA device pointers on the device that was current at plan creation;
- *     "host" pointers are ordinary host memory (pinned memory makes the copies asynchronous).
+ *   - "dev" pointers are CUDA device pointers on the device that was current at plan creation (the
+ *     plan's device); "host" pointers are ordinary host memory (pinned memory makes the copies
+ *     asynchronous).  Devices: every call that touches the GPU switches to the plan's device for its
+ *     duration and restores the caller's current device before it returns, so plans on several devices can
+ *     be driven from one process and one thread whatever device is current; shared-memory opt-ins and
+ *     occupancies are cached per device.  Threads: different plans may be used from different host
+ *     threads concurrently; one plan must not be used by two threads at the same time.
  *   - The caller owns rho and phi; rho is read-only; rho and phi must not overlap.  The plan owns
  *     the spectrum, twiddle tables and workspace.  fsp_solve allocates nothing and does not
  *     synchronise the host: it is ordered on the stream given at plan creation.
@@ -65,7 +70,7 @@ enum {
     FSP_OK = 0,
     FSP_ERR_INVALID_ARG = -1,     /* null pointer, N_d outside [2,1024], h <= 0, bad enum             */
     FSP_ERR_NOT_PRECOMPUTED = -2, /* fsp_solve / getters before fsp_precompute_green                 */
-    FSP_ERR_OUT_OF_MEMORY = -3,   /* device allocation failed (e.g. FSP_VICO at 512^3: (4N)^3 grid)  */
+    FSP_ERR_OUT_OF_MEMORY = -3,   /* device allocation failed (e.g. FSP_VICO at 1024^3: (4N)^3 lattice) */
     FSP_ERR_CUDA = -4,            /* a CUDA runtime call or kernel launch failed                     */
     FSP_ERR_NO_DEVICE = -5        /* no CUDA device / not an sm_100 device                           */
 };
@@ -118,7 +123,8 @@ int fsp_plan_set_spacing(fsp_plan* p, const double* h);
  * Fills the plan-owned real-space table T[dx][dy][dz] (0 <= d_d <= N_d, the kernel at displacement
  * (dx hx, dy hy, dz hz)) and the spectrum F{G2} of its 8-case mirror, with the
  * factor hx hy hz / (8 Nx Ny Nz) of PAPER.md:80 folded in.  Transient device memory is allocated
- * and freed inside the call (FSP_VICO: a (4Nx)(4Ny)(4Nz) complex grid).  Synchronises the
+ * and freed inside the call (FSP_VICO: the C2R half spectrum of the (4N)^3 lattice, (2Nx+1)(4Ny)(4Nz) complex
+ * values, 8.6 GB at 256^3; FSP_VICO_2: (2Nx+1)(2Ny+1)(2Nz+1) reals).  Synchronises the
  * stream before returning.  Re-callable (e.g. after fsp_plan_set_param).
  */
 int fsp_precompute_green(fsp_plan* p);
@@ -193,6 +199,15 @@ double fsp_model_bytes_per_field_solve(const fsp_plan* p, int with_phi);
 /* Oversampling factors (m_x, m_y, m_z) used by the last fsp_precompute_green of a VG algorithm
  * (4,4,4 for FSP_VICO and FSP_VICO_2); m_out: host pointer to 3 ints. */
 int fsp_get_vg_factors(const fsp_plan* p, int* m_out);
+
+/* Does the frequency lattice of the plan's Vico-Greengard algorithm keep the periodic images of the truncated kernel
+ * out of the table?  PAPER.md:92-94: L = alpha x diagonal and a fixed 4x oversampling; the kernel of radius L is
+ * periodised with period m_d L_d and used up to displacement L_d, so the condition is m_d L_d >= L + L_d on every
+ * axis (R17).  *safe_out = 1 if it holds for the factors the plan would use NOW (m = 4 for FSP_VICO and
+ * FSP_VICO_2; the per-axis factors of FSP_VICO_SAFE, which satisfy it by construction; FSP_HOCKNEY: always 1), else
+ * 0: on such a box (longer than about 2.7 times its shortest side) FSP_VICO / FSP_VICO_2 alias silently and
+ * FSP_VICO_SAFE is the algorithm to use.  No GPU work; callable before fsp_precompute_green. */
+int fsp_vg_lattice_is_safe(const fsp_plan* p, int* safe_out);
 
 /* Copies the real-space table T, (Nx+1)(Ny+1)(Nz+1) doubles in C order, to host memory. */
 int fsp_get_green_table(const fsp_plan* p, double* T_host);

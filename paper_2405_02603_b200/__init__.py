@@ -5,4 +5,4 @@ Vico-Greengard spectra, pruned + fused fp64 FFT convolution in hand-written sm_1
 ``workloads`` holds the seeded synthetic inputs; ``build`` compiles the library in-tree.
 """
 from . import binding, workloads  # noqa: F401
-from .binding import HOCKNEY, VICO, VICO_2, FspError, Plan  # noqa: F401
+from .binding import HOCKNEY, VICO, VICO_2, VICO_SAFE, FspError, Plan  # noqa: F401

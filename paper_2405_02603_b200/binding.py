@@ -43,6 +43,7 @@ SIGNATURES = {
     "fsp_precompute_peak_bytes": (_sz, [_vp]),
     "fsp_model_bytes_per_solve": (_d, [_vp, _dp]),
     "fsp_get_vg_factors": (_i, [_vp, _c.POINTER(_i)]),
+    "fsp_vg_lattice_is_safe": (_i, [_vp, _c.POINTER(_i)]),
     "fsp_get_green_table": (_i, [_vp, _dp]),
     "fsp_get_green_spectrum": (_i, [_vp, _dp]),
     "fsp_set_profiling": (_i, [_vp, _i]),
@@ -179,6 +180,12 @@ def get_vg_factors(plan: int):
     return tuple(int(v) for v in m)
 
 
+def vg_lattice_is_safe(plan: int) -> bool:
+    ok = _i(0)
+    _chk(lib().fsp_vg_lattice_is_safe(plan, ctypes.byref(ok)), "fsp_vg_lattice_is_safe")
+    return bool(ok.value)
+
+
 def get_green_table(plan: int, N) -> np.ndarray:
     T = np.empty(tuple(n + 1 for n in N), dtype=np.float64)
     _chk(lib().fsp_get_green_table(plan, T.ctypes.data_as(_dp)), "fsp_get_green_table")
@@ -268,6 +275,9 @@ class Plan:
 
     def vg_factors(self):
         return get_vg_factors(self.handle)
+
+    def vg_lattice_is_safe(self) -> bool:
+        return vg_lattice_is_safe(self.handle)
 
     def green_table(self) -> np.ndarray:
         return get_green_table(self.handle, self.N)

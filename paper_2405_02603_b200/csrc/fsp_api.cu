@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <atomic>
 #include <vector>
 
 #include <cuda.h>
@@ -17,7 +18,7 @@
 
 using namespace fsp;
 
-#define FSP_VERSION_NUM 110
+#define FSP_VERSION_NUM 200
 
 struct fsp_plan {
     int Nx = 0, Ny = 0, Nz = 0;   // transform mesh: each a power of two (the caller's mesh when that is one)
@@ -223,18 +224,45 @@ int make_tensor_map(CUtensorMap* tm, void* base, int rank, const cuuint64_t* dim
     return r == CUDA_SUCCESS ? FSP_OK : FSP_ERR_CUDA;
 }
 
+// ---- per-device caches -------------------------------------------------------------------------------
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) and the occupancy of a kernel belong to a DEVICE, not to the
+// process: every launch helper keeps one slot per device (zero = not yet queried; the query is idempotent, so two
+// host threads racing on a slot do no harm).
+constexpr int kMaxDevices = 64;
+struct OccCache { std::atomic<int> v[kMaxDevices]; };
+template <class Kern>
+int cached_occupancy(OccCache& c, int dev, Kern kern, int threads, size_t smem, int* occ_out) {
+    int o = c.v[dev].load(std::memory_order_acquire);
+    if (o == 0) {
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, kern, threads, smem));
+        if (o < 1) return FSP_ERR_CUDA;
+        c.v[dev].store(o, std::memory_order_release);
+    }
+    *occ_out = o;
+    return FSP_OK;
+}
+// Every entry point runs on the plan's device and restores the caller's current device on return.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+};
+
 // ---- kernel launch helpers (one template instantiation per FFT length) ---------------------------
 template <int M>
 int launch_fwd_y_t(fsp_plan* p, int kx0, double2* B2, int nplanes) {
     using Y = TileY<M>;
     const long ntiles = (long)nplanes * (p->Nz / Y::KW);
     const size_t smem = Y::smem_bytes();
-    static int occ = 0;
-    if (occ == 0) {
-        CU(cudaFuncSetAttribute(k_fwd_y_t<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_fwd_y_t<M>, Y::THREADS, smem));
-        if (occ < 1) return FSP_ERR_CUDA;
-    }
+    static OccCache cache;   // per device: function attributes and occupancy belong to the device
+    int occ = 0;
+    { const int rc_ = cached_occupancy(cache, p->device, k_fwd_y_t<M>, Y::THREADS, smem, &occ); if (rc_ != FSP_OK) return rc_; }
     long grid = (long)p->sm_count * occ;
     if (grid > ntiles) grid = ntiles;
     k_fwd_y_t<M><<<(unsigned)grid, Y::THREADS, smem, p->stream>>>(p->tmB1y, B2, p->LTy, p->Wy, p->Nz, kx0, ntiles);
@@ -246,12 +274,9 @@ int launch_fwd_y(fsp_plan* p, const double2* B1, double2* B2, int nplanes) {
     constexpr int G = TileGroups<Cfg>::G;
     const long ntiles = (long)nplanes * (p->Nz / kW);
     const size_t smem = sizeof(double2) * (size_t)(2 * M + G * M * kW);
-    static int occ = 0;
-    if (occ == 0) {
-        CU(cudaFuncSetAttribute(k_fwd_y<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_fwd_y<M>, G * kW * Cfg::T, smem));
-        if (occ < 1) return FSP_ERR_CUDA;
-    }
+    static OccCache cache;   // per device: function attributes and occupancy belong to the device
+    int occ = 0;
+    { const int rc_ = cached_occupancy(cache, p->device, k_fwd_y<M>, G * kW * Cfg::T, smem, &occ); if (rc_ != FSP_OK) return rc_; }
     long grid = (ntiles + G - 1) / G;
     if (grid > (long)p->sm_count * occ) grid = (long)p->sm_count * occ;
     k_fwd_y<M><<<(unsigned)grid, G * kW * Cfg::T, smem, p->stream>>>(B1, B2, p->Wy, p->Nz, ntiles);
@@ -263,12 +288,9 @@ int launch_inv_y_impl(fsp_plan* p, const double2* B2, double2* B1, int nplanes, 
     constexpr int G = TileGroups<Cfg>::G;
     const long ntiles = (long)nplanes * (p->Nz / kW);
     const size_t smem = sizeof(double2) * (size_t)(2 * M + G * M * kW);
-    static int occ = 0;
-    if (occ == 0) {
-        CU(cudaFuncSetAttribute(k_inv_y<M, DER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_inv_y<M, DER>, G * kW * Cfg::T, smem));
-        if (occ < 1) return FSP_ERR_CUDA;
-    }
+    static OccCache cache;   // per device: function attributes and occupancy belong to the device
+    int occ = 0;
+    { const int rc_ = cached_occupancy(cache, p->device, k_inv_y<M, DER>, G * kW * Cfg::T, smem, &occ); if (rc_ != FSP_OK) return rc_; }
     long grid = (ntiles + G - 1) / G;
     if (grid > (long)p->sm_count * occ) grid = (long)p->sm_count * occ;
     k_inv_y<M, DER><<<(unsigned)grid, G * kW * Cfg::T, smem, p->stream>>>(B2, B1, p->Wy, p->Nz, ntiles, kder);
@@ -285,12 +307,9 @@ int launch_conv_z_p_impl(fsp_plan* p, double2* B2, const double* G, int nplanes,
     using Z = ConvZP<M>;
     const long nsteps = (long)nplanes * (2 * p->Ny) / Z::G;   // pair steps: G pencils each
     const size_t smem = Z::smem_bytes();
-    static int occ = 0;
-    if (occ == 0) {
-        CU(cudaFuncSetAttribute(k_conv_z_p<M, DER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_conv_z_p<M, DER>, Z::WARPS * 32, smem));
-        if (occ < 1) return FSP_ERR_CUDA;
-    }
+    static OccCache cache;   // per device: function attributes and occupancy belong to the device
+    int occ = 0;
+    { const int rc_ = cached_occupancy(cache, p->device, k_conv_z_p<M, DER>, Z::WARPS * 32, smem, &occ); if (rc_ != FSP_OK) return rc_; }
     long grid = (long)p->sm_count * occ;
     const long need = (nsteps + Z::PAIRS - 1) / Z::PAIRS;
     if (grid > need) grid = need;
@@ -302,12 +321,9 @@ int launch_conv_z_s_impl(fsp_plan* p, double2* B2, const double* G, int nplanes,
     using Z = ConvZS;
     const long nsteps = (long)nplanes * (2 * p->Ny);   // pair steps: one pencil each
     const size_t smem = Z::smem_bytes();
-    static int occ = 0;
-    if (occ == 0) {
-        CU(cudaFuncSetAttribute(k_conv_z_s<DER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_conv_z_s<DER>, Z::WARPS * 32, smem));
-        if (occ < 1) return FSP_ERR_CUDA;
-    }
+    static OccCache cache;   // per device: function attributes and occupancy belong to the device
+    int occ = 0;
+    { const int rc_ = cached_occupancy(cache, p->device, k_conv_z_s<DER>, Z::WARPS * 32, smem, &occ); if (rc_ != FSP_OK) return rc_; }
     long grid = (long)p->sm_count * occ;
     const long need = (nsteps + Z::PAIRS - 1) / Z::PAIRS;
     if (grid > need) grid = need;
@@ -319,12 +335,9 @@ int launch_conv_z_f_impl(fsp_plan* p, double2* B2, const double* G, int nplanes,
     using Z = ConvZF<M2>;
     const long ngroups = (long)nplanes * (2 * p->Ny) / Z::G;
     const size_t smem = Z::smem_bytes();
-    static int occ = 0;
-    if (occ == 0) {
-        CU(cudaFuncSetAttribute(k_conv_z_f<M2, DER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_conv_z_f<M2, DER>, Z::WARPS * 32, smem));
-        if (occ < 1) return FSP_ERR_CUDA;
-    }
+    static OccCache cache;   // per device: function attributes and occupancy belong to the device
+    int occ = 0;
+    { const int rc_ = cached_occupancy(cache, p->device, k_conv_z_f<M2, DER>, Z::WARPS * 32, smem, &occ); if (rc_ != FSP_OK) return rc_; }
     long grid = (long)p->sm_count * occ;
     const long need = (ngroups + Z::WARPS - 1) / Z::WARPS;
     if (grid > need) grid = need;
@@ -343,12 +356,9 @@ int launch_conv_z_w_impl(fsp_plan* p, double2* B2, const double* G, int nplanes,
     using Z = ConvZ<M>;
     const long ngroups = (long)nplanes * (2 * p->Ny) / Z::G;
     const size_t smem = Z::smem_bytes();
-    static int occ = 0;  // CTAs per SM, queried once per transform length
-    if (occ == 0) {
-        CU(cudaFuncSetAttribute(k_conv_z_w<M, DER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_conv_z_w<M, DER>, Z::WARPS * 32, smem));
-        if (occ < 1) return FSP_ERR_CUDA;
-    }
+    static OccCache cache;   // per device: function attributes and occupancy belong to the device
+    int occ = 0;
+    { const int rc_ = cached_occupancy(cache, p->device, k_conv_z_w<M, DER>, Z::WARPS * 32, smem, &occ); if (rc_ != FSP_OK) return rc_; }
     long grid = (long)p->sm_count * occ;
     const long need = (ngroups + Z::WARPS - 1) / Z::WARPS;
     if (grid > need) grid = need;
@@ -367,7 +377,9 @@ int launch_fwd_x(fsp_plan* p, const double* rho) {
     constexpr int G = TileGroups<Cfg>::G;
     const long ntiles = (long)p->Ny * (p->Nz / kW);
     const size_t smem = sizeof(double2) * (size_t)(4 * M + G * M * kW + G * 2 * M * kW);
-    CU(cudaFuncSetAttribute(k_fwd_x_r2c<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    static OccCache cache;
+    int occ = 0;
+    { const int rc_ = cached_occupancy(cache, p->device, k_fwd_x_r2c<M>, G * kW * Cfg::T, smem, &occ); if (rc_ != FSP_OK) return rc_; }
     k_fwd_x_r2c<M><<<(unsigned)((ntiles + G - 1) / G), G * kW * Cfg::T, smem, p->stream>>>(rho, p->B1, p->Wx, p->Ny, p->Nz, ntiles);
     return FSP_OK;
 }
@@ -377,7 +389,9 @@ int launch_inv_x_impl(fsp_plan* p, double* phi, double kder) {
     constexpr int G = TileGroups<Cfg>::G;
     const long ntiles = (long)p->Ny * (p->Nz / kW);
     const size_t smem = sizeof(double2) * (size_t)(4 * M + G * M * kW);
-    CU(cudaFuncSetAttribute(k_inv_x_c2r<M, DER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    static OccCache cache;
+    int occ = 0;
+    { const int rc_ = cached_occupancy(cache, p->device, k_inv_x_c2r<M, DER>, G * kW * Cfg::T, smem, &occ); if (rc_ != FSP_OK) return rc_; }
     k_inv_x_c2r<M, DER><<<(unsigned)((ntiles + G - 1) / G), G * kW * Cfg::T, smem, p->stream>>>(p->B1, phi, p->Wx, p->Ny, p->Nz, ntiles, kder);
     return FSP_OK;
 }
@@ -417,12 +431,9 @@ int launch_fwd_x_t(fsp_plan* p) {
     using X_ = TileX<M>;
     const long plane = (long)p->Ny * p->Nz, ntiles = plane / X_::KC;
     const size_t smem = X_::smem_bytes();
-    static int occ = 0;
-    if (occ == 0) {
-        CU(cudaFuncSetAttribute(k_fwd_x_t<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_fwd_x_t<M>, X_::THREADS, smem));
-        if (occ < 1) return FSP_ERR_CUDA;
-    }
+    static OccCache cache;   // per device: function attributes and occupancy belong to the device
+    int occ = 0;
+    { const int rc_ = cached_occupancy(cache, p->device, k_fwd_x_t<M>, X_::THREADS, smem, &occ); if (rc_ != FSP_OK) return rc_; }
     long grid = (long)p->sm_count * occ;
     if (grid > ntiles) grid = ntiles;
     k_fwd_x_t<M><<<(unsigned)grid, X_::THREADS, smem, p->stream>>>(p->tmRho, p->B1, p->LTx, p->Wx, plane, ntiles);
@@ -481,12 +492,9 @@ int launch_inv_y_t_impl(fsp_plan* p, const CUtensorMap& tm, double2* B1, int npl
     using Y = TileYI<M>;
     const long ntiles = (long)nplanes * (p->Nz / Y::KW);
     const size_t smem = Y::smem_bytes();
-    static int occ = 0;
-    if (occ == 0) {
-        CU(cudaFuncSetAttribute(k_inv_y_t<M, DER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_inv_y_t<M, DER>, Y::THREADS, smem));
-        if (occ < 1) return FSP_ERR_CUDA;
-    }
+    static OccCache cache;   // per device: function attributes and occupancy belong to the device
+    int occ = 0;
+    { const int rc_ = cached_occupancy(cache, p->device, k_inv_y_t<M, DER>, Y::THREADS, smem, &occ); if (rc_ != FSP_OK) return rc_; }
     long grid = (long)p->sm_count * occ;
     if (grid > ntiles) grid = ntiles;
     k_inv_y_t<M, DER><<<(unsigned)grid, Y::THREADS, smem, p->stream>>>(tm, B1, p->LTy, p->Wy, p->Nz, ntiles, kder);
@@ -512,12 +520,9 @@ int launch_inv_x_t_impl(fsp_plan* p, double* phi, double kder) {
     using X_ = TileXI<M>;
     const long plane = (long)p->Ny * p->Nz, ntiles = plane / X_::KC;
     const size_t smem = X_::smem_bytes();
-    static int occ = 0;
-    if (occ == 0) {
-        CU(cudaFuncSetAttribute(k_inv_x_t<M, DER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_inv_x_t<M, DER>, X_::THREADS, smem));
-        if (occ < 1) return FSP_ERR_CUDA;
-    }
+    static OccCache cache;   // per device: function attributes and occupancy belong to the device
+    int occ = 0;
+    { const int rc_ = cached_occupancy(cache, p->device, k_inv_x_t<M, DER>, X_::THREADS, smem, &occ); if (rc_ != FSP_OK) return rc_; }
     long grid = (long)p->sm_count * occ;
     if (grid > ntiles) grid = ntiles;
     k_inv_x_t<M, DER><<<(unsigned)grid, X_::THREADS, smem, p->stream>>>(p->tmB1x, p->B1, phi, p->LTx, p->Wx, plane, ntiles, kder);
@@ -823,6 +828,7 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
     cudaDeviceProp prop{};
     if (cudaGetDevice(&p->device) != cudaSuccess || cudaGetDeviceProperties(&prop, p->device) != cudaSuccess) rc = FSP_ERR_NO_DEVICE;
     if (rc == FSP_OK && prop.major != 10) rc = FSP_ERR_NO_DEVICE;  // the library holds sm_100a code only
+    if (rc == FSP_OK && (p->device < 0 || p->device >= kMaxDevices)) rc = FSP_ERR_NO_DEVICE;
     const size_t n1 = (size_t)(Nx + 1) * Ny * Nz, n2 = (size_t)(Nx + 1) * 2 * Ny * Nz;
     const size_t nt = (size_t)(Nx + 1) * (Ny + 1) * (Nz + 1);
     if (rc == FSP_OK && p->padded) rc = dev_alloc(&p->rho_pad, (size_t)Nx * Ny * Nz, &p->bytes);
@@ -907,6 +913,7 @@ int fsp_plan_set_spacing(fsp_plan* p, const double* h) {
 
 int fsp_precompute_green(fsp_plan* p) {
     if (!p) return FSP_ERR_INVALID_ARG;
+    DeviceGuard dev_guard(p->device);
     p->precomputed = false;
     int rc = precompute_impl(p);
     if (rc != FSP_OK) {
@@ -921,6 +928,7 @@ int fsp_precompute_green(fsp_plan* p) {
 int fsp_solve(fsp_plan* p, const double* rho_dev, double* phi_dev) {
     if (!p || !rho_dev || !phi_dev || rho_dev == phi_dev) return FSP_ERR_INVALID_ARG;
     if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
+    DeviceGuard dev_guard(p->device);
     double* phi_user = nullptr;
     if (p->padded) {   // embed, solve on the transform mesh, crop
         int rce = embed_rho(p, rho_dev);
@@ -975,6 +983,7 @@ int fsp_solve(fsp_plan* p, const double* rho_dev, double* phi_dev) {
 int fsp_solve_host(fsp_plan* p, const double* rho_host, double* phi_host) {
     if (!p || !rho_host || !phi_host) return FSP_ERR_INVALID_ARG;
     if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
+    DeviceGuard dev_guard(p->device);
     const size_t v = user_volume(p);
     if (!p->rho_stage) {
         int rc = dev_alloc(&p->rho_stage, v, &p->bytes);
@@ -990,29 +999,9 @@ int fsp_solve_host(fsp_plan* p, const double* rho_host, double* phi_host) {
     return FSP_OK;
 }
 
-int fsp_solve_host_batch(fsp_plan* p, int n, const double* const* rho_hosts, double* const* phi_hosts) {
-    if (!p || n < 0 || (n > 0 && (!rho_hosts || !phi_hosts))) return FSP_ERR_INVALID_ARG;
-    for (int i = 0; i < n; ++i)
-        if (!rho_hosts[i] || !phi_hosts[i]) return FSP_ERR_INVALID_ARG;
-    if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
-    if (n == 0) return FSP_OK;
-    const size_t v = user_volume(p);
+// the pipeline of fsp_solve_host_batch (the caller drains the three streams if this returns an error)
+static int batch_pipeline(fsp_plan* p, int n, const double* const* rho_hosts, double* const* phi_hosts, size_t v) {
     int rc;
-    if (!p->rho_stage) {
-        if ((rc = dev_alloc(&p->rho_stage, v, &p->bytes)) != FSP_OK) return rc;
-        if ((rc = dev_alloc(&p->phi_stage, v, &p->bytes)) != FSP_OK) return rc;
-    }
-    if (!p->rho_stage2) {
-        if ((rc = dev_alloc(&p->rho_stage2, v, &p->bytes)) != FSP_OK) return rc;
-        if ((rc = dev_alloc(&p->phi_stage2, v, &p->bytes)) != FSP_OK) return rc;
-        CU(cudaStreamCreateWithFlags(&p->s_h2d, cudaStreamNonBlocking));
-        CU(cudaStreamCreateWithFlags(&p->s_d2h, cudaStreamNonBlocking));
-        for (int i = 0; i < 2; ++i) {
-            CU(cudaEventCreateWithFlags(&p->ev_h2d[i], cudaEventDisableTiming));
-            CU(cudaEventCreateWithFlags(&p->ev_solve[i], cudaEventDisableTiming));
-            CU(cudaEventCreateWithFlags(&p->ev_d2h[i], cudaEventDisableTiming));
-        }
-    }
     double* rs[2] = {p->rho_stage, p->rho_stage2};
     double* ps[2] = {p->phi_stage, p->phi_stage2};
     // earlier work on the plan's stream may still use the staging buffers
@@ -1041,9 +1030,43 @@ int fsp_solve_host_batch(fsp_plan* p, int n, const double* const* rho_hosts, dou
     return FSP_OK;
 }
 
+int fsp_solve_host_batch(fsp_plan* p, int n, const double* const* rho_hosts, double* const* phi_hosts) {
+    if (!p || n < 0 || (n > 0 && (!rho_hosts || !phi_hosts))) return FSP_ERR_INVALID_ARG;
+    for (int i = 0; i < n; ++i)
+        if (!rho_hosts[i] || !phi_hosts[i]) return FSP_ERR_INVALID_ARG;
+    if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
+    if (n == 0) return FSP_OK;
+    DeviceGuard dev_guard(p->device);
+    const size_t v = user_volume(p);
+    int rc;
+    if (!p->rho_stage) {
+        if ((rc = dev_alloc(&p->rho_stage, v, &p->bytes)) != FSP_OK) return rc;
+        if ((rc = dev_alloc(&p->phi_stage, v, &p->bytes)) != FSP_OK) return rc;
+    }
+    if (!p->rho_stage2) {
+        if ((rc = dev_alloc(&p->rho_stage2, v, &p->bytes)) != FSP_OK) return rc;
+        if ((rc = dev_alloc(&p->phi_stage2, v, &p->bytes)) != FSP_OK) return rc;
+        CU(cudaStreamCreateWithFlags(&p->s_h2d, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithFlags(&p->s_d2h, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            CU(cudaEventCreateWithFlags(&p->ev_h2d[i], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&p->ev_solve[i], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&p->ev_d2h[i], cudaEventDisableTiming));
+        }
+    }
+    rc = batch_pipeline(p, n, rho_hosts, phi_hosts, v);
+    if (rc != FSP_OK) {
+        // copies to and from the caller's buffers may still be in flight: drain before handing them back
+        cudaStreamSynchronize(p->s_h2d); cudaStreamSynchronize(p->stream); cudaStreamSynchronize(p->s_d2h);
+        (void)cudaGetLastError();
+    }
+    return rc;
+}
+
 int fsp_solve_field(fsp_plan* p, const double* rho_dev, double* phi_dev, double* E_dev) {
     if (!p || !rho_dev || !E_dev || rho_dev == phi_dev || rho_dev == E_dev) return FSP_ERR_INVALID_ARG;
     if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
+    DeviceGuard dev_guard(p->device);
     const size_t n2 = (size_t)(p->Nx + 1) * 2 * p->Ny * p->Nz, V = user_volume(p);
     int rc;
     if (p->padded) {
@@ -1057,13 +1080,19 @@ int fsp_solve_field(fsp_plan* p, const double* rho_dev, double* phi_dev, double*
         return r != FSP_OK ? r : crop_out(p, dst);
     };
     if (!p->B3) {   // first field solve of this plan: the buffer that receives the derivative spectra
-        if ((rc = dev_alloc(&p->B3, n2, &p->bytes)) != FSP_OK) return rc;
+        double2* b3 = nullptr;
+        if ((rc = dev_alloc(&b3, n2, nullptr)) != FSP_OK) return rc;
         if (p->tile_y) {
             const cuuint64_t dims[4] = {(cuuint64_t)2 * p->Nz, 2, (cuuint64_t)p->Ny, (cuuint64_t)(p->Nx + 1)};
             const cuuint64_t strides[3] = {(cuuint64_t)p->Nz * 16, (cuuint64_t)2 * p->Nz * 16, (cuuint64_t)2 * p->Ny * p->Nz * 16};
             const cuuint32_t box[4] = {2 * (cuuint32_t)(p->Ny == 1024 ? 4 : kW), 1, (cuuint32_t)(p->Ny < 256 ? p->Ny : 256), 1};
-            if ((rc = make_tensor_map(&p->tmB3y, p->B3, 4, dims, strides, box)) != FSP_OK) return rc;
+            if ((rc = make_tensor_map(&p->tmB3y, b3, 4, dims, strides, box)) != FSP_OK) {
+                cudaFree(b3);   // B3 stays null: the next call starts over instead of reading through a bad map
+                return rc;
+            }
         }
+        p->B3 = b3;
+        p->bytes += n2 * sizeof(double2);
     }
     const int planes = p->Nx + 1;
     const double PI = 3.14159265358979323846;
@@ -1095,6 +1124,7 @@ int fsp_solve_field(fsp_plan* p, const double* rho_dev, double* phi_dev, double*
 int fsp_solve_field_host(fsp_plan* p, const double* rho_host, double* phi_host, double* E_host) {
     if (!p || !rho_host || !E_host) return FSP_ERR_INVALID_ARG;
     if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
+    DeviceGuard dev_guard(p->device);
     const size_t v = user_volume(p);
     int rc;
     if (!p->rho_stage) {
@@ -1119,6 +1149,7 @@ double fsp_model_bytes_per_field_solve(const fsp_plan* p, int with_phi) {
 
 int fsp_destroy(fsp_plan* p) {
     if (!p) return FSP_ERR_INVALID_ARG;
+    DeviceGuard dev_guard(p->device);
     cudaStreamSynchronize(p->stream);
     free_plan_memory(p);
     (void)cudaGetLastError();
@@ -1156,9 +1187,21 @@ int fsp_get_vg_factors(const fsp_plan* p, int* m_out) {
     return FSP_OK;
 }
 
+int fsp_vg_lattice_is_safe(const fsp_plan* p, int* safe_out) {
+    if (!p || !safe_out) return FSP_ERR_INVALID_ARG;
+    *safe_out = 1;
+    if (p->algorithm == FSP_HOCKNEY || p->algorithm == FSP_VICO_SAFE) return FSP_OK;
+    const double Ld[3] = {p->Nx * p->h[0], p->Ny * p->h[1], p->Nz * p->h[2]};
+    const double L = p->alpha * std::sqrt(Ld[0] * Ld[0] + Ld[1] * Ld[1] + Ld[2] * Ld[2]);
+    for (int d = 0; d < 3; ++d)
+        if (4.0 * Ld[d] < L + Ld[d]) *safe_out = 0;
+    return FSP_OK;
+}
+
 int fsp_get_green_table(const fsp_plan* p, double* T_host) {
     if (!p || !T_host) return FSP_ERR_INVALID_ARG;
     if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
+    DeviceGuard dev_guard(p->device);
     const size_t nt = (size_t)(p->Nx + 1) * (p->Ny + 1) * (p->Nz + 1);
     CU(cudaStreamSynchronize(p->stream));
     if (p->padded) {   // the caller's block (Ux+1)(Uy+1)(Uz+1) of the table of the transform mesh
@@ -1178,6 +1221,7 @@ int fsp_get_green_spectrum(const fsp_plan* p, double* Ghat_host) {
     if (!p || !Ghat_host) return FSP_ERR_INVALID_ARG;
     if (p->padded) return FSP_ERR_INVALID_ARG;   // the spectrum lives on the transform mesh, not the caller's
     if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
+    DeviceGuard dev_guard(p->device);
     const size_t nt = (size_t)(p->Nx + 1) * (p->Ny + 1) * (p->Nz + 1);
     CU(cudaStreamSynchronize(p->stream));
     CU(cudaMemcpy(Ghat_host, p->Goct, nt * sizeof(double), cudaMemcpyDeviceToHost));
@@ -1193,6 +1237,7 @@ int fsp_set_profiling(fsp_plan* p, int on) {
 
 int fsp_get_kernel_times(fsp_plan* p, float* ms, int* n_solves) {
     if (!p || !ms || !n_solves) return FSP_ERR_INVALID_ARG;
+    DeviceGuard dev_guard(p->device);
     for (int i = 0; i < FSP_NUM_SOLVE_KERNELS; ++i) ms[i] = 0.0f;
     const size_t n = p->events_used / 6;
     if (n > 0) CU(cudaEventSynchronize(p->events[p->events_used - 1]));

@@ -411,3 +411,40 @@ def test_repeated_solves_are_bitwise_identical_at_bench_sizes(N):
         E1 = E1.clone()
         _, E2 = p.solve_field(rho, want_phi=False)
         assert torch.equal(E1, E2)
+
+
+def test_vg_lattice_query_flags_elongated_boxes():
+    """PAPER.md:92-94 taken literally aliases when 4 L_d < L + L_d (R17): the library says so."""
+    with binding.Plan((16, 16, 16), (1 / 16,) * 3, binding.VICO_2) as p:
+        assert p.vg_lattice_is_safe()
+    for alg, safe in ((binding.VICO_2, False), (binding.VICO, False), (binding.VICO_SAFE, True), (binding.HOCKNEY, True)):
+        with binding.Plan((32, 32, 128), (1 / 32,) * 3, alg) as p:   # the 1 x 1 x 4 box of config 4
+            assert p.vg_lattice_is_safe() is safe
+    with binding.Plan((16, 16, 16), (1 / 16,) * 3, binding.VICO_2) as p:
+        with pytest.raises(binding.FspError):
+            binding.plan_set_param(p.handle, binding.PARAM_ALPHA, 1.0)   # PAPER.md:92: alpha > 1
+
+
+def test_plans_on_two_devices_from_one_process():
+    """Function attributes and occupancies are cached per device and every call runs on the plan's device whatever
+    device is current (include/fsp.h "Devices").  Needs two GPUs: skipped on the one-GPU boxes."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    w = W.random_density((256, 128, 256), seed=8)   # tile kernels on x and y, k_conv_z_f: all need the > 48 KB opt-in
+    ref = oracle.OraclePlan(w.N, w.h, oracle.HOCKNEY).precompute_green().solve(w.rho)
+    plans, outs = [], []
+    for dev in (0, 1):
+        torch.cuda.set_device(dev)
+        plans.append(binding.Plan(w.N, w.h, binding.HOCKNEY))
+    torch.cuda.set_device(0)   # both plans are now driven with device 0 current
+    for dev, p in enumerate(plans):
+        p.precompute_green()
+        rho = torch.from_numpy(w.rho).to(f"cuda:{dev}")
+        phi = torch.empty_like(rho)
+        p.solve(rho, phi)
+        outs.append(phi)
+    assert torch.cuda.current_device() == 0
+    for dev, (p, phi) in enumerate(zip(plans, outs)):
+        torch.cuda.synchronize(dev)
+        check(phi.cpu().numpy(), ref)
+        p.destroy()
