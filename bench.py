@@ -42,6 +42,7 @@ def parse_args():
     ap.add_argument("--alg", default="HE", choices=sorted(ALGS))
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-extras", action="store_true", help="skip the 256^3 / VG2 side measurements")
+    ap.add_argument("--print-kernels-sha", action="store_true", help="print the sha16 profiles/ncu_traffic.csv records")
     return ap.parse_args()
 
 
@@ -120,62 +121,158 @@ def _sample_workload(wname: str, edge: int):
     return W.config1(edge)
 
 
-def oracle_time_solves(wname: str, alg: str, steps: int, warmup: int, budget_s: float):
-    """Times the oracle's solve (PAPER.md:67-82 steps 1-5, un-pruned, radix-2 FFT) as it stands on the
-    host cores.  Returns (seconds per solve of the sample, sample workload, threads, description)."""
+def _full_edge(wname: str) -> int:
+    return {"512": 512, "256": 256, "beam": 512, "64": 64}[wname]
+
+
+def _free_host_bytes() -> int:
+    try:
+        for line in open("/proc/meminfo"):
+            if line.startswith("MemAvailable:"):
+                return int(line.split()[1]) * 1024
+    except OSError:
+        pass
+    return 0
+
+
+def _oracle_bytes(w) -> int:
+    """Host memory of one oracle solve: F{G2} and the padded density, both complex on the (2N)^3 grid."""
+    return 2 * 16 * 8 * w.N[0] * w.N[1] * w.N[2]
+
+
+def oracle_plan_for(w, alg: str):
+    """The oracle's spectrum for this mesh.  The solve (PAPER.md:67-82 steps 1-5) is the same code for every
+    algorithm once F{G2} exists, so VG spectra are built by the cheap VICO_2 route for timing purposes."""
     import oracle
-    oalg = {"HE": oracle.HOCKNEY, "VG": oracle.VICO, "VG2": oracle.VICO_2, "VGS": oracle.VICO_SAFE}[alg]
-    # calibrate on 32^3, then take the largest edge whose (steps+warmup) solves fit the budget
-    w = _sample_workload(wname, 32)
-    pl = oracle.OraclePlan(w.N, w.h, oracle.HOCKNEY).precompute_green()
-    pl.solve(w.rho)
-    t0 = time.perf_counter(); pl.solve(w.rho); t32 = time.perf_counter() - t0
-    edge = 32
-    for cand in (64, 128):
-        est = t32 * (cand / 32) ** 3 * 1.4 * (steps + warmup + 1)   # +1: spectrum build; 1.4: log factor, cache
-        if est <= budget_s:
-            edge = cand
-    w = _sample_workload(wname, edge)
-    # VICO's (4N)^3 table is not needed for timing the solve: the solve is identical for every
-    # algorithm given the spectrum; VG spectra are built with the cheap VICO_2 route.
-    pl = oracle.OraclePlan(w.N, w.h, oracle.VICO_2 if oalg != oracle.HOCKNEY else oalg).precompute_green()
+    oalg = oracle.HOCKNEY if alg == "HE" else oracle.VICO_2
+    return oracle.OraclePlan(w.N, w.h, oalg).precompute_green()
+
+
+def oracle_time_mesh(w, alg: str, steps: int, warmup: int):
+    """Seconds per oracle solve (un-pruned radix-2 FFT convolution, as it stands) of workload w on the host cores."""
+    pl = oracle_plan_for(w, alg)
     for _ in range(warmup):
         pl.solve(w.rho)
     t0 = time.perf_counter()
     for _ in range(steps):
         pl.solve(w.rho)
-    dt = (time.perf_counter() - t0) / max(steps, 1)
-    desc = (f"oracle O2 (oracle/fsp_oracle.c, un-pruned radix-2 FFT convolution) full solve of the same "
-            f"density on a {w.N[0]}x{w.N[1]}x{w.N[2]} mesh, {steps} solve(s); grid-points/s scaled to the "
-            f"workload's V (FFT log factor ignored: flatters the CPU by <= 25%)")
-    return dt, w, oracle.num_threads(), desc
+    return (time.perf_counter() - t0) / max(steps, 1)
+
+
+def pick_sample_edge(wname: str, alg: str, nsolves: int, budget_s: float) -> int:
+    """Largest mesh edge (a power of two up to the workload's own) whose nsolves oracle solves (+ one spectrum build)
+    fit budget_s and host memory; calibrated on a 64^3 solve with the n log n factor and a margin."""
+    import math
+    w = _sample_workload(wname, 64)
+    pl = oracle_plan_for(w, alg)
+    pl.solve(w.rho)
+    t0 = time.perf_counter(); pl.solve(w.rho); t64 = time.perf_counter() - t0
+    V64 = w.N[0] * w.N[1] * w.N[2]
+    edge = 64
+    for cand in (128, 256, 512):
+        if cand > _full_edge(wname):
+            break
+        wc_pts = (cand ** 3) if wname != "beam" else (cand ** 3) // 16
+        est = t64 * (wc_pts / V64) * (math.log2(2 * cand) / 7.0) * 1.3 * (nsolves + 1.5)
+        mem = 2 * 16 * 8 * wc_pts
+        if est <= budget_s and mem <= 0.5 * max(_free_host_bytes(), 8 << 30):
+            edge = cand
+    return edge
 
 
 def run_reference(args):
-    """--impl reference: the oracle is the reference arm for this tier (no reference code exists)."""
+    """--impl reference: the oracle is the reference arm for this tier (no reference code exists).  Each step is one
+    oracle solve of the SAME analytic density on the largest mesh whose K + W solves end within a few minutes on this
+    box's host cores; ms_per_step is the time measured for that mesh, which config.workload names; the figure scaled
+    to the GPU arm's mesh sits in its own key."""
+    import math
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    from paper_2405_02603_b200 import workloads as W  # noqa: F401  (input generators only)
+    import oracle
     cfg_idx, _, _, wdesc = WORKLOADS[args.workload]
-    dt, w, threads, desc = oracle_time_solves(args.workload, args.alg, args.steps, args.warmup, budget_s=150.0)
+    edge = pick_sample_edge(args.workload, args.alg, args.steps + args.warmup, budget_s=150.0)
+    w = _sample_workload(args.workload, edge)
+    dt = oracle_time_mesh(w, args.alg, args.steps, args.warmup)
+    threads = oracle.num_threads()
     Vs = w.N[0] * w.N[1] * w.N[2]
     V = workload_points(args.workload)
-    pts_per_s = Vs / dt
-    value = pts_per_s / V
+    full = Vs == V
+    mesh = f"{w.N[0]}x{w.N[1]}x{w.N[2]}"
+    # n log n rule of BASELINE.md section 3: time ~ V log2(2 N_max)
+    rule = (V / Vs) * (math.log2(2 * _full_edge(args.workload)) / math.log2(2 * max(w.N)))
+    desc = (f"oracle O2 (oracle/fsp_oracle.c: PAPER.md:67-82 steps 1-5, un-pruned, textbook radix-2 FFT, OpenMP over "
+            f"pencils), one full solve of the workload's analytic density on a {mesh} mesh per step, {threads} threads")
     line = {
-        "impl": "reference", "metric": "solves/s", "value": value, "unit": "solves/s",
-        "grid_points_per_s": pts_per_s, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": dt * 1e3 * (V / Vs), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "impl": "reference", "metric": "solves/s", "value": 1.0 / dt, "unit": "solves/s",
+        "grid_points_per_s": Vs / dt, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": wdesc, "baseline_config_index": cfg_idx, "algorithm": args.alg,
-                   "note": "ms_per_step is the sample's time scaled by V_workload/V_sample"},
-        "cpu_baseline": {"value": value, "unit": "solves/s", "cores": threads, "kind": "oracle", "sample": desc},
-        "e2e": {"value": value, "unit": "solves/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "config": {"workload": (wdesc if full else f"{mesh} sample of " + wdesc), "mesh": list(w.N),
+                   "baseline_config_index": cfg_idx, "algorithm": args.alg, "is_full_workload": full,
+                   "note": "value and ms_per_step are MEASURED on the mesh named here; see scaled_to_workload"},
+        "scaled_to_workload": {"value": 1.0 / (dt * rule), "unit": "solves/s", "ms_per_step": dt * 1e3 * rule,
+                               "extrapolated": not full, "rule": "time x (V / V_sample) x log2(2N) / log2(2N_sample)"},
+        "cpu_baseline": {"value": 1.0 / dt, "unit": "solves/s", "cores": threads, "kind": "oracle", "sample": desc},
+        "e2e": {"value": 1.0 / dt, "unit": "solves/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line))
     return 0
+
+
+def cpu_baseline_leg(wname: str, alg: str, V: int):
+    """The oracle, as it stands, on this box's host cores, beside the GPU figure (a reported baseline, not the target,
+    and a deliberately plain program: no speed-up is formed from it).  SURVEY 8(d) / BASELINE.md section 3: a full
+    oracle solve of the 256^3 density (all cores, and one thread at 128^3), and of the workload's own mesh when host
+    memory and about half a minute allow; otherwise the 256^3 time scaled by V log(2N) and labelled extrapolated."""
+    import math
+    import oracle
+    threads = oracle.num_threads()
+    out = {"unit": "solves/s", "cores": threads, "kind": "oracle", "nproc": os.cpu_count(),
+           "what": "oracle/fsp_oracle.c: PAPER.md:67-82 steps 1-5 un-pruned, textbook radix-2 FFT, OpenMP over pencils "
+                   "(plain by design; a tuned CPU FFT would be several times faster)"}
+    full_edge = _full_edge(wname)
+    e1 = min(256, full_edge)
+    w1 = _sample_workload(wname, e1)
+    t1 = oracle_time_mesh(w1, alg, steps=2, warmup=1)
+    V1 = w1.N[0] * w1.N[1] * w1.N[2]
+    out["mesh_256"] = {"mesh": list(w1.N), "s_per_solve": t1, "solves_per_s": 1.0 / t1, "grid_points_per_s": V1 / t1, "steps": 2}
+    rule = (V / V1) * (math.log2(2 * full_edge) / math.log2(2 * max(w1.N)))
+    value, sample, extrapolated = 1.0 / (t1 * rule), None, V1 != V
+    if V1 == V:
+        sample = f"2 full oracle solves of the workload itself ({w1.N[0]}x{w1.N[1]}x{w1.N[2]})"
+    else:
+        wf = None
+        need = 2 * 16 * 8 * V
+        if need <= 0.6 * _free_host_bytes() and t1 * rule <= 60.0:
+            try:
+                wf = _sample_workload(wname, full_edge)
+                tf = oracle_time_mesh(wf, alg, steps=1, warmup=0)
+                value, extrapolated = 1.0 / tf, False
+                sample = (f"one full oracle solve of the workload itself ({wf.N[0]}x{wf.N[1]}x{wf.N[2]}, "
+                          f"{need / 2 ** 30:.0f} GiB of host arrays), no warm-up")
+                out["mesh_full"] = {"mesh": list(wf.N), "s_per_solve": tf, "solves_per_s": 1.0 / tf, "steps": 1}
+            except MemoryError:
+                wf = None
+        if wf is None:
+            sample = (f"2 full oracle solves of the same density on {w1.N[0]}x{w1.N[1]}x{w1.N[2]}, scaled to the workload "
+                      f"by V log2(2N) (x {rule:.2f}): EXTRAPOLATED")
+    out.update({"value": value, "sample": sample, "extrapolated": extrapolated, "grid_points_per_s": value * V})
+    try:   # one thread, 128^3 (SURVEY 8(d): single-thread time beside the all-cores one)
+        ws = _sample_workload(wname, min(128, full_edge))
+        pl = oracle_plan_for(ws, alg)
+        oracle.set_num_threads(1)
+        t0 = time.perf_counter(); pl.solve(ws.rho); ts = time.perf_counter() - t0
+        oracle.set_num_threads(threads)
+        Vs = ws.N[0] * ws.N[1] * ws.N[2]
+        rs = (V / Vs) * (math.log2(2 * full_edge) / math.log2(2 * max(ws.N)))
+        out["single_thread"] = {"mesh": list(ws.N), "s_per_solve": ts, "cores": 1,
+                                "scaled_to_workload_solves_per_s": 1.0 / (ts * rs), "extrapolated": True}
+    except Exception as ex:
+        oracle.set_num_threads(threads)
+        out["single_thread"] = {"error": repr(ex)[:120]}
+    return out
 
 
 # ------------------------------------------------------------------------------------------------
@@ -311,9 +408,11 @@ def run_b200(args):
     kernels = [{"name": names[i], "ms": kms[i], "model_bytes": model_k[i],
                 "achieved_gbs": model_k[i] / (kms[i] * 1e-3) / 1e9 if kms[i] > 0 else None,
                 "share": kms[i] / sum(kms)} for i in range(len(kms))]
+    traffic, traffic_stale = _ncu_traffic(names[dom], args.workload)
     roofline = {"bound": "hbm", "kernel": names[dom], "achieved": kernels[dom]["achieved_gbs"], "peak": peak,
-                "unit": "GB/s", "frac": kernels[dom]["achieved_gbs"] / peak, "traffic": _ncu_traffic(names[dom], args.workload),
-                "peak_source": peak_src,
+                "unit": "GB/s", "frac": kernels[dom]["achieved_gbs"] / peak, "traffic": traffic,
+                "traffic_source": "profiles/ncu_traffic.csv (ncu --set full capture, not this run)",
+                "traffic_source_stale": traffic_stale, "peak_source": peak_src,
                 "whole_solve": {"model_bytes": model_total, "achieved": model_total / (ms * 1e-3) / 1e9,
                                 "frac": model_total / (ms * 1e-3) / 1e9 / peak,
                                 "frac_of_nominal_8TBs": model_total / (ms * 1e-3) / 1e9 / 8000.0},
@@ -390,22 +489,7 @@ def run_b200(args):
     if world == 1 and not args.no_extras:
         line["also"] = extras(args, peak)
     if world == 1 and rank == 0 and not args.no_cpu_baseline:
-        dt, ws, threads, desc = oracle_time_solves(args.workload, args.alg, steps=2, warmup=1, budget_s=25.0)
-        pts = ws.N[0] * ws.N[1] * ws.N[2] / dt
-        line["cpu_baseline"] = {"value": pts / V, "unit": "solves/s", "cores": threads, "kind": "oracle",
-                                "sample": desc, "grid_points_per_s": pts}
-        try:   # single-thread time beside the all-cores one (one 64^3 solve, same code)
-            import oracle
-            w1 = _sample_workload(args.workload, 64)
-            p1 = oracle.OraclePlan(w1.N, w1.h, oracle.HOCKNEY).precompute_green()
-            oracle.set_num_threads(1)
-            p1.solve(w1.rho)
-            t0 = time.perf_counter(); p1.solve(w1.rho); t1 = time.perf_counter() - t0
-            oracle.set_num_threads(threads)
-            line["cpu_baseline"]["single_thread"] = {"value": (64 ** 3 / t1) / V, "unit": "solves/s", "cores": 1,
-                                                     "sample": "one 64^3 solve, grid-points/s scaled to the workload's V"}
-        except Exception as ex:
-            line["cpu_baseline"]["single_thread"] = {"error": repr(ex)[:120]}
+        line["cpu_baseline"] = cpu_baseline_leg(args.workload, args.alg, V)
     if rank == 0:
         print(json.dumps(line))
     if dist:
@@ -413,20 +497,36 @@ def run_b200(args):
     return 0
 
 
+KERNEL_SOURCES = ("solve_kernels.cuh", "fft_warp.cuh", "fft_engine.cuh", "tma.cuh")
+
+
+def kernel_sources_sha16() -> str:
+    """sha256 (first 16 hex digits) of the solve kernels' sources: profiles/ncu_traffic.csv records the value its
+    capture was made with, so that a traffic figure measured on other kernels is flagged instead of silently reused."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in KERNEL_SOURCES:
+        h.update(open(os.path.join(ROOT, "paper_2405_02603_b200", "csrc", f), "rb").read())
+    return h.hexdigest()[:16]
+
+
 def _ncu_traffic(kernel: str, wname: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
-    committed `ncu --set full` summary under profiles/ (null until one exists for this workload)."""
+    """(dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, stale?) from the committed
+    `ncu --set full` summary under profiles/ (null until one exists for this workload).  The figure is NOT measured
+    by this run (a bench number is never taken under a profiler): it is stale when the kernel sources have changed
+    since the capture."""
     path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
     if not os.path.exists(path):
-        return None
+        return None, None
     try:
         for line in open(path):
             f = line.strip().split(",")
             if len(f) >= 3 and f[0] == wname and f[1] == kernel:
-                return float(f[2])
+                stale = not (len(f) >= 5 and f[4] == kernel_sources_sha16())
+                return float(f[2]), stale
     except Exception:
-        return None
-    return None
+        return None, None
+    return None, None
 
 
 def extras(args, peak):
@@ -545,4 +645,7 @@ def cufft_comparison(wname, steps):
 
 if __name__ == "__main__":
     a = parse_args()
+    if a.print_kernels_sha:
+        print(kernel_sources_sha16())
+        sys.exit(0)
     sys.exit(run_reference(a) if a.impl == "reference" else run_b200(a))
