@@ -536,7 +536,9 @@ def extras(args, peak):
     import torch
     from paper_2405_02603_b200 import binding, workloads as W
     out = {}
-    todo = [("256", "HE"), ("beam", "HE"), ("beam", "VGS"), (args.workload, "VG2" if args.alg == "HE" else "HE")]
+    # ("256", "VG"): BASELINE config 3 names the plain Vico-Greengard precompute (1024^3 lattice)
+    todo = [("256", "HE"), ("256", "VG"), ("256", "VG2"), ("beam", "HE"), ("beam", "VGS"),
+            (args.workload, "VG2" if args.alg == "HE" else "HE")]
     for wname, alg in todo:
         if (wname, alg) == (args.workload, args.alg):
             continue
@@ -557,7 +559,8 @@ def extras(args, peak):
                                      "grid_points_per_s": V * 1e3 / ms, "steps": steps,
                                      "model_gbs": model_total / (ms * 1e-3) / 1e9,
                                      "frac_of_measured_peak": model_total / (ms * 1e-3) / 1e9 / peak,
-                                     "precompute_green_s": t_pre, "rel_l2_vs_closed_form": _analytic_error(w, phi)}
+                                     "precompute_green_s": t_pre, "precompute_peak_bytes": plan.precompute_peak_bytes,
+                                     "rel_l2_vs_closed_form": _analytic_error(w, phi)}
         del rho, phi
     # field output: phi and E = -grad phi in one call, against 4 separate solves' worth of work
     for wname in ("256", args.workload):

@@ -242,6 +242,17 @@ int cached_occupancy(OccCache& c, int dev, Kern kern, int threads, size_t smem, 
     *occ_out = o;
     return FSP_OK;
 }
+// shared-memory opt-in of a precompute kernel whose request varies with the transform length: raised only when a launch
+// needs more than any earlier one on this device (setting the attribute before every launch costs milliseconds)
+template <class Kern>
+int cached_smem_optin(OccCache& c, int dev, Kern kern, size_t smem) {
+    if (c.v[dev].load(std::memory_order_acquire) < (int)smem) {
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        c.v[dev].store((int)smem, std::memory_order_release);
+    }
+    return FSP_OK;
+}
+
 // Every entry point runs on the plan's device and restores the caller's current device on return.
 struct DeviceGuard {
     int prev = -1;
@@ -577,9 +588,25 @@ int crop_out(fsp_plan* p, double* dst_user) {          // dst <- phi_pad restric
 }
 int next_pow2_min8(int n) { int q = 8; while (q < n) q *= 2; return q; }
 
-// batched DCT-I along one axis of a real 3-D array (C order), output pruned to nout along that axis
+// batched DCT-I along one axis of a real 3-D array (C order), output pruned to nout along that axis.
+// fill != nullptr (axis 2 only): the input array does not exist, its values are G_L evaluated inside the kernel.
+template <int C>
+int launch_dct1_tile(fsp_plan* p, const double* in, double* out, int n, int nout, long nA, long nB, const long* ai,
+                     const long* ao, double scale, size_t smem, int threads, const GLFill* fill) {
+    if (fill) {
+        { static OccCache optin; const int rc_ = cached_smem_optin(optin, p->device, k_dct1_tile<C, true>, smem); if (rc_ != FSP_OK) return rc_; }
+        k_dct1_tile<C, true><<<(unsigned)(nA * ((nB + C - 1) / C)), threads, smem, p->stream>>>(
+            in, out, n, nout, nB, ai[0], ai[1], ai[2], ao[0], ao[1], ao[2], scale, *fill);
+    } else {
+        { static OccCache optin; const int rc_ = cached_smem_optin(optin, p->device, k_dct1_tile<C, false>, smem); if (rc_ != FSP_OK) return rc_; }
+        k_dct1_tile<C, false><<<(unsigned)(nA * ((nB + C - 1) / C)), threads, smem, p->stream>>>(
+            in, out, n, nout, nB, ai[0], ai[1], ai[2], ao[0], ao[1], ao[2], scale, GLFill{0.0, 0.0, 0.0, 0.0, 0});
+    }
+    CU(cudaGetLastError());
+    return FSP_OK;
+}
 int dct1_axis(fsp_plan* p, const double* in, double* out, const long in_dims[3], const long out_dims[3],
-              int axis, int n, int nout, double scale) {
+              int axis, int n, int nout, double scale, const GLFill* fill = nullptr) {
     const long is[3] = {in_dims[1] * in_dims[2], in_dims[2], 1};
     const long os[3] = {out_dims[1] * out_dims[2], out_dims[2], 1};
     const int o1 = (axis + 1) % 3, o2 = (axis + 2) % 3;
@@ -590,23 +617,16 @@ int dct1_axis(fsp_plan* p, const double* in, double* out, const long in_dims[3],
         const long nA = in_dims[adim], nB = in_dims[bdim];
         auto tile_smem = [&](int C) { return sizeof(double2) * ((size_t)n + (size_t)C * Lf); };
         const long args_in[3] = {is[adim], is[bdim], is[axis]}, args_out[3] = {os[adim], os[bdim], os[axis]};
-        if (tile_smem(8) <= 72 * 1024) {   // at least 3 CTAs per SM: the stages are latency-bound
-            CU(cudaFuncSetAttribute(k_dct1_tile<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_smem(8)));
-            k_dct1_tile<8><<<(unsigned)(nA * ((nB + 7) / 8)), 512, tile_smem(8), p->stream>>>(
-                in, out, n, nout, nB, args_in[0], args_in[1], args_in[2], args_out[0], args_out[1], args_out[2], scale);
-            CU(cudaGetLastError());
-            return FSP_OK;
-        }
-        if (tile_smem(4) <= 200 * 1024) {
-            CU(cudaFuncSetAttribute(k_dct1_tile<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_smem(4)));
-            k_dct1_tile<4><<<(unsigned)(nA * ((nB + 3) / 4)), tile_smem(4) <= 76 * 1024 ? 256 : 1024, tile_smem(4), p->stream>>>(
-                in, out, n, nout, nB, args_in[0], args_in[1], args_in[2], args_out[0], args_out[1], args_out[2], scale);
-            CU(cudaGetLastError());
-            return FSP_OK;
-        }
+        // several CTAs per SM: the Stockham stages are latency-bound (one butterfly per thread between two barriers)
+        if (tile_smem(8) <= 72 * 1024) return launch_dct1_tile<8>(p, in, out, n, nout, nA, nB, args_in, args_out, scale, tile_smem(8), 512, fill);
+        if (tile_smem(4) <= 76 * 1024) return launch_dct1_tile<4>(p, in, out, n, nout, nA, nB, args_in, args_out, scale, tile_smem(4), 256, fill);
+        if (tile_smem(2) <= 100 * 1024) return launch_dct1_tile<2>(p, in, out, n, nout, nA, nB, args_in, args_out, scale, tile_smem(2), 512, fill);
+        if (tile_smem(4) <= 200 * 1024) return launch_dct1_tile<4>(p, in, out, n, nout, nA, nB, args_in, args_out, scale, tile_smem(4), 1024, fill);
+        if (tile_smem(2) <= 200 * 1024) return launch_dct1_tile<2>(p, in, out, n, nout, nA, nB, args_in, args_out, scale, tile_smem(2), 512, fill);
     }
+    if (fill) return FSP_ERR_INVALID_ARG;   // (lengths beyond the tile kernels: m_d N_d > 7264 is rejected before)
     const size_t smem = sizeof(double2) * 2 * (size_t)Lf;
-    CU(cudaFuncSetAttribute(k_dct1_pencils, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    { static OccCache optin; const int rc_ = cached_smem_optin(optin, p->device, k_dct1_pencils, smem); if (rc_ != FSP_OK) return rc_; }
     int threads = Lf / 2 < 256 ? (Lf / 2 < 32 ? 32 : Lf / 2) : 256;
     k_dct1_pencils<<<(unsigned)(n1 * n2), threads, smem, p->stream>>>(in, out, n, nout, is[axis], os[axis], n2,
                                                                       is[o1], is[o2], os[o1], os[o2], scale);
@@ -625,7 +645,7 @@ AxisTiling axis_tiling(const long dims[3], int axis) {
 
 template <int C>
 int launch_ifft_tile(fsp_plan* p, double2* data, int Lf, long nA, long nB, long sA, long sB, long sK, size_t smem) {
-    CU(cudaFuncSetAttribute(k_ifft_tile<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    { static OccCache optin; const int rc_ = cached_smem_optin(optin, p->device, k_ifft_tile<C>, smem); if (rc_ != FSP_OK) return rc_; }
     k_ifft_tile<C><<<(unsigned)(nA * ((nB + C - 1) / C)), smem <= 72 * 1024 ? 512 : 1024, smem, p->stream>>>(data, Lf, nB, sA, sB, sK);
     CU(cudaGetLastError());
     return FSP_OK;
@@ -646,7 +666,7 @@ int ifft_axis(fsp_plan* p, double2* data, const long dims[3], int axis, long nA_
 template <int C>
 int launch_c2r_tile(fsp_plan* p, const double2* in, double* out, int Lf, int nout, long nA, long nB, const AxisTiling& ti,
                     const AxisTiling& to, double scale, size_t smem) {
-    CU(cudaFuncSetAttribute(k_c2r_tile<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    { static OccCache optin; const int rc_ = cached_smem_optin(optin, p->device, k_c2r_tile<C>, smem); if (rc_ != FSP_OK) return rc_; }
     k_c2r_tile<C><<<(unsigned)(nA * ((nB + C - 1) / C)), smem <= 72 * 1024 ? 512 : 1024, smem, p->stream>>>(
         in, out, Lf, nout, nB, ti.sA, ti.sB, ti.sK, to.sA, to.sB, to.sK, scale);
     CU(cudaGetLastError());
@@ -718,32 +738,68 @@ int precompute_impl(fsp_plan* p) {
             if (sizeof(double2) * 4 * (size_t)(nx > ny ? (nx > nz ? nx : nz) : (ny > nz ? ny : nz)) > 227 * 1024)
                 return FSP_ERR_INVALID_ARG;
             const double vscale = 1.0 / (((double)m[0] * Nx * hx) * ((double)m[1] * Ny * hy) * ((double)m[2] * Nz * hz));
-            const long fd[3] = {nx + 1L, ny + 1L, nz + 1L};
-            const long ad[3] = {fd[0], fd[1], Nz + 1};
-            const long bd[3] = {fd[0], Ny + 1, Nz + 1};
-            double *f = nullptr, *a = nullptr, *b = nullptr;
-            int rc = dev_alloc(&f, (size_t)fd[0] * fd[1] * fd[2], &peak);
-            if (rc != FSP_OK) return rc;
-            tmp.ptrs.push_back(f);
-            rc = dev_alloc(&a, (size_t)ad[0] * ad[1] * ad[2], &peak);
-            if (rc != FSP_OK) return rc;
-            tmp.ptrs.push_back(a);
-            rc = dev_alloc(&b, (size_t)bd[0] * bd[1] * bd[2], &peak);
-            if (rc != FSP_OK) return rc;
-            tmp.ptrs.push_back(b);
-            k_fill_gl_vg2<<<grid_for(fd[0] * fd[1] * fd[2], blk), blk, 0, p->stream>>>(f, Nx, Ny, Nz, hx, hy, hz, L, m[0], m[1], m[2]);
-            CU(cudaGetLastError());
-            if ((rc = dct1_axis(p, f, a, fd, ad, 2, nz, Nz + 1, 1.0)) != FSP_OK) return rc;
-            if ((rc = dct1_axis(p, a, b, ad, bd, 1, ny, Ny + 1, 1.0)) != FSP_OK) return rc;
+            // The lattice f[kx][ky][kz] is never stored: the z pass evaluates G_L itself (k_dct1_tile<., FILL>).  It runs
+            // a chunk of kx planes at a time through a[kx][ky][dz] (in the plan's workspace B1), the y pass takes the
+            // chunk to b[kx][dy][dz] (workspace B2), the x pass b -> T.  No transient memory when the workspace holds
+            // a plane of a and the whole of b (always for the paper's m = 4), else it is allocated.
+            const long Kx = nx + 1L, Ky = ny + 1L;
+            if (sizeof(double2) * 5 * (size_t)nz > 200 * 1024) {
+                // the z transform is too long for the tile kernels (m_z N_z > 5120): the unfused route, lattice in memory
+                const long fd[3] = {nx + 1L, ny + 1L, nz + 1L};
+                const long ad[3] = {fd[0], fd[1], Nz + 1};
+                const long bd[3] = {fd[0], Ny + 1, Nz + 1};
+                double *f = nullptr, *a = nullptr, *b = nullptr;
+                int rc = dev_alloc(&f, (size_t)fd[0] * fd[1] * fd[2], &peak);
+                if (rc != FSP_OK) return rc;
+                tmp.ptrs.push_back(f);
+                if ((rc = dev_alloc(&a, (size_t)ad[0] * ad[1] * ad[2], &peak)) != FSP_OK) return rc;
+                tmp.ptrs.push_back(a);
+                if ((rc = dev_alloc(&b, (size_t)bd[0] * bd[1] * bd[2], &peak)) != FSP_OK) return rc;
+                tmp.ptrs.push_back(b);
+                k_fill_gl_vg2<<<grid_for(fd[0] * fd[1] * fd[2], blk), blk, 0, p->stream>>>(f, Nx, Ny, Nz, hx, hy, hz, L, m[0], m[1], m[2]);
+                CU(cudaGetLastError());
+                if ((rc = dct1_axis(p, f, a, fd, ad, 2, nz, Nz + 1, 1.0)) != FSP_OK) return rc;
+                if ((rc = dct1_axis(p, a, b, ad, bd, 1, ny, Ny + 1, 1.0)) != FSP_OK) return rc;
+                if ((rc = dct1_axis(p, b, p->T, bd, tdims, 0, nx, Nx + 1, vscale)) != FSP_OK) return rc;
+            } else {
+            const size_t plane_a = (size_t)Ky * (Nz + 1), count_b = (size_t)Kx * (Ny + 1) * (Nz + 1);
+            const size_t cap1 = (size_t)(Nx + 1) * Ny * Nz * 2, cap2 = 2 * cap1;   // doubles in B1, B2
+            double *a = reinterpret_cast<double*>(p->B1), *b = reinterpret_cast<double*>(p->B2);
+            long chunk = (long)(cap1 / plane_a);
+            int rc;
+            if (chunk < 1) {
+                chunk = Kx < 64 ? Kx : 64;
+                if ((rc = dev_alloc(&a, (size_t)chunk * plane_a, &peak)) != FSP_OK) return rc;
+                tmp.ptrs.push_back(a);
+            }
+            if (chunk > Kx) chunk = Kx;
+            if (count_b > cap2) {
+                if ((rc = dev_alloc(&b, count_b, &peak)) != FSP_OK) return rc;
+                tmp.ptrs.push_back(b);
+            }
+            const double PI2 = 6.28318530717958647692;
+            for (long a0 = 0; a0 < Kx; a0 += chunk) {
+                const long nc = Kx - a0 < chunk ? Kx - a0 : chunk;
+                const long fd[3] = {nc, Ky, nz + 1L};
+                const long ad[3] = {nc, Ky, Nz + 1};
+                const long bd[3] = {nc, Ny + 1, Nz + 1};
+                const GLFill gl{PI2 / ((double)m[0] * Nx * hx), PI2 / ((double)m[1] * Ny * hy), PI2 / ((double)m[2] * Nz * hz), L, a0};
+                if ((rc = dct1_axis(p, nullptr, a, fd, ad, 2, nz, Nz + 1, 1.0, &gl)) != FSP_OK) return rc;
+                if ((rc = dct1_axis(p, a, b + (size_t)a0 * (Ny + 1) * (Nz + 1), ad, bd, 1, ny, Ny + 1, 1.0)) != FSP_OK) return rc;
+            }
+            const long bd[3] = {Kx, Ny + 1, Nz + 1};
             if ((rc = dct1_axis(p, b, p->T, bd, tdims, 0, nx, Nx + 1, vscale)) != FSP_OK) return rc;
+            }
         }
     }
     // Ghat octant = 3-D DCT-I of T (size N_d + 1 per axis)
     {
-        double* u = nullptr;
-        int rc = dev_alloc(&u, (size_t)tcount, &peak);
-        if (rc != FSP_OK) return rc;
-        tmp.ptrs.push_back(u);
+        double* u = reinterpret_cast<double*>(p->B1);   // the solve's workspace serves as scratch when it is big enough
+        int rc = FSP_OK;
+        if ((size_t)tcount > (size_t)(Nx + 1) * Ny * Nz * 2) {
+            if ((rc = dev_alloc(&u, (size_t)tcount, &peak)) != FSP_OK) return rc;
+            tmp.ptrs.push_back(u);
+        }
         if ((rc = dct1_axis(p, p->T, p->Goct, tdims, tdims, 2, Nz, Nz + 1, 1.0)) != FSP_OK) return rc;
         if ((rc = dct1_axis(p, p->Goct, u, tdims, tdims, 1, Ny, Ny + 1, 1.0)) != FSP_OK) return rc;
         if ((rc = dct1_axis(p, u, p->Goct, tdims, tdims, 0, Nx, Nx + 1, 1.0)) != FSP_OK) return rc;

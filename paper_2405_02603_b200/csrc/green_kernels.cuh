@@ -167,10 +167,14 @@ __device__ __forceinline__ double2* smem_stockham(double2* a, double2* b, const 
 // ONE complex sequence -- both transforms are real, so they come out as Re and Im of the result; (2) the
 // tile is chosen along the contiguous dimension, so that global accesses are full sectors; the twiddles
 // come from a shared-memory table filled once per CTA.  Shared memory: [tw: Lf/2][a: C/2*Lf][b: C/2*Lf].
-template <int C>
+// FILL: the input is not read but evaluated in place, element k of pencil (a, b) = G_L(gl.sa (gl.a0 + a), gl.sb b,
+// gl.sk k) (first pass of the modified Vico-Greengard precompute: the (2N+1)^3 lattice of PAPER.md:100-102 is never
+// written to memory).
+struct GLFill { double sa, sb, sk, L; long a0; };
+template <int C, bool FILL = false>
 __global__ void k_dct1_tile(const double* __restrict__ in, double* __restrict__ out, int n, int nout,
                             long nB, long sA_in, long sB_in, long sK_in, long sA_out, long sB_out,
-                            long sK_out, double scale) {
+                            long sK_out, double scale, const GLFill gl) {
     extern __shared__ double2 sm[];
     const int Lf = 2 * n, half = n, S = C / 2;
     double2* tw = sm;
@@ -193,7 +197,11 @@ __global__ void k_dct1_tile(const double* __restrict__ in, double* __restrict__ 
         int k, c;
         if (sK_in == 1) { k = e % (n + 1); c = e / (n + 1); }   // contiguous transform axis: k fastest
         else { c = e % C; k = e / C; }                          // strided axis: pencils fastest
-        const double v = c < nc ? src[(long)c * sB_in + (long)k * sK_in] : 0.0;
+        double v = 0.0;
+        if (c < nc) {
+            if constexpr (FILL) v = vg_GL(gl.sa * (double)(gl.a0 + ia), gl.sb * (double)(b0 + c), gl.sk * (double)k, gl.L);
+            else v = src[(long)c * sB_in + (long)k * sK_in];
+        }
         const long sq = (long)(c >> 1) * Lf;
         af[2 * (sq + k) + (c & 1)] = v;
         if (k > 0 && k < n) af[2 * (sq + Lf - k) + (c & 1)] = v;
