@@ -42,6 +42,9 @@ def parse_args():
     ap.add_argument("--alg", default="HE", choices=sorted(ALGS))
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-extras", action="store_true", help="skip the 256^3 / VG2 side measurements")
+    ap.add_argument("--sharded", action="store_true",
+                    help="ONE solve split over the ranks (slab decomposition, SURVEY 8(f) N5) instead of N replicas; "
+                         "a side mode with its own JSON line, launched under torchrun like --gpus N")
     ap.add_argument("--print-kernels-sha", action="store_true", help="print the sha16 profiles/ncu_traffic.csv records")
     return ap.parse_args()
 
@@ -510,6 +513,98 @@ def kernel_sources_sha16() -> str:
     return h.hexdigest()[:16]
 
 
+def run_sharded(args):
+    """One solve of the workload split into y-slabs over WORLD_SIZE ranks (include/fsp.h "slab decomposition").  Each
+    rank: K1 on its slab, P2P transpose, K2-K4 on its kx planes, transpose back, K5; a stream synchronisation and a
+    barrier between the three phases.  Workspace addresses travel between the processes as CUDA IPC handles.  When
+    there are fewer devices than ranks (the one-GPU boxes) the ranks share devices and the barriers go over gloo: no
+    kernel ever waits on another rank's kernel, so this is safe; the number then says nothing about scaling.
+    Strong scaling: the mesh is fixed, value = solves/s of the whole job.  Rank 0 checks the result against fsp_solve."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2405_02603_b200 import binding, workloads as W
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    ndev = torch.cuda.device_count()
+    if ndev == 0:
+        raise SystemExit("bench.py --sharded: no CUDA device")
+    dev = local % ndev
+    torch.cuda.set_device(dev)
+    shared_devices = world > ndev
+    if world > 1:
+        dist.init_process_group("gloo" if shared_devices else "nccl", **({} if shared_devices else {"device_id": torch.device("cuda", dev)}))
+    barrier = (lambda: dist.barrier()) if world > 1 else (lambda: None)
+    cfg_idx, builder, kw, wdesc = WORKLOADS[args.workload]
+    w = getattr(W, builder)(**kw)
+    N, V = w.N, int(np.prod(w.N))
+    yl = N[1] // world
+    plan = binding.ShardedPlan(N, w.h, ALGS[args.alg], rank, world)
+    plan.precompute_green()
+    b1x, b1y, _, _ = plan.buffers()
+    if world > 1:
+        mine = (binding.ipc_get_handle(b1x), binding.ipc_get_handle(b1y))
+        allh = [None] * world
+        dist.all_gather_object(allh, mine)
+        px = [b1x if r == rank else binding.ipc_open_handle(allh[r][0]) for r in range(world)]
+        py = [b1y if r == rank else binding.ipc_open_handle(allh[r][1]) for r in range(world)]
+    else:
+        px, py = [b1x], [b1y]
+    plan.set_peers(px, py)
+    rho = torch.from_numpy(np.ascontiguousarray(w.rho[:, rank * yl:(rank + 1) * yl, :])).cuda()
+    phi = torch.empty_like(rho)
+
+    def solve():
+        for ph in range(3):
+            plan.phase(ph, rho, phi)
+            torch.cuda.synchronize()
+            barrier()
+
+    for _ in range(args.warmup):
+        solve()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        solve()
+    dt = (time.perf_counter() - t0) / args.steps
+    if world > 1:
+        t = torch.tensor([dt], dtype=torch.float64)
+        if not shared_devices:
+            t = t.cuda()
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dt = float(t.item())
+    # parity of the assembled field against the single-GPU solve (rank 0 gathers the slabs through the host)
+    slabs = [None] * world
+    if world > 1:
+        dist.all_gather_object(slabs, phi.cpu().numpy())
+    else:
+        slabs = [phi.cpu().numpy()]
+    err = None
+    if rank == 0:
+        full = np.concatenate(slabs, axis=1)
+        with binding.Plan(N, w.h, ALGS[args.alg]) as p1:
+            one = p1.precompute_green().solve(torch.from_numpy(w.rho).cuda()).cpu().numpy()
+        err = float(np.abs(full - one).max() / np.abs(one).max())
+        nx1 = N[0] + 1
+        line = {"mode": "sharded", "metric": "solves/s", "value": 1.0 / dt, "unit": "solves/s", "grid_points_per_s": V / dt,
+                "n_gpus": world, "devices_used": min(world, ndev), "ranks_share_devices": shared_devices,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+                "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": wdesc, "mesh": list(N), "algorithm": args.alg, "parallelism": f"y-slabs over {world} ranks, "
+                           "2 P2P transposes + 2 host barriers per solve", "timing": "host clock, max over ranks (phases end in "
+                           "stream syncs and barriers)"},
+                "p2p_bytes_per_gpu_per_solve": 2 * 16 * nx1 * yl * N[2] * (world - 1) // world,
+                "max_rel_diff_vs_single_gpu_solve": err, "plan_bytes_per_rank": plan.bytes,
+                "gpu_launches": 7 * args.steps}
+        print(json.dumps(line))
+    barrier()
+    plan.destroy()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
 def _ncu_traffic(kernel: str, wname: str):
     """(dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, stale?) from the committed
     `ncu --set full` summary under profiles/ (null until one exists for this workload).  The figure is NOT measured
@@ -651,4 +746,6 @@ if __name__ == "__main__":
     if a.print_kernels_sha:
         print(kernel_sources_sha16())
         sys.exit(0)
+    if a.sharded and a.impl != "reference":
+        sys.exit(run_sharded(a))
     sys.exit(run_reference(a) if a.impl == "reference" else run_b200(a))

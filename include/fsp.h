@@ -180,6 +180,58 @@ int fsp_solve_field_host(fsp_plan* p, const double* rho_host, double* phi_host, 
 /* Frees everything the plan owns (synchronises its stream first). */
 int fsp_destroy(fsp_plan* p);
 
+/* ---- slab decomposition over several GPUs -----------------------------------------------------
+ * the paper runs its large meshes on many GPUs (heFFTe pencils, MPI all-to-all).  Here one solve
+ * is split over P GPUs with ONE global transpose each way:
+ *   rank r owns the y-slab rho_r[x][yl][z], yl < Ny/P, and the same slab of phi;
+ *   phase 0: K1 (R2C along x) on the slab, then every rank writes, through peer memory (NVLink P2P stores, no pack
+ *            buffer), the kx planes [k0_s, k0_s + np_s) of its result into rank s's y-z workspace B1y_s[kxl][y][z];
+ *   phase 1: K2, K3, K4 on the rank's own kx planes (spectrum rows of those planes only), then the transpose back
+ *            into every rank's x workspace B1x_r[kx][yl][z];
+ *   phase 2: K5 (C2R along x) on the slab.
+ * Between phases ALL ranks must have finished the previous phase (the caller synchronises its stream and runs a
+ * barrier, e.g. torch.distributed.barrier(); two barriers per solve, nothing else crosses ranks).  Bytes leaving a GPU
+ * per solve: 2 x 16 (Nx+1)(Ny/P) Nz (P-1)/P.  Power-of-two meshes with Ny % P == 0, P <= 16, (Ny/P) Nz >= 64.
+ * The Green precompute is replicated: every rank computes the whole octant and keeps the rows of its planes
+ * (stated limitation: the transient and the (N+1)^3 table are not sharded yet).
+ * Verified on ONE device with P plans in one process (phases run in turn, tests/test_gpu_sharded.py) and, for the
+ * index arithmetic, by a world-size-2 CPU test; NOT yet measured on a multi-GPU node.
+ */
+typedef struct fsp_sharded_plan fsp_sharded_plan;
+
+/* kx planes [*k0_out, *k0_out + *np_out) of rank `rank`: contiguous slabs of the Nx + 1 planes. */
+int fsp_shard_planes(int Nx, int nranks, int rank, int* k0_out, int* np_out);
+
+/* The block rank src_rank sends to dst_rank (direction 0: forward transpose B1x -> B1y; 1: backward B1y -> B1x) as
+ * out6 = {nrun, run_len, src_off, src_stride, dst_off, dst_stride} in complex (16-byte) elements: run i covers
+ * src[src_off + i src_stride + j] -> dst[dst_off + i dst_stride + j], j < run_len.  Host only (no GPU needed). */
+int fsp_shard_block(int Nx, int Ny, int Nz, int nranks, int src_rank, int dst_rank, int direction, long long* out6);
+
+/* plan for rank `rank` of `nranks` on the current device; stream as in fsp_plan_create. */
+int fsp_sharded_create(fsp_sharded_plan** out, int Nx, int Ny, int Nz, const double* h, int algorithm,
+                       void* cuda_stream, int rank, int nranks);
+int fsp_sharded_set_param(fsp_sharded_plan* sp, int which, double value);
+int fsp_sharded_precompute_green(fsp_sharded_plan* sp);
+
+/* Device pointers (and sizes) of this rank's two transpose targets; the caller makes them known to every rank
+ * (same process: the pointers themselves; one process per GPU: fsp_ipc_get_handle / fsp_ipc_open_handle). */
+int fsp_sharded_buffers(const fsp_sharded_plan* sp, void** b1x_out, void** b1y_out, size_t* b1x_bytes, size_t* b1y_bytes);
+
+/* peer_b1x[s], peer_b1y[s]: addresses, valid on THIS device, of rank s's buffers, s < nranks (own entries included). */
+int fsp_sharded_set_peers(fsp_sharded_plan* sp, void* const* peer_b1x, void* const* peer_b1y);
+
+/* One phase (0, 1, 2; see above) of one solve, asynchronous on the plan's stream.  rho_slab_dev (phase 0) and
+ * phi_slab_dev (phase 2): Nx * (Ny/P) * Nz doubles, [x][yl][z]; ignored in the other phases. */
+int fsp_sharded_solve_phase(fsp_sharded_plan* sp, int phase, const double* rho_slab_dev, double* phi_slab_dev);
+
+size_t fsp_sharded_bytes(const fsp_sharded_plan* sp);
+int fsp_sharded_destroy(fsp_sharded_plan* sp);
+
+/* cudaIpcGetMemHandle / cudaIpcOpenMemHandle / cudaIpcCloseMemHandle on 64-byte handles (host pointers). */
+int fsp_ipc_get_handle(void* dev_ptr, void* handle64_out);
+int fsp_ipc_open_handle(const void* handle64, void** dev_ptr_out);
+int fsp_ipc_close_handle(void* dev_ptr);
+
 /* ---- queries and test hooks (no hot-path cost) ------------------------------------------------ */
 
 /* Device bytes the plan holds between solves (workspace + spectrum + tables [+ staging]). */

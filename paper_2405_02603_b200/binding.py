@@ -48,6 +48,19 @@ SIGNATURES = {
     "fsp_get_green_spectrum": (_i, [_vp, _dp]),
     "fsp_set_profiling": (_i, [_vp, _i]),
     "fsp_get_kernel_times": (_i, [_vp, _c.POINTER(_c.c_float), _c.POINTER(_i)]),
+    "fsp_shard_planes": (_i, [_i, _i, _i, _c.POINTER(_i), _c.POINTER(_i)]),
+    "fsp_shard_block": (_i, [_i, _i, _i, _i, _i, _i, _i, _c.POINTER(_c.c_longlong)]),
+    "fsp_sharded_create": (_i, [_c.POINTER(_vp), _i, _i, _i, _dp, _i, _vp, _i, _i]),
+    "fsp_sharded_set_param": (_i, [_vp, _i, _d]),
+    "fsp_sharded_precompute_green": (_i, [_vp]),
+    "fsp_sharded_buffers": (_i, [_vp, _c.POINTER(_vp), _c.POINTER(_vp), _c.POINTER(_sz), _c.POINTER(_sz)]),
+    "fsp_sharded_set_peers": (_i, [_vp, _c.POINTER(_vp), _c.POINTER(_vp)]),
+    "fsp_sharded_solve_phase": (_i, [_vp, _i, _vp, _vp]),
+    "fsp_sharded_bytes": (_sz, [_vp]),
+    "fsp_sharded_destroy": (_i, [_vp]),
+    "fsp_ipc_get_handle": (_i, [_vp, _vp]),
+    "fsp_ipc_open_handle": (_i, [_vp, _c.POINTER(_vp)]),
+    "fsp_ipc_close_handle": (_i, [_vp]),
     "fsp_kernel_name": (_c.c_char_p, [_i]),
     "fsp_strerror": (_c.c_char_p, [_i]),
     "fsp_version": (_i, []),
@@ -318,3 +331,81 @@ class Plan:
             self.destroy()
         except Exception:
             pass
+
+
+# ---- slab decomposition (include/fsp.h "slab decomposition over several GPUs") ---------------------------------
+def shard_planes(Nx: int, nranks: int, rank: int):
+    k0, npl = _i(0), _i(0)
+    _chk(lib().fsp_shard_planes(Nx, nranks, rank, ctypes.byref(k0), ctypes.byref(npl)), "fsp_shard_planes")
+    return int(k0.value), int(npl.value)
+
+
+def shard_block(Nx: int, Ny: int, Nz: int, nranks: int, src_rank: int, dst_rank: int, direction: int):
+    """(nrun, run_len, src_off, src_stride, dst_off, dst_stride) in complex elements."""
+    out = (ctypes.c_longlong * 6)()
+    _chk(lib().fsp_shard_block(Nx, Ny, Nz, nranks, src_rank, dst_rank, direction, out), "fsp_shard_block")
+    return tuple(int(v) for v in out)
+
+
+class ShardedPlan:
+    """Rank `rank` of `nranks` of one solve split into y-slabs (marshalling only; the caller provides the barriers
+    between the three phases and tells every rank where the others' workspaces are)."""
+
+    def __init__(self, N, h, algorithm: int, rank: int, nranks: int, stream: int = 0):
+        self.N = tuple(int(v) for v in N)
+        self.rank, self.nranks = rank, nranks
+        hh = (ctypes.c_double * 3)(*[float(v) for v in np.broadcast_to(np.asarray(h, dtype=np.float64), (3,))])
+        out = ctypes.c_void_p()
+        _chk(lib().fsp_sharded_create(ctypes.byref(out), *self.N, hh, algorithm, ctypes.c_void_p(stream), rank, nranks),
+             "fsp_sharded_create")
+        self.handle = out.value
+        self.slab = (self.N[0], self.N[1] // nranks, self.N[2])
+
+    def precompute_green(self):
+        _chk(lib().fsp_sharded_precompute_green(self.handle), "fsp_sharded_precompute_green")
+        return self
+
+    def buffers(self):
+        """(B1x address, B1y address, B1x bytes, B1y bytes) of this rank's transpose targets."""
+        a, b, na, nb = ctypes.c_void_p(), ctypes.c_void_p(), ctypes.c_size_t(), ctypes.c_size_t()
+        _chk(lib().fsp_sharded_buffers(self.handle, ctypes.byref(a), ctypes.byref(b), ctypes.byref(na), ctypes.byref(nb)),
+             "fsp_sharded_buffers")
+        return a.value, b.value, na.value, nb.value
+
+    def set_peers(self, b1x_addrs, b1y_addrs):
+        n = self.nranks
+        xa = (ctypes.c_void_p * n)(*b1x_addrs)
+        ya = (ctypes.c_void_p * n)(*b1y_addrs)
+        _chk(lib().fsp_sharded_set_peers(self.handle, xa, ya), "fsp_sharded_set_peers")
+
+    def phase(self, which: int, rho_slab=None, phi_slab=None):
+        _chk(lib().fsp_sharded_solve_phase(self.handle, which, _ptr(rho_slab) if rho_slab is not None else None,
+                                           _ptr(phi_slab) if phi_slab is not None else None), "fsp_sharded_solve_phase")
+
+    @property
+    def bytes(self) -> int:
+        return int(lib().fsp_sharded_bytes(self.handle))
+
+    def destroy(self):
+        if self.handle:
+            _chk(lib().fsp_sharded_destroy(self.handle), "fsp_sharded_destroy")
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+
+def ipc_get_handle(dev_ptr: int) -> bytes:
+    buf = ctypes.create_string_buffer(64)
+    _chk(lib().fsp_ipc_get_handle(dev_ptr, ctypes.cast(buf, ctypes.c_void_p)), "fsp_ipc_get_handle")
+    return buf.raw
+
+
+def ipc_open_handle(handle: bytes) -> int:
+    buf = ctypes.create_string_buffer(handle, 64)
+    out = ctypes.c_void_p()
+    _chk(lib().fsp_ipc_open_handle(ctypes.cast(buf, ctypes.c_void_p), ctypes.byref(out)), "fsp_ipc_open_handle")
+    return out.value

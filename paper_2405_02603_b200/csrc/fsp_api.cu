@@ -15,6 +15,7 @@
 #include "../../include/fsp.h"
 #include "green_kernels.cuh"
 #include "solve_kernels.cuh"
+#include "shard.cuh"
 
 using namespace fsp;
 
@@ -39,6 +40,11 @@ struct fsp_plan {
     double* LTzs = nullptr; // Nz = 512: constants of the 32-lane transform (k_conv_z_s): stage 2 [32][16], shuffled level [2][16]
     double* LTzf = nullptr; // Nz = 256, 512: stage-2 constants of the padded transform of 2 Nz points (k_conv_z_f)
     int k3_variant = 0;     // FSP_PARAM_K3_VARIANT
+    // shape of the workspace (sharded plans): a whole plan holds Nx + 1 kx planes and runs all five passes
+    int stage = 0;          // 0: whole solve; 1: x passes only (K1, K5); 2: the y-z-y middle only (K2, K3, K4)
+    int planes = 0;         // kx planes held by B1 (stage 2), B2 and Gk; Nx + 1 unless stage 2 of a sharded plan
+    int kx0 = 0;            // global index of the first of them
+    size_t b1_count = 0, b2_count = 0;   // complex elements allocated in B1, B2
     bool gk_natural = false; // Gk rows in natural order (k_conv_z_f) instead of [E | O] (decided by the last precompute)
     double* LTy = nullptr;  // the same for the y transform (tile kernels)
     bool tile_y = false;    // K2/K4 tile kernels (TMA-staged) are used
@@ -763,7 +769,7 @@ int precompute_impl(fsp_plan* p) {
                 if ((rc = dct1_axis(p, b, p->T, bd, tdims, 0, nx, Nx + 1, vscale)) != FSP_OK) return rc;
             } else {
             const size_t plane_a = (size_t)Ky * (Nz + 1), count_b = (size_t)Kx * (Ny + 1) * (Nz + 1);
-            const size_t cap1 = (size_t)(Nx + 1) * Ny * Nz * 2, cap2 = 2 * cap1;   // doubles in B1, B2
+            const size_t cap1 = p->b1_count * 2, cap2 = p->b2_count * 2;   // doubles in B1, B2
             double *a = reinterpret_cast<double*>(p->B1), *b = reinterpret_cast<double*>(p->B2);
             long chunk = (long)(cap1 / plane_a);
             int rc;
@@ -796,7 +802,7 @@ int precompute_impl(fsp_plan* p) {
     {
         double* u = reinterpret_cast<double*>(p->B1);   // the solve's workspace serves as scratch when it is big enough
         int rc = FSP_OK;
-        if ((size_t)tcount > (size_t)(Nx + 1) * Ny * Nz * 2) {
+        if ((size_t)tcount > p->b1_count * 2) {
             if ((rc = dev_alloc(&u, (size_t)tcount, &peak)) != FSP_OK) return rc;
             tmp.ptrs.push_back(u);
         }
@@ -807,10 +813,12 @@ int precompute_impl(fsp_plan* p) {
     // scale: hx hy hz / (8 Nx Ny Nz) (inverse DFT) / 2 (K1 produces 2X)
     const double gscale = hx * hy * hz / (8.0 * (double)Nx * (double)Ny * (double)Nz) * 0.5;
     {
-        const long gk_total = (long)(Nx + 1) * (Ny + 1) * (Nz + 2);
+        // (a sharded plan keeps the rows of its own kx planes only)
+        const long gk_total = (long)p->planes * (Ny + 1) * (Nz + 2);
+        const double* goct = p->Goct + (size_t)p->kx0 * (Ny + 1) * (Nz + 1);
         p->gk_natural = (Nz == 256 || Nz == 512) && p->k3_variant == 0;
-        if (p->gk_natural) k_layout_spectrum_nat<<<grid_for(gk_total, blk), blk, 0, p->stream>>>(p->Goct, p->Gk, Nx, Ny, Nz, gscale);
-        else k_layout_spectrum_oct<<<grid_for(gk_total, blk), blk, 0, p->stream>>>(p->Goct, p->Gk, Nx, Ny, Nz, gscale);
+        if (p->gk_natural) k_layout_spectrum_nat<<<grid_for(gk_total, blk), blk, 0, p->stream>>>(goct, p->Gk, p->planes - 1, Ny, Nz, gscale);
+        else k_layout_spectrum_oct<<<grid_for(gk_total, blk), blk, 0, p->stream>>>(goct, p->Gk, p->planes - 1, Ny, Nz, gscale);
     }
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(p->stream));
@@ -855,7 +863,9 @@ const char* fsp_kernel_name(int i) {
     return (i >= 0 && i < FSP_NUM_SOLVE_KERNELS) ? names[i] : "";
 }
 
-int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int algorithm, void* cuda_stream) {
+// stage / kx0 / planes: see fsp_plan.  Stages 1 and 2 are the two halves of a sharded plan (power-of-two meshes only).
+static int plan_create_impl(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int algorithm, void* cuda_stream,
+                            int stage, int kx0, int planes_req) {
     if (!out) return FSP_ERR_INVALID_ARG;
     *out = nullptr;
     if (!h || !(h[0] > 0.0) || !(h[1] > 0.0) || !(h[2] > 0.0)) return FSP_ERR_INVALID_ARG;
@@ -885,20 +895,25 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
     if (cudaGetDevice(&p->device) != cudaSuccess || cudaGetDeviceProperties(&prop, p->device) != cudaSuccess) rc = FSP_ERR_NO_DEVICE;
     if (rc == FSP_OK && prop.major != 10) rc = FSP_ERR_NO_DEVICE;  // the library holds sm_100a code only
     if (rc == FSP_OK && (p->device < 0 || p->device >= kMaxDevices)) rc = FSP_ERR_NO_DEVICE;
-    const size_t n1 = (size_t)(Nx + 1) * Ny * Nz, n2 = (size_t)(Nx + 1) * 2 * Ny * Nz;
+    if (stage != 0 && p->padded) rc = FSP_ERR_INVALID_ARG;
+    const int planes = stage == 2 ? planes_req : Nx + 1;
+    p->stage = stage; p->planes = planes; p->kx0 = stage == 2 ? kx0 : 0;
+    const bool want_x = stage != 2, want_yz = stage != 1;
+    const size_t n1 = (size_t)planes * Ny * Nz, n2 = (size_t)planes * 2 * Ny * Nz;
     const size_t nt = (size_t)(Nx + 1) * (Ny + 1) * (Nz + 1);
+    p->b1_count = n1; p->b2_count = want_yz ? n2 : 0;
     if (rc == FSP_OK && p->padded) rc = dev_alloc(&p->rho_pad, (size_t)Nx * Ny * Nz, &p->bytes);
     if (rc == FSP_OK && p->padded) rc = dev_alloc(&p->phi_pad, (size_t)Nx * Ny * Nz, &p->bytes);
     if (rc == FSP_OK && p->padded && cudaMemset(p->rho_pad, 0, sizeof(double) * (size_t)Nx * Ny * Nz) != cudaSuccess) rc = FSP_ERR_CUDA;
     if (rc == FSP_OK) rc = dev_alloc(&p->B1, n1, &p->bytes);
-    if (rc == FSP_OK) rc = dev_alloc(&p->B2, n2, &p->bytes);
+    if (rc == FSP_OK && want_yz) rc = dev_alloc(&p->B2, n2, &p->bytes);
     p->sm_count = prop.multiProcessorCount > 0 ? prop.multiProcessorCount : 148;
-    if (rc == FSP_OK) rc = dev_alloc(&p->Gk, (size_t)(Nx + 1) * (Ny + 1) * (Nz + 2), &p->bytes);
-    if (rc == FSP_OK) rc = make_z_lane_table(p);
-    if (rc == FSP_OK && Nz == 512) rc = make_lane_table_512s(&p->LTzs, &p->bytes);
-    if (rc == FSP_OK && Nz == 512) rc = lane_table_for<1024>(&p->LTzf, &p->bytes);
-    if (rc == FSP_OK && Nz == 256) rc = lane_table_for<512>(&p->LTzf, &p->bytes);
-    p->tile_x = (Nx == 128 || Nx == 256 || Nx == 512 || Nx == 1024) && ((long)Ny * Nz) % kC == 0;
+    if (rc == FSP_OK && want_yz) rc = dev_alloc(&p->Gk, (size_t)planes * (Ny + 1) * (Nz + 2), &p->bytes);
+    if (rc == FSP_OK && want_yz) rc = make_z_lane_table(p);
+    if (rc == FSP_OK && want_yz && Nz == 512) rc = make_lane_table_512s(&p->LTzs, &p->bytes);
+    if (rc == FSP_OK && want_yz && Nz == 512) rc = lane_table_for<1024>(&p->LTzf, &p->bytes);
+    if (rc == FSP_OK && want_yz && Nz == 256) rc = lane_table_for<512>(&p->LTzf, &p->bytes);
+    p->tile_x = want_x && (Nx == 128 || Nx == 256 || Nx == 512 || Nx == 1024) && ((long)Ny * Nz) % kC == 0;
     if (rc == FSP_OK && p->tile_x) rc = make_x_lane_table(p);
     if (rc == FSP_OK && p->tile_x) {
         const cuuint64_t plane = (cuuint64_t)Ny * Nz;
@@ -907,26 +922,26 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
         const cuuint32_t box[3] = {2 * (cuuint32_t)(Nx == 1024 ? 8 : kC), 1, (cuuint32_t)(Nx / 2 < 256 ? Nx / 2 : 256)};   // TileXI<M>::KC columns
         rc = make_tensor_map(&p->tmB1x, p->B1, 3, dims, strides, box);
     }
-    p->tile_y = (Ny == 128 || Ny == 256 || Ny == 512 || Ny == 1024) && Nz >= kW;
+    p->tile_y = want_yz && (Ny == 128 || Ny == 256 || Ny == 512 || Ny == 1024) && Nz >= kW;
     const cuuint32_t kwy = Ny == 1024 ? 4 : kW;   // TileY<M>::KW: columns per tile of the y tile kernels
     if (rc == FSP_OK && p->tile_y) rc = make_y_lane_table(p);
     if (rc == FSP_OK && p->tile_y) {
-        const cuuint64_t dims[3] = {(cuuint64_t)2 * Nz, (cuuint64_t)Ny, (cuuint64_t)(Nx + 1)};
+        const cuuint64_t dims[3] = {(cuuint64_t)2 * Nz, (cuuint64_t)Ny, (cuuint64_t)planes};
         const cuuint64_t strides[2] = {(cuuint64_t)Nz * 16, (cuuint64_t)Ny * Nz * 16};
         const cuuint32_t box[3] = {2 * kwy, (cuuint32_t)(Ny < 256 ? Ny : 256), 1};
         rc = make_tensor_map(&p->tmB1y, p->B1, 3, dims, strides, box);
     }
     if (rc == FSP_OK && p->tile_y) {
-        const cuuint64_t dims[4] = {(cuuint64_t)2 * Nz, 2, (cuuint64_t)Ny, (cuuint64_t)(Nx + 1)};
+        const cuuint64_t dims[4] = {(cuuint64_t)2 * Nz, 2, (cuuint64_t)Ny, (cuuint64_t)planes};
         const cuuint64_t strides[3] = {(cuuint64_t)Nz * 16, (cuuint64_t)2 * Nz * 16, (cuuint64_t)2 * Ny * Nz * 16};
         const cuuint32_t box[4] = {2 * kwy, 1, (cuuint32_t)(Ny < 256 ? Ny : 256), 1};
         rc = make_tensor_map(&p->tmB2y, p->B2, 4, dims, strides, box);
     }
-    if (rc == FSP_OK) rc = dev_alloc(&p->T, nt, &p->bytes);
-    if (rc == FSP_OK) rc = dev_alloc(&p->Goct, nt, &p->bytes);
-    if (rc == FSP_OK) rc = make_table(&p->Wx, 2 * Nx, &p->bytes);
-    if (rc == FSP_OK) rc = make_table(&p->Wy, 2 * Ny, &p->bytes);
-    if (rc == FSP_OK) rc = make_table(&p->Wz, 2 * Nz, &p->bytes);
+    if (rc == FSP_OK && want_yz) rc = dev_alloc(&p->T, nt, &p->bytes);
+    if (rc == FSP_OK && want_yz) rc = dev_alloc(&p->Goct, nt, &p->bytes);
+    if (rc == FSP_OK && want_x) rc = make_table(&p->Wx, 2 * Nx, &p->bytes);
+    if (rc == FSP_OK && want_yz) rc = make_table(&p->Wy, 2 * Ny, &p->bytes);
+    if (rc == FSP_OK && want_yz) rc = make_table(&p->Wz, 2 * Nz, &p->bytes);
     if (rc != FSP_OK) {
         free_plan_memory(p);
         delete p;
@@ -934,6 +949,10 @@ int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int
     }
     *out = p;
     return FSP_OK;
+}
+
+int fsp_plan_create(fsp_plan** out, int Nx, int Ny, int Nz, const double* h, int algorithm, void* cuda_stream) {
+    return plan_create_impl(out, Nx, Ny, Nz, h, algorithm, cuda_stream, 0, 0, 0);
 }
 
 int fsp_plan_set_param(fsp_plan* p, int which, double value) {
@@ -968,7 +987,7 @@ int fsp_plan_set_spacing(fsp_plan* p, const double* h) {
 }
 
 int fsp_precompute_green(fsp_plan* p) {
-    if (!p) return FSP_ERR_INVALID_ARG;
+    if (!p || p->stage == 1) return FSP_ERR_INVALID_ARG;
     DeviceGuard dev_guard(p->device);
     p->precomputed = false;
     int rc = precompute_impl(p);
@@ -983,6 +1002,7 @@ int fsp_precompute_green(fsp_plan* p) {
 
 int fsp_solve(fsp_plan* p, const double* rho_dev, double* phi_dev) {
     if (!p || !rho_dev || !phi_dev || rho_dev == phi_dev) return FSP_ERR_INVALID_ARG;
+    if (p->stage != 0) return FSP_ERR_INVALID_ARG;
     if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
     DeviceGuard dev_guard(p->device);
     double* phi_user = nullptr;
@@ -1121,6 +1141,7 @@ int fsp_solve_host_batch(fsp_plan* p, int n, const double* const* rho_hosts, dou
 
 int fsp_solve_field(fsp_plan* p, const double* rho_dev, double* phi_dev, double* E_dev) {
     if (!p || !rho_dev || !E_dev || rho_dev == phi_dev || rho_dev == E_dev) return FSP_ERR_INVALID_ARG;
+    if (p->stage != 0) return FSP_ERR_INVALID_ARG;
     if (!p->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
     DeviceGuard dev_guard(p->device);
     const size_t n2 = (size_t)(p->Nx + 1) * 2 * p->Ny * p->Nz, V = user_volume(p);
@@ -1305,6 +1326,163 @@ int fsp_get_kernel_times(fsp_plan* p, float* ms, int* n_solves) {
         }
     *n_solves = (int)n;
     p->events_used = 0;
+    return FSP_OK;
+}
+
+
+// ---- sharded plan (slab decomposition, shard.cuh) ----------------------------------------------------------
+struct fsp_sharded_plan {
+    fsp_plan* px = nullptr;    // x stage on the y-slab: mesh (Nx, Ny / P, Nz); its B1 is B1x
+    fsp_plan* pyz = nullptr;   // y-z-y middle on this rank's kx planes: mesh (Nx, Ny, Nz); its B1 is B1y
+    int rank = 0, nranks = 1, Nx = 0, Ny = 0, Nz = 0, k0 = 0, np = 0;
+    double2* peer_b1y[kMaxRanks] = {};   // every rank's B1y (forward transpose target), device-accessible from here
+    double2* peer_b1x[kMaxRanks] = {};   // every rank's B1x (backward transpose target)
+    bool peers_set = false;
+};
+
+static int shard_scatter(fsp_sharded_plan* sp, int direction) {
+    ShardCopyArgs a;
+    long longest = 0;
+    for (int s = 0; s < sp->nranks; ++s) {
+        a.dst[s] = direction == 0 ? sp->peer_b1y[s] : sp->peer_b1x[s];
+        a.blk[s] = shard_block(sp->Nx, sp->Ny, sp->Nz, sp->nranks, sp->rank, s, direction);
+        const long t = a.blk[s].nrun * a.blk[s].run_len;
+        if (t > longest) longest = t;
+    }
+    const double2* src = direction == 0 ? sp->px->B1 : sp->pyz->B1;
+    dim3 grid(grid_for(longest, 256), (unsigned)sp->nranks);
+    k_shard_copy<<<grid, 256, 0, sp->px->stream>>>(src, a);
+    CU(cudaGetLastError());
+    return FSP_OK;
+}
+
+int fsp_shard_planes(int Nx, int nranks, int rank, int* k0_out, int* np_out) {
+    if (Nx < 1 || nranks < 1 || nranks > kMaxRanks || rank < 0 || rank >= nranks || !k0_out || !np_out) return FSP_ERR_INVALID_ARG;
+    shard_planes(Nx, nranks, rank, k0_out, np_out);
+    return FSP_OK;
+}
+
+int fsp_shard_block(int Nx, int Ny, int Nz, int nranks, int src_rank, int dst_rank, int direction, long long* out6) {
+    if (Nx < 1 || Ny < 1 || Nz < 1 || nranks < 1 || nranks > kMaxRanks || Ny % nranks != 0 || src_rank < 0 || src_rank >= nranks ||
+        dst_rank < 0 || dst_rank >= nranks || (direction != 0 && direction != 1) || !out6)
+        return FSP_ERR_INVALID_ARG;
+    const ShardBlock b = shard_block(Nx, Ny, Nz, nranks, src_rank, dst_rank, direction);
+    out6[0] = b.nrun; out6[1] = b.run_len; out6[2] = b.src_off; out6[3] = b.src_stride; out6[4] = b.dst_off; out6[5] = b.dst_stride;
+    return FSP_OK;
+}
+
+int fsp_sharded_create(fsp_sharded_plan** out, int Nx, int Ny, int Nz, const double* h, int algorithm, void* cuda_stream,
+                       int rank, int nranks) {
+    if (!out) return FSP_ERR_INVALID_ARG;
+    *out = nullptr;
+    auto pow2 = [](int n) { return n >= 8 && (n & (n - 1)) == 0; };
+    if (!pow2(Nx) || !pow2(Ny) || !pow2(Nz) || Nx > 1024 || Ny > 1024 || Nz > 1024) return FSP_ERR_INVALID_ARG;
+    if (nranks < 1 || nranks > kMaxRanks || rank < 0 || rank >= nranks || Ny % nranks != 0 || Nx + 1 < nranks) return FSP_ERR_INVALID_ARG;
+    const long slab_plane = (long)(Ny / nranks) * Nz;   // columns of the x stage
+    if (slab_plane < 64) return FSP_ERR_INVALID_ARG;
+    fsp_sharded_plan* sp = new (std::nothrow) fsp_sharded_plan();
+    if (!sp) return FSP_ERR_OUT_OF_MEMORY;
+    sp->rank = rank; sp->nranks = nranks; sp->Nx = Nx; sp->Ny = Ny; sp->Nz = Nz;
+    shard_planes(Nx, nranks, rank, &sp->k0, &sp->np);
+    // the x stage sees the y-slab as a mesh of its own: K1 and K5 only need Ny_loc * Nz columns of length Nx
+    // (K1 and K5 only see "plane = Ny_loc * Nz columns": the slab is handed to them as a mesh Nx x Ny' x Nz' with the
+    // same number of columns and both factors powers of two >= 8, whatever Ny / P is)
+    const int nz_x = (int)(slab_plane / 8 < 1024 ? slab_plane / 8 : 1024), ny_x = (int)(slab_plane / nz_x);
+    int rc = plan_create_impl(&sp->px, Nx, ny_x, nz_x, h, algorithm, cuda_stream, 1, 0, 0);
+    if (rc == FSP_OK) rc = plan_create_impl(&sp->pyz, Nx, Ny, Nz, h, algorithm, cuda_stream, 2, sp->k0, sp->np);
+    if (rc != FSP_OK) {
+        if (sp->px) fsp_destroy(sp->px);
+        if (sp->pyz) fsp_destroy(sp->pyz);
+        delete sp;
+        return rc;
+    }
+    *out = sp;
+    return FSP_OK;
+}
+
+int fsp_sharded_set_param(fsp_sharded_plan* sp, int which, double value) {
+    if (!sp) return FSP_ERR_INVALID_ARG;
+    return fsp_plan_set_param(sp->pyz, which, value);
+}
+
+int fsp_sharded_precompute_green(fsp_sharded_plan* sp) {
+    if (!sp) return FSP_ERR_INVALID_ARG;
+    return fsp_precompute_green(sp->pyz);
+}
+
+int fsp_sharded_buffers(const fsp_sharded_plan* sp, void** b1x_out, void** b1y_out, size_t* b1x_bytes, size_t* b1y_bytes) {
+    if (!sp || !b1x_out || !b1y_out) return FSP_ERR_INVALID_ARG;
+    *b1x_out = sp->px->B1;
+    *b1y_out = sp->pyz->B1;
+    if (b1x_bytes) *b1x_bytes = sp->px->b1_count * sizeof(double2);
+    if (b1y_bytes) *b1y_bytes = sp->pyz->b1_count * sizeof(double2);
+    return FSP_OK;
+}
+
+int fsp_sharded_set_peers(fsp_sharded_plan* sp, void* const* peer_b1x, void* const* peer_b1y) {
+    if (!sp || !peer_b1x || !peer_b1y) return FSP_ERR_INVALID_ARG;
+    for (int s = 0; s < sp->nranks; ++s) {
+        if (!peer_b1x[s] || !peer_b1y[s]) return FSP_ERR_INVALID_ARG;
+        sp->peer_b1x[s] = static_cast<double2*>(peer_b1x[s]);
+        sp->peer_b1y[s] = static_cast<double2*>(peer_b1y[s]);
+    }
+    if (sp->peer_b1x[sp->rank] != sp->px->B1 || sp->peer_b1y[sp->rank] != sp->pyz->B1) return FSP_ERR_INVALID_ARG;
+    sp->peers_set = true;
+    return FSP_OK;
+}
+
+int fsp_sharded_solve_phase(fsp_sharded_plan* sp, int phase, const double* rho_slab_dev, double* phi_slab_dev) {
+    if (!sp || phase < 0 || phase > 2) return FSP_ERR_INVALID_ARG;
+    if (!sp->peers_set) return FSP_ERR_INVALID_ARG;
+    if (!sp->pyz->precomputed) return FSP_ERR_NOT_PRECOMPUTED;
+    DeviceGuard dev_guard(sp->px->device);
+    int rc;
+    if (phase == 0) {          // K1 on the y-slab, then the forward transpose into every rank's B1y
+        if (!rho_slab_dev) return FSP_ERR_INVALID_ARG;
+        if ((rc = do_fwd_x(sp->px, rho_slab_dev)) != FSP_OK) return rc;
+        return shard_scatter(sp, 0);
+    }
+    if (phase == 1) {          // K2, K3, K4 on this rank's kx planes, then the backward transpose into every rank's B1x
+        fsp_plan* q = sp->pyz;
+        if ((rc = do_fwd_y(q, 0, q->B2, sp->np)) != FSP_OK) return rc;
+        if ((rc = do_conv_z(q, q->B2, 0, sp->np)) != FSP_OK) return rc;
+        if ((rc = do_inv_y(q, q->B2, q->B1, sp->np)) != FSP_OK) return rc;
+        return shard_scatter(sp, 1);
+    }
+    if (!phi_slab_dev) return FSP_ERR_INVALID_ARG;
+    if ((rc = do_inv_x(sp->px, phi_slab_dev)) != FSP_OK) return rc;   // K5 on the y-slab
+    CU(cudaGetLastError());
+    return FSP_OK;
+}
+
+size_t fsp_sharded_bytes(const fsp_sharded_plan* sp) { return sp ? sp->px->bytes + sp->pyz->bytes : 0; }
+
+int fsp_sharded_destroy(fsp_sharded_plan* sp) {
+    if (!sp) return FSP_ERR_INVALID_ARG;
+    fsp_destroy(sp->px);
+    fsp_destroy(sp->pyz);
+    delete sp;
+    return FSP_OK;
+}
+
+// thin wrappers over the CUDA IPC calls, so that one-process-per-GPU launches can exchange the workspace addresses that
+// fsp_sharded_set_peers needs (handle: 64 bytes, sent between ranks by the caller, e.g. torch.distributed all_gather)
+int fsp_ipc_get_handle(void* dev_ptr, void* handle64_out) {
+    if (!dev_ptr || !handle64_out) return FSP_ERR_INVALID_ARG;
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "handle size");
+    CU(cudaIpcGetMemHandle(static_cast<cudaIpcMemHandle_t*>(handle64_out), dev_ptr));
+    return FSP_OK;
+}
+int fsp_ipc_open_handle(const void* handle64, void** dev_ptr_out) {
+    if (!handle64 || !dev_ptr_out) return FSP_ERR_INVALID_ARG;
+    cudaIpcMemHandle_t hnd;
+    std::memcpy(&hnd, handle64, sizeof(hnd));
+    CU(cudaIpcOpenMemHandle(dev_ptr_out, hnd, cudaIpcMemLazyEnablePeerAccess));
+    return FSP_OK;
+}
+int fsp_ipc_close_handle(void* dev_ptr) {
+    if (!dev_ptr) return FSP_ERR_INVALID_ARG;
+    CU(cudaIpcCloseMemHandle(dev_ptr));
     return FSP_OK;
 }
 

@@ -779,8 +779,9 @@ k_conv_z_f(double2* __restrict__ B2, const double* __restrict__ Gk, const double
                     if constexpr (DER) {
                         // signed mode of kz = t + T i: kz below M, kz - M2 above, zero at the Nyquist index kz = M
                         // (t = 0, i = R/2); the factor -i itself is applied to the final result (F^-1 is linear)
-                        double cf = gk * fma(kap.z, (double)(i < H ? T * i : T * i - M2), fz0);
-                        if (i == H) cf = t == 0 ? gk * fp : cf;
+                        // (fz0 = fp + kap.z t, so at t = 0 the Nyquist factor fp is fz0 itself)
+                        const double off = (double)(i < H ? T * i : T * i - M2);
+                        const double cf = gk * ((i == H && t == 0) ? fz0 : fma(kap.z, off, fz0));
                         vr[i] *= cf; vi[i] *= -cf;
                     } else {
                         vr[i] *= gk; vi[i] *= -gk;
