@@ -74,15 +74,19 @@ __device__ __forceinline__ double sin64(int k) { return cos64(k - 16); }
 
 // ---- r-point DFT, in place, on elements re[0], re[S], re[2S], ... (natural order in and out) ---
 template <int r, int S>
-__device__ __forceinline__ void dft_inplace(double* re, double* im) {
+__device__ __forceinline__ void dft_pfa(double* re, double* im);
+
+// r a power of two (decimation in time); dft_inplace below dispatches on r
+template <int r, int S>
+__device__ __forceinline__ void dft_pow2(double* re, double* im) {
     if constexpr (r == 2) {
         double ar = re[0], ai = im[0], br = re[S], bi = im[S];
         re[0] = ar + br; im[0] = ai + bi;
         re[S] = ar - br; im[S] = ai - bi;
     } else if constexpr (r > 2) {
         constexpr int H = r / 2;
-        dft_inplace<H, 2 * S>(re, im);          // even-indexed inputs
-        dft_inplace<H, 2 * S>(re + S, im + S);  // odd-indexed inputs
+        dft_pow2<H, 2 * S>(re, im);          // even-indexed inputs
+        dft_pow2<H, 2 * S>(re + S, im + S);  // odd-indexed inputs
         double er[H], ei[H], qr[H], qi[H];
 #pragma unroll
         for (int k = 0; k < H; ++k) {
@@ -115,6 +119,83 @@ __device__ __forceinline__ void dft_inplace(double* re, double* im) {
             }
         }
     }
+}
+
+// ---- radices 3 and 5, and 6, 12, 10, 20 by the prime-factor algorithm (meshes 3 * 2^k, 5 * 2^k) ----
+// Forward sign exp(-2 pi i ..).  Constants: sin(2 pi/3), cos/sin(2 pi/5), cos/sin(4 pi/5), 40 digits.
+template <int S>
+__device__ __forceinline__ void dft3(double* re, double* im) {
+    constexpr double s3 = 0.8660254037844386467637231707529361834714;
+    const double ar = re[S] + re[2 * S], ai = im[S] + im[2 * S], br = re[S] - re[2 * S], bi = im[S] - im[2 * S];
+    const double tr = fma(-0.5, ar, re[0]), ti = fma(-0.5, ai, im[0]);
+    re[0] += ar; im[0] += ai;
+    // X1 = t - i s b,  X2 = t + i s b   (-i (br + i bi) = bi - i br)
+    re[S] = fma(s3, bi, tr); im[S] = fma(-s3, br, ti);
+    re[2 * S] = fma(-s3, bi, tr); im[2 * S] = fma(s3, br, ti);
+}
+template <int S>
+__device__ __forceinline__ void dft5(double* re, double* im) {
+    constexpr double c1 = 0.3090169943749474241022934171828190588602, c2 = -0.8090169943749474241022934171828190588602;
+    constexpr double s1 = 0.9510565162951535721164393333793821434057, s2 = 0.5877852522924731291687059546390727685977;
+    const double a1r = re[S] + re[4 * S], a1i = im[S] + im[4 * S], b1r = re[S] - re[4 * S], b1i = im[S] - im[4 * S];
+    const double a2r = re[2 * S] + re[3 * S], a2i = im[2 * S] + im[3 * S], b2r = re[2 * S] - re[3 * S], b2i = im[2 * S] - im[3 * S];
+    const double x0r = re[0], x0i = im[0];
+    const double t1r = fma(c2, a2r, fma(c1, a1r, x0r)), t1i = fma(c2, a2i, fma(c1, a1i, x0i));
+    const double t2r = fma(c1, a2r, fma(c2, a1r, x0r)), t2i = fma(c1, a2i, fma(c2, a1i, x0i));
+    const double u1r = fma(s2, b2r, s1 * b1r), u1i = fma(s2, b2i, s1 * b1i);
+    const double u2r = fma(-s1, b2r, s2 * b1r), u2i = fma(-s1, b2i, s2 * b1i);
+    re[0] = x0r + a1r + a2r; im[0] = x0i + a1i + a2i;
+    // X1 = t1 - i u1, X4 = t1 + i u1, X2 = t2 - i u2, X3 = t2 + i u2   (-i u = u.i - i u.r)
+    re[S] = t1r + u1i; im[S] = t1i - u1r;
+    re[4 * S] = t1r - u1i; im[4 * S] = t1i + u1r;
+    re[2 * S] = t2r + u2i; im[2 * S] = t2i - u2r;
+    re[3 * S] = t2r - u2i; im[3 * S] = t2i + u2r;
+}
+
+__host__ __device__ constexpr int mod_inverse(int a, int m) {   // a^-1 mod m (a, m coprime, m small)
+    for (int x = 1; x < m; ++x)
+        if ((a * x) % m == 1) return x;
+    return 1;
+}
+
+// r = A * B with A in {2, 4}, B in {3, 5} coprime: Good-Thomas.  With n = (B n1 + A n2) mod r and k = k1 (mod A),
+// k = k2 (mod B):  X[k] = sum_n1 w_A^(n1 k1) sum_n2 w_B^(n2 k2) x[n]  -- no twiddles between the two passes.
+template <int r, int S>
+__device__ __forceinline__ void dft_pfa(double* re, double* im) {
+    constexpr int B = (r % 3 == 0) ? 3 : 5, A = r / B;
+    static_assert(A * B == r && (A == 2 || A == 4), "prime-factor radices: 6, 12, 10, 20");
+    double tr[r], ti[r];
+    // pass 1: B-point transforms over n2 for each n1; result k2 kept in the slot (n1, k2)
+#pragma unroll
+    for (int n1 = 0; n1 < A; ++n1) {
+        double ur[B], ui[B];
+#pragma unroll
+        for (int n2 = 0; n2 < B; ++n2) { ur[n2] = re[S * ((B * n1 + A * n2) % r)]; ui[n2] = im[S * ((B * n1 + A * n2) % r)]; }
+        if constexpr (B == 3) dft3<1>(ur, ui); else dft5<1>(ur, ui);
+#pragma unroll
+        for (int k2 = 0; k2 < B; ++k2) { tr[n1 * B + k2] = ur[k2]; ti[n1 * B + k2] = ui[k2]; }
+    }
+    // pass 2: A-point transforms over n1 for each k2; X[k] with k = k1 (mod A), k = k2 (mod B) by the CRT
+#pragma unroll
+    for (int k2 = 0; k2 < B; ++k2) {
+        double ur[A], ui[A];
+#pragma unroll
+        for (int n1 = 0; n1 < A; ++n1) { ur[n1] = tr[n1 * B + k2]; ui[n1] = ti[n1 * B + k2]; }
+        dft_pow2<A, 1>(ur, ui);
+#pragma unroll
+        for (int k1 = 0; k1 < A; ++k1) {
+            const int k = (k1 * B * mod_inverse(B % A, A) + k2 * A * mod_inverse(A % B, B)) % r;
+            re[S * k] = ur[k1]; im[S * k] = ui[k1];
+        }
+    }
+}
+
+template <int r, int S>
+__device__ __forceinline__ void dft_inplace(double* re, double* im) {
+    if constexpr (r == 3) dft3<S>(re, im);
+    else if constexpr (r == 5) dft5<S>(re, im);
+    else if constexpr (r == 6 || r == 12 || r == 10 || r == 20) dft_pfa<r, S>(re, im);
+    else dft_pow2<r, S>(re, im);
 }
 
 // ---- r-point DFT, strictly in place ------------------------------------------------------------
@@ -182,6 +263,22 @@ template <> struct FftCfg<128> : FftCfgT<128, 16, 16, 8, 1> {};
 template <> struct FftCfg<256> : FftCfgT<256, 16, 16, 16, 1> {};
 template <> struct FftCfg<512> : FftCfgT<512, 8, 8, 8, 8> {};
 template <> struct FftCfg<1024> : FftCfgT<1024, 16, 16, 16, 4> {};
+// 3 * 2^k and 5 * 2^k: power-of-two stages first (the scatter of a stage assumes that the radices
+// before it multiply to a power of two), the stage that carries the factor 3 or 5 last
+template <> struct FftCfg<6> : FftCfgT<6, 6, 6, 1, 1> {};
+template <> struct FftCfg<12> : FftCfgT<12, 12, 12, 1, 1> {};
+template <> struct FftCfg<24> : FftCfgT<24, 12, 2, 12, 1> {};
+template <> struct FftCfg<48> : FftCfgT<48, 12, 4, 12, 1> {};
+template <> struct FftCfg<96> : FftCfgT<96, 12, 4, 2, 12> {};
+template <> struct FftCfg<192> : FftCfgT<192, 12, 4, 4, 12> {};
+template <> struct FftCfg<384> : FftCfgT<384, 24, 8, 4, 12> {};
+template <> struct FftCfg<768> : FftCfgT<768, 24, 8, 8, 12> {};
+template <> struct FftCfg<10> : FftCfgT<10, 10, 10, 1, 1> {};
+template <> struct FftCfg<20> : FftCfgT<20, 20, 20, 1, 1> {};
+template <> struct FftCfg<40> : FftCfgT<40, 20, 2, 20, 1> {};
+template <> struct FftCfg<80> : FftCfgT<80, 20, 4, 20, 1> {};
+template <> struct FftCfg<160> : FftCfgT<160, 20, 4, 2, 20> {};
+template <> struct FftCfg<320> : FftCfgT<320, 20, 4, 4, 20> {};
 
 // ---- one stage: twiddle (if Ns > 1) and butterflies ----------------------------------------------
 // W: table of exp(-2 pi i n / LTAB), n < LTAB, in shared memory; LTAB a multiple of Ns*r.

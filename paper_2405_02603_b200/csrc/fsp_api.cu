@@ -420,6 +420,18 @@ int launch_inv_x(fsp_plan* p, double* phi, double kder) {
 
 #define DISPATCH_YZ(fn, M, ...)                          \
     switch (M) {                                         \
+        case 12: return fn<12>(__VA_ARGS__);             \
+        case 24: return fn<24>(__VA_ARGS__);             \
+        case 48: return fn<48>(__VA_ARGS__);             \
+        case 96: return fn<96>(__VA_ARGS__);             \
+        case 192: return fn<192>(__VA_ARGS__);           \
+        case 384: return fn<384>(__VA_ARGS__);           \
+        case 768: return fn<768>(__VA_ARGS__);           \
+        case 20: return fn<20>(__VA_ARGS__);             \
+        case 40: return fn<40>(__VA_ARGS__);             \
+        case 80: return fn<80>(__VA_ARGS__);             \
+        case 160: return fn<160>(__VA_ARGS__);           \
+        case 320: return fn<320>(__VA_ARGS__);           \
         case 8: return fn<8>(__VA_ARGS__);               \
         case 16: return fn<16>(__VA_ARGS__);             \
         case 32: return fn<32>(__VA_ARGS__);             \
@@ -432,6 +444,18 @@ int launch_inv_x(fsp_plan* p, double* phi, double kder) {
     }
 #define DISPATCH_X(fn, M, ...)                           \
     switch (M) {                                         \
+        case 6: return fn<6>(__VA_ARGS__);               \
+        case 12: return fn<12>(__VA_ARGS__);             \
+        case 24: return fn<24>(__VA_ARGS__);             \
+        case 48: return fn<48>(__VA_ARGS__);             \
+        case 96: return fn<96>(__VA_ARGS__);             \
+        case 192: return fn<192>(__VA_ARGS__);           \
+        case 384: return fn<384>(__VA_ARGS__);           \
+        case 10: return fn<10>(__VA_ARGS__);             \
+        case 20: return fn<20>(__VA_ARGS__);             \
+        case 40: return fn<40>(__VA_ARGS__);             \
+        case 80: return fn<80>(__VA_ARGS__);             \
+        case 160: return fn<160>(__VA_ARGS__);           \
         case 4: return fn<4>(__VA_ARGS__);               \
         case 8: return fn<8>(__VA_ARGS__);               \
         case 16: return fn<16>(__VA_ARGS__);             \
@@ -495,13 +519,89 @@ int do_fwd_y(fsp_plan* p, int kx0, double2* B2, int np) {
         case 1024: return fn<1024>(__VA_ARGS__);         \
         default: return FSP_ERR_INVALID_ARG;             \
     }
-int do_conv_z_w(fsp_plan* p, double2* B2, const double* G, int np, double2* out, const DerK* kap) { DISPATCH_W(launch_conv_z_w, p->Nz, p, B2, G, np, out, kap) }
+template <int M, bool DER>
+int launch_conv_z_g_impl(fsp_plan* p, double2* B2, const double* G, int nplanes, double2* out, const DerK kap) {
+    using Cfg = FftCfg<M>;
+    constexpr int GT = TileGroups<Cfg>::G;
+    const long npencils = (long)nplanes * (2 * p->Ny);
+    const size_t smem = sizeof(double2) * (size_t)(2 * M + GT * M * kW);
+    static OccCache cache;
+    int occ = 0;
+    { const int rc_ = cached_occupancy(cache, p->device, k_conv_z_g<M, DER>, GT * kW * Cfg::T, smem, &occ); if (rc_ != FSP_OK) return rc_; }
+    long grid = (npencils + (long)GT * kW - 1) / ((long)GT * kW);
+    if (grid > (long)p->sm_count * occ) grid = (long)p->sm_count * occ;
+    k_conv_z_g<M, DER><<<(unsigned)grid, GT * kW * Cfg::T, smem, p->stream>>>(B2, G, p->Wz, p->Ny, npencils, out, kap);
+    return FSP_OK;
+}
+template <int M>
+int launch_conv_z_g(fsp_plan* p, double2* B2, const double* G, int np, double2* out, const DerK* kap) {
+    if (kap) return launch_conv_z_g_impl<M, true>(p, B2, G, np, out, *kap);
+    return launch_conv_z_g_impl<M, false>(p, B2, G, np, nullptr, DerK{0.0, 0.0, 0.0, 0});
+}
+template <int M2, bool DER>
+int launch_conv_z_g2_impl(fsp_plan* p, double2* B2, const double* G, int nplanes, double2* out, const DerK kap) {
+    using Cfg = FftCfg<M2>;
+    constexpr int GT = TileGroups<Cfg>::G;
+    const long npencils = (long)nplanes * (2 * p->Ny);
+    const size_t smem = sizeof(double2) * (size_t)(M2 + GT * M2 * kW);
+    static OccCache cache;
+    int occ = 0;
+    { const int rc_ = cached_occupancy(cache, p->device, k_conv_z_g2<M2, DER>, GT * kW * Cfg::T, smem, &occ); if (rc_ != FSP_OK) return rc_; }
+    long grid = (npencils + (long)GT * kW - 1) / ((long)GT * kW);
+    if (grid > (long)p->sm_count * occ) grid = (long)p->sm_count * occ;
+    k_conv_z_g2<M2, DER><<<(unsigned)grid, GT * kW * Cfg::T, smem, p->stream>>>(B2, G, p->Wz, p->Ny, npencils, out, kap);
+    return FSP_OK;
+}
+template <int M2>
+int launch_conv_z_g2(fsp_plan* p, double2* B2, const double* G, int np, double2* out, const DerK* kap) {
+    if (kap) return launch_conv_z_g2_impl<M2, true>(p, B2, G, np, out, *kap);
+    return launch_conv_z_g2_impl<M2, false>(p, B2, G, np, nullptr, DerK{0.0, 0.0, 0.0, 0});
+}
+bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+// Nz = 3 * 2^k, 5 * 2^k whose doubled length has an engine configuration: k_conv_z_g2 (natural-order spectrum rows)
+bool z_uses_g2(int Nz) { return Nz == 24 || Nz == 48 || Nz == 96 || Nz == 192 || Nz == 384 || Nz == 40 || Nz == 80 || Nz == 160; }
+int do_conv_z_w(fsp_plan* p, double2* B2, const double* G, int np, double2* out, const DerK* kap) {
+    if (!is_pow2(p->Nz)) {   // 3 * 2^k, 5 * 2^k: the CTA-level kernels on the mixed-radix engine
+        if (p->gk_natural) {
+            switch (p->Nz) {
+                case 24: return launch_conv_z_g2<48>(p, B2, G, np, out, kap);
+                case 48: return launch_conv_z_g2<96>(p, B2, G, np, out, kap);
+                case 96: return launch_conv_z_g2<192>(p, B2, G, np, out, kap);
+                case 192: return launch_conv_z_g2<384>(p, B2, G, np, out, kap);
+                case 384: return launch_conv_z_g2<768>(p, B2, G, np, out, kap);
+                case 40: return launch_conv_z_g2<80>(p, B2, G, np, out, kap);
+                case 80: return launch_conv_z_g2<160>(p, B2, G, np, out, kap);
+                case 160: return launch_conv_z_g2<320>(p, B2, G, np, out, kap);
+                default: return FSP_ERR_INVALID_ARG;
+            }
+        }
+        switch (p->Nz) {
+            case 12: return launch_conv_z_g<12>(p, B2, G, np, out, kap);
+            case 24: return launch_conv_z_g<24>(p, B2, G, np, out, kap);
+            case 48: return launch_conv_z_g<48>(p, B2, G, np, out, kap);
+            case 96: return launch_conv_z_g<96>(p, B2, G, np, out, kap);
+            case 192: return launch_conv_z_g<192>(p, B2, G, np, out, kap);
+            case 384: return launch_conv_z_g<384>(p, B2, G, np, out, kap);
+            case 768: return launch_conv_z_g<768>(p, B2, G, np, out, kap);
+            case 20: return launch_conv_z_g<20>(p, B2, G, np, out, kap);
+            case 40: return launch_conv_z_g<40>(p, B2, G, np, out, kap);
+            case 80: return launch_conv_z_g<80>(p, B2, G, np, out, kap);
+            case 160: return launch_conv_z_g<160>(p, B2, G, np, out, kap);
+            case 320: return launch_conv_z_g<320>(p, B2, G, np, out, kap);
+            default: return FSP_ERR_INVALID_ARG;
+        }
+    }
+    DISPATCH_W(launch_conv_z_w, p->Nz, p, B2, G, np, out, kap)
+}
 // planes [kx0, kx0 + np) of the spectrum go with the np planes stored at B2.
 // kap == nullptr: in place (phi); otherwise B2 -> out with the derivative factor (whole volume only, kx0 = 0).
 int do_conv_z(fsp_plan* p, double2* B2, int kx0, int np, double2* out = nullptr, const DerK* kap = nullptr) {
     return do_conv_z_w(p, B2, p->Gk + (size_t)kx0 * (p->Ny + 1) * (p->Nz + 2), np, out, kap);
 }
-int make_z_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Nz, &p->LTz, &p->bytes) }
+int make_z_lane_table(fsp_plan* p) {
+    if (!is_pow2(p->Nz)) return FSP_OK;   // k_conv_z_g reads the root table only
+    DISPATCH_W(lane_table_for, p->Nz, &p->LTz, &p->bytes)
+}
 int make_x_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Nx / 2, &p->LTx, &p->bytes) }
 int make_y_lane_table(fsp_plan* p) { DISPATCH_W(lane_table_for, p->Ny, &p->LTy, &p->bytes) }
 template <int M, bool DER>
@@ -593,6 +693,16 @@ int crop_out(fsp_plan* p, double* dst_user) {          // dst <- phi_pad restric
     return FSP_OK;
 }
 int next_pow2_min8(int n) { int q = 8; while (q < n) q *= 2; return q; }
+// smallest transform length >= n that has kernels: 2^k, 3 * 2^k, 5 * 2^k between 8 and 1024.
+// pow2_only: the plain Vico-Greengard precompute (its 4N-point FFTs are power-of-two code)
+// z_axis: the kernels bundle 8 adjacent z columns, so Nz must be a multiple of 8 (12 and 20 are x / y lengths only)
+int next_supported_size(int n, bool pow2_only, bool z_axis) {
+    if (pow2_only) return next_pow2_min8(n);
+    static const int sizes[] = {8, 12, 16, 20, 24, 32, 40, 48, 64, 80, 96, 128, 160, 192, 256, 320, 384, 512, 768, 1024};
+    for (int s : sizes)
+        if (s >= n && !(z_axis && s % 8 != 0)) return s;
+    return 1024;
+}
 
 // batched DCT-I along one axis of a real 3-D array (C order), output pruned to nout along that axis.
 // fill != nullptr (axis 2 only): the input array does not exist, its values are G_L evaluated inside the kernel.
@@ -618,6 +728,25 @@ int dct1_axis(fsp_plan* p, const double* in, double* out, const long in_dims[3],
     const int o1 = (axis + 1) % 3, o2 = (axis + 2) % 3;
     const long n1 = in_dims[o1], n2 = in_dims[o2];
     const int Lf = 2 * n;
+    if ((n & (n - 1)) != 0) {   // not a power of two: the cosine sum as written (k_dct1_direct)
+        const int bdim = axis == 2 ? 1 : 2, adim = axis == 2 ? 0 : (axis == 0 ? 1 : 0);
+        const long nA = in_dims[adim], nB = in_dims[bdim];
+        const long ai[3] = {is[adim], is[bdim], is[axis]}, ao[3] = {os[adim], os[bdim], os[axis]};
+        constexpr int C = 8;
+        const size_t smem = sizeof(double) * ((size_t)2 * n + (size_t)(n + 1) * C);
+        if (smem > 200 * 1024) return FSP_ERR_INVALID_ARG;
+        if (fill) {
+            { static OccCache optin; const int rc_ = cached_smem_optin(optin, p->device, k_dct1_direct<C, true>, smem); if (rc_ != FSP_OK) return rc_; }
+            k_dct1_direct<C, true><<<(unsigned)(nA * ((nB + C - 1) / C)), 256, smem, p->stream>>>(
+                in, out, n, nout, nB, ai[0], ai[1], ai[2], ao[0], ao[1], ao[2], scale, *fill);
+        } else {
+            { static OccCache optin; const int rc_ = cached_smem_optin(optin, p->device, k_dct1_direct<C, false>, smem); if (rc_ != FSP_OK) return rc_; }
+            k_dct1_direct<C, false><<<(unsigned)(nA * ((nB + C - 1) / C)), 256, smem, p->stream>>>(
+                in, out, n, nout, nB, ai[0], ai[1], ai[2], ao[0], ao[1], ao[2], scale, GLFill{0.0, 0.0, 0.0, 0.0, 0});
+        }
+        CU(cudaGetLastError());
+        return FSP_OK;
+    }
     {   // tile kernel: C pencils per CTA along the contiguous dimension (z; y when the transform axis is z)
         const int bdim = axis == 2 ? 1 : 2, adim = axis == 2 ? 0 : (axis == 0 ? 1 : 0);
         const long nA = in_dims[adim], nB = in_dims[bdim];
@@ -749,7 +878,7 @@ int precompute_impl(fsp_plan* p) {
             // chunk to b[kx][dy][dz] (workspace B2), the x pass b -> T.  No transient memory when the workspace holds
             // a plane of a and the whole of b (always for the paper's m = 4), else it is allocated.
             const long Kx = nx + 1L, Ky = ny + 1L;
-            if (sizeof(double2) * 5 * (size_t)nz > 200 * 1024) {
+            if ((nz & (nz - 1)) == 0 && sizeof(double2) * 5 * (size_t)nz > 200 * 1024) {
                 // the z transform is too long for the tile kernels (m_z N_z > 5120): the unfused route, lattice in memory
                 const long fd[3] = {nx + 1L, ny + 1L, nz + 1L};
                 const long ad[3] = {fd[0], fd[1], Nz + 1};
@@ -816,7 +945,7 @@ int precompute_impl(fsp_plan* p) {
         // (a sharded plan keeps the rows of its own kx planes only)
         const long gk_total = (long)p->planes * (Ny + 1) * (Nz + 2);
         const double* goct = p->Goct + (size_t)p->kx0 * (Ny + 1) * (Nz + 1);
-        p->gk_natural = (Nz == 256 || Nz == 512) && p->k3_variant == 0;
+        p->gk_natural = (Nz == 256 || Nz == 512 || z_uses_g2(Nz)) && p->k3_variant == 0;
         if (p->gk_natural) k_layout_spectrum_nat<<<grid_for(gk_total, blk), blk, 0, p->stream>>>(goct, p->Gk, p->planes - 1, Ny, Nz, gscale);
         else k_layout_spectrum_oct<<<grid_for(gk_total, blk), blk, 0, p->stream>>>(goct, p->Gk, p->planes - 1, Ny, Nz, gscale);
     }
@@ -872,8 +1001,9 @@ static int plan_create_impl(fsp_plan** out, int Nx, int Ny, int Nz, const double
     if (!std::isfinite(h[0]) || !std::isfinite(h[1]) || !std::isfinite(h[2])) return FSP_ERR_INVALID_ARG;
     if (Nx < 2 || Ny < 2 || Nz < 2 || Nx > 1024 || Ny > 1024 || Nz > 1024) return FSP_ERR_INVALID_ARG;
     const int Ux = Nx, Uy = Ny, Uz = Nz;
-    // the transforms are power-of-two: any other mesh is embedded in the next one (R19)
-    Nx = next_pow2_min8(Ux); Ny = next_pow2_min8(Uy); Nz = next_pow2_min8(Uz);
+    // transform lengths are 2^k, 3 * 2^k or 5 * 2^k: any other mesh is embedded in the next such mesh (R19)
+    Nx = next_supported_size(Ux, algorithm == FSP_VICO, false); Ny = next_supported_size(Uy, algorithm == FSP_VICO, false);
+    Nz = next_supported_size(Uz, algorithm == FSP_VICO, true);
     if (algorithm != FSP_HOCKNEY && algorithm != FSP_VICO && algorithm != FSP_VICO_2 && algorithm != FSP_VICO_SAFE) return FSP_ERR_INVALID_ARG;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {

@@ -217,6 +217,52 @@ __global__ void k_dct1_tile(const double* __restrict__ in, double* __restrict__ 
     }
 }
 
+// DCT-I of pencils whose length is not a power of two (meshes 3 * 2^k, 5 * 2^k): the cosine sum as
+// written, out[d] = sum_k w_k in[k] cos(pi k d / n), O(n * nout) per pencil -- a once-per-plan step on meshes the
+// paper never uses; the cosines come from a shared-memory table cos(pi m / n), m < 2n, indexed by (k d) mod 2n.
+// Same tile geometry and FILL option as k_dct1_tile; shared memory: [table: 2n doubles][input: (n+1) * C doubles].
+template <int C, bool FILL = false>
+__global__ void k_dct1_direct(const double* __restrict__ in, double* __restrict__ out, int n, int nout, long nB,
+                              long sA_in, long sB_in, long sK_in, long sA_out, long sB_out, long sK_out,
+                              double scale, const GLFill gl) {
+    extern __shared__ double smd[];
+    double* ct = smd;               // 2n
+    double* x = smd + 2 * n;        // (n + 1) * C, [k][c]
+    const long tilesB = (nB + C - 1) / C;
+    const long ia = blockIdx.x / tilesB, b0 = (blockIdx.x % tilesB) * C;
+    const int nc = (int)(nB - b0 < C ? nB - b0 : C);
+    const double* src = in + ia * sA_in + b0 * sB_in;
+    double* dst = out + ia * sA_out + b0 * sB_out;
+    for (int m = threadIdx.x; m < 2 * n; m += blockDim.x) ct[m] = cospi((double)m / (double)n);
+    const int total = (n + 1) * C;
+    for (int e = threadIdx.x; e < total; e += blockDim.x) {
+        int k, c;
+        if (sK_in == 1) { k = e % (n + 1); c = e / (n + 1); }
+        else { c = e % C; k = e / C; }
+        double v = 0.0;
+        if (c < nc) {
+            if constexpr (FILL) v = vg_GL(gl.sa * (double)(gl.a0 + ia), gl.sb * (double)(b0 + c), gl.sk * (double)k, gl.L);
+            else v = src[(long)c * sB_in + (long)k * sK_in];
+        }
+        x[k * C + c] = (k == 0 || k == n) ? v : 2.0 * v;   // endpoint weight 1, interior weight 2
+    }
+    __syncthreads();
+    const int ototal = nout * C;
+    for (int e = threadIdx.x; e < ototal; e += blockDim.x) {
+        int d, c;
+        if (sK_out == 1) { d = e % nout; c = e / nout; }
+        else { c = e % C; d = e / C; }
+        double acc = 0.0;
+        int idx = 0;   // (k d) mod 2n
+        for (int k = 0; k <= n; ++k) {
+            acc = fma(x[k * C + c], ct[idx], acc);
+            idx += d;
+            if (idx >= 2 * n) idx -= 2 * n;
+        }
+        if (c < nc) dst[(long)c * sB_out + (long)d * sK_out] = scale * acc;
+    }
+}
+
 // Unscaled inverse complex DFT (sign +) of length Lf along one axis for a TILE of C adjacent pencils per CTA, in
 // place or out of place (plain VG, y and z axes of the half-spectrum lattice).  Same tiling as k_dct1_tile: the C
 // pencils are adjacent along the contiguous dimension, so the strided axes are read and written in full sectors

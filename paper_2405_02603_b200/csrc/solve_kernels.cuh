@@ -366,6 +366,135 @@ k_inv_y_t(const __grid_constant__ CUtensorMap tmB2, double2* __restrict__ B1, co
     }
 }
 
+// ============================================================ K3 for any supported Nz (3 * 2^k, 5 * 2^k): conv_z_g
+// CTA-level kernel on the register engine of fft_engine.cuh (any radix mix), used where the warp-level kernels do
+// not apply (Nz not a power of two).  Tile = kW pencils that follow one another in memory (pencil
+// q = (kx, ky), M contiguous points each); thread (c, t) = (pencil of the tile, lane of the pencil), c fastest, so
+// that the exchange buffer [position][kW] is conflict free.  Per pencil: both half-spectrum branches one after the
+// other (even: FFT_M(x); odd: FFT_M(x w^n)), times the octant spectrum row [E | O], inverse, y = y_e + conj(w^n) y_o.
+template <int M, bool DER = false>
+__global__ void __launch_bounds__(TileGroups<FftCfg<M>>::G* kW* FftCfg<M>::T)
+k_conv_z_g(double2* __restrict__ B2, const double* __restrict__ Gk, const double2* __restrict__ Wg, int Ny,
+           long npencils, double2* __restrict__ out, const DerK kap) {
+    using Cfg = FftCfg<M>;
+    constexpr int R = Cfg::R, T = Cfg::T, G = TileGroups<Cfg>::G, LTAB = 2 * M, ROW = M + 2;
+    extern __shared__ double2 smem[];
+    double2* Ws = smem;                 // LTAB: exp(-2 pi i n / 2M)
+    double2* xb = smem + LTAB;          // G * M * kW
+    load_table<LTAB>(Ws, Wg);
+    const int tid = threadIdx.x;
+    const int g = tid / (kW * T), lt = tid % (kW * T);
+    const int c = lt % kW, t = lt / kW;
+    double2* buf = xb + g * (M * kW) + c;
+    const int ny2 = 2 * Ny;
+    __syncthreads();
+    for (long tile0 = (long)blockIdx.x * G; tile0 * kW < npencils; tile0 += (long)gridDim.x * G) {
+        const long q = (tile0 + g) * kW + c;
+        const bool valid = q < npencils;
+        const int kx = valid ? (int)(q / ny2) : 0, ky = valid ? (int)(q % ny2) : 0;
+        const int qy = ky <= Ny ? ky : ny2 - ky;
+        double2* base = B2 + (valid ? q : 0) * M;
+        double2* obase = DER ? out + (valid ? q : 0) * M : base;
+        const double* grow = Gk + ((long)kx * (Ny + 1) + qy) * ROW;
+        double fp = 0.0;
+        if constexpr (DER) fp = kap.x * signed_mode(kx, kap.Nx) + kap.y * signed_mode(ky, Ny);
+        double xr[R], xi[R], vr[R], vi[R];
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            const double2 v = valid ? base[t + T * i] : make_double2(0.0, 0.0);
+            xr[i] = v.x; xi[i] = v.y; vr[i] = v.x; vi[i] = v.y;
+        }
+        // even branch: Y_e[j] = Ghat[2j] FFT_M(x)[j], y_e = IFFT_M(Y_e) (kept in vr, vi)
+        fft_forward<Cfg, kW, LTAB>(vr, vi, t, buf, Ws);
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            const int j = t + T * i;
+            double gk = __ldg(grow + (j <= M - j ? j : M - j));
+            if constexpr (DER) gk *= fp + kap.z * signed_mode(2 * j, M);
+            vr[i] *= gk; vi[i] *= gk;
+        }
+        fft_inverse<Cfg, kW, LTAB>(vr, vi, t, buf, Ws);
+        // odd branch: x[n] w^n, Y_o[j] = Ghat[2j+1] FFT_M(.)[j], y_o = IFFT_M(Y_o)
+#pragma unroll
+        for (int i = 0; i < R; ++i) cmul(xr[i], xi[i], Ws[t + T * i]);
+        fft_forward<Cfg, kW, LTAB>(xr, xi, t, buf, Ws);
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            const int j = t + T * i;
+            double gk = __ldg(grow + M / 2 + 1 + (j <= M - 1 - j ? j : M - 1 - j));
+            if constexpr (DER) gk *= fp + kap.z * signed_mode(2 * j + 1, M);
+            xr[i] *= gk; xi[i] *= gk;
+        }
+        fft_inverse<Cfg, kW, LTAB>(xr, xi, t, buf, Ws);
+        if (valid) {
+#pragma unroll
+            for (int i = 0; i < R; ++i) {
+                cmul_conj(xr[i], xi[i], Ws[t + T * i]);
+                const double yr = vr[i] + xr[i], yi = vi[i] + xi[i];
+                obase[t + T * i] = DER ? make_double2(yi, -yr) : make_double2(yr, yi);   // DER: -i y
+            }
+        }
+    }
+}
+
+// ================================================ K3 for Nz = 3 * 2^k, 5 * 2^k with a kernel of length 2 Nz: conv_z_g2
+// The same tile scheme as k_conv_z_g, but each pencil is transformed as ONE zero-padded sequence of M2 = 2 Nz points
+// (forward, times Ghat in natural order, inverse, first half kept) instead of two half-length branches each way:
+// one register set instead of two (no spills at R = 24), no pre-twiddle, no final sum.  The zero half is fed to the
+// first stage as zeros and the discarded half is computed and dropped (the engine's stages are generic; the pruned
+// first / last radix-2 levels of k_conv_z_f do not exist for these radices).
+template <int M2, bool DER = false>
+__global__ void __launch_bounds__(TileGroups<FftCfg<M2>>::G* kW* FftCfg<M2>::T)
+k_conv_z_g2(double2* __restrict__ B2, const double* __restrict__ Gk, const double2* __restrict__ Wg, int Ny,
+            long npencils, double2* __restrict__ out, const DerK kap) {
+    using Cfg = FftCfg<M2>;
+    constexpr int R = Cfg::R, T = Cfg::T, G = TileGroups<Cfg>::G, LTAB = M2, M = M2 / 2, ROW = M + 2;
+    extern __shared__ double2 smem[];
+    double2* Ws = smem;                 // LTAB: exp(-2 pi i n / M2)
+    double2* xb = smem + LTAB;          // G * M2 * kW
+    load_table<LTAB>(Ws, Wg);
+    const int tid = threadIdx.x;
+    const int g = tid / (kW * T), lt = tid % (kW * T);
+    const int c = lt % kW, t = lt / kW;
+    double2* buf = xb + g * (M2 * kW) + c;
+    const int ny2 = 2 * Ny;
+    __syncthreads();
+    for (long tile0 = (long)blockIdx.x * G; tile0 * kW < npencils; tile0 += (long)gridDim.x * G) {
+        const long q = (tile0 + g) * kW + c;
+        const bool valid = q < npencils;
+        const int kx = valid ? (int)(q / ny2) : 0, ky = valid ? (int)(q % ny2) : 0;
+        const int qy = ky <= Ny ? ky : ny2 - ky;
+        double2* base = B2 + (valid ? q : 0) * M;
+        double2* obase = DER ? out + (valid ? q : 0) * M : base;
+        const double* grow = Gk + ((long)kx * (Ny + 1) + qy) * ROW;
+        double fp = 0.0;
+        if constexpr (DER) fp = kap.x * signed_mode(kx, kap.Nx) + kap.y * signed_mode(ky, Ny);
+        double vr[R], vi[R];
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            const int n = t + T * i;
+            const double2 v = (valid && n < M) ? base[n] : make_double2(0.0, 0.0);
+            vr[i] = v.x; vi[i] = v.y;
+        }
+        fft_forward<Cfg, kW, LTAB>(vr, vi, t, buf, Ws);
+#pragma unroll
+        for (int i = 0; i < R; ++i) {
+            const int kz = t + T * i;
+            double gk = __ldg(grow + (kz <= M ? kz : M2 - kz));
+            if constexpr (DER) gk *= fp + kap.z * signed_mode(kz, M);
+            vr[i] *= gk; vi[i] *= gk;
+        }
+        fft_inverse<Cfg, kW, LTAB>(vr, vi, t, buf, Ws);
+        if (valid) {
+#pragma unroll
+            for (int i = 0; i < R; ++i) {
+                const int n = t + T * i;
+                if (n < M) obase[n] = DER ? make_double2(vi[i], -vr[i]) : make_double2(vr[i], vi[i]);   // DER: -i y
+            }
+        }
+    }
+}
+
 // ============================================================================== K3 (v2): conv_z_w
 // One pencil per group of 2T lanes of a warp: lanes with b = 0 run the even
 // half-spectrum branch, lanes with b = 1 the odd one, each a two-stage single-exchange FFT of
@@ -1269,7 +1398,7 @@ k_fwd_x_r2c(const double* __restrict__ rho, double2* __restrict__ B1, const doub
             for (int o = 0; o < 2; ++o) {
                 const int k = 2 * (t + T * i) + o;
                 const double2 a = Z[k * kW];
-                const double2 bq = Z[((N - k) & (N - 1)) * kW];
+                const double2 bq = Z[(k == 0 ? 0 : N - k) * kW];
                 const double br = bq.x, bi = -bq.y;            // B = conj(Z[N-k])
                 const double sr = a.x + br, si = a.y + bi;     // A + B
                 double dr = a.x - br, di = a.y - bi;           // A - B

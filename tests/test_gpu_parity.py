@@ -335,11 +335,20 @@ def test_degenerate_densities(N):
 
 
 # ---------------------------------------------------------------- any mesh size (R19)
+SIZES = (8, 12, 16, 20, 24, 32, 40, 48, 64, 80, 96, 128, 160, 192, 256, 320, 384, 512, 768, 1024)
+
+
+def transform_mesh(N):
+    """The mesh the transforms run on (include/fsp.h): per axis the next length 2^k, 3 * 2^k or 5 * 2^k >= max(N_d, 8);
+    Nz a multiple of 8."""
+    return tuple(next(s for s in SIZES if s >= n and not (d == 2 and s % 8)) for d, n in enumerate(N))
+
+
 def _ref_on_enclosing_box(alg, N, h, rho):
-    """R19: the transforms run on the next power-of-two mesh N' >= max(N, 8).  The convolution on the caller's
+    """R19: the transforms run on the next supported mesh N' >= max(N, 8) (2^k, 3 * 2^k, 5 * 2^k).  The convolution on the caller's
     mesh needs the table at displacements below N only, so the reference is the paper's steps 1-5 on the 2N grid
     (oracle O2, direct DFT for these lengths) with the table of the enclosing box -- for HE the very same table."""
-    Np = tuple(max(8, 1 << (n - 1).bit_length()) for n in N)
+    Np = transform_mesh(N)
     T = oracle.green_table(alg, Np, h)[: N[0] + 1, : N[1] + 1, : N[2] + 1].copy()
     return T, oracle.solve_with_spectrum(oracle.green_spectrum(T), h, rho)
 
@@ -386,7 +395,8 @@ def test_any_mesh_size_field_and_accuracy():
         _, E2 = p.solve_field(torch.from_numpy(w2.rho).cuda(), want_phi=False)
         E2 = E2.cpu().numpy()
     # the spectral gradient lives on the transform mesh (period 2 N' h): reference = oracle on the embedded density
-    Np = (32, 16, 64)
+    Np = transform_mesh((20, 12, 36))
+    assert Np == (20, 12, 40)
     emb = np.zeros(Np)
     emb[:20, :12, :36] = w2.rho
     _, Eo = oracle.OraclePlan(Np, w2.h, oracle.HOCKNEY).precompute_green().solve_field(emb)
@@ -448,3 +458,37 @@ def test_plans_on_two_devices_from_one_process():
         torch.cuda.synchronize(dev)
         check(phi.cpu().numpy(), ref)
         p.destroy()
+
+
+# ---------------------------------------------------------------- mixed-radix meshes
+@pytest.mark.parametrize("alg", ["HE", "VG2"])
+@pytest.mark.parametrize("N", [(96, 96, 96), (384, 48, 24), (40, 80, 160), (12, 20, 24), (24, 12, 40), (192, 24, 48),
+                               (20, 320, 8), (768, 8, 8), (8, 768, 8), (8, 8, 768), (8, 16, 320), (48, 16, 80), (160, 8, 192)])
+def test_mixed_radix_meshes_run_natively_on_the_callers_mesh(N, alg):
+    """N_d = 3 * 2^k, 5 * 2^k: radix-3 / radix-5 stages (prime-factor butterflies 6, 12, 10, 20) instead of embedding in
+    the next power of two; reference = the oracle ON THE CALLER'S MESH (its direct O(n^2) DFT; for VG the table of
+    the caller's box: the paper's result, no enclosing-box reading needed)."""
+    assert transform_mesh(N) == tuple(N)
+    w = W.random_density(N, seed=sum(N) + 7)
+    with binding.Plan(w.N, w.h, ALGS[alg][0]) as p:
+        p.precompute_green()
+        got = gpu_solve(p, w.rho)
+        T = p.green_table()
+        G = p.green_spectrum()      # native mesh: the spectrum is available (not an embedded plan)
+    op = oracle.OraclePlan(w.N, w.h, ALGS[alg][1]).precompute_green()
+    assert np.abs(T - op.T).max() <= 1e-13 * np.abs(op.T).max()
+    Go = op.Ghat.real[: N[0] + 1, : N[1] + 1, : N[2] + 1]
+    assert np.abs(G - Go).max() <= 1e-12 * np.abs(Go).max()
+    check(got, op.solve(w.rho))
+
+
+def test_mixed_radix_field_output():
+    w = W.random_density((48, 40, 24), seed=5)
+    with binding.Plan(w.N, w.h, binding.HOCKNEY) as p:
+        p.precompute_green()
+        phi, E = p.solve_field(torch.from_numpy(w.rho).cuda())
+        phi, E = phi.cpu().numpy(), E.cpu().numpy()
+    phi_o, E_o = oracle.OraclePlan(w.N, w.h, oracle.HOCKNEY).precompute_green().solve_field(w.rho)
+    check(phi, phi_o)
+    for d in range(3):
+        check(E[d], E_o[d])
