@@ -82,7 +82,10 @@ enum {
                             has to exceed the largest displacement), else FSP_ERR_INVALID_ARG       */
     FSP_PARAM_CHUNK_PLANES = 2, /* kx-planes per pass of the y-z-y middle (0 = all at once); takes
                                   effect at the next fsp_solve; does not change results             */
-    FSP_PARAM_K3_VARIANT = 3 /* kernel of the z pass at Nz = 256, 512 (kept for A/B measurements): 0 (default) =
+    FSP_PARAM_K2_VARIANT = 4, /* kernel of the forward y pass at Ny = 512 (kept for A/B measurements): 0 (default) = the
+                                zero-padded column of 2 Ny points in one group (k_fwd_y_f); 1 = two half-length
+                                branches in two groups (k_fwd_y_t).  Takes effect at the next fsp_solve          */
+    FSP_PARAM_K3_VARIANT = 3, /* kernel of the z pass at Nz = 256, 512 (kept for A/B measurements): 0 (default) =
                                 the whole zero-padded pencil in one lane group (k_conv_z_f); 1 = two half-
                                 length branches in a warp pair (k_conv_z_p); 2 (Nz = 512) = the pair scheme
                                 with 32 lanes per branch (k_conv_z_s).  Invalidates the spectrum (its row

@@ -239,14 +239,16 @@ __device__ __forceinline__ void fft512s_forward(double (&re)[16], double (&im)[1
 // E[position][CW] (conflict free without padding) and every global access a full line.  The T lanes of
 // a column sit in different warps, so the two syncs are named barriers over the group.
 // Ec = E + c;  bar_id: the group's barrier.
-template <class Cfg, int CW>
+// LO1 = 4: the first radix-2 level of stage 1 is skipped (zero-padded input: the caller has put x_i into the register
+// of x_(i + R1/2) = 0, see fft2_padded_pass).
+template <class Cfg, int CW, int LO1 = 2>
 __device__ __forceinline__ void fft2_forward_tile(double (&re)[Cfg::R], double (&im)[Cfg::R], int t,
                                                   double2* __restrict__ Ec, int bar_id,
                                                   const double (&cc)[Cfg::NB2][LaneTw<Cfg::R2>::NC],
                                                   const double (&tn)[Cfg::NB2][LaneTw<Cfg::R2>::NC]) {
     constexpr int R = Cfg::R, R1 = Cfg::R1, R2 = Cfg::R2, T = Cfg::T, NB1 = Cfg::NB1, NB2 = Cfg::NB2;
 #pragma unroll
-    for (int m = 0; m < NB1; ++m) dft_br<R1, NB1>(&re[m], &im[m]);
+    for (int m = 0; m < NB1; ++m) dft_br<R1, NB1, LO1, R1>(&re[m], &im[m]);
     bar_sync(bar_id, CW * T);  // earlier readers of E are done
 #pragma unroll
     for (int m = 0; m < NB1; ++m) {

@@ -47,6 +47,8 @@ struct fsp_plan {
     size_t b1_count = 0, b2_count = 0;   // complex elements allocated in B1, B2
     bool gk_natural = false; // Gk rows in natural order (k_conv_z_f) instead of [E | O] (decided by the last precompute)
     double* LTy = nullptr;  // the same for the y transform (tile kernels)
+    double* LTyf = nullptr; // Ny = 512: stage-2 constants of the padded 1024-point y transform (k_fwd_y_f)
+    int k2_variant = 0;     // FSP_PARAM_K2_VARIANT
     bool tile_y = false;    // K2/K4 tile kernels (TMA-staged) are used
     double* LTx = nullptr;  // lane-constant twiddles of the x transform (length Nx/2)
     bool tile_x = false;    // K1 tile kernel is used
@@ -285,6 +287,19 @@ int launch_fwd_y_t(fsp_plan* p, int kx0, double2* B2, int nplanes) {
     k_fwd_y_t<M><<<(unsigned)grid, Y::THREADS, smem, p->stream>>>(p->tmB1y, B2, p->LTy, p->Wy, p->Nz, kx0, ntiles);
     return FSP_OK;
 }
+template <int M2>
+int launch_fwd_y_f(fsp_plan* p, int kx0, double2* B2, int nplanes) {
+    using Y = TileYF<M2>;
+    const long ntiles = (long)nplanes * (p->Nz / Y::KW);
+    const size_t smem = Y::smem_bytes();
+    static OccCache cache;
+    int occ = 0;
+    { const int rc_ = cached_occupancy(cache, p->device, k_fwd_y_f<M2>, Y::THREADS, smem, &occ); if (rc_ != FSP_OK) return rc_; }
+    long grid = (long)p->sm_count * occ;
+    if (grid > ntiles) grid = ntiles;
+    k_fwd_y_f<M2><<<(unsigned)grid, Y::THREADS, smem, p->stream>>>(p->tmB1y, B2, p->LTyf, p->Nz, kx0, ntiles);
+    return FSP_OK;
+}
 template <int M>
 int launch_fwd_y(fsp_plan* p, const double2* B1, double2* B2, int nplanes) {
     using Cfg = FftCfg<M>;
@@ -500,6 +515,7 @@ int do_fwd_x(fsp_plan* p, const double* rho) {
 int do_fwd_y(fsp_plan* p, int kx0, double2* B2, int np) {
     if (p->tile_y) {
         if (p->Ny == 1024) return launch_fwd_y_t<1024>(p, kx0, B2, np);
+        if (p->Ny == 512 && p->k2_variant == 0) return launch_fwd_y_f<1024>(p, kx0, B2, np);
         if (p->Ny == 512) return launch_fwd_y_t<512>(p, kx0, B2, np);
         if (p->Ny == 256) return launch_fwd_y_t<256>(p, kx0, B2, np);
         return launch_fwd_y_t<128>(p, kx0, B2, np);
@@ -956,7 +972,7 @@ int precompute_impl(fsp_plan* p) {
 }
 
 void free_plan_memory(fsp_plan* p) {
-    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->B3); cudaFree(p->rho_pad); cudaFree(p->phi_pad); cudaFree(p->E_stage); cudaFree(p->rho_stage2); cudaFree(p->phi_stage2); cudaFree(p->Gk); cudaFree(p->LTz); cudaFree(p->LTzs); cudaFree(p->LTzf); cudaFree(p->LTy); cudaFree(p->LTx); cudaFree(p->T); cudaFree(p->Goct);
+    cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->B3); cudaFree(p->rho_pad); cudaFree(p->phi_pad); cudaFree(p->E_stage); cudaFree(p->rho_stage2); cudaFree(p->phi_stage2); cudaFree(p->Gk); cudaFree(p->LTz); cudaFree(p->LTzs); cudaFree(p->LTzf); cudaFree(p->LTy); cudaFree(p->LTyf); cudaFree(p->LTx); cudaFree(p->T); cudaFree(p->Goct);
     cudaFree(p->Wx); cudaFree(p->Wy); cudaFree(p->Wz); cudaFree(p->rho_stage); cudaFree(p->phi_stage);
     for (cudaEvent_t e : p->events) cudaEventDestroy(e);
     p->events.clear();
@@ -1055,6 +1071,7 @@ static int plan_create_impl(fsp_plan** out, int Nx, int Ny, int Nz, const double
     p->tile_y = want_yz && (Ny == 128 || Ny == 256 || Ny == 512 || Ny == 1024) && Nz >= kW;
     const cuuint32_t kwy = Ny == 1024 ? 4 : kW;   // TileY<M>::KW: columns per tile of the y tile kernels
     if (rc == FSP_OK && p->tile_y) rc = make_y_lane_table(p);
+    if (rc == FSP_OK && p->tile_y && Ny == 512) rc = lane_table_for<1024>(&p->LTyf, &p->bytes);
     if (rc == FSP_OK && p->tile_y) {
         const cuuint64_t dims[3] = {(cuuint64_t)2 * Nz, (cuuint64_t)Ny, (cuuint64_t)planes};
         const cuuint64_t strides[2] = {(cuuint64_t)Nz * 16, (cuuint64_t)Ny * Nz * 16};
@@ -1091,6 +1108,11 @@ int fsp_plan_set_param(fsp_plan* p, int which, double value) {
     if (which == FSP_PARAM_CHUNK_PLANES) {
         if (value < 0.0 || value > 4096.0) return FSP_ERR_INVALID_ARG;
         p->chunk_planes = (int)value;
+        return FSP_OK;
+    }
+    if (which == FSP_PARAM_K2_VARIANT) {
+        if (value != 0.0 && value != 1.0) return FSP_ERR_INVALID_ARG;
+        p->k2_variant = (int)value;
         return FSP_OK;
     }
     if (which == FSP_PARAM_K3_VARIANT) {

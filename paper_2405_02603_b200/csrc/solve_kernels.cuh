@@ -201,6 +201,77 @@ k_fwd_y_t(const __grid_constant__ CUtensorMap tmB1, double2* __restrict__ B2, co
     }
 }
 
+// ================================================================================= K2 (v3): fwd_y_f
+// The tile kernel with ONE group per tile that transforms the whole zero-padded column of M2 = 2 Ny points (as
+// k_conv_z_f does along z): the tile is read from shared memory once instead of twice, there is no pre-twiddle
+// x[n] w^n and no twiddle table; the first radix-2 level of stage 1 is a register copy made while loading.
+// Ny = 512: M2 = 1024 = 32 x 32, 8 columns x 32 lanes = 256 threads, 32 points per lane.
+template <int M2>
+struct TileYF {
+    using Cfg = Fft2Cfg<M2>;
+    static constexpr int M = M2 / 2;                 // Ny
+    static constexpr int T = Cfg::T, R = Cfg::R, KW = kW;
+    static constexpr int THREADS = KW * T;
+    static constexpr int NC = LaneTw<Cfg::R2>::NC;
+    static constexpr int BOXR = M < 256 ? M : 256;
+    static_assert(Cfg::NB1 == 1 && Cfg::NB2 == 1, "one butterfly per lane and stage");
+    // [mbarriers: 128 B][X: M*KW][E: M2*KW]
+    static constexpr size_t smem_bytes() { return 128 + sizeof(double2) * (size_t)(M * KW + M2 * KW); }
+};
+
+template <int M2>
+__global__ void __launch_bounds__(TileYF<M2>::THREADS, 1)
+k_fwd_y_f(const __grid_constant__ CUtensorMap tmB1, double2* __restrict__ B2, const double* __restrict__ lane_g,
+          int Nz, int kx0, long ntiles) {
+    using Y = TileYF<M2>;
+    using Cfg = typename Y::Cfg;
+    constexpr int R = Y::R, T = Y::T, NC = Y::NC, KW = Y::KW, M = Y::M, H = R / 2;
+    extern __shared__ __align__(128) unsigned char smraw[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smraw);
+    double2* X = reinterpret_cast<double2*>(smraw + 128);
+    double2* E = X + M * KW;
+    const int tid = threadIdx.x;
+    const int c = tid % KW, t = tid / KW;
+    double cc[1][NC], tn[1][NC];
+#pragma unroll
+    for (int i = 0; i < NC; ++i) {
+        cc[0][i] = lane_g[t * 2 * NC + i];
+        tn[0][i] = lane_g[t * 2 * NC + NC + i];
+    }
+    if (tid == 0) { mbar_init(full, 1); mbar_fence_init(); }
+    __syncthreads();
+    const int nzb = Nz / KW;
+    auto issue = [&](long tile) {   // one thread: arm the barrier, then one TMA per box of rows
+        const int kx = (int)(tile / nzb), zb = (int)(tile % nzb);
+        mbar_arrive_expect_tx(full, (uint32_t)(M * KW * sizeof(double2)));
+#pragma unroll
+        for (int r0 = 0; r0 < M; r0 += Y::BOXR) tma_load_3d(X + r0 * KW, &tmB1, full, zb * KW * 2, r0, kx0 + kx);
+    };
+    long tile = blockIdx.x;
+    if (tid == 0 && tile < ntiles) issue(tile);
+    uint32_t parity = 0;
+    double2* Ec = E + c;
+    for (; tile < ntiles; tile += gridDim.x) {
+        const long kx = tile / nzb;
+        const int zb = (int)(tile % nzb);
+        double vr[R], vi[R];
+        mbar_wait(full, parity);
+        parity ^= 1;
+#pragma unroll
+        for (int i = 0; i < H; ++i) {   // rows t + T i < Ny; the zero half: (x_i, 0) -> (x_i, x_i)
+            const double2 v = X[(t + T * i) * KW + c];
+            vr[i] = v.x; vi[i] = v.y;
+            vr[i + H] = v.x; vi[i + H] = v.y;
+        }
+        __syncthreads();   // every thread holds its part of the tile: X may be refilled
+        if (tid == 0 && tile + gridDim.x < ntiles) issue(tile + gridDim.x);
+        fft2_forward_tile<Cfg, KW, 4>(vr, vi, t, Ec, 1, cc, tn);
+        double2* out = B2 + ((kx * M2) * (long)Nz + zb * KW + c);
+#pragma unroll
+        for (int i = 0; i < R; ++i) out[(long)(t + T * i) * Nz] = make_double2(vr[i], vi[i]);
+    }
+}
+
 // ====================================================================================== K4: inv_y
 // DER: input row ky is multiplied by -i kder m'(ky) first (E_y of the field output, see DerK)
 template <int M, bool DER = false>

@@ -107,6 +107,17 @@ def test_z_pass_kernel_variants_full_field(N, variant):
         check(E[d], E_o[d])
 
 
+def test_forward_y_kernel_variants_are_both_correct():
+    """FSP_PARAM_K2_VARIANT at Ny = 512: the padded-column kernel (default) and the two-branch tile kernel, full field,
+    264 tiles on 148 CTAs (the persistent loop iterates)."""
+    w = W.random_density((32, 512, 64), seed=77)
+    ref = oracle.OraclePlan(w.N, w.h, oracle.HOCKNEY).precompute_green().solve(w.rho)
+    for variant in (0, 1):
+        with binding.Plan(w.N, w.h, binding.HOCKNEY) as p:
+            binding.plan_set_param(p.handle, binding.PARAM_K2_VARIANT, variant)
+            check(gpu_solve(p.precompute_green(), w.rho), ref)
+
+
 # ---- (b) BASELINE configs 3 and 4, full field against O2 with the oracle's own table -------------------------
 @pytest.mark.parametrize("alg", ["HE", "VG2"])
 def test_config3_256_full_field_against_the_oracle(alg):
