@@ -1226,7 +1226,12 @@ k_fwd_x_t(const __grid_constant__ CUtensorMap tmRho, double2* __restrict__ B1, c
         }
     const double2 lam_n = Wg[2 * t];          // w_N^t     (Wg[m] = exp(-2 pi i m / 2N))
     const double2 lam_k = Wg[2 * t + grp];    // w_2N^(2t+g)
-    if (tid == 0) { mbar_init(full, 1); mbar_fence_init(); }
+    // full: the tile has landed in X; empty (full + 1): every thread holds its part of it.  The two groups are NOT
+    // synchronised with one another: group 1 (which has the pre-twiddle on top) falls behind until it reads a tile just
+    // before group 0 wants the next one, and from then on the shared-memory phases of one group run under the fp64
+    // phases of the other (a CTA-wide barrier here kept all 16 warps in the same phase)
+    uint64_t* empty = full + 1;
+    if (tid == 0) { mbar_init(full, 1); mbar_init(empty, X_::THREADS); mbar_fence_init(); }
     __syncthreads();
     auto issue = [&](long tile) {
         mbar_arrive_expect_tx(full, (uint32_t)(N * KC * sizeof(double)));
@@ -1247,8 +1252,11 @@ k_fwd_x_t(const __grid_constant__ CUtensorMap tmRho, double2* __restrict__ B1, c
             vr[i] = Xd[(2 * n) * KC + c];
             vi[i] = Xd[(2 * n + 1) * KC + c];
         }
-        __syncthreads();   // X may be refilled
-        if (tid == 0 && tile + gridDim.x < ntiles) issue(tile + gridDim.x);
+        mbar_arrive(empty);
+        if (tid == GT && tile + gridDim.x < ntiles) {   // first thread of group 1: X may be refilled once both groups hold the tile
+            mbar_wait(empty, parity ^ 1);
+            issue(tile + gridDim.x);
+        }
         if (grp) {   // z[n] w_N^n,  w_N^n = w_N^t w_32^i
             UntangleFwd<M>::run([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
