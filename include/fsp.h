@@ -85,12 +85,13 @@ enum {
     FSP_PARAM_K2_VARIANT = 4, /* kernel of the forward y pass at Ny = 512 (kept for A/B measurements): 0 (default) = the
                                 zero-padded column of 2 Ny points in one group (k_fwd_y_f); 1 = two half-length
                                 branches in two groups (k_fwd_y_t).  Takes effect at the next fsp_solve          */
-    FSP_PARAM_K3_VARIANT = 3, /* kernel of the z pass at Nz = 256, 512 (kept for A/B measurements): 0 (default) =
-                                the whole zero-padded pencil in one lane group (k_conv_z_f); 1 = two half-
-                                length branches in a warp pair (k_conv_z_p); 2 (Nz = 512) = the pair scheme
-                                with 32 lanes per branch (k_conv_z_s).  Invalidates the spectrum (its row
-                                layout follows the kernel): call fsp_precompute_green again.  Results agree
-                                to rounding, all within the tolerances of DESIGN.md                  */
+    FSP_PARAM_K3_VARIANT = 3  /* kernel of the z pass (kept for A/B measurements).  0 (default): the whole zero-padded
+                                pencil in one lane group (k_conv_z_f, Nz = 256, 512; the prime-factor kernel
+                                k_conv_z_pf at Nz = 96, 192, 384; k_conv_z_g2 at the other 3 * 2^k, 5 * 2^k).  1: two
+                                half-length branches (k_conv_z_p, k_conv_z_g).  2: Nz = 512: the pair scheme with 32
+                                lanes per branch (k_conv_z_s); Nz = 96, 192, 384: k_conv_z_g2.  Invalidates the
+                                spectrum (its row layout follows the kernel): call fsp_precompute_green again.
+                                Results agree to rounding, all within the tolerances of DESIGN.md       */
 };
 
 /* number of kernels one fsp_solve launches (the five passes of DESIGN.md "The path") */

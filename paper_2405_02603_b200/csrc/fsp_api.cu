@@ -45,6 +45,7 @@ struct fsp_plan {
     int planes = 0;         // kx planes held by B1 (stage 2), B2 and Gk; Nx + 1 unless stage 2 of a sharded plan
     int kx0 = 0;            // global index of the first of them
     size_t b1_count = 0, b2_count = 0;   // complex elements allocated in B1, B2
+    bool gk_pfa = false;     // Gk rows hold all 2 Nz entries in CRT order (k_conv_z_pf, Nz = 96, 192, 384)
     bool gk_natural = false; // Gk rows in natural order (k_conv_z_f) instead of [E | O] (decided by the last precompute)
     double* LTy = nullptr;  // the same for the y transform (tile kernels)
     double* LTyf = nullptr; // Ny = 512: stage-2 constants of the padded 1024-point y transform (k_fwd_y_f)
@@ -573,11 +574,39 @@ int launch_conv_z_g2(fsp_plan* p, double2* B2, const double* G, int np, double2*
     if (kap) return launch_conv_z_g2_impl<M2, true>(p, B2, G, np, out, *kap);
     return launch_conv_z_g2_impl<M2, false>(p, B2, G, np, nullptr, DerK{0.0, 0.0, 0.0, 0});
 }
+template <int P, bool DER>
+int launch_conv_z_pf_impl(fsp_plan* p, double2* B2, const double* G, int nplanes, double2* out, const DerK kap) {
+    using Z = ConvZPF<P>;
+    const long ngroups = (long)nplanes * (2 * p->Ny) / Z::G;
+    const size_t smem = Z::smem_bytes();
+    static OccCache cache;
+    int occ = 0;
+    { const int rc_ = cached_occupancy(cache, p->device, k_conv_z_pf<P, DER>, Z::WARPS * 32, smem, &occ); if (rc_ != FSP_OK) return rc_; }
+    long grid = (long)p->sm_count * occ;
+    const long need = (ngroups + Z::WARPS - 1) / Z::WARPS;
+    if (grid > need) grid = need;
+    k_conv_z_pf<P, DER><<<(unsigned)grid, Z::WARPS * 32, smem, p->stream>>>(B2, G, p->LTzf, p->Ny, ngroups, out, kap);
+    return FSP_OK;
+}
+template <int P>
+int launch_conv_z_pf(fsp_plan* p, double2* B2, const double* G, int np, double2* out, const DerK* kap) {
+    if (kap) return launch_conv_z_pf_impl<P, true>(p, B2, G, np, out, *kap);
+    return launch_conv_z_pf_impl<P, false>(p, B2, G, np, nullptr, DerK{0.0, 0.0, 0.0, 0});
+}
 bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+// Nz = 3 * 2^k with a warp-level prime-factor kernel (2 Nz = 3 P, P = 64, 128, 256)
+bool z_uses_pf(int Nz) { return Nz == 96 || Nz == 192 || Nz == 384; }
+// doubles per spectrum row as ALLOCATED: Nz + 2 (octant rows, natural or [E | O]); 2 Nz where the prime-factor kernel may run
+size_t gk_row(int Nz) { return z_uses_pf(Nz) ? (size_t)2 * Nz : (size_t)Nz + 2; }
 // Nz = 3 * 2^k, 5 * 2^k whose doubled length has an engine configuration: k_conv_z_g2 (natural-order spectrum rows)
 bool z_uses_g2(int Nz) { return Nz == 24 || Nz == 48 || Nz == 96 || Nz == 192 || Nz == 384 || Nz == 40 || Nz == 80 || Nz == 160; }
 int do_conv_z_w(fsp_plan* p, double2* B2, const double* G, int np, double2* out, const DerK* kap) {
-    if (!is_pow2(p->Nz)) {   // 3 * 2^k, 5 * 2^k: the CTA-level kernels on the mixed-radix engine
+    if (!is_pow2(p->Nz)) {   // 3 * 2^k, 5 * 2^k: the prime-factor warp kernel, else the CTA-level kernels on the mixed-radix engine
+        if (p->gk_pfa) {
+            if (p->Nz == 384) return launch_conv_z_pf<256>(p, B2, G, np, out, kap);
+            if (p->Nz == 192) return launch_conv_z_pf<128>(p, B2, G, np, out, kap);
+            return launch_conv_z_pf<64>(p, B2, G, np, out, kap);
+        }
         if (p->gk_natural) {
             switch (p->Nz) {
                 case 24: return launch_conv_z_g2<48>(p, B2, G, np, out, kap);
@@ -612,7 +641,7 @@ int do_conv_z_w(fsp_plan* p, double2* B2, const double* G, int np, double2* out,
 // planes [kx0, kx0 + np) of the spectrum go with the np planes stored at B2.
 // kap == nullptr: in place (phi); otherwise B2 -> out with the derivative factor (whole volume only, kx0 = 0).
 int do_conv_z(fsp_plan* p, double2* B2, int kx0, int np, double2* out = nullptr, const DerK* kap = nullptr) {
-    return do_conv_z_w(p, B2, p->Gk + (size_t)kx0 * (p->Ny + 1) * (p->Nz + 2), np, out, kap);
+    return do_conv_z_w(p, B2, p->Gk + (size_t)kx0 * (p->Ny + 1) * (p->gk_pfa ? (size_t)2 * p->Nz : (size_t)p->Nz + 2), np, out, kap);
 }
 int make_z_lane_table(fsp_plan* p) {
     if (!is_pow2(p->Nz)) return FSP_OK;   // k_conv_z_g reads the root table only
@@ -961,8 +990,13 @@ int precompute_impl(fsp_plan* p) {
         // (a sharded plan keeps the rows of its own kx planes only)
         const long gk_total = (long)p->planes * (Ny + 1) * (Nz + 2);
         const double* goct = p->Goct + (size_t)p->kx0 * (Ny + 1) * (Nz + 1);
-        p->gk_natural = (Nz == 256 || Nz == 512 || z_uses_g2(Nz)) && p->k3_variant == 0;
-        if (p->gk_natural) k_layout_spectrum_nat<<<grid_for(gk_total, blk), blk, 0, p->stream>>>(goct, p->Gk, p->planes - 1, Ny, Nz, gscale);
+        p->gk_pfa = z_uses_pf(Nz) && p->k3_variant == 0;
+        p->gk_natural = !p->gk_pfa && ((Nz == 256 || Nz == 512) ? p->k3_variant == 0 : (z_uses_g2(Nz) && p->k3_variant != 1));
+        if (p->gk_pfa) {
+            const int P = 2 * Nz / 3, c1 = P * (P % 3 == 1 ? 1 : 2), c2 = 3 * (P == 256 ? 171 : 43);
+            const long tot = (long)p->planes * (Ny + 1) * 2 * Nz;
+            k_layout_spectrum_pfa<<<grid_for(tot, blk), blk, 0, p->stream>>>(goct, p->Gk, p->planes - 1, Ny, Nz, P, c1, c2, gscale);
+        } else if (p->gk_natural) k_layout_spectrum_nat<<<grid_for(gk_total, blk), blk, 0, p->stream>>>(goct, p->Gk, p->planes - 1, Ny, Nz, gscale);
         else k_layout_spectrum_oct<<<grid_for(gk_total, blk), blk, 0, p->stream>>>(goct, p->Gk, p->planes - 1, Ny, Nz, gscale);
     }
     CU(cudaGetLastError());
@@ -1054,7 +1088,10 @@ static int plan_create_impl(fsp_plan** out, int Nx, int Ny, int Nz, const double
     if (rc == FSP_OK) rc = dev_alloc(&p->B1, n1, &p->bytes);
     if (rc == FSP_OK && want_yz) rc = dev_alloc(&p->B2, n2, &p->bytes);
     p->sm_count = prop.multiProcessorCount > 0 ? prop.multiProcessorCount : 148;
-    if (rc == FSP_OK && want_yz) rc = dev_alloc(&p->Gk, (size_t)planes * (Ny + 1) * (Nz + 2), &p->bytes);
+    if (rc == FSP_OK && want_yz) rc = dev_alloc(&p->Gk, (size_t)planes * (Ny + 1) * gk_row(Nz), &p->bytes);
+    if (rc == FSP_OK && want_yz && Nz == 384) rc = lane_table_for<256>(&p->LTzf, &p->bytes);
+    if (rc == FSP_OK && want_yz && Nz == 192) rc = lane_table_for<128>(&p->LTzf, &p->bytes);
+    if (rc == FSP_OK && want_yz && Nz == 96) rc = lane_table_for<64>(&p->LTzf, &p->bytes);
     if (rc == FSP_OK && want_yz) rc = make_z_lane_table(p);
     if (rc == FSP_OK && want_yz && Nz == 512) rc = make_lane_table_512s(&p->LTzs, &p->bytes);
     if (rc == FSP_OK && want_yz && Nz == 512) rc = lane_table_for<1024>(&p->LTzf, &p->bytes);

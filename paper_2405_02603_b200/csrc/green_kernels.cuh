@@ -375,4 +375,20 @@ __global__ void k_layout_spectrum_nat(const double* __restrict__ Goct, double* _
     }
 }
 
+// Spectrum layout for k_conv_z_pf (Nz = 3 P / 2): all M2 = 2 Nz = 3 P entries of a row in CRT order,
+//   Gk[row * M2 + k1 * P + k2] = scale * Goct[row][min(k, M2 - k)],   k = k1 (mod 3), k = k2 (mod P)
+__global__ void k_layout_spectrum_pfa(const double* __restrict__ Goct, double* __restrict__ Gk, int Nx, int Ny,
+                                      int Nz, int P, int c1, int c2, double scale) {
+    const long row = 2L * Nz;
+    const long total = (long)(Nx + 1) * (Ny + 1) * row;
+    for (long o = blockIdx.x * (long)blockDim.x + threadIdx.x; o < total; o += (long)gridDim.x * blockDim.x) {
+        const int c = (int)(o % row);
+        const long pr = o / row;
+        const int k1 = c / P, k2 = c % P;
+        const int k = (int)(((long)c1 * k1 + (long)c2 * k2) % row);
+        const int idx = k <= Nz ? k : (int)row - k;
+        Gk[o] = scale * Goct[pr * (Nz + 1) + idx];
+    }
+}
+
 }  // namespace fsp

@@ -86,7 +86,8 @@ def test_full_field_of_the_field_output_where_loops_iterate(N):
 
 
 @pytest.mark.parametrize("N,variant", [((32, 32, 512), 1), ((32, 32, 512), 2), ((64, 32, 256), 1), ((16, 64, 512), 0),
-                                       ((16, 24, 96), 1)])   # last: the branch kernel k_conv_z_g where k_conv_z_g2 is the default
+                                       ((16, 24, 96), 1), ((16, 24, 96), 2), ((40, 12, 192), 0)])
+# (.., 96): default = the prime-factor warp kernel k_conv_z_pf; 1 = the branch kernel k_conv_z_g; 2 = k_conv_z_g2
 def test_z_pass_kernel_variants_full_field(N, variant):
     """FSP_PARAM_K3_VARIANT: the branch-pair kernels of the z pass (k_conv_z_p, k_conv_z_s) stay selectable for A/B
     measurements; each against the oracle, phi and the field (the DER variants), where the persistent loops iterate."""
