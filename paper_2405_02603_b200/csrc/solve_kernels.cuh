@@ -973,6 +973,10 @@ k_conv_z_f(double2* __restrict__ B2, const double* __restrict__ Gk, const double
                 mbar_wait(gbar, gpar);
                 gpar ^= 1;
                 const double fz0 = fp + kap.z * (double)t;   // DER only
+                double kzv = kap.z;
+                // opaque to the compiler: otherwise the 32 products kap.z * offset are formed once per kernel, spilled to
+                // local memory and re-read for every pencil (35 doubles of spills)
+                if constexpr (DER) asm volatile("" : "+d"(kzv));
 #pragma unroll
                 for (int i = 0; i < R; ++i) {
                     const double gk = i < H ? gA[T * i] : gB[-T * i];
@@ -981,7 +985,7 @@ k_conv_z_f(double2* __restrict__ B2, const double* __restrict__ Gk, const double
                         // (t = 0, i = R/2); the factor -i itself is applied to the final result (F^-1 is linear)
                         // (fz0 = fp + kap.z t, so at t = 0 the Nyquist factor fp is fz0 itself)
                         const double off = (double)(i < H ? T * i : T * i - M2);
-                        const double cf = gk * ((i == H && t == 0) ? fz0 : fma(kap.z, off, fz0));
+                        const double cf = gk * ((i == H && t == 0) ? fz0 : fma(kzv, off, fz0));
                         vr[i] *= cf; vi[i] *= -cf;
                     } else {
                         vr[i] *= gk; vi[i] *= -gk;
@@ -1503,6 +1507,8 @@ k_inv_x_t(const __grid_constant__ CUtensorMap tmB1, const double2* __restrict__ 
         double zr[R], zi[R];
         mbar_wait(&full[grp], parity);
         parity ^= 1;
+        double kdv = kder;   // opaque: keeps the 2 R mode factors from being formed once per kernel and spilled (DER only)
+        if constexpr (DER) asm volatile("" : "+d"(kdv));
         UntangleFwd<M>::run([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             const int j = t + T * i;
@@ -1511,9 +1517,9 @@ k_inv_x_t(const __grid_constant__ CUtensorMap tmB1, const double2* __restrict__ 
             if (grp) bq = Ec[(M - 1 - j) * KC];
             else bq = (j == 0) ? XN[c] : Ec[(M - j) * KC];
             if constexpr (DER) {   // k = (2t + grp) + 2T i: a lane constant plus a compile-time multiple
-                const double ck = fma(kder * (double)(2 * T), (double)i, kd0);
+                const double ck = fma(kdv * (double)(2 * T), (double)i, kd0);
                 mul_minus_i(a.x, a.y, ck);
-                mul_minus_i(bq.x, bq.y, (i == 0 && kd0 == 0.0) ? 0.0 : kder * (double)N - ck);   // N - k; row N is the Nyquist row
+                mul_minus_i(bq.x, bq.y, (i == 0 && kd0 == 0.0) ? 0.0 : kdv * (double)N - ck);   // N - k; row N is the Nyquist row
             }
             const double br = bq.x, bi = -bq.y;
             const double sr = a.x + br, si = a.y + bi;
