@@ -45,6 +45,10 @@ struct fsp_plan {
     int planes = 0;         // kx planes held by B1 (stage 2), B2 and Gk; Nx + 1 unless stage 2 of a sharded plan
     int kx0 = 0;            // global index of the first of them
     size_t b1_count = 0, b2_count = 0;   // complex elements allocated in B1, B2
+    // warp-level DCT-I of the precompute: per transform length M, the lane-constant table and the roots exp(-2 pi i m / 2M)
+    std::vector<int> dct_len;
+    std::vector<double*> dct_lane;
+    std::vector<double2*> dct_roots;
     bool gk_pfa = false;     // Gk rows hold all 2 Nz entries in CRT order (k_conv_z_pf, Nz = 96, 192, 384)
     bool gk_natural = false; // Gk rows in natural order (k_conv_z_f) instead of [E | O] (decided by the last precompute)
     double* LTy = nullptr;  // the same for the y transform (tile kernels)
@@ -749,6 +753,48 @@ int next_supported_size(int n, bool pow2_only, bool z_axis) {
     return 1024;
 }
 
+// tables of k_dct1_warp<M> for this plan (built on first use, freed with the plan)
+template <int M>
+int dct_warp_tables(fsp_plan* p, double** lane, double2** roots) {
+    for (size_t i = 0; i < p->dct_len.size(); ++i)
+        if (p->dct_len[i] == M) { *lane = p->dct_lane[i]; *roots = p->dct_roots[i]; return FSP_OK; }
+    double* l = nullptr;
+    double2* r = nullptr;
+    int rc = lane_table_for<M>(&l, &p->bytes);
+    if (rc != FSP_OK) return rc;
+    std::vector<double2> hst((size_t)M + 1);
+    for (int m = 0; m <= M; ++m) hst[m] = unit_root(m, 2L * M);
+    if ((rc = upload_table(&r, hst, &p->bytes)) != FSP_OK) { cudaFree(l); return rc; }
+    p->dct_len.push_back(M); p->dct_lane.push_back(l); p->dct_roots.push_back(r);
+    *lane = l; *roots = r;
+    return FSP_OK;
+}
+template <int M>
+int launch_dct1_warp(fsp_plan* p, const double* in, double* out, int nout, long nA, long nB, const long* ai, const long* ao,
+                     double scale, const GLFill* fill) {
+    using Cfg = Fft2Cfg<M>;
+    constexpr int G = 32 / Cfg::T, WARPS = 8;
+    double* lane = nullptr;
+    double2* roots = nullptr;
+    int rc = dct_warp_tables<M>(p, &lane, &roots);
+    if (rc != FSP_OK) return rc;
+    const size_t smem = sizeof(double2) * (size_t)(WARPS * G * Cfg::BUF);
+    const long ngroups = (nA * nB + G - 1) / G;
+    long grid = (ngroups + WARPS - 1) / WARPS;
+    if (grid > (long)p->sm_count) grid = p->sm_count;
+    if (fill) {
+        { static OccCache optin; const int rc_ = cached_smem_optin(optin, p->device, k_dct1_warp<M, true>, smem); if (rc_ != FSP_OK) return rc_; }
+        k_dct1_warp<M, true><<<(unsigned)grid, WARPS * 32, smem, p->stream>>>(in, out, nout, nA, nB, ai[0], ai[1], ai[2], ao[0], ao[1], ao[2],
+                                                                          scale, *fill, lane, roots);
+    } else {
+        { static OccCache optin; const int rc_ = cached_smem_optin(optin, p->device, k_dct1_warp<M, false>, smem); if (rc_ != FSP_OK) return rc_; }
+        k_dct1_warp<M, false><<<(unsigned)grid, WARPS * 32, smem, p->stream>>>(in, out, nout, nA, nB, ai[0], ai[1], ai[2], ao[0], ao[1], ao[2],
+                                                                           scale, GLFill{0.0, 0.0, 0.0, 0.0, 0}, lane, roots);
+    }
+    CU(cudaGetLastError());
+    return FSP_OK;
+}
+
 // batched DCT-I along one axis of a real 3-D array (C order), output pruned to nout along that axis.
 // fill != nullptr (axis 2 only): the input array does not exist, its values are G_L evaluated inside the kernel.
 template <int C>
@@ -791,6 +837,21 @@ int dct1_axis(fsp_plan* p, const double* in, double* out, const long in_dims[3],
         }
         CU(cudaGetLastError());
         return FSP_OK;
+    }
+    if (n >= 8 && n <= 1024) {   // the warp-level transform of the solve, one pencil per lane group (k_dct1_warp)
+        const int bdim = axis == 2 ? 1 : 2, adim = axis == 2 ? 0 : (axis == 0 ? 1 : 0);
+        const long nA = in_dims[adim], nB = in_dims[bdim];
+        const long ai[3] = {is[adim], is[bdim], is[axis]}, ao[3] = {os[adim], os[bdim], os[axis]};
+        switch (n) {
+            case 8: return launch_dct1_warp<8>(p, in, out, nout, nA, nB, ai, ao, scale, fill);
+            case 16: return launch_dct1_warp<16>(p, in, out, nout, nA, nB, ai, ao, scale, fill);
+            case 32: return launch_dct1_warp<32>(p, in, out, nout, nA, nB, ai, ao, scale, fill);
+            case 64: return launch_dct1_warp<64>(p, in, out, nout, nA, nB, ai, ao, scale, fill);
+            case 128: return launch_dct1_warp<128>(p, in, out, nout, nA, nB, ai, ao, scale, fill);
+            case 256: return launch_dct1_warp<256>(p, in, out, nout, nA, nB, ai, ao, scale, fill);
+            case 512: return launch_dct1_warp<512>(p, in, out, nout, nA, nB, ai, ao, scale, fill);
+            default: return launch_dct1_warp<1024>(p, in, out, nout, nA, nB, ai, ao, scale, fill);
+        }
     }
     {   // tile kernel: C pencils per CTA along the contiguous dimension (z; y when the transform axis is z)
         const int bdim = axis == 2 ? 1 : 2, adim = axis == 2 ? 0 : (axis == 0 ? 1 : 0);
@@ -1006,6 +1067,9 @@ int precompute_impl(fsp_plan* p) {
 }
 
 void free_plan_memory(fsp_plan* p) {
+    for (double* q : p->dct_lane) cudaFree(q);
+    for (double2* q : p->dct_roots) cudaFree(q);
+    p->dct_lane.clear(); p->dct_roots.clear(); p->dct_len.clear();
     cudaFree(p->B1); cudaFree(p->B2); cudaFree(p->B3); cudaFree(p->rho_pad); cudaFree(p->phi_pad); cudaFree(p->E_stage); cudaFree(p->rho_stage2); cudaFree(p->phi_stage2); cudaFree(p->Gk); cudaFree(p->LTz); cudaFree(p->LTzs); cudaFree(p->LTzf); cudaFree(p->LTy); cudaFree(p->LTyf); cudaFree(p->LTx); cudaFree(p->T); cudaFree(p->Goct);
     cudaFree(p->Wx); cudaFree(p->Wy); cudaFree(p->Wz); cudaFree(p->rho_stage); cudaFree(p->phi_stage);
     for (cudaEvent_t e : p->events) cudaEventDestroy(e);
