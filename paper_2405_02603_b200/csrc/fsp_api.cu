@@ -578,28 +578,30 @@ int launch_conv_z_g2(fsp_plan* p, double2* B2, const double* G, int np, double2*
     if (kap) return launch_conv_z_g2_impl<M2, true>(p, B2, G, np, out, *kap);
     return launch_conv_z_g2_impl<M2, false>(p, B2, G, np, nullptr, DerK{0.0, 0.0, 0.0, 0});
 }
-template <int P, bool DER>
+template <int B, int P, bool DER>
 int launch_conv_z_pf_impl(fsp_plan* p, double2* B2, const double* G, int nplanes, double2* out, const DerK kap) {
-    using Z = ConvZPF<P>;
+    using Z = ConvZPF<B, P>;
     const long ngroups = (long)nplanes * (2 * p->Ny) / Z::G;
     const size_t smem = Z::smem_bytes();
     static OccCache cache;
     int occ = 0;
-    { const int rc_ = cached_occupancy(cache, p->device, k_conv_z_pf<P, DER>, Z::WARPS * 32, smem, &occ); if (rc_ != FSP_OK) return rc_; }
+    { const int rc_ = cached_occupancy(cache, p->device, k_conv_z_pf<B, P, DER>, Z::WARPS * 32, smem, &occ); if (rc_ != FSP_OK) return rc_; }
     long grid = (long)p->sm_count * occ;
     const long need = (ngroups + Z::WARPS - 1) / Z::WARPS;
     if (grid > need) grid = need;
-    k_conv_z_pf<P, DER><<<(unsigned)grid, Z::WARPS * 32, smem, p->stream>>>(B2, G, p->LTzf, p->Ny, ngroups, out, kap);
+    k_conv_z_pf<B, P, DER><<<(unsigned)grid, Z::WARPS * 32, smem, p->stream>>>(B2, G, p->LTzf, p->Ny, ngroups, out, kap);
     return FSP_OK;
 }
-template <int P>
+template <int B, int P>
 int launch_conv_z_pf(fsp_plan* p, double2* B2, const double* G, int np, double2* out, const DerK* kap) {
-    if (kap) return launch_conv_z_pf_impl<P, true>(p, B2, G, np, out, *kap);
-    return launch_conv_z_pf_impl<P, false>(p, B2, G, np, nullptr, DerK{0.0, 0.0, 0.0, 0});
+    if (kap) return launch_conv_z_pf_impl<B, P, true>(p, B2, G, np, out, *kap);
+    return launch_conv_z_pf_impl<B, P, false>(p, B2, G, np, nullptr, DerK{0.0, 0.0, 0.0, 0});
 }
 bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
-// Nz = 3 * 2^k with a warp-level prime-factor kernel (2 Nz = 3 P, P = 64, 128, 256)
-bool z_uses_pf(int Nz) { return Nz == 96 || Nz == 192 || Nz == 384; }
+// Nz = 3 * 2^k, 5 * 2^k with a warp-level prime-factor kernel (2 Nz = B P, B = 3: P = 16 .. 256, B = 5: P = 16 .. 64)
+// (Nz = 320 would need 5 x 16 complex registers per lane and 233 KB of shared memory, Nz = 768 3 x 32: CTA-level kernel)
+bool z_uses_pf(int Nz) { return Nz == 24 || Nz == 48 || Nz == 96 || Nz == 192 || Nz == 384 || Nz == 40 || Nz == 80 || Nz == 160; }
+int pf_radix(int Nz) { return Nz % 3 == 0 ? 3 : 5; }
 // doubles per spectrum row as ALLOCATED: Nz + 2 (octant rows, natural or [E | O]); 2 Nz where the prime-factor kernel may run
 size_t gk_row(int Nz) { return z_uses_pf(Nz) ? (size_t)2 * Nz : (size_t)Nz + 2; }
 // Nz = 3 * 2^k, 5 * 2^k whose doubled length has an engine configuration: k_conv_z_g2 (natural-order spectrum rows)
@@ -607,9 +609,17 @@ bool z_uses_g2(int Nz) { return Nz == 24 || Nz == 48 || Nz == 96 || Nz == 192 ||
 int do_conv_z_w(fsp_plan* p, double2* B2, const double* G, int np, double2* out, const DerK* kap) {
     if (!is_pow2(p->Nz)) {   // 3 * 2^k, 5 * 2^k: the prime-factor warp kernel, else the CTA-level kernels on the mixed-radix engine
         if (p->gk_pfa) {
-            if (p->Nz == 384) return launch_conv_z_pf<256>(p, B2, G, np, out, kap);
-            if (p->Nz == 192) return launch_conv_z_pf<128>(p, B2, G, np, out, kap);
-            return launch_conv_z_pf<64>(p, B2, G, np, out, kap);
+            switch (p->Nz) {
+                case 384: return launch_conv_z_pf<3, 256>(p, B2, G, np, out, kap);
+                case 192: return launch_conv_z_pf<3, 128>(p, B2, G, np, out, kap);
+                case 96: return launch_conv_z_pf<3, 64>(p, B2, G, np, out, kap);
+                case 48: return launch_conv_z_pf<3, 32>(p, B2, G, np, out, kap);
+                case 24: return launch_conv_z_pf<3, 16>(p, B2, G, np, out, kap);
+                case 160: return launch_conv_z_pf<5, 64>(p, B2, G, np, out, kap);
+                case 80: return launch_conv_z_pf<5, 32>(p, B2, G, np, out, kap);
+                case 40: return launch_conv_z_pf<5, 16>(p, B2, G, np, out, kap);
+                default: return FSP_ERR_INVALID_ARG;
+            }
         }
         if (p->gk_natural) {
             switch (p->Nz) {
@@ -1054,7 +1064,8 @@ int precompute_impl(fsp_plan* p) {
         p->gk_pfa = z_uses_pf(Nz) && p->k3_variant == 0;
         p->gk_natural = !p->gk_pfa && ((Nz == 256 || Nz == 512) ? p->k3_variant == 0 : (z_uses_g2(Nz) && p->k3_variant != 1));
         if (p->gk_pfa) {
-            const int P = 2 * Nz / 3, c1 = P * (P % 3 == 1 ? 1 : 2), c2 = 3 * (P == 256 ? 171 : 43);
+            const int B = pf_radix(Nz), P = 2 * Nz / B;
+            const int c1 = P * mod_inverse(P % B, B), c2 = B * mod_inverse(B % P, P);   // k = (c1 k1 + c2 k2) mod 2 Nz
             const long tot = (long)p->planes * (Ny + 1) * 2 * Nz;
             k_layout_spectrum_pfa<<<grid_for(tot, blk), blk, 0, p->stream>>>(goct, p->Gk, p->planes - 1, Ny, Nz, P, c1, c2, gscale);
         } else if (p->gk_natural) k_layout_spectrum_nat<<<grid_for(gk_total, blk), blk, 0, p->stream>>>(goct, p->Gk, p->planes - 1, Ny, Nz, gscale);
@@ -1153,9 +1164,15 @@ static int plan_create_impl(fsp_plan** out, int Nx, int Ny, int Nz, const double
     if (rc == FSP_OK && want_yz) rc = dev_alloc(&p->B2, n2, &p->bytes);
     p->sm_count = prop.multiProcessorCount > 0 ? prop.multiProcessorCount : 148;
     if (rc == FSP_OK && want_yz) rc = dev_alloc(&p->Gk, (size_t)planes * (Ny + 1) * gk_row(Nz), &p->bytes);
-    if (rc == FSP_OK && want_yz && Nz == 384) rc = lane_table_for<256>(&p->LTzf, &p->bytes);
-    if (rc == FSP_OK && want_yz && Nz == 192) rc = lane_table_for<128>(&p->LTzf, &p->bytes);
-    if (rc == FSP_OK && want_yz && Nz == 96) rc = lane_table_for<64>(&p->LTzf, &p->bytes);
+    if (rc == FSP_OK && want_yz && z_uses_pf(Nz)) {   // stage-2 constants of the P-point sub-transforms, P = 2 Nz / B
+        switch (2 * Nz / pf_radix(Nz)) {
+            case 256: rc = lane_table_for<256>(&p->LTzf, &p->bytes); break;
+            case 128: rc = lane_table_for<128>(&p->LTzf, &p->bytes); break;
+            case 64: rc = lane_table_for<64>(&p->LTzf, &p->bytes); break;
+            case 32: rc = lane_table_for<32>(&p->LTzf, &p->bytes); break;
+            default: rc = lane_table_for<16>(&p->LTzf, &p->bytes); break;
+        }
+    }
     if (rc == FSP_OK && want_yz) rc = make_z_lane_table(p);
     if (rc == FSP_OK && want_yz && Nz == 512) rc = make_lane_table_512s(&p->LTzs, &p->bytes);
     if (rc == FSP_OK && want_yz && Nz == 512) rc = lane_table_for<1024>(&p->LTzf, &p->bytes);

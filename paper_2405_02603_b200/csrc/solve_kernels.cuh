@@ -1000,39 +1000,39 @@ k_conv_z_f(double2* __restrict__ B2, const double* __restrict__ Gk, const double
     }
 }
 
-// ============================================ K3 for Nz = 3 * 2^k (96, 192, 384): conv_z_pf, prime-factor warp kernel
-// The zero-padded pencil of M2 = 2 Nz = 3 P points (P = 64, 128, 256) by the Good-Thomas map: with n = (P n1 + 3 n2) mod
-// M2 on the input side and k = k1 (mod 3), k = k2 (mod P) (CRT) on the output side,
-//     X[k] = sum_n1 w_3^(n1 k1) sum_n2 w_P^(n2 k2) x[n]
-// -- three P-point transforms (the warp-level two-stage transform of fft_warp.cuh, lane-constant twiddles, exchange
-// private to the lane group) and a radix-3 butterfly across them in registers, NO twiddles in between.  The DFT
-// matrix is symmetric, so the same code also maps a CRT-ordered input to an (P n1 + 3 n2)-ordered output: the forward
+// =============================== K3 for Nz = 3 * 2^k (24 .. 384) and 5 * 2^k (40 .. 160): conv_z_pf, prime-factor warp kernel
+// The zero-padded pencil of M2 = 2 Nz = B P points (B = 3 or 5, P = 16 .. 256) by the Good-Thomas map: with n = (P n1 + B n2)
+// mod M2 on the input side and k = k1 (mod B), k = k2 (mod P) (CRT) on the output side,
+//     X[k] = sum_n1 w_B^(n1 k1) sum_n2 w_P^(n2 k2) x[n]
+// -- B P-point transforms (the warp-level two-stage transform of fft_warp.cuh, lane-constant twiddles, exchange
+// private to the lane group) and a radix-B butterfly across them in registers, NO twiddles in between.  The DFT
+// matrix is symmetric, so the same code also maps a CRT-ordered input to an (P n1 + B n2)-ordered output: the forward
 // pass leaves the spectrum in CRT order (the spectrum rows are stored in that order, k_layout_spectrum_pfa), the
 // inverse pass (IFFT(Y) = conj(FFT(conj Y)), the same copy of the code) returns to the order the pencil was loaded in.
 // Against the CTA-level engine (k_conv_z_g2): no twiddle table, no CTA barriers, 8 free-running warps.
-template <int P>
+template <int B, int P>
 struct ConvZPF {
     using Cfg = Fft2Cfg<P>;
-    static constexpr int M2 = 3 * P, M = M2 / 2;           // M = Nz
+    static constexpr int M2 = B * P, M = M2 / 2;           // M = Nz
     static constexpr int T = Cfg::T, R = Cfg::R;
     static constexpr int G = 32 / T;                       // pencils per warp
     static constexpr int WARPS = 8;
     static constexpr int ROW = M2;                         // doubles per spectrum row (CRT order, all M2 entries)
     static constexpr int NC = LaneTw<Cfg::R2>::NC;
-    static constexpr int C1 = P * (P % 3 == 1 ? 1 : 2);    // k = (C1 k1 + C2 k2) mod M2:  P * (P^-1 mod 3)
-    static constexpr int C2 = 3 * (P == 128 ? 43 : (P == 256 ? 171 : 43));   // 3 * (3^-1 mod P): 43 (64), 43 (128), 171 (256)
-    static_assert((3 * (C2 / 3)) % P == 1 && C1 % 3 == 1, "CRT constants");
+    static constexpr int C1 = P * mod_inverse(P % B, B);   // k = (C1 k1 + C2 k2) mod M2:  P * (P^-1 mod B)
+    static constexpr int C2 = B * mod_inverse(B % P, P);   //                              B * (B^-1 mod P)
+    static_assert((B == 3 || B == 5) && C2 % P == 1 && C1 % B == 1, "CRT constants");
     // [exchange: WARPS*G*BUF double2][rows: WARPS*G*ROW doubles][mbarriers: WARPS]
     static constexpr size_t smem_bytes() {
         return sizeof(double2) * (size_t)(WARPS * G * Cfg::BUF) + sizeof(double) * (size_t)(WARPS * G * ROW) + 8 * WARPS;
     }
 };
 
-template <int P, bool DER = false>
-__global__ void __launch_bounds__(ConvZPF<P>::WARPS * 32, 1)
+template <int B, int P, bool DER = false>
+__global__ void __launch_bounds__(ConvZPF<B, P>::WARPS * 32, 1)
 k_conv_z_pf(double2* __restrict__ B2, const double* __restrict__ Gk, const double* __restrict__ lane_g, int Ny,
             long ngroups, double2* __restrict__ out, const DerK kap) {
-    using Z = ConvZPF<P>;
+    using Z = ConvZPF<B, P>;
     using Cfg = typename Z::Cfg;
     constexpr int M = Z::M, M2 = Z::M2, R = Z::R, T = Z::T, G = Z::G, WARPS = Z::WARPS, NC = Z::NC, NB2 = Cfg::NB2;
     extern __shared__ double2 smem[];
@@ -1077,13 +1077,13 @@ k_conv_z_pf(double2* __restrict__ B2, const double* __restrict__ Gk, const doubl
                 bulk_load(gall + (warp * G + gg) * Z::ROW, Gk + ((long)kx2 * (Ny + 1) + qy2) * Z::ROW, Z::ROW * 8, gbar);
             }
         }
-        // slot (n1, i) <-> n = (P n1 + 3 (t + T i)) mod M2; the padded half (n >= M) is zero
-        double vr[3][R], vi[3][R];
+        // slot (n1, i) <-> n = (P n1 + B (t + T i)) mod M2; the padded half (n >= M) is zero
+        double vr[B][R], vi[B][R];
 #pragma unroll
-        for (int n1 = 0; n1 < 3; ++n1)
+        for (int n1 = 0; n1 < B; ++n1)
 #pragma unroll
             for (int i = 0; i < R; ++i) {
-                int n = P * n1 + 3 * (t + T * i);
+                int n = P * n1 + B * (t + T * i);
                 n -= n >= M2 ? M2 : 0;
                 const double2 v = n < M ? base[n] : make_double2(0.0, 0.0);
                 vr[n1][i] = v.x; vi[n1][i] = v.y;
@@ -1091,19 +1091,21 @@ k_conv_z_pf(double2* __restrict__ B2, const double* __restrict__ Gk, const doubl
 #pragma unroll 1
         for (int pass = 0; pass < 2; ++pass) {
 #pragma unroll
-            for (int n1 = 0; n1 < 3; ++n1) fft2_forward_lc<Cfg>(vr[n1], vi[n1], t, buf, cc, tn);
+            for (int n1 = 0; n1 < B; ++n1) fft2_forward_lc<Cfg>(vr[n1], vi[n1], t, buf, cc, tn);
 #pragma unroll
-            for (int i = 0; i < R; ++i) {   // radix 3 across the three sub-transforms (register stride R)
-                double ar[3] = {vr[0][i], vr[1][i], vr[2][i]}, ai[3] = {vi[0][i], vi[1][i], vi[2][i]};
-                dft3<1>(ar, ai);
-                vr[0][i] = ar[0]; vr[1][i] = ar[1]; vr[2][i] = ar[2];
-                vi[0][i] = ai[0]; vi[1][i] = ai[1]; vi[2][i] = ai[2];
+            for (int i = 0; i < R; ++i) {   // radix B across the B sub-transforms (register stride R)
+                double ar[B], ai[B];
+#pragma unroll
+                for (int n1 = 0; n1 < B; ++n1) { ar[n1] = vr[n1][i]; ai[n1] = vi[n1][i]; }
+                if constexpr (B == 3) dft3<1>(ar, ai); else dft5<1>(ar, ai);
+#pragma unroll
+                for (int n1 = 0; n1 < B; ++n1) { vr[n1][i] = ar[n1]; vi[n1][i] = ai[n1]; }
             }
-            if (pass == 0) {   // slot (k1, i) now holds X[k], k = k1 (mod 3), k = t + T i (mod P); Y = conj(Ghat X)
+            if (pass == 0) {   // slot (k1, i) now holds X[k], k = k1 (mod B), k = t + T i (mod P); Y = conj(Ghat X)
                 mbar_wait(gbar, gpar);
                 gpar ^= 1;
 #pragma unroll
-                for (int k1 = 0; k1 < 3; ++k1)
+                for (int k1 = 0; k1 < B; ++k1)
 #pragma unroll
                     for (int i = 0; i < R; ++i) {
                         double gk = gst[k1 * P + t + T * i];
@@ -1117,10 +1119,10 @@ k_conv_z_pf(double2* __restrict__ B2, const double* __restrict__ Gk, const doubl
         }
         // v = FFT(conj(Ghat X)) = conj(y), back in the order of the load; the kept half
 #pragma unroll
-        for (int n1 = 0; n1 < 3; ++n1)
+        for (int n1 = 0; n1 < B; ++n1)
 #pragma unroll
             for (int i = 0; i < R; ++i) {
-                int n = P * n1 + 3 * (t + T * i);
+                int n = P * n1 + B * (t + T * i);
                 n -= n >= M2 ? M2 : 0;
                 if (n < M) obase[n] = DER ? make_double2(-vi[n1][i], -vr[n1][i]) : make_double2(vr[n1][i], -vi[n1][i]);
             }
