@@ -196,8 +196,9 @@ int fsp_destroy(fsp_plan* p);
  * Between phases ALL ranks must have finished the previous phase (the caller synchronises its stream and runs a
  * barrier, e.g. torch.distributed.barrier(); two barriers per solve, nothing else crosses ranks).  Bytes leaving a GPU
  * per solve: 2 x 16 (Nx+1)(Ny/P) Nz (P-1)/P.  Power-of-two meshes with Ny % P == 0, P <= 16, (Ny/P) Nz >= 64.
- * The Green precompute is replicated: every rank computes the whole octant and keeps the rows of its planes
- * (stated limitation: the transient and the (N+1)^3 table are not sharded yet).
+ * The Green precompute is replicated: every rank computes the whole table and octant (2 x 8 (N+1)^3 bytes, allocated
+ * for the duration of fsp_sharded_precompute_green only and reported by its peak) and keeps the spectrum rows of its
+ * own planes; between solves a rank holds its slab of the workspace and those rows, nothing of full size.
  * Verified on ONE device with P plans in one process (phases run in turn, tests/test_gpu_sharded.py) and, for the
  * index arithmetic, by a world-size-2 CPU test; NOT yet measured on a multi-GPU node.
  */

@@ -951,6 +951,16 @@ int precompute_impl(fsp_plan* p) {
     ScopedFree tmp;
     size_t peak = 0;
     const int blk = 256;
+    struct TransientTables {   // sharded plan, y-z stage: T and Goct live for the duration of this call only
+        fsp_plan* p; bool on;
+        ~TransientTables() { if (on) { cudaFree(p->T); cudaFree(p->Goct); p->T = nullptr; p->Goct = nullptr; } }
+    } transient{p, false};
+    if (p->stage == 2) {
+        int rc = dev_alloc(&p->T, (size_t)tcount, &peak);
+        if (rc == FSP_OK) rc = dev_alloc(&p->Goct, (size_t)tcount, &peak);
+        transient.on = true;
+        if (rc != FSP_OK) return rc;
+    }
 
     if (p->algorithm == FSP_HOCKNEY) {
         k_fill_he<<<grid_for(tcount, blk), blk, 0, p->stream>>>(p->T, Nx, Ny, Nz, hx, hy, hz, p->g0);
@@ -1202,8 +1212,9 @@ static int plan_create_impl(fsp_plan** out, int Nx, int Ny, int Nz, const double
         const cuuint32_t box[4] = {2 * kwy, 1, (cuuint32_t)(Ny < 256 ? Ny : 256), 1};
         rc = make_tensor_map(&p->tmB2y, p->B2, 4, dims, strides, box);
     }
-    if (rc == FSP_OK && want_yz) rc = dev_alloc(&p->T, nt, &p->bytes);
-    if (rc == FSP_OK && want_yz) rc = dev_alloc(&p->Goct, nt, &p->bytes);
+    // (the y-z stage of a sharded plan holds the table and the un-normalised octant only while its precompute runs)
+    if (rc == FSP_OK && want_yz && stage == 0) rc = dev_alloc(&p->T, nt, &p->bytes);
+    if (rc == FSP_OK && want_yz && stage == 0) rc = dev_alloc(&p->Goct, nt, &p->bytes);
     if (rc == FSP_OK && want_x) rc = make_table(&p->Wx, 2 * Nx, &p->bytes);
     if (rc == FSP_OK && want_yz) rc = make_table(&p->Wy, 2 * Ny, &p->bytes);
     if (rc == FSP_OK && want_yz) rc = make_table(&p->Wz, 2 * Nz, &p->bytes);
