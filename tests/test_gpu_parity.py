@@ -492,3 +492,31 @@ def test_mixed_radix_field_output():
     check(phi, phi_o)
     for d in range(3):
         check(E[d], E_o[d])
+
+
+def test_plan_on_a_side_stream_and_two_plans_interleaved():
+    """All work of a plan is enqueued on the stream given at creation (include/fsp.h): a plan on a non-default stream, and
+    two plans on two streams whose solves are interleaved from one host thread, give the results of the default stream."""
+    w = W.random_density((128, 256, 64), seed=31)
+    with binding.Plan(w.N, w.h, binding.HOCKNEY) as p0:
+        ref = gpu_solve(p0.precompute_green(), w.rho)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    rho = torch.from_numpy(w.rho).cuda()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s1):
+        p1 = binding.Plan(w.N, w.h, binding.HOCKNEY)
+    with torch.cuda.stream(s2):
+        p2 = binding.Plan(w.N, w.h, binding.VICO_2)
+    assert p1.stream == s1.cuda_stream and p2.stream == s2.cuda_stream and p1.stream != p2.stream
+    p1.precompute_green(); p2.precompute_green()
+    a = [torch.empty_like(rho) for _ in range(3)]
+    b = [torch.empty_like(rho) for _ in range(3)]
+    for i in range(3):
+        p1.solve(rho, a[i])
+        p2.solve(rho, b[i])
+    s1.synchronize(); s2.synchronize()
+    for i in range(3):
+        assert np.array_equal(a[i].cpu().numpy(), ref)
+        assert torch.equal(b[i], b[0])
+    check(b[0].cpu().numpy(), oracle.OraclePlan(w.N, w.h, oracle.VICO_2).precompute_green().solve(w.rho))
+    p1.destroy(); p2.destroy()
