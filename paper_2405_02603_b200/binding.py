@@ -21,6 +21,7 @@ ERRORS = {0: "FSP_OK", -1: "FSP_ERR_INVALID_ARG", -2: "FSP_ERR_NOT_PRECOMPUTED",
           -3: "FSP_ERR_OUT_OF_MEMORY", -4: "FSP_ERR_CUDA", -5: "FSP_ERR_NO_DEVICE"}
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
+# the in-tree library; FSP_LIB selects another build of the SAME library (A/B measurements of kernel variants), never a fallback
 LIB_PATH = os.environ.get("FSP_LIB", os.path.join(_HERE, "libfsp.so"))
 _lib = None
 
