@@ -822,17 +822,14 @@ int launch_dct1_tile(fsp_plan* p, const double* in, double* out, int n, int nout
     CU(cudaGetLastError());
     return FSP_OK;
 }
-int dct1_axis(fsp_plan* p, const double* in, double* out, const long in_dims[3], const long out_dims[3],
-              int axis, int n, int nout, double scale, const GLFill* fill = nullptr) {
-    const long is[3] = {in_dims[1] * in_dims[2], in_dims[2], 1};
-    const long os[3] = {out_dims[1] * out_dims[2], out_dims[2], 1};
-    const int o1 = (axis + 1) % 3, o2 = (axis + 2) % 3;
-    const long n1 = in_dims[o1], n2 = in_dims[o2];
+// DCT-I of an nA x nB grid of pencils with explicit strides: element k of pencil (a, b) at in[a ai[0] + b ai[1] + k ai[2]],
+// output d at out[a ao[0] + b ao[1] + d ao[2]]; b is the dimension the kernels coalesce over.  kNoTileKernel when none of
+// the pencil-grid kernels takes this length.
+constexpr int kNoTileKernel = 1;
+int dct1_strided(fsp_plan* p, const double* in, double* out, int n, int nout, long nA, long nB, const long ai[3],
+                 const long ao[3], double scale, const GLFill* fill) {
     const int Lf = 2 * n;
     if ((n & (n - 1)) != 0) {   // not a power of two: the cosine sum as written (k_dct1_direct)
-        const int bdim = axis == 2 ? 1 : 2, adim = axis == 2 ? 0 : (axis == 0 ? 1 : 0);
-        const long nA = in_dims[adim], nB = in_dims[bdim];
-        const long ai[3] = {is[adim], is[bdim], is[axis]}, ao[3] = {os[adim], os[bdim], os[axis]};
         constexpr int C = 8;
         const size_t smem = sizeof(double) * ((size_t)2 * n + (size_t)(n + 1) * C);
         if (smem > 200 * 1024) return FSP_ERR_INVALID_ARG;
@@ -849,9 +846,6 @@ int dct1_axis(fsp_plan* p, const double* in, double* out, const long in_dims[3],
         return FSP_OK;
     }
     if (n >= 8 && n <= 1024) {   // the warp-level transform of the solve, one pencil per lane group (k_dct1_warp)
-        const int bdim = axis == 2 ? 1 : 2, adim = axis == 2 ? 0 : (axis == 0 ? 1 : 0);
-        const long nA = in_dims[adim], nB = in_dims[bdim];
-        const long ai[3] = {is[adim], is[bdim], is[axis]}, ao[3] = {os[adim], os[bdim], os[axis]};
         switch (n) {
             case 8: return launch_dct1_warp<8>(p, in, out, nout, nA, nB, ai, ao, scale, fill);
             case 16: return launch_dct1_warp<16>(p, in, out, nout, nA, nB, ai, ao, scale, fill);
@@ -863,18 +857,28 @@ int dct1_axis(fsp_plan* p, const double* in, double* out, const long in_dims[3],
             default: return launch_dct1_warp<1024>(p, in, out, nout, nA, nB, ai, ao, scale, fill);
         }
     }
-    {   // tile kernel: C pencils per CTA along the contiguous dimension (z; y when the transform axis is z)
-        const int bdim = axis == 2 ? 1 : 2, adim = axis == 2 ? 0 : (axis == 0 ? 1 : 0);
-        const long nA = in_dims[adim], nB = in_dims[bdim];
-        auto tile_smem = [&](int C) { return sizeof(double2) * ((size_t)n + (size_t)C * Lf); };
-        const long args_in[3] = {is[adim], is[bdim], is[axis]}, args_out[3] = {os[adim], os[bdim], os[axis]};
-        // several CTAs per SM: the Stockham stages are latency-bound (one butterfly per thread between two barriers)
-        if (tile_smem(8) <= 72 * 1024) return launch_dct1_tile<8>(p, in, out, n, nout, nA, nB, args_in, args_out, scale, tile_smem(8), 512, fill);
-        if (tile_smem(4) <= 76 * 1024) return launch_dct1_tile<4>(p, in, out, n, nout, nA, nB, args_in, args_out, scale, tile_smem(4), 256, fill);
-        if (tile_smem(2) <= 100 * 1024) return launch_dct1_tile<2>(p, in, out, n, nout, nA, nB, args_in, args_out, scale, tile_smem(2), 512, fill);
-        if (tile_smem(4) <= 200 * 1024) return launch_dct1_tile<4>(p, in, out, n, nout, nA, nB, args_in, args_out, scale, tile_smem(4), 1024, fill);
-        if (tile_smem(2) <= 200 * 1024) return launch_dct1_tile<2>(p, in, out, n, nout, nA, nB, args_in, args_out, scale, tile_smem(2), 512, fill);
-    }
+    // Stockham tile kernel, C pencils per CTA.  Several CTAs per SM: the stages are latency-bound (one butterfly per
+    // thread between two barriers)
+    auto tile_smem = [&](int C) { return sizeof(double2) * ((size_t)n + (size_t)C * Lf); };
+    if (tile_smem(8) <= 72 * 1024) return launch_dct1_tile<8>(p, in, out, n, nout, nA, nB, ai, ao, scale, tile_smem(8), 512, fill);
+    if (tile_smem(4) <= 76 * 1024) return launch_dct1_tile<4>(p, in, out, n, nout, nA, nB, ai, ao, scale, tile_smem(4), 256, fill);
+    if (tile_smem(2) <= 100 * 1024) return launch_dct1_tile<2>(p, in, out, n, nout, nA, nB, ai, ao, scale, tile_smem(2), 512, fill);
+    if (tile_smem(4) <= 200 * 1024) return launch_dct1_tile<4>(p, in, out, n, nout, nA, nB, ai, ao, scale, tile_smem(4), 1024, fill);
+    if (tile_smem(2) <= 200 * 1024) return launch_dct1_tile<2>(p, in, out, n, nout, nA, nB, ai, ao, scale, tile_smem(2), 512, fill);
+    return kNoTileKernel;
+}
+// the same along one axis of a C-order array: pencils tiled along the contiguous dimension (z; y when the axis is z)
+int dct1_axis(fsp_plan* p, const double* in, double* out, const long in_dims[3], const long out_dims[3],
+              int axis, int n, int nout, double scale, const GLFill* fill = nullptr) {
+    const long is[3] = {in_dims[1] * in_dims[2], in_dims[2], 1};
+    const long os[3] = {out_dims[1] * out_dims[2], out_dims[2], 1};
+    const int o1 = (axis + 1) % 3, o2 = (axis + 2) % 3;
+    const long n1 = in_dims[o1], n2 = in_dims[o2];
+    const int Lf = 2 * n;
+    const int bdim = axis == 2 ? 1 : 2, adim = axis == 2 ? 0 : (axis == 0 ? 1 : 0);
+    const long ai[3] = {is[adim], is[bdim], is[axis]}, ao[3] = {os[adim], os[bdim], os[axis]};
+    const int rc = dct1_strided(p, in, out, n, nout, in_dims[adim], in_dims[bdim], ai, ao, scale, fill);
+    if (rc != kNoTileKernel) return rc;
     if (fill) return FSP_ERR_INVALID_ARG;   // (lengths beyond the tile kernels: m_d N_d > 7264 is rejected before)
     const size_t smem = sizeof(double2) * 2 * (size_t)Lf;
     { static OccCache optin; const int rc_ = cached_smem_optin(optin, p->device, k_dct1_pencils, smem); if (rc_ != FSP_OK) return rc_; }
@@ -882,6 +886,24 @@ int dct1_axis(fsp_plan* p, const double* in, double* out, const long in_dims[3],
     k_dct1_pencils<<<(unsigned)(n1 * n2), threads, smem, p->stream>>>(in, out, n, nout, is[axis], os[axis], n2,
                                                                       is[o1], is[o2], os[o1], os[o2], scale);
     CU(cudaGetLastError());
+    return FSP_OK;
+}
+// the y pass followed by the x pass of a 3-D DCT-I, src[a < na][b < nb][z < nz1] -> dst[Nx+1][Ny+1][nz1], through an
+// intermediate `mid` stored [dy][a][z] -- dy OUTERMOST, so that the x pass reads pencils whose elements are nz1 doubles
+// apart instead of (Ny+1) nz1 (2 MB at 512^3: one page per element).  y_only / x_only run one half (chunked callers).
+int dct1_y_then_x(fsp_plan* p, const double* src, double* mid, double* dst, long na_total, long a0, long na, long nb_in,
+                  long nz1, int ny, int nyout, int nx, int nxout, double scale, bool do_y, bool do_x) {
+    int rc;
+    if (do_y) {   // src[a][ky][z] (chunk of na planes starting at plane a0 of na_total) -> mid[dy][a0 + a][z]
+        const long ai[3] = {nb_in * nz1, 1, nz1}, ao[3] = {nz1, 1, na_total * nz1};
+        rc = dct1_strided(p, src, mid + (size_t)a0 * nz1, ny, nyout, na, nz1, ai, ao, 1.0, nullptr);
+        if (rc != FSP_OK) return rc == kNoTileKernel ? FSP_ERR_INVALID_ARG : rc;
+    }
+    if (do_x) {   // mid[dy][kx][z] -> dst[dx][dy][z]
+        const long ai[3] = {na_total * nz1, 1, nz1}, ao[3] = {nz1, 1, (long)nyout * nz1};
+        rc = dct1_strided(p, mid, dst, nx, nxout, nyout, nz1, ai, ao, scale, nullptr);
+        if (rc != FSP_OK) return rc == kNoTileKernel ? FSP_ERR_INVALID_ARG : rc;
+    }
     return FSP_OK;
 }
 
@@ -1043,13 +1065,11 @@ int precompute_impl(fsp_plan* p) {
                 const long nc = Kx - a0 < chunk ? Kx - a0 : chunk;
                 const long fd[3] = {nc, Ky, nz + 1L};
                 const long ad[3] = {nc, Ky, Nz + 1};
-                const long bd[3] = {nc, Ny + 1, Nz + 1};
                 const GLFill gl{PI2 / ((double)m[0] * Nx * hx), PI2 / ((double)m[1] * Ny * hy), PI2 / ((double)m[2] * Nz * hz), L, a0};
                 if ((rc = dct1_axis(p, nullptr, a, fd, ad, 2, nz, Nz + 1, 1.0, &gl)) != FSP_OK) return rc;
-                if ((rc = dct1_axis(p, a, b + (size_t)a0 * (Ny + 1) * (Nz + 1), ad, bd, 1, ny, Ny + 1, 1.0)) != FSP_OK) return rc;
+                if ((rc = dct1_y_then_x(p, a, b, nullptr, Kx, a0, nc, Ky, Nz + 1, ny, Ny + 1, nx, Nx + 1, 1.0, true, false)) != FSP_OK) return rc;
             }
-            const long bd[3] = {Kx, Ny + 1, Nz + 1};
-            if ((rc = dct1_axis(p, b, p->T, bd, tdims, 0, nx, Nx + 1, vscale)) != FSP_OK) return rc;
+            if ((rc = dct1_y_then_x(p, nullptr, b, p->T, Kx, 0, Kx, Ky, Nz + 1, ny, Ny + 1, nx, Nx + 1, vscale, false, true)) != FSP_OK) return rc;
             }
         }
     }
@@ -1062,8 +1082,7 @@ int precompute_impl(fsp_plan* p) {
             tmp.ptrs.push_back(u);
         }
         if ((rc = dct1_axis(p, p->T, p->Goct, tdims, tdims, 2, Nz, Nz + 1, 1.0)) != FSP_OK) return rc;
-        if ((rc = dct1_axis(p, p->Goct, u, tdims, tdims, 1, Ny, Ny + 1, 1.0)) != FSP_OK) return rc;
-        if ((rc = dct1_axis(p, u, p->Goct, tdims, tdims, 0, Nx, Nx + 1, 1.0)) != FSP_OK) return rc;
+        if ((rc = dct1_y_then_x(p, p->Goct, u, p->Goct, Nx + 1, 0, Nx + 1, Ny + 1, Nz + 1, Ny, Ny + 1, Nx, Nx + 1, 1.0, true, true)) != FSP_OK) return rc;
     }
     // scale: hx hy hz / (8 Nx Ny Nz) (inverse DFT) / 2 (K1 produces 2X)
     const double gscale = hx * hy * hz / (8.0 * (double)Nx * (double)Ny * (double)Nz) * 0.5;
