@@ -6,14 +6,40 @@
 //   VG2:    G_L on the (2N+1)^3 lattice, DCT-I per axis, restricted to d <= N.
 //   all: Ghat = F{G2} of the 8-case mirror = 3-D DCT-I of T (G2 is real and even).
 //
-// These kernels are NOT on the per-solve path and are written for clarity, not speed: one CTA
-// transforms one pencil with a radix-2 Stockham FFT in shared memory; twiddles come from
-// sincospi() in fp64.
+// These kernels are NOT on the per-solve path (once per plan, again when the spacing changes).  Powers of two between
+// 8 and 1024 run on the warp-level transform of the solve (k_dct1_warp), other lengths on a Stockham tile kernel or the
+// cosine sum as written.
 #pragma once
 #include <cuda_runtime.h>
 #include "fft_warp.cuh"
 
 namespace fsp {
+
+// sin(x) up to sign for 0 <= x < 2^20 pi: x - n pi by a two-constant Cody-Waite reduction (n pi_hi is formed inside the
+// fma and the difference is exactly representable, so the reduced argument carries one rounding), then the Taylor
+// polynomial through x^21 on [-pi/2, pi/2] (first omitted term 1.3e-18 relative).  Eq. 3 needs sin^2 only, so the
+// factor (-1)^n is never formed.  A third of the instructions of sin(): no quadrant select, no conversions, no slow path
+// (the lattice argument is at most (L/2) pi sqrt(sum 1/h_d^2), 2.4e3 at 512^3; beyond the bound the library is called).
+constexpr double kSinModPiMax = 3.0e6;
+__device__ __forceinline__ double sin_mod_pi_nocheck(double x) {
+    const double RND = 6755399441055744.0;   // 1.5 * 2^52: adding and subtracting it rounds to the nearest integer
+    const double n = __dadd_rn(__fma_rn(x, 0.31830988618379067154, RND), -RND);
+    double f = __fma_rn(-n, 3.141592653589793116, x);
+    f = __fma_rn(-n, 1.2246467991473532e-16, f);
+    const double t = f * f;
+    double p = 1.0 / 51090942171709440000.0;
+    p = fma(p, t, -1.0 / 121645100408832000.0);
+    p = fma(p, t, 1.0 / 355687428096000.0);
+    p = fma(p, t, -1.0 / 1307674368000.0);
+    p = fma(p, t, 1.0 / 6227020800.0);
+    p = fma(p, t, -1.0 / 39916800.0);
+    p = fma(p, t, 1.0 / 362880.0);
+    p = fma(p, t, -1.0 / 5040.0);
+    p = fma(p, t, 1.0 / 120.0);
+    p = fma(p, t, -1.0 / 6.0);
+    return fma(f * t, p, f);
+}
+__device__ __forceinline__ double sin_mod_pi(double x) { return x > kSinModPiMax ? sin(x) : sin_mod_pi_nocheck(x); }
 
 // Eq. 3 with the s -> 0 limit L^2/2.
 // (1/|s| by rsqrt: one reciprocal square root instead of a square root and a division -- the fill is evaluated inside
@@ -22,7 +48,16 @@ __device__ __forceinline__ double vg_GL(double sx, double sy, double sz, double 
     const double s2 = sx * sx + sy * sy + sz * sz;
     if (s2 == 0.0) return 0.5 * L * L;
     const double r = rsqrt(s2);
-    const double q = sin(0.5 * L * (s2 * r)) * r;
+    const double q = sin_mod_pi(0.5 * L * (s2 * r)) * r;
+    return 2.0 * q * q;
+}
+// The same without a branch, for arguments known to stay below kSinModPiMax (the caller checks the largest one of its
+// pencil): independent evaluations then interleave in one instruction stream.  s = 0: s2 is raised to 1e-300, where
+// sin(x) = x to the last bit and the formula returns its own limit 2 (L/2)^2.
+__device__ __forceinline__ double vg_GL_straight(double s2xy, double sz, double halfL) {
+    const double s2 = fmax(fma(sz, sz, s2xy), 1.0e-300);
+    const double r = rsqrt(s2);
+    const double q = sin_mod_pi_nocheck(halfL * (s2 * r)) * r;
     return 2.0 * q * q;
 }
 
@@ -306,9 +341,15 @@ k_dct1_warp(const double* __restrict__ in, double* __restrict__ out, int nout, l
         if constexpr (FILL) {   // every lattice value once (each enters the even extension twice): through the exchange buffer
             double* xs = reinterpret_cast<double*>(buf);
             __syncwarp();   // the previous pencil's exchange has been read back
+            const double sxv = gl.sa * (double)(gl.a0 + ia), syv = gl.sb * (double)ib, s2xy = sxv * sxv + syv * syv;
+            const double szmax = gl.sk * (double)M, halfL = 0.5 * gl.L;
+            if (halfL * sqrt(fma(szmax, szmax, s2xy)) < kSinModPiMax) {   // (uniform over the lane group)
 #pragma unroll 8
-            for (int k = t; k <= M; k += T)   // (unrolled: eight independent sin / rsqrt chains in flight per lane)
-                xs[k] = vg_GL(gl.sa * (double)(gl.a0 + ia), gl.sb * (double)ib, gl.sk * (double)k, gl.L);
+                for (int k = t; k <= M; k += T)   // (unrolled, no branch: eight independent sin / rsqrt chains per lane)
+                    xs[k] = vg_GL_straight(s2xy, gl.sk * (double)k, halfL);
+            } else {
+                for (int k = t; k <= M; k += T) xs[k] = vg_GL(sxv, syv, gl.sk * (double)k, gl.L);
+            }
             __syncwarp();
         }
 #pragma unroll
