@@ -72,7 +72,8 @@ enum {
     FSP_ERR_NOT_PRECOMPUTED = -2, /* fsp_solve / getters before fsp_precompute_green                 */
     FSP_ERR_OUT_OF_MEMORY = -3,   /* device allocation failed (e.g. FSP_VICO at 1024^3: (4N)^3 lattice) */
     FSP_ERR_CUDA = -4,            /* a CUDA runtime call or kernel launch failed                     */
-    FSP_ERR_NO_DEVICE = -5        /* no CUDA device / not an sm_100 device                           */
+    FSP_ERR_NO_DEVICE = -5,       /* no CUDA device / not an sm_100 device                           */
+    FSP_ERR_STATIC_CAPACITY = -6  /* fsp_green_spectrum_static: table larger than FSP_STATIC_MAX_DOUBLES */
 };
 
 /* parameters settable before fsp_precompute_green */
@@ -273,6 +274,31 @@ int fsp_get_green_table(const fsp_plan* p, double* T_host);
  * (Nx+1)(Ny+1)(Nz+1) doubles in C order (F{G2} is real and even), to host memory.  Power-of-two meshes
  * only: on an embedded mesh the spectrum belongs to the transform mesh (FSP_ERR_INVALID_ARG). */
 int fsp_get_green_spectrum(const fsp_plan* p, double* Ghat_host);
+
+/*
+ * spectrum_static(T) -- the last step of the Green precompute, T -> F{G2} octant, WITHOUT any allocation.
+ *
+ * For callers that cannot call cudaMalloc where the spectrum has to be refreshed (the spacing changes whenever the bunch
+ * moves): under CUDA graph capture, in a serving loop, in harnesses that forbid it.  Computes what
+ * fsp_precompute_green leaves behind fsp_get_green_spectrum,
+ *     Ghat[kx][ky][kz] = sum_d w_dx w_dy w_dz T[dx][dy][dz] cos(pi kx dx/Nx) cos(pi ky dy/Ny) cos(pi kz dz/Nz),
+ * w = 1 at d = 0 and d = N_d, 2 between -- the 3-D DCT-I of the table, which IS the DFT of the mirrored G2
+ * (G2 is real and even) -- as three passes of cosine sums (k_dct1_direct, any N_d).
+ *   T_dev      device pointer, (Nx+1)(Ny+1)(Nz+1) doubles in C order (the layout of fsp_get_green_table); read-only
+ *   Ghat_dev   device pointer, same shape; written; must not overlap T_dev.  Both on the CURRENT device
+ *   Nx,Ny,Nz   1 <= N_d <= 512 and (Nx+1)(Ny+1)(Nz+1) <= FSP_STATIC_MAX_DOUBLES (a 64^3 mesh: 65^3 entries);
+ *              a larger table gives FSP_ERR_STATIC_CAPACITY and launches nothing
+ *   cuda_stream  the three kernels are enqueued there; no host synchronisation
+ * Scratch: the intermediate between the second and the third pass lives in a file-scope `static __device__` array of
+ * FSP_STATIC_MAX_DOUBLES doubles (2.2 MB) that every GPU holds from the moment it loads libfsp.so until the process
+ * exits.  No cudaMalloc, cudaFree or allocating library call is made, on the first call or later (the first call on a
+ * device resolves the array's device address with cudaGetSymbolAddress: make one call before starting a capture).
+ * ALL calls on one device share that array: two calls that overlap on the GPU (different streams, or graphs replayed
+ * concurrently) race and give garbage; calls on one stream are ordered and safe.  The array keeps the last call's
+ * contents; nothing in it has to start at zero (every entry that is read was written by the same call's second pass).
+ */
+#define FSP_STATIC_MAX_DOUBLES 274625 /* 65^3 */
+int fsp_green_spectrum_static(const double* T_dev, double* Ghat_dev, int Nx, int Ny, int Nz, void* cuda_stream);
 
 /*
  * Per-kernel timing.  With profiling on, fsp_solve brackets each of its kernels with CUDA events

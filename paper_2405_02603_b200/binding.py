@@ -47,6 +47,7 @@ SIGNATURES = {
     "fsp_vg_lattice_is_safe": (_i, [_vp, _c.POINTER(_i)]),
     "fsp_get_green_table": (_i, [_vp, _dp]),
     "fsp_get_green_spectrum": (_i, [_vp, _dp]),
+    "fsp_green_spectrum_static": (_i, [_vp, _vp, _i, _i, _i, _vp]),
     "fsp_set_profiling": (_i, [_vp, _i]),
     "fsp_get_kernel_times": (_i, [_vp, _c.POINTER(_c.c_float), _c.POINTER(_i)]),
     "fsp_shard_planes": (_i, [_i, _i, _i, _c.POINTER(_i), _c.POINTER(_i)]),
@@ -210,6 +211,17 @@ def get_green_spectrum(plan: int, N) -> np.ndarray:
     G = np.empty(tuple(n + 1 for n in N), dtype=np.float64)
     _chk(lib().fsp_get_green_spectrum(plan, G.ctypes.data_as(_dp)), "fsp_get_green_spectrum")
     return G
+
+
+STATIC_MAX_DOUBLES = 274625   # FSP_STATIC_MAX_DOUBLES (65^3)
+ERR_STATIC_CAPACITY = -6
+
+
+def green_spectrum_static(T_dev, Ghat_dev, N, stream: int = 0) -> None:
+    """fsp_green_spectrum_static: T -> spectrum octant on the current device, scratch in the library's static device
+    array, no allocation.  T_dev, Ghat_dev: contiguous fp64 CUDA tensors of shape (Nx+1, Ny+1, Nz+1)."""
+    _chk(lib().fsp_green_spectrum_static(_ptr(T_dev), _ptr(Ghat_dev), int(N[0]), int(N[1]), int(N[2]),
+                                         ctypes.c_void_p(int(stream) or None)), "fsp_green_spectrum_static")
 
 
 def set_profiling(plan: int, on: bool) -> None:

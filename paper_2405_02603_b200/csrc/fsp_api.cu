@@ -1137,6 +1137,7 @@ const char* fsp_strerror(int code) {
         case FSP_ERR_OUT_OF_MEMORY: return "device memory allocation failed";
         case FSP_ERR_CUDA: return "CUDA runtime or kernel launch error";
         case FSP_ERR_NO_DEVICE: return "no usable CUDA device";
+        case FSP_ERR_STATIC_CAPACITY: return "table larger than the static scratch array (FSP_STATIC_MAX_DOUBLES)";
         default: return "unknown error code";
     }
 }
@@ -1787,3 +1788,68 @@ int fsp_ipc_close_handle(void* dev_ptr) {
 }
 
 }  // extern "C"
+
+// ---- the allocation-free entry point (include/fsp.h: fsp_green_spectrum_static) -------------------------------------
+// The scratch of the 3-D DCT-I (the array between the y pass and the x pass) as a file-scope device array.  In HOST code
+// the name g_static_scratch is a stand-in, not a device address: the address the kernels get comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+static __device__ __align__(256) double g_static_scratch[FSP_STATIC_MAX_DOUBLES];
+
+namespace {
+constexpr int kStaticMaxDevices = 64;
+std::atomic<double*> g_static_scratch_ptr[kStaticMaxDevices];   // zero-initialised: not yet resolved on that device
+
+int static_scratch_address(double** out) {
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return FSP_ERR_NO_DEVICE;
+    double* ptr = g_static_scratch_ptr[dev].load(std::memory_order_acquire);
+    if (!ptr) {   // (two threads may both resolve it: same answer, no allocation either way)
+        CU(cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), g_static_scratch));
+        if (!ptr) return FSP_ERR_CUDA;
+        g_static_scratch_ptr[dev].store(ptr, std::memory_order_release);
+    }
+    *out = ptr;
+    return FSP_OK;
+}
+
+// one pass of cosine sums over an nA x nB grid of pencils (strides as in dct1_strided); n <= 512: 25 KB of shared memory
+// at most, below the 48 KB that need no opt-in.
+// C = 4 on purpose: the instantiation must be one that the plan path (dct1_strided: C = 8) never launches.  That path
+// sets cudaFuncAttributeMaxDynamicSharedMemorySize of ITS kernel to the largest request seen so far, which LOWERS the
+// limit below the default 48 KB while only short transforms have run -- a launch from here with a longer one would then
+// fail, or not, depending on which plans the process has created before.  This kernel's attribute is never touched.
+int static_dct1_pass(const double* in, double* out, int n, long nA, long nB, const long ai[3], const long ao[3],
+                     cudaStream_t stream) {
+    constexpr int C = 4;
+    const size_t smem = sizeof(double) * ((size_t)2 * n + (size_t)(n + 1) * C);
+    k_dct1_direct<C, false><<<(unsigned)(nA * ((nB + C - 1) / C)), 256, smem, stream>>>(
+        in, out, n, n + 1, nB, ai[0], ai[1], ai[2], ao[0], ao[1], ao[2], 1.0, GLFill{0.0, 0.0, 0.0, 0.0, 0});
+    CU(cudaGetLastError());
+    return FSP_OK;
+}
+}  // namespace
+
+extern "C" int fsp_green_spectrum_static(const double* T_dev, double* Ghat_dev, int Nx, int Ny, int Nz, void* cuda_stream) {
+    if (!T_dev || !Ghat_dev || T_dev == Ghat_dev) return FSP_ERR_INVALID_ARG;
+    if (Nx < 1 || Ny < 1 || Nz < 1 || Nx > 512 || Ny > 512 || Nz > 512) return FSP_ERR_INVALID_ARG;
+    const long X = Nx + 1L, Y = Ny + 1L, Z = Nz + 1L;
+    if (X * Y * Z > (long)FSP_STATIC_MAX_DOUBLES) return FSP_ERR_STATIC_CAPACITY;
+    double* mid = nullptr;
+    int rc = static_scratch_address(&mid);
+    if (rc != FSP_OK) return rc;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    {   // z pass: T[x][y][z] -> Ghat[x][y][kz]
+        const long ai[3] = {Y * Z, Z, 1}, ao[3] = {Y * Z, Z, 1};
+        if ((rc = static_dct1_pass(T_dev, Ghat_dev, Nz, X, Y, ai, ao, stream)) != FSP_OK) return rc;
+    }
+    {   // y pass: Ghat[x][y][kz] -> mid[ky][x][kz]  (ky outermost: the x pass reads pencils Z doubles apart)
+        const long ai[3] = {Y * Z, 1, Z}, ao[3] = {Z, 1, X * Z};
+        if ((rc = static_dct1_pass(Ghat_dev, mid, Ny, X, Z, ai, ao, stream)) != FSP_OK) return rc;
+    }
+    {   // x pass: mid[ky][x][kz] -> Ghat[kx][ky][kz]
+        const long ai[3] = {X * Z, 1, Z}, ao[3] = {Z, 1, Y * Z};
+        if ((rc = static_dct1_pass(mid, Ghat_dev, Nx, Y, Z, ai, ao, stream)) != FSP_OK) return rc;
+    }
+    return FSP_OK;
+}

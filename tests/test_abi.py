@@ -35,7 +35,7 @@ def test_header_symbols_are_exported(libpath):
 def test_static_queries_and_error_strings(libpath):
     assert binding.version() >= 100
     assert [binding.kernel_name(i) for i in range(5)] == ["k_fwd_x_r2c", "k_fwd_y", "k_conv_z", "k_inv_y", "k_inv_x_c2r"]
-    for code in (0, -1, -2, -3, -4, -5):
+    for code in (0, -1, -2, -3, -4, -5, -6):
         assert binding.strerror(code) and "unknown" not in binding.strerror(code)
     assert "unknown" in binding.strerror(-99)
 
