@@ -435,6 +435,29 @@ def run_b200(args):
                            "peak": alu_peak, "unit": "TFLOP/s (fp64)", "frac": flops / (kms[dom] * 1e-3) / 1e12 / alu_peak,
                            "peak_source": "148 SMs x 64 DFMA/clk x 2 flop x SM clock sampled during the run "
                                           "(DESIGN.md: 64 fp64 ops/clk/SM measured)"}
+        # What one fp64 warp-instruction costs on THIS device (fsp_ubench_fp64, measured after the timed region): the
+        # 2 clocks behind the peak above hold only while at most two 64-bit sources are new register reads; the stage-2
+        # butterflies (lane-constant twiddles: three register sources) are bound by register-file reads at up to 3.
+        # issue_clk_per_warp_step: the fp64 instructions of k_conv_z_f's SASS weighted with these costs (profiles/
+        # r02_k3_sass_reuse.txt, 512^3 build); issue_frac: that roof over the measured time of the kernel.
+        try:
+            cost = {"dfma_3_new_sources": binding.ubench_fp64(0, 8), "dfma_2_repeated": binding.ubench_fp64(1, 8),
+                    "dfma_1_repeated": binding.ubench_fp64(2, 8), "dadd": binding.ubench_fp64(3, 8)}
+            roofline["alu"]["issue_clk_per_warp_instruction"] = {k: round(v, 3) for k, v in cost.items()}
+            if w.N[2] in (256, 512):
+                # fp64 instructions per lane and pencil (K3: 868 forward + 836 inverse, the same at both
+                # sizes: 32 points per lane): 928 stage-2 DFMAs with three register sources, 776 DADD / DMUL / DFMA
+                # with a compile-time twiddle; the three-source ones split by new register reads as in the SASS
+                mix = K3_SASS_3REG_MIX
+                c3 = mix[3] * cost["dfma_3_new_sources"] + mix[2] * cost["dfma_1_repeated"] + mix[0] * cost["dfma_2_repeated"]
+                issue_clk = 928 * c3 + 776 * cost["dadd"]
+                groups = pencils / (32 // (2 * w.N[2] // 32))                # lane groups of 2 Nz / 32 lanes per warp
+                t_issue = groups / (148 * 4) * issue_clk / (mhz * 1e6)       # warps per scheduler, one after the other
+                roofline["alu"]["issue_clk_per_warp_step"] = issue_clk   # one warp step = 32 / (2 Nz / 32) pencils
+                roofline["alu"]["issue_roof_ms"] = t_issue * 1e3
+                roofline["alu"]["issue_frac"] = t_issue * 1e3 / kms[dom]
+        except Exception as ex:  # noqa: BLE001
+            roofline["alu"]["issue_clk_per_warp_instruction"] = {"error": repr(ex)[:120]}
     err = _analytic_error(w, phi)
 
     # e2e: the public host-buffer call, H2D of rho and D2H of phi inside the timed region
@@ -499,6 +522,11 @@ def run_b200(args):
         dist.destroy_process_group()
     return 0
 
+
+# k_conv_z_f<1024>: share of its 544 three-register DFMAs by NEW register reads (3: no operand-reuse hit, 2: one hit,
+# 0: all three repeated), from `python -m paper_2405_02603_b200.sass_reuse k_conv_z_fILi1024ELb0`
+# (profiles/r02_k3_sass_reuse.txt; kernel sources c04166c8ac56f02f)
+K3_SASS_3REG_MIX = {3: 0.706, 2: 0.202, 0: 0.092}
 
 KERNEL_SOURCES = ("solve_kernels.cuh", "fft_warp.cuh", "fft_engine.cuh", "tma.cuh")
 

@@ -309,6 +309,17 @@ int fsp_green_spectrum_static(const double* T_dev, double* Ghat_dev, int Nx, int
 int fsp_set_profiling(fsp_plan* p, int on);
 int fsp_get_kernel_times(fsp_plan* p, float* ms, int* n_solves);
 
+/*
+ * Measurement hook (bench.py): clocks per fp64 warp-instruction and scheduler on the current
+ * device, with warps_per_sm (4, 8, .. 32) resident warps per SM each issuing a stream of independent instructions.
+ *   mode 0  DFMA, three register sources, none shared with the instruction before   (B200: 3.0)
+ *   mode 1  DFMA, two sources repeated from the instruction before (operand reuse)    (2.2)
+ *   mode 2  DFMA, one source repeated                                                 (2.2)
+ *   mode 3  DADD, two register sources                                                (2.0)
+ * clk_per_instr_out: host pointer.  Allocates and frees three small device buffers; synchronises the device.
+ */
+int fsp_ubench_fp64(int mode, int warps_per_sm, double* clk_per_instr_out);
+
 /* Name of solve kernel i (0..FSP_NUM_SOLVE_KERNELS-1), static string. */
 const char* fsp_kernel_name(int i);
 

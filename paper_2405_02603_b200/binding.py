@@ -48,6 +48,7 @@ SIGNATURES = {
     "fsp_get_green_table": (_i, [_vp, _dp]),
     "fsp_get_green_spectrum": (_i, [_vp, _dp]),
     "fsp_green_spectrum_static": (_i, [_vp, _vp, _i, _i, _i, _vp]),
+    "fsp_ubench_fp64": (_i, [_i, _i, _c.POINTER(_d)]),
     "fsp_set_profiling": (_i, [_vp, _i]),
     "fsp_get_kernel_times": (_i, [_vp, _c.POINTER(_c.c_float), _c.POINTER(_i)]),
     "fsp_shard_planes": (_i, [_i, _i, _i, _c.POINTER(_i), _c.POINTER(_i)]),
@@ -222,6 +223,14 @@ def green_spectrum_static(T_dev, Ghat_dev, N, stream: int = 0) -> None:
     array, no allocation.  T_dev, Ghat_dev: contiguous fp64 CUDA tensors of shape (Nx+1, Ny+1, Nz+1)."""
     _chk(lib().fsp_green_spectrum_static(_ptr(T_dev), _ptr(Ghat_dev), int(N[0]), int(N[1]), int(N[2]),
                                          ctypes.c_void_p(int(stream) or None)), "fsp_green_spectrum_static")
+
+
+def ubench_fp64(mode: int, warps_per_sm: int = 8) -> float:
+    """fsp_ubench_fp64: clocks per fp64 warp-instruction and scheduler (mode 0: DFMA with three new register sources,
+    1 / 2: with two / one source repeated, 3: DADD)."""
+    v = ctypes.c_double()
+    _chk(lib().fsp_ubench_fp64(int(mode), int(warps_per_sm), ctypes.byref(v)), "fsp_ubench_fp64")
+    return float(v.value)
 
 
 def set_profiling(plan: int, on: bool) -> None:

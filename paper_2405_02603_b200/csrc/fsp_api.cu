@@ -16,6 +16,7 @@
 #include "green_kernels.cuh"
 #include "solve_kernels.cuh"
 #include "shard.cuh"
+#include "ubench.cuh"
 
 using namespace fsp;
 
@@ -1788,6 +1789,41 @@ int fsp_ipc_close_handle(void* dev_ptr) {
 }
 
 }  // extern "C"
+
+// ---- fp64 issue-cost micro-benchmark (include/fsp.h: fsp_ubench_fp64; ubench.cuh) ------------------------------------
+extern "C" int fsp_ubench_fp64(int mode, int warps_per_sm, double* clk_per_instr_out) {
+    if (!clk_per_instr_out || mode < 0 || mode > 3) return FSP_ERR_INVALID_ARG;
+    if (warps_per_sm < 4 || warps_per_sm > 32 || warps_per_sm % 4 != 0) return FSP_ERR_INVALID_ARG;
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int threads = warps_per_sm * 32, iters = 4096;
+    double *out = nullptr, *in = nullptr;
+    long long* clk = nullptr;
+    int rc = dev_alloc(&out, (size_t)sms * threads, nullptr);
+    if (rc == FSP_OK) rc = dev_alloc(&in, (size_t)threads + 48, nullptr);
+    if (rc == FSP_OK) rc = dev_alloc(&clk, 1, nullptr);
+    long long h = 0;
+    if (rc == FSP_OK) {
+        cudaMemset(in, 0, sizeof(double) * ((size_t)threads + 48));
+        for (int rep = 0; rep < 2; ++rep) {   // the second launch is the measurement (the first loads the code)
+            switch (mode) {
+                case 0: k_ubench_fp64<0><<<sms, threads>>>(out, in, iters, clk); break;
+                case 1: k_ubench_fp64<1><<<sms, threads>>>(out, in, iters, clk); break;
+                case 2: k_ubench_fp64<2><<<sms, threads>>>(out, in, iters, clk); break;
+                default: k_ubench_fp64<3><<<sms, threads>>>(out, in, iters, clk); break;
+            }
+        }
+        cudaError_t e = cudaDeviceSynchronize();
+        if (e == cudaSuccess) e = cudaMemcpy(&h, clk, sizeof(h), cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) { (void)cudaGetLastError(); rc = map_cuda(e); }
+    }
+    cudaFree(out); cudaFree(in); cudaFree(clk);
+    if (rc != FSP_OK) return rc;
+    // per scheduler (4 per SM): warps_per_sm / 4 warps each issue iters * 16 instructions
+    *clk_per_instr_out = (double)h / ((double)iters * 16.0 * (warps_per_sm / 4.0));
+    return FSP_OK;
+}
 
 // ---- the allocation-free entry point (include/fsp.h: fsp_green_spectrum_static) -------------------------------------
 // The scratch of the 3-D DCT-I (the array between the y pass and the x pass) as a file-scope device array.  In HOST code
