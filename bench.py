@@ -494,6 +494,16 @@ def run_b200(args):
                             "d2h_bytes_per_step": 8 * V,
                             "matches_device_solve": bool(all(torch.equal(b.cuda(), phi) for b in ring_p))}
         del ring_r, ring_p, rl, pl
+        # the headline end-to-end figure is the throughput call (a stream of solves is what the metric, solves/s, is
+        # about): every step's rho still crosses PCIe in and every phi out inside the timed region; the one-call-per-step
+        # figure stays beside it
+        if e2e["pipelined"]["matches_device_solve"]:
+            single = {k: e2e[k] for k in ("value", "unit", "ms_per_step", "what", "matches_device_solve")}
+            e2e.update({"value": e2e["pipelined"]["value"], "ms_per_step": e2e["pipelined"]["ms_per_step"],
+                        "what": "fsp_solve_host_batch over the K steps: H2D of step i+1 and D2H of step i-1 overlap the "
+                                "five kernels of step i (ring of 3 pinned buffers each way); every step copies its own "
+                                "rho in and phi out inside the timed region",
+                        "matches_device_solve": True, "single_call": single})
     except Exception as ex:   # never fail the bench line on the extra leg
         e2e["pipelined"] = {"error": repr(ex)[:200]}
     plan_bytes, pre_peak = plan.bytes, plan.precompute_peak_bytes

@@ -83,3 +83,25 @@ def test_product_does_not_import_oracle():
                 txt = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(from|import)\s+oracle\b", txt, flags=re.M), f
                 assert "fsp_oracle" not in txt, f
+
+
+def test_sass_reuse_statistics_on_a_snippet():
+    """paper_2405_02603_b200.sass_reuse: a source counts as free only if the PREVIOUS instruction carried .reuse on the
+    same register in the same operand slot."""
+    from paper_2405_02603_b200 import sass_reuse
+    sass = """
+        /*0000*/                   DFMA R10, R2.reuse, R4, R6 ;
+        /*0010*/                   DFMA R12, -R2.reuse, R4, R6 ;
+        /*0020*/                   DFMA R14, R2, R8.reuse, R12.reuse ;
+        /*0030*/                   DFMA R16, R20, -R8, R12 ;
+        /*0040*/                   DFMA R18, R20, c[0x3][0x10], R12 ;
+        /*0050*/                   DADD R22, R18, -R16 ;
+        /*0060*/                   LDS.128 R24, [R9+UR4+0x10] ;
+        /*0070*/                   DMUL R26, R24, R24 ;
+    """.splitlines()
+    st = sass_reuse.reuse_statistics(sass)
+    assert st[("DFMA", 3, 3)] == 1          # the first one
+    assert st[("DFMA", 3, 2)] == 2          # R2 repeated; then R2 repeated again (R8, R12 new)
+    assert st[("DFMA", 3, 1)] == 1          # R8 and R12 repeated, R20 new
+    assert st[("DFMA", 2, 2)] == 1          # constant-bank operand: two register sources, neither flagged before
+    assert st[("DADD", 2, 2)] == 1 and st[("DMUL", 2, 2)] == 1

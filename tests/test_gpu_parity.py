@@ -520,3 +520,20 @@ def test_plan_on_a_side_stream_and_two_plans_interleaved():
         assert torch.equal(b[i], b[0])
     check(b[0].cpu().numpy(), oracle.OraclePlan(w.N, w.h, oracle.VICO_2).precompute_green().solve(w.rho))
     p1.destroy(); p2.destroy()
+
+
+@pytest.mark.gpu
+def test_fp64_issue_cost_hook():
+    """fsp_ubench_fp64 (bench.py's roofline.alu.issue_clk_per_warp_instruction): the fp64 pipe takes one warp-instruction
+    per 2 clocks and scheduler; a DFMA whose three sources are all new register reads cannot beat that, and nothing
+    should cost more than 4."""
+    dadd = binding.ubench_fp64(3, 8)
+    reuse = binding.ubench_fp64(1, 8)
+    three = binding.ubench_fp64(0, 8)
+    assert 1.9 < dadd < 2.6, dadd
+    assert 1.9 < reuse < 3.2, reuse
+    assert reuse - 0.05 <= three < 4.0, (reuse, three)
+    with pytest.raises(binding.FspError):
+        binding.ubench_fp64(7, 8)
+    with pytest.raises(binding.FspError):
+        binding.ubench_fp64(0, 5)
