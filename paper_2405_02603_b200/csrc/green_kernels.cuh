@@ -51,12 +51,24 @@ __device__ __forceinline__ double vg_GL(double sx, double sy, double sz, double 
     const double q = sin_mod_pi(0.5 * L * (s2 * r)) * r;
     return 2.0 * q * q;
 }
-// The same without a branch, for arguments known to stay below kSinModPiMax (the caller checks the largest one of its
-// pencil): independent evaluations then interleave in one instruction stream.  s = 0: s2 is raised to 1e-300, where
-// sin(x) = x to the last bit and the formula returns its own limit 2 (L/2)^2.
+// 1/sqrt(x) without the special-case branch of rsqrt() (whose slow-path call splits every evaluation into basic blocks
+// of its own and keeps independent evaluations from interleaving): fp32 seed, two Newton steps in fp64 (relative error
+// 1e-7 -> 1.5e-14 -> 3e-28, i.e. the rounding of the last step).  x in [kRsqrtMin, kRsqrtMax] (the fp32 range).
+constexpr double kRsqrtMin = 1.0e-35, kRsqrtMax = 1.0e37;
+__device__ __forceinline__ double rsqrt_straight(double x) {
+    const double y0 = (double)rsqrtf((float)x);
+    const double hx = 0.5 * x;
+    double e = fma(-hx * y0, y0, 0.5);
+    const double y1 = fma(y0, e, y0);
+    e = fma(-hx * y1, y1, 0.5);
+    return fma(y1, e, y1);
+}
+// Eq. 3 without a branch, for arguments known to stay below kSinModPiMax and s^2 inside the range of rsqrt_straight or
+// zero (the caller checks its pencil): independent evaluations then interleave in one instruction stream.  s = 0: s^2 is
+// raised to kRsqrtMin, where sin(x) = x to the last bit and the formula returns its own limit 2 (L/2)^2.
 __device__ __forceinline__ double vg_GL_straight(double s2xy, double sz, double halfL) {
-    const double s2 = fmax(fma(sz, sz, s2xy), 1.0e-300);
-    const double r = rsqrt(s2);
+    const double s2 = fmax(fma(sz, sz, s2xy), kRsqrtMin);
+    const double r = rsqrt_straight(s2);
     const double q = sin_mod_pi_nocheck(halfL * (s2 * r)) * r;
     return 2.0 * q * q;
 }
@@ -343,10 +355,17 @@ k_dct1_warp(const double* __restrict__ in, double* __restrict__ out, int nout, l
             __syncwarp();   // the previous pencil's exchange has been read back
             const double sxv = gl.sa * (double)(gl.a0 + ia), syv = gl.sb * (double)ib, s2xy = sxv * sxv + syv * syv;
             const double szmax = gl.sk * (double)M, halfL = 0.5 * gl.L;
-            if (halfL * sqrt(fma(szmax, szmax, s2xy)) < kSinModPiMax) {   // (uniform over the lane group)
+            const double s2max = fma(szmax, szmax, s2xy);
+            // (uniform over the lane group) arguments in the range of the branch-free forms: sin below its bound, every
+            // non-zero s^2 of the pencil inside the fp32 range of the rsqrt seed
+            if (halfL * sqrt(s2max) < kSinModPiMax && s2max < kRsqrtMax && gl.sk * gl.sk > kRsqrtMin &&
+                (s2xy == 0.0 || s2xy > kRsqrtMin)) {
+                // M / T full rounds with a compile-time trip count (no bound check, no branch: the evaluations of a
+                // lane interleave, eight sin / rsqrt chains in flight), then the one entry k = M
 #pragma unroll 8
-                for (int k = t; k <= M; k += T)   // (unrolled, no branch: eight independent sin / rsqrt chains per lane)
-                    xs[k] = vg_GL_straight(s2xy, gl.sk * (double)k, halfL);
+                for (int i = 0; i < M / T; ++i) xs[t + T * i] = vg_GL_straight(s2xy, gl.sk * (double)(t + T * i), halfL);
+                const double last = vg_GL_straight(s2xy, szmax, halfL);
+                if (t == 0) xs[M] = last;
             } else {
                 for (int k = t; k <= M; k += T) xs[k] = vg_GL(sxv, syv, gl.sk * (double)k, gl.L);
             }
