@@ -724,6 +724,13 @@ def extras(args, peak):
                                          "frac_of_measured_peak": model / (ms * 1e-3) / 1e9 / peak,
                                          "plan_bytes": plan.bytes}
         del rho, phi, E
+    # fsp_solve allocates nothing and never synchronises, so a caller can capture it into a CUDA graph (a PIC loop
+    # captures its whole time step): K solves per replay against the same K plain calls, on the plan's own stream
+    for wname in ("64", "256"):
+        try:
+            out[f"graph_replay_{wname}_HE"] = graph_replay_leg(wname)
+        except Exception as e:   # an extra line must never fail the bench
+            out[f"graph_replay_{wname}_HE"] = {"error": repr(e)[:200]}
     for wname, steps in (("256", 20), ("512", 5)):
         try:
             torch.cuda.empty_cache()
@@ -732,6 +739,47 @@ def extras(args, peak):
             out[f"cufft_unpruned_{wname}"] = {"error": repr(e)[:200]}
     torch.cuda.empty_cache()
     return out
+
+
+def graph_replay_leg(wname, K=20, reps=20):
+    import torch
+    from paper_2405_02603_b200 import binding, workloads as W
+    _, builder, kw, wdesc = WORKLOADS[wname]
+    w = getattr(W, builder)(**kw)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st), binding.Plan(w.N, w.h, binding.HOCKNEY, stream=st.cuda_stream) as plan:
+        plan.precompute_green()
+        rho = torch.from_numpy(w.rho).cuda()
+        phi = torch.empty_like(rho)
+        for _ in range(3):
+            plan.solve(rho, phi)
+        st.synchronize()
+        ref = phi.clone()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            for _ in range(K):
+                plan.solve(rho, phi)
+        phi.zero_()
+        g.replay()
+        st.synchronize()
+        same = bool(torch.equal(phi, ref))
+
+        def per_solve_ms(f):
+            f()
+            st.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(st)
+            for _ in range(reps):
+                f()
+            e1.record(st)
+            e1.synchronize()
+            return e0.elapsed_time(e1) / reps / K
+
+        t_graph = per_solve_ms(g.replay)
+        t_plain = per_solve_ms(lambda: [plan.solve(rho, phi) for _ in range(K)])
+        del g
+    return {"workload": wdesc, "solves_per_replay": K, "ms_per_solve_graph": t_graph, "ms_per_solve_plain": t_plain,
+            "bit_identical": same}
 
 
 def cufft_comparison(wname, steps):

@@ -537,3 +537,35 @@ def test_fp64_issue_cost_hook():
         binding.ubench_fp64(7, 8)
     with pytest.raises(binding.FspError):
         binding.ubench_fp64(0, 5)
+
+
+@pytest.mark.gpu
+def test_solve_can_be_captured_into_a_cuda_graph():
+    """fsp_solve allocates nothing and does not synchronise the host (include/fsp.h): a caller may capture it on the
+    plan's stream and replay it; the replay is bit-identical to the plain call, also with a new density in the same
+    buffer."""
+    N = (32, 64, 48)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st), binding.Plan(N, (0.1, 0.05, 0.07), binding.HOCKNEY, stream=st.cuda_stream) as p:
+        p.precompute_green()
+        g0 = torch.Generator(device="cuda").manual_seed(5)
+        rho = torch.randn(N, dtype=torch.float64, device="cuda", generator=g0)
+        phi = torch.empty_like(rho)
+        p.solve(rho, phi)          # (first call: tensor maps for this rho are encoded on the host)
+        st.synchronize()
+        ref = phi.clone()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=st):
+            p.solve(rho, phi)
+        phi.zero_()
+        graph.replay()
+        st.synchronize()
+        assert torch.equal(phi, ref)
+        rho.copy_(torch.randn(N, dtype=torch.float64, device="cuda", generator=g0))
+        graph.replay()
+        st.synchronize()
+        got = phi.clone()
+        p.solve(rho, phi)
+        st.synchronize()
+        assert torch.equal(got, phi)
+        del graph
