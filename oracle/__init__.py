@@ -18,6 +18,8 @@ from .oracle import (  # noqa: F401
     build,
     dct1,
     direct_sum,
+    direct_sum_mixed,
+    solve_mixed,
     fft1d,
     fft3d,
     green_spectrum,

@@ -27,6 +27,9 @@
  *                                        scale by hxhyhz, restrict.
  *   orc_solve_field      PAPER.md:227-231 (Eq. A.1)  E = -grad phi, spectral gradient on the doubled
  *                                        grid (8(f) N3, R18): steps 1-4, times -i k_d, inverse FFT, restrict.
+ *   orc_solve_mixed /    PAPER.md:67, 72  periodic directions (8(f) N4, R20): "double the computational grid in the
+ *   orc_direct_sum_mixed                 non-periodic directions" only; G made periodic along a periodic direction
+ *                                        with the period of the domain (nearest image); the same sum written out.
  *
  * Pins (tests/test_oracle_*.py, all -m "not gpu"): numpy brute force on tiny grids, numpy.fft on
  * random vectors, the closed-form Gaussian potential with second-order (HE) and
@@ -632,4 +635,92 @@ int orc_green_table_vg_entries(long Nx, long Ny, long Nz, const double h[3], dou
         for (int a = 0; a < 3; ++a) free(c[a]);
     }
     return err ? ORC_ENOMEM : ORC_OK;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Mixed periodic / open directions (PAPER.md:67 step 1: "Double the computational grid in
+ * the non-periodic directions (those which have open boundary conditions)"; reading R20).
+ * periodic[d] != 0: direction d is periodic with the period of the domain, L_d = N_d h_d.  The grid is NOT
+ * doubled along d and rho is not padded there; step 3's "circular shifting and making G periodic"
+ * along d is the nearest-image kernel G2[i] = T[min(i, N_d - i)], i < N_d.  Open directions as
+ * in orc_solve: doubled, zero-padded, mirrored.  T: the (Nx+1)(Ny+1)(Nz+1) table of orc_green_table_*.
+ * ------------------------------------------------------------------------------------------ */
+int orc_solve_mixed(long Nx, long Ny, long Nz, const double h[3], const double* T, const int periodic[3],
+                    int method, const double* rho, double* phi) {
+    if (Nx < 1 || Ny < 1 || Nz < 1 || !h || !T || !periodic || !rho || !phi) return ORC_EINVAL;
+    const long N[3] = {Nx, Ny, Nz};
+    long D[3];
+    for (int d = 0; d < 3; ++d) D[d] = periodic[d] ? N[d] : 2 * N[d];   /* step 1 */
+    size_t total = (size_t)D[0] * D[1] * D[2];
+    double* r2 = (double*)calloc(2 * total, sizeof(double));
+    double* g2 = (double*)calloc(2 * total, sizeof(double));
+    if (!r2 || !g2) { free(r2); free(g2); return ORC_ENOMEM; }
+    for (long i = 0; i < Nx; ++i)                                          /* step 2 */
+        for (long j = 0; j < Ny; ++j)
+            for (long k = 0; k < Nz; ++k)
+                r2[2 * (((size_t)i * D[1] + j) * D[2] + k)] = rho[((size_t)i * Ny + j) * Nz + k];
+    for (long i = 0; i < D[0]; ++i) {                                      /* step 3 */
+        long dx = i <= D[0] - i ? i : D[0] - i;   /* both cases: the distance to the nearest period of the grid */
+        for (long j = 0; j < D[1]; ++j) {
+            long dy = j <= D[1] - j ? j : D[1] - j;
+            for (long k = 0; k < D[2]; ++k) {
+                long dz = k <= D[2] - k ? k : D[2] - k;
+                g2[2 * (((size_t)i * D[1] + j) * D[2] + k)] = T[(dx * (Ny + 1) + dy) * (Nz + 1) + dz];
+            }
+        }
+    }
+    int rc = orc_fft3d(D[0], D[1], D[2], r2, -1, method);                  /* step 4 */
+    if (rc == ORC_OK) rc = orc_fft3d(D[0], D[1], D[2], g2, -1, method);
+    if (rc == ORC_OK) {
+        for (size_t o = 0; o < total; ++o) {
+            double ar = r2[2 * o], ai = r2[2 * o + 1], br = g2[2 * o], bi = g2[2 * o + 1];
+            r2[2 * o] = ar * br - ai * bi;
+            r2[2 * o + 1] = ar * bi + ai * br;
+        }
+        rc = orc_fft3d(D[0], D[1], D[2], r2, +1, method);
+    }
+    if (rc == ORC_OK) {
+        double scale = h[0] * h[1] * h[2] / (double)total;
+        for (long i = 0; i < Nx; ++i)                                      /* step 5 */
+            for (long j = 0; j < Ny; ++j)
+                for (long k = 0; k < Nz; ++k)
+                    phi[((size_t)i * Ny + j) * Nz + k] = scale * r2[2 * (((size_t)i * D[1] + j) * D[2] + k)];
+    }
+    free(r2);
+    free(g2);
+    return rc;
+}
+
+/* The same result as a plain sum (Def. O1 with the nearest image along the periodic directions):
+ *   phi[i] = hx hy hz sum_j T[|i - j|*] rho[j],  |i - j|*_d = min(|i_d - j_d|, N_d - |i_d - j_d|) if d is periodic,
+ *                                                             |i_d - j_d| otherwise.
+ * idx / npts / long double accumulation as in orc_direct_sum. */
+int orc_direct_sum_mixed(long Nx, long Ny, long Nz, const double h[3], const double* T, const int periodic[3],
+                         const double* rho, long npts, const long* idx, double* out) {
+    if (Nx < 1 || Ny < 1 || Nz < 1 || !h || !T || !periodic || !rho || !out) return ORC_EINVAL;
+    long V = Nx * Ny * Nz;
+    if (!idx) npts = V;
+    long double w = (long double)h[0] * (long double)h[1] * (long double)h[2];
+#pragma omp parallel for schedule(dynamic, 1)
+    for (long p = 0; p < npts; ++p) {
+        long f = idx ? idx[p] : p;
+        long i = f / (Ny * Nz), j = (f / Nz) % Ny, k = f % Nz;
+        long double acc = 0.0L;
+        for (long a = 0; a < Nx; ++a) {
+            long dx = labs(i - a);
+            if (periodic[0] && Nx - dx < dx) dx = Nx - dx;
+            for (long b = 0; b < Ny; ++b) {
+                long dy = labs(j - b);
+                if (periodic[1] && Ny - dy < dy) dy = Ny - dy;
+                for (long c = 0; c < Nz; ++c) {
+                    long dz = labs(k - c);
+                    if (periodic[2] && Nz - dz < dz) dz = Nz - dz;
+                    acc += (long double)T[(dx * (Ny + 1) + dy) * (Nz + 1) + dz] *
+                           (long double)rho[((size_t)a * Ny + b) * Nz + c];
+                }
+            }
+        }
+        out[p] = (double)(w * acc);
+    }
+    return ORC_OK;
 }

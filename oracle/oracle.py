@@ -65,6 +65,9 @@ def _load():
         lib.orc_solve_field.argtypes = [L, L, L, _dp, _dp, I, _dp, _dp, _dp]
         lib.orc_direct_sum.argtypes = [L, L, L, _dp, _dp, _dp, L, _lp, _dp]
         lib.orc_green_table_vg_entries.argtypes = [L, L, L, _dp, D, _lp, L, _lp, _dp]
+        _ip = ctypes.POINTER(ctypes.c_int)
+        lib.orc_solve_mixed.argtypes = [L, L, L, _dp, _dp, _ip, I, _dp, _dp]
+        lib.orc_direct_sum_mixed.argtypes = [L, L, L, _dp, _dp, _ip, _dp, L, _lp, _dp]
         _lib = lib
     return _lib
 
@@ -271,6 +274,45 @@ def direct_sum(T: np.ndarray, h, rho: np.ndarray, idx: np.ndarray | None = None)
     out = np.empty(idx.size, dtype=np.float64)
     _check(lib.orc_direct_sum(Nx, Ny, Nz, _d(h), _d(T), _d(rho), idx.size, idx.ctypes.data_as(_lp),
                               _d(out)), "direct_sum")
+    return out
+
+
+def _mask3(periodic):
+    m = (ctypes.c_int * 3)(*[int(bool(v)) for v in periodic])
+    return m
+
+
+def solve_mixed(T: np.ndarray, h, rho: np.ndarray, periodic, method: int = 0) -> np.ndarray:
+    """PAPER.md:67-82 with step 1 taken literally: only the non-periodic directions are doubled; along a periodic
+    direction G is the nearest-image kernel of period N_d h_d (R20).  periodic: three booleans."""
+    rho = np.ascontiguousarray(rho, dtype=np.float64)
+    T = np.ascontiguousarray(T, dtype=np.float64)
+    Nx, Ny, Nz = rho.shape
+    assert T.shape == (Nx + 1, Ny + 1, Nz + 1)
+    h = _h3(h)
+    phi = np.empty_like(rho)
+    _check(_load().orc_solve_mixed(Nx, Ny, Nz, _d(h), _d(T), _mask3(periodic), int(method), _d(rho), _d(phi)),
+           "solve_mixed")
+    return phi
+
+
+def direct_sum_mixed(T: np.ndarray, h, rho: np.ndarray, periodic, idx: np.ndarray | None = None) -> np.ndarray:
+    """Def. O1 with the nearest image along the periodic directions, at all points or at flat indices ``idx``."""
+    rho = np.ascontiguousarray(rho, dtype=np.float64)
+    T = np.ascontiguousarray(T, dtype=np.float64)
+    Nx, Ny, Nz = rho.shape
+    assert T.shape == (Nx + 1, Ny + 1, Nz + 1)
+    h = _h3(h)
+    lib = _load()
+    if idx is None:
+        out = np.empty(rho.size, dtype=np.float64)
+        _check(lib.orc_direct_sum_mixed(Nx, Ny, Nz, _d(h), _d(T), _mask3(periodic), _d(rho), rho.size, None, _d(out)),
+               "direct_sum_mixed")
+        return out.reshape(rho.shape)
+    idx = np.ascontiguousarray(idx, dtype=np.int64)
+    out = np.empty(idx.size, dtype=np.float64)
+    _check(lib.orc_direct_sum_mixed(Nx, Ny, Nz, _d(h), _d(T), _mask3(periodic), _d(rho), idx.size,
+                                    idx.ctypes.data_as(_lp), _d(out)), "direct_sum_mixed")
     return out
 
 

@@ -571,3 +571,74 @@ def test_field_of_point_charges_matches_fft_path():
     got = oracle.field_of_point_charges(T, h, charges, pts)
     ref = np.stack([E[:, p[0], p[1], p[2]] for p in pts])
     assert np.abs(got - ref).max() < 1e-12 * np.abs(E).max()
+
+
+# ---------------------------------------------------------------- mixed periodic / open directions (8(f) N4, R20)
+MASKS = [(1, 0, 0), (0, 1, 0), (0, 0, 1), (1, 1, 0), (0, 1, 1), (1, 1, 1)]
+
+
+def _brute_mixed(T, h, rho, periodic):
+    """numpy, written here: phi[i] = h^3 sum_j T[nearest-image |i - j| along periodic axes, |i - j| otherwise] rho[j]."""
+    N = rho.shape
+    ax = []
+    for d in range(3):
+        i = np.arange(N[d])
+        dist = np.abs(i[:, None] - i[None, :])
+        if periodic[d]:
+            dist = np.minimum(dist, N[d] - dist)
+        ax.append(dist)
+    K = T[ax[0][:, None, None, :, None, None], ax[1][None, :, None, None, :, None], ax[2][None, None, :, None, None, :]]
+    return float(np.prod(h)) * np.einsum("ijkabc,abc->ijk", K, rho)
+
+
+@pytest.mark.parametrize("periodic", MASKS)
+def test_mixed_solve_and_direct_sum_match_numpy_brute_force(periodic):
+    N, h = (4, 6, 8), (0.3, 0.2, 0.25)
+    rng = np.random.default_rng(11)
+    rho = rng.standard_normal(N)
+    T = oracle.green_table(oracle.HOCKNEY, N, h)
+    ref = _brute_mixed(T, h, rho, periodic)
+    assert rel_max(oracle.direct_sum_mixed(T, h, rho, periodic), ref) < 1e-13
+    assert rel_max(oracle.solve_mixed(T, h, rho, periodic), ref) < 1e-13
+    idx = np.array([0, 5, 77, rho.size - 1])
+    assert np.allclose(oracle.direct_sum_mixed(T, h, rho, periodic, idx), ref.ravel()[idx], rtol=0, atol=1e-13 * np.abs(ref).max())
+
+
+def test_mixed_with_no_periodic_direction_is_the_open_solve():
+    w = W.config1()
+    p = oracle.OraclePlan(w.N, w.h, oracle.HOCKNEY).precompute_green()
+    assert rel_max(oracle.solve_mixed(p.T, w.h, w.rho, (0, 0, 0)), p.solve(w.rho)) < 1e-14
+
+
+def test_fully_periodic_is_a_cyclic_convolution_numpy_fft():
+    """All three directions periodic: no doubling at all, phi = h^3 ifftn(fftn(rho) fftn(G_nearest_image))."""
+    N, h = (8, 12, 16), (0.1, 0.15, 0.05)
+    rng = np.random.default_rng(3)
+    rho = rng.standard_normal(N)
+    T = oracle.green_table(oracle.HOCKNEY, N, h)
+    ix = [np.minimum(np.arange(n), n - np.arange(n)) for n in N]
+    G = T[np.ix_(*ix)]
+    ref = float(np.prod(h)) * np.fft.ifftn(np.fft.fftn(rho) * np.fft.fftn(G)).real
+    assert rel_max(oracle.solve_mixed(T, h, rho, (1, 1, 1)), ref) < 1e-13
+
+
+def test_mixed_point_source_and_translation_along_the_periodic_axis():
+    """A unit point source gives h^3 times the nearest-image kernel; shifting rho cyclically along a periodic axis
+    shifts phi cyclically (and does NOT along an open one)."""
+    N, h = (8, 8, 16), (0.2, 0.2, 0.1)
+    T = oracle.green_table(oracle.HOCKNEY, N, h)
+    rho = np.zeros(N)
+    rho[6, 1, 3] = 1.0
+    phi = oracle.solve_mixed(T, h, rho, (1, 0, 0))
+    w = float(np.prod(h))
+    # x periodic: the source at x = 6 is 3 cells from x = 1 through the boundary (|1 - 6| = 5 > 8 - 5)
+    assert abs(phi[1, 1, 3] - w * T[3, 0, 0]) < 1e-15 * abs(phi[1, 1, 3]) + 1e-18
+    # y open: plain distance
+    assert abs(phi[6, 7, 3] - w * T[0, 6, 0]) < 1e-15 * abs(phi[6, 7, 3]) + 1e-18
+    rng = np.random.default_rng(5)
+    r = rng.standard_normal(N)
+    a = oracle.solve_mixed(T, h, r, (1, 0, 0))
+    b = oracle.solve_mixed(T, h, np.roll(r, 3, axis=0), (1, 0, 0))
+    assert rel_max(b, np.roll(a, 3, axis=0)) < 1e-13
+    c = oracle.solve_mixed(T, h, np.roll(r, 3, axis=1), (1, 0, 0))
+    assert rel_max(c, np.roll(a, 3, axis=1)) > 1e-3
