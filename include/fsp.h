@@ -86,6 +86,18 @@ enum {
     FSP_PARAM_K2_VARIANT = 4, /* kernel of the forward y pass at Ny = 512 (kept for A/B measurements): 0 (default) = the
                                 zero-padded column of 2 Ny points in one group (k_fwd_y_f); 1 = two half-length
                                 branches in two groups (k_fwd_y_t).  Takes effect at the next fsp_solve          */
+    FSP_PARAM_PERIODIC = 5, /* periodic directions (PAPER.md:67 step 1: only "the non-periodic directions (those which have
+                              open boundary conditions)" are doubled; reading R20).  value = bit
+                              mask, 1: x, 2: y, 4: z; default 0 = all open (the paper's configurations).  Along a periodic
+                              direction d the result is the CYCLIC convolution of period N_d with the kernel made periodic
+                              by "circular shifting": G at the nearest image, displacement
+                              min(|i - j|, N_d - |i - j|) h_d; rho is taken as N_d-periodic there, nothing is padded.
+                              (The nearest image only: the lattice sum of 1/r over all images does not converge and the
+                              paper gives no other rule.)  FSP_HOCKNEY only, and only on meshes that are transformed at
+                              their own size (2^k, 3 2^k, 5 2^k), else FSP_ERR_INVALID_ARG.  Same five kernels and the same
+                              cost as the open solve: the periodic kernel's spectrum on the doubled grid has zero odd bins.
+                              fsp_get_green_table then returns the folded table T'[i] = T[min(i, N_d - i)].  Invalidates
+                              the spectrum: call fsp_precompute_green again                                        */
     FSP_PARAM_K3_VARIANT = 3  /* kernel of the z pass (kept for A/B measurements).  0 (default): the whole zero-padded
                                 pencil in one lane group (k_conv_z_f, Nz = 256, 512; the prime-factor kernel
                                 k_conv_z_pf at Nz = 96, 192, 384; k_conv_z_g2 at the other 3 * 2^k, 5 * 2^k).  1: two

@@ -15,7 +15,7 @@ import os
 import numpy as np
 
 HOCKNEY, VICO, VICO_2, VICO_SAFE = 0, 1, 2, 3           # include/fsp.h, PAPER.md:199 (+ DESIGN.md R17)
-PARAM_G0, PARAM_ALPHA, PARAM_CHUNK_PLANES, PARAM_K3_VARIANT, PARAM_K2_VARIANT = 0, 1, 2, 3, 4
+PARAM_G0, PARAM_ALPHA, PARAM_CHUNK_PLANES, PARAM_K3_VARIANT, PARAM_K2_VARIANT, PARAM_PERIODIC = 0, 1, 2, 3, 4, 5
 NUM_SOLVE_KERNELS = 5
 ERRORS = {0: "FSP_OK", -1: "FSP_ERR_INVALID_ARG", -2: "FSP_ERR_NOT_PRECOMPUTED",
           -3: "FSP_ERR_OUT_OF_MEMORY", -4: "FSP_ERR_CUDA", -5: "FSP_ERR_NO_DEVICE"}
@@ -248,7 +248,7 @@ class Plan:
     """plan -> precompute_green -> solve* -> destroy, on the current torch CUDA stream by default."""
 
     def __init__(self, N, h, algorithm: int, stream: int | None = None, g0: float | None = None,
-                 alpha: float | None = None):
+                 alpha: float | None = None, periodic=None):
         self.N = tuple(int(v) for v in N)
         self.h = tuple(float(v) for v in np.broadcast_to(np.asarray(h, dtype=np.float64), (3,)))
         self.algorithm = int(algorithm)
@@ -261,6 +261,13 @@ class Plan:
             plan_set_param(self.handle, PARAM_G0, g0)
         if alpha is not None:
             plan_set_param(self.handle, PARAM_ALPHA, alpha)
+        if periodic is not None and any(periodic):   # three booleans (x, y, z): FSP_PARAM_PERIODIC
+            try:
+                plan_set_param(self.handle, PARAM_PERIODIC, sum(1 << d for d in range(3) if periodic[d]))
+            except FspError:
+                destroy(self.handle)
+                self.handle = None
+                raise
 
     def precompute_green(self):
         precompute_green(self.handle)

@@ -55,6 +55,7 @@ struct fsp_plan {
     double* LTy = nullptr;  // the same for the y transform (tile kernels)
     double* LTyf = nullptr; // Ny = 512: stage-2 constants of the padded 1024-point y transform (k_fwd_y_f)
     int k2_variant = 0;     // FSP_PARAM_K2_VARIANT
+    int periodic = 0;       // FSP_PARAM_PERIODIC: bit d set = direction d periodic (nearest-image kernel of period N_d h_d)
     bool tile_y = false;    // K2/K4 tile kernels (TMA-staged) are used
     double* LTx = nullptr;  // lane-constant twiddles of the x transform (length Nx/2)
     bool tile_x = false;    // K1 tile kernel is used
@@ -988,6 +989,10 @@ int precompute_impl(fsp_plan* p) {
     if (p->algorithm == FSP_HOCKNEY) {
         k_fill_he<<<grid_for(tcount, blk), blk, 0, p->stream>>>(p->T, Nx, Ny, Nz, hx, hy, hz, p->g0);
         CU(cudaGetLastError());
+        if (p->periodic) {   // (set_param has checked: FSP_HOCKNEY, mesh not embedded)
+            k_fold_periodic<<<grid_for(tcount, blk), blk, 0, p->stream>>>(p->T, Nx, Ny, Nz, p->periodic);
+            CU(cudaGetLastError());
+        }
     } else {
         const double Lx = Nx * hx, Ly = Ny * hy, Lz = Nz * hz;
         const double L = p->alpha * std::sqrt(Lx * Lx + Ly * Ly + Lz * Lz);
@@ -1263,6 +1268,15 @@ int fsp_plan_set_param(fsp_plan* p, int which, double value) {
     if (which == FSP_PARAM_K2_VARIANT) {
         if (value != 0.0 && value != 1.0) return FSP_ERR_INVALID_ARG;
         p->k2_variant = (int)value;
+        return FSP_OK;
+    }
+    if (which == FSP_PARAM_PERIODIC) {
+        const int mask = (int)value;
+        if (value != (double)mask || mask < 0 || mask > 7) return FSP_ERR_INVALID_ARG;
+        // the nearest-image kernel is defined for the 1/r table; the period must be the caller's N_d, so no embedding
+        if (mask != 0 && (p->algorithm != FSP_HOCKNEY || p->padded)) return FSP_ERR_INVALID_ARG;
+        p->periodic = mask;
+        p->precomputed = false;
         return FSP_OK;
     }
     if (which == FSP_PARAM_K3_VARIANT) {

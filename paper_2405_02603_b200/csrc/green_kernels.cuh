@@ -73,6 +73,25 @@ __device__ __forceinline__ double vg_GL_straight(double s2xy, double sz, double 
     return 2.0 * q * q;
 }
 
+// Periodic directions (R20): along a periodic direction d the kernel is made
+// periodic with the period of the domain, T'[i] = T[min(i, N_d - i)], i <= N_d.  Its mirror image on the doubled grid
+// (what the DCT-I below transforms) is then exactly the N_d-periodic repetition of the nearest-image kernel, whose
+// 2 N_d-point spectrum has zero odd bins: the five solve kernels, unchanged, compute the CYCLIC convolution of period
+// N_d along d and the free-space one along the others.  In place: an entry is rewritten only if one of its indices
+// folds, and the entries it is copied from (all indices <= N_d / 2 along the periodic directions) never are.
+__global__ void k_fold_periodic(double* __restrict__ T, int Nx, int Ny, int Nz, int mask) {
+    const long total = (long)(Nx + 1) * (Ny + 1) * (Nz + 1);
+    for (long o = blockIdx.x * (long)blockDim.x + threadIdx.x; o < total; o += (long)gridDim.x * blockDim.x) {
+        const int dz = (int)(o % (Nz + 1));
+        const int dy = (int)((o / (Nz + 1)) % (Ny + 1));
+        const int dx = (int)(o / ((long)(Nz + 1) * (Ny + 1)));
+        const int fx = (mask & 1) && Nx - dx < dx ? Nx - dx : dx;
+        const int fy = (mask & 2) && Ny - dy < dy ? Ny - dy : dy;
+        const int fz = (mask & 4) && Nz - dz < dz ? Nz - dz : dz;
+        if (fx != dx || fy != dy || fz != dz) T[o] = T[((long)fx * (Ny + 1) + fy) * (Nz + 1) + fz];
+    }
+}
+
 __global__ void k_fill_he(double* __restrict__ T, int Nx, int Ny, int Nz, double hx, double hy,
                           double hz, double g0) {
     const long total = (long)(Nx + 1) * (Ny + 1) * (Nz + 1);
