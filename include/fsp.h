@@ -18,13 +18,16 @@
  * fallback.  One GPU, one plan = one mesh; fp64 throughout.  eps0 = 1: the caller divides by eps0.
  *
  * Conventions
- *   - Mesh Nx x Ny x Nz, spacings h[0..2] = hx, hy, hz, 2 <= N_d <= 1024.  The transforms
- *     are power-of-two (the paper's sizes all are): a mesh with another N_d is embedded
- *     in the next power-of-two mesh N'_d >= max(N_d, 8) (zero density outside, result cropped; DESIGN.md
- *     R19).  The cyclic convolution is exact for any period >= 2 N_d - 1, so FSP_HOCKNEY gives the paper's
- *     result for the caller's mesh; the Vico-Greengard table is that of the enclosing box N'_d h_d
- *     (a larger truncation radius L, same free-space kernel); the spectral gradient of fsp_solve_field
- *     has period 2 N'_d h_d.  Cost and memory are those of the N' mesh.
+ *   - Mesh Nx x Ny x Nz, spacings h[0..2] = hx, hy, hz, 2 <= N_d <= 1024.  Transform lengths
+ *     are 2^k (the paper's sizes all are), 3 2^k and 5 2^k between 8 and 1024 (Nz a multiple
+ *     of 8): on such a mesh nothing is embedded and every algorithm gives the paper's result for the caller's
+ *     mesh.  A mesh with another N_d is embedded in the next such mesh N'_d >= max(N_d, 8) (zero density
+ *     outside, result cropped; R19).  The cyclic convolution is exact for any period >= 2 N_d - 1,
+ *     so FSP_HOCKNEY still gives the paper's result for the caller's mesh; the Vico-Greengard table is then
+ *     that of the enclosing box N'_d h_d (a larger truncation radius L, same free-space kernel); the spectral
+ *     gradient of fsp_solve_field has period 2 N'_d h_d.  Cost and memory are those of the N' mesh.
+ *     (FSP_VICO, the plain 4x-oversampled precompute, takes power-of-two transform meshes only: every other
+ *     mesh is embedded in the next power of two.)
  *   - rho, phi: dense fp64 arrays of shape (Nx, Ny, Nz) in C order, index (ix*Ny + iy)*Nz + iz,
  *     iz fastest.  The sample position inside a cell does not matter (translation invariance).
  *   - "dev" pointers are CUDA device pointers on the device that was current at plan creation (the
