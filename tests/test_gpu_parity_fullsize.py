@@ -143,6 +143,31 @@ def test_config4_beam_full_field_against_the_oracle(alg):
     check(got, ref)
 
 
+def _host_memory_available_gib():
+    try:
+        import psutil
+        return psutil.virtual_memory().available / 2 ** 30
+    except Exception:   # noqa: BLE001
+        return 0.0
+
+
+@pytest.mark.skipif(_host_memory_available_gib() < 60.0, reason="the oracle's 1024^3 complex arrays need about 40 GiB of host memory")
+def test_config5_512_full_field_against_the_oracle():
+    """BASELINE config 5, the bench workload itself (512^3, Gaussian sigma = 0.05, HE), FULL field against the oracle's
+    un-pruned 1024^3 complex FFT convolution (two arrays of 17 GB on the host, about a minute on 16 cores): the sampled
+    check of test_gpu_parity.py::test_full_size_sampled_against_plain_definition cannot exclude a fault confined to a
+    few tiles of the launch configuration the bench times; this can."""
+    w = W.config5()
+    with binding.Plan(w.N, w.h, binding.HOCKNEY) as p:
+        got = gpu_solve(p.precompute_green(), w.rho)
+    T = oracle_table("HE", w.N, w.h)
+    G = oracle.green_spectrum(T)
+    del T
+    ref = oracle.solve_with_spectrum(G, w.h, w.rho)
+    del G
+    check(got, ref)
+
+
 # ---- (c) Vico-Greengard tables at size -----------------------------------------------------------------------
 @pytest.mark.parametrize("name,alg", [("256", "VG2"), ("beam", "VG2"), ("beam", "VGS")])
 def test_vg_table_at_size_against_the_oracle_table(name, alg):
