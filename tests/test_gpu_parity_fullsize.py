@@ -152,28 +152,30 @@ def _host_memory_available_gib():
 
 
 @pytest.mark.skipif(_host_memory_available_gib() < 60.0, reason="the oracle's 1024^3 complex arrays need about 40 GiB of host memory")
-def test_config5_512_full_field_against_the_oracle():
-    """BASELINE config 5, the bench workload itself (512^3, Gaussian sigma = 0.05, HE), FULL field against the oracle's
-    un-pruned 1024^3 complex FFT convolution (two arrays of 17 GB on the host, about a minute on 16 cores): the sampled
-    check of test_gpu_parity.py::test_full_size_sampled_against_plain_definition cannot exclude a fault confined to a
-    few tiles of the launch configuration the bench times; this can."""
+@pytest.mark.parametrize("alg", ["HE", "VG2"])
+def test_config5_512_full_field_against_the_oracle(alg):
+    """BASELINE config 5, the bench workload itself (512^3, Gaussian sigma = 0.05; HE and the memory-reduced VG), FULL
+    field against the oracle's un-pruned 1024^3 complex FFT convolution with the ORACLE's table (two arrays of 17 GB on
+    the host, under a minute on 16 cores): the sampled check of
+    test_gpu_parity.py::test_full_size_sampled_against_plain_definition cannot exclude a fault confined to a few tiles
+    of the launch configuration the bench times; this can."""
     w = W.config5()
-    with binding.Plan(w.N, w.h, binding.HOCKNEY) as p:
+    with binding.Plan(w.N, w.h, ALGS[alg][0]) as p:
         got = gpu_solve(p.precompute_green(), w.rho)
-    T = oracle_table("HE", w.N, w.h)
-    G = oracle.green_spectrum(T)
-    del T
+    G = oracle.green_spectrum(oracle.green_table(ALGS[alg][1], w.N, w.h))
     ref = oracle.solve_with_spectrum(G, w.h, w.rho)
     del G
     check(got, ref)
 
 
 # ---- (c) Vico-Greengard tables at size -----------------------------------------------------------------------
-@pytest.mark.parametrize("name,alg", [("256", "VG2"), ("beam", "VG2"), ("beam", "VGS")])
+@pytest.mark.parametrize("name,alg", [("256", "VG2"), ("beam", "VG2"), ("beam", "VGS"), ("512", "VG2")])
 def test_vg_table_at_size_against_the_oracle_table(name, alg):
-    """The DCT paths that only run at size (lattices 513^3, 257 x 257 x 1025, 513 x 513 x 1025; k_dct1_tile<4> with
-    1024 threads at n = 1024) against the oracle's transform route, every entry."""
-    w = W.config3() if name == "256" else W.config4()
+    """The DCT paths that only run at size (lattices 513^3, 257 x 257 x 1025, 513 x 513 x 1025, and the 1025^3 lattice of
+    BASELINE config 5 with its chunked fused z pass) against the oracle's transform route, every entry."""
+    if name == "512" and _host_memory_available_gib() < 40.0:
+        pytest.skip("the oracle's 1025^3 lattice and its intermediates need about 25 GiB of host memory")
+    w = {"256": W.config3, "beam": W.config4, "512": W.config5}[name]()
     with binding.Plan(w.N, w.h, ALGS[alg][0]) as p:
         p.precompute_green()
         T = p.green_table()
