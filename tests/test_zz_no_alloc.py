@@ -26,9 +26,7 @@ def _static_path(T):
     N = tuple(n - 1 for n in T.shape)
     Td = torch.from_numpy(T).cuda()
     Gd = torch.full_like(Td, float("nan"))
-    before = torch.cuda.memory_allocated()
     binding.green_spectrum_static(Td, Gd, N, torch.cuda.current_stream().cuda_stream)
-    assert torch.cuda.memory_allocated() == before
     torch.cuda.synchronize()
     return Gd.cpu().numpy()
 
@@ -59,14 +57,18 @@ def test_static_spectrum_same_result_on_immediate_repeat():
     assert np.array_equal(G1, G2)
     assert _rel_l2(G1, G_ref) < REL_TOL
     # no device memory is taken by a call (after the first one, which may load the kernels' module)
+    # (device-wide free memory as the driver reports it: the library does not go through torch's allocator, and
+    # garbage left by earlier tests is collected first so that nothing is released in between)
+    import gc
     Td = torch.from_numpy(T).cuda()
     Gd = torch.empty_like(Td)
+    gc.collect()
     torch.cuda.synchronize()
     free_before, _ = torch.cuda.mem_get_info()
     binding.green_spectrum_static(Td, Gd, (32, 32, 32), torch.cuda.current_stream().cuda_stream)
     torch.cuda.synchronize()
     free_after, _ = torch.cuda.mem_get_info()
-    assert free_after == free_before
+    assert free_after >= free_before
     assert np.array_equal(Gd.cpu().numpy(), G1)
 
 
