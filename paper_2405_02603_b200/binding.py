@@ -15,7 +15,7 @@ import os
 import numpy as np
 
 HOCKNEY, VICO, VICO_2, VICO_SAFE = 0, 1, 2, 3           # include/fsp.h, PAPER.md:199 (+ DESIGN.md R17)
-PARAM_G0, PARAM_ALPHA, PARAM_CHUNK_PLANES, PARAM_K3_VARIANT, PARAM_K2_VARIANT, PARAM_PERIODIC = 0, 1, 2, 3, 4, 5
+PARAM_G0, PARAM_ALPHA, PARAM_CHUNK_PLANES, PARAM_K3_VARIANT, PARAM_K2_VARIANT, PARAM_PERIODIC, PARAM_PERIODIC_FAST_Z = 0, 1, 2, 3, 4, 5, 6
 NUM_SOLVE_KERNELS = 5
 ERRORS = {0: "FSP_OK", -1: "FSP_ERR_INVALID_ARG", -2: "FSP_ERR_NOT_PRECOMPUTED",
           -3: "FSP_ERR_OUT_OF_MEMORY", -4: "FSP_ERR_CUDA", -5: "FSP_ERR_NO_DEVICE"}

@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfsp.so")
 SOURCES = ["fsp_api.cu"]
-HEADERS = ["fft_engine.cuh", "fft_warp.cuh", "solve_kernels.cuh", "green_kernels.cuh", "tma.cuh", "shard.cuh", "ubench.cuh", os.path.join("..", "..", "include", "fsp.h")]
+HEADERS = ["fft_engine.cuh", "fft_warp.cuh", "solve_kernels.cuh", "green_kernels.cuh", "tma.cuh", "shard.cuh", "ubench.cuh", "periodic_kernels.cuh", os.path.join("..", "..", "include", "fsp.h")]
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17",

@@ -87,3 +87,25 @@ def test_periodic_is_rejected_where_it_is_not_defined():
         with pytest.raises(binding.FspError):
             binding.plan_set_param(p.handle, binding.PARAM_PERIODIC, 1.5)
         binding.plan_set_param(p.handle, binding.PARAM_PERIODIC, 0)
+
+
+@pytest.mark.parametrize("N,h", [((16, 8, 512), (0.1, 0.2, 0.01)), ((8, 16, 256), (0.1, 0.1, 0.02))])
+def test_periodic_z_on_nz_point_transforms(N, h):
+    """k_conv_z_periodic (periodic z at Nz = 256, 512: Nz-point transforms instead of the padded 2 Nz) against the
+    oracle's literal step 1, full field, and against the doubled-grid kernel (FSP_PARAM_PERIODIC_FAST_Z = 0)."""
+    rng = np.random.default_rng(N[2])
+    rho = rng.standard_normal(N)
+    To = oracle.green_table(oracle.HOCKNEY, N, h)
+    for periodic in ((0, 0, 1), (1, 0, 1)):
+        ref = oracle.solve_mixed(To, h, rho, periodic)
+        got = {}
+        for fast in (1, 0):
+            with binding.Plan(N, h, binding.HOCKNEY, periodic=periodic) as p:
+                binding.plan_set_param(p.handle, binding.PARAM_PERIODIC_FAST_Z, fast)
+                p.precompute_green()
+                phi = p.solve(torch.from_numpy(rho).cuda())
+                torch.cuda.synchronize()
+                got[fast] = phi.cpu().numpy()
+            assert rel_l2(got[fast], ref) <= L2_TOL, (fast, rel_l2(got[fast], ref))
+            assert rel_max(got[fast], ref) <= MAX_TOL, (fast, rel_max(got[fast], ref))
+        assert not np.array_equal(got[0], got[1])   # (two different kernels ran)
