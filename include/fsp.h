@@ -99,10 +99,10 @@ enum {
                               paper gives no other rule.)  FSP_HOCKNEY only, and only on meshes that are transformed at
                               their own size (2^k, 3 2^k, 5 2^k), else FSP_ERR_INVALID_ARG.  Same five kernels and the same
                               cost as the open solve: the periodic kernel's spectrum on the doubled grid has zero odd bins
-                              (a periodic z at Nz = 256, 512 is cheaper, see FSP_PARAM_PERIODIC_FAST_Z).
+                              (a periodic z with Nz = 2^k is cheaper, see FSP_PARAM_PERIODIC_FAST_Z).
                               fsp_get_green_table then returns the folded table T'[i] = T[min(i, N_d - i)].  Invalidates
                               the spectrum: call fsp_precompute_green again                                        */
-    FSP_PARAM_PERIODIC_FAST_Z = 6, /* 1 (default): a periodic z direction at Nz = 256 or 512 runs the z pass on Nz-point
+    FSP_PARAM_PERIODIC_FAST_Z = 6, /* 1 (default): a periodic z direction with Nz a power of two runs the z pass on Nz-point
                                      transforms (k_conv_z_periodic: the saving PAPER.md:67's step 1 implies, along z);
                                      0: the doubled-grid kernel as for every other case.  Same result to rounding; takes
                                      effect at the next fsp_solve (fsp_solve_field always uses the doubled-grid kernels) */

@@ -56,7 +56,7 @@ struct fsp_plan {
     double* LTy = nullptr;  // the same for the y transform (tile kernels)
     double* LTyf = nullptr; // Ny = 512: stage-2 constants of the padded 1024-point y transform (k_fwd_y_f)
     int k2_variant = 0;     // FSP_PARAM_K2_VARIANT
-    bool periodic_fast_z = true;   // FSP_PARAM_PERIODIC_FAST_Z: periodic z at Nz = 256, 512 by Nz-point transforms (k_conv_z_periodic)
+    bool periodic_fast_z = true;   // FSP_PARAM_PERIODIC_FAST_Z: periodic z (Nz = 2^k) by Nz-point transforms (k_conv_z_periodic)
     int periodic = 0;       // FSP_PARAM_PERIODIC: bit d set = direction d periodic (nearest-image kernel of period N_d h_d)
     bool tile_y = false;    // K2/K4 tile kernels (TMA-staged) are used
     double* LTx = nullptr;  // lane-constant twiddles of the x transform (length Nx/2)
@@ -658,26 +658,45 @@ int do_conv_z_w(fsp_plan* p, double2* B2, const double* G, int np, double2* out,
 }
 // planes [kx0, kx0 + np) of the spectrum go with the np planes stored at B2.
 // kap == nullptr: in place (phi); otherwise B2 -> out with the derivative factor (whole volume only, kx0 = 0).
-// periodic z (FSP_PARAM_PERIODIC bit 4) on natural-order rows: Nz-point transforms instead of the padded 2 Nz (k_conv_z_periodic)
-template <int M>
-int launch_conv_z_periodic(fsp_plan* p, double2* B2, const double* G, int nplanes) {
+// periodic z (FSP_PARAM_PERIODIC bit 4) on power-of-two Nz: Nz-point transforms instead of the padded 2 Nz (k_conv_z_periodic)
+template <int M, bool NATURAL>
+int launch_conv_z_periodic_impl(fsp_plan* p, double2* B2, const double* G, int nplanes) {
     using Z = ConvZPer<M>;
-    const long ngroups = (long)nplanes * (2 * p->Ny) / Z::G;
+    const long npencils = (long)nplanes * (2 * p->Ny), ngroups = (npencils + Z::G - 1) / Z::G;
     const size_t smem = Z::smem_bytes();
     static OccCache cache;
     int occ = 0;
-    { const int rc_ = cached_occupancy(cache, p->device, k_conv_z_periodic<M>, Z::WARPS * 32, smem, &occ); if (rc_ != FSP_OK) return rc_; }
+    { const int rc_ = cached_occupancy(cache, p->device, k_conv_z_periodic<M, NATURAL>, Z::WARPS * 32, smem, &occ); if (rc_ != FSP_OK) return rc_; }
     long grid = (long)p->sm_count * occ;
     const long need = (ngroups + Z::WARPS - 1) / Z::WARPS;
     if (grid > need) grid = need;
-    k_conv_z_periodic<M><<<(unsigned)grid, Z::WARPS * 32, smem, p->stream>>>(B2, G, p->LTz, p->Ny, ngroups);
+    k_conv_z_periodic<M, NATURAL><<<(unsigned)grid, Z::WARPS * 32, smem, p->stream>>>(B2, G, p->LTz, p->Ny, ngroups, npencils);
     CU(cudaGetLastError());
     return FSP_OK;
 }
+template <int M>
+int launch_conv_z_periodic(fsp_plan* p, double2* B2, const double* G, int nplanes) {
+    // natural-order rows exist where k_conv_z_f runs (Nz = 256, 512), [E | O] rows elsewhere
+    if constexpr (M == 256 || M == 512) {
+        if (p->gk_natural) return launch_conv_z_periodic_impl<M, true>(p, B2, G, nplanes);
+    }
+    if (p->gk_natural) return FSP_ERR_INVALID_ARG;
+    return launch_conv_z_periodic_impl<M, false>(p, B2, G, nplanes);
+}
 int do_conv_z(fsp_plan* p, double2* B2, int kx0, int np, double2* out = nullptr, const DerK* kap = nullptr) {
-    if ((p->periodic & 4) && p->periodic_fast_z && !out && !kap && p->gk_natural && !p->gk_pfa && (p->Nz == 256 || p->Nz == 512)) {
+    if ((p->periodic & 4) && p->periodic_fast_z && !out && !kap && !p->gk_pfa && is_pow2(p->Nz) && p->LTz) {
         const double* G = p->Gk + (size_t)kx0 * (p->Ny + 1) * ((size_t)p->Nz + 2);
-        return p->Nz == 512 ? launch_conv_z_periodic<512>(p, B2, G, np) : launch_conv_z_periodic<256>(p, B2, G, np);
+        switch (p->Nz) {
+            case 8: return launch_conv_z_periodic<8>(p, B2, G, np);
+            case 16: return launch_conv_z_periodic<16>(p, B2, G, np);
+            case 32: return launch_conv_z_periodic<32>(p, B2, G, np);
+            case 64: return launch_conv_z_periodic<64>(p, B2, G, np);
+            case 128: return launch_conv_z_periodic<128>(p, B2, G, np);
+            case 256: return launch_conv_z_periodic<256>(p, B2, G, np);
+            case 512: return launch_conv_z_periodic<512>(p, B2, G, np);
+            case 1024: return launch_conv_z_periodic<1024>(p, B2, G, np);
+            default: break;
+        }
     }
     return do_conv_z_w(p, B2, p->Gk + (size_t)kx0 * (p->Ny + 1) * (p->gk_pfa ? (size_t)2 * p->Nz : (size_t)p->Nz + 2), np, out, kap);
 }

@@ -4,8 +4,8 @@
 // FSP_PARAM_PERIODIC works with the unchanged doubled-grid kernels because the folded table's spectrum has zero odd bins.
 // Along z that wastes half of K3, the dominant kernel: the cyclic convolution of period Nz needs Nz-point transforms only,
 //     y = IDFT_Nz( G_Nz . DFT_Nz(x) ),   G_Nz[j] = Ghat_2Nz[2j] / 2,
-// and the 1/(2 Nz) folded into the stored spectrum is exactly (1/Nz)(1/2): the rows are used as they are, entry
-// min(2 kz, 2 Nz - 2 kz) of the natural-order row (k_layout_spectrum_nat; Ghat is even in kz).  No padding, no pruning:
+// and the 1/(2 Nz) folded into the stored spectrum is exactly (1/Nz)(1/2): the rows are used as they are, the even
+// entries of either row layout (Ghat is even in kz).  No padding, no pruning:
 // one pencil of Nz points per lane group of Fft2Cfg<Nz>, forward, times Ghat, inverse by IFFT(Y) = conj(FFT(conj Y)) on
 // ONE copy of the transform code, in place in B2.  Same layout of B2 as K3 (the x and y passes are the doubled-grid ones).
 #pragma once
@@ -21,10 +21,10 @@ struct ConvZPer {
     static constexpr size_t smem_bytes() { return sizeof(double2) * (size_t)(WARPS * G * Cfg::BUF); }
 };
 
-template <int M>
+template <int M, bool NATURAL>
 __global__ void __launch_bounds__(ConvZPer<M>::WARPS * 32, 1)
 k_conv_z_periodic(double2* __restrict__ B2, const double* __restrict__ Gk, const double* __restrict__ lane_g, int Ny,
-                  long ngroups) {
+                  long ngroups, long npencils) {
     using Z = ConvZPer<M>;
     using Cfg = typename Z::Cfg;
     constexpr int R = Z::R, T = Z::T, G = Z::G, WARPS = Z::WARPS, NC = LaneTw<Cfg::R2>::NC, NB2 = Cfg::NB2;
@@ -42,7 +42,14 @@ k_conv_z_periodic(double2* __restrict__ B2, const double* __restrict__ Gk, const
         }
     const long ny2 = 2L * Ny;
     for (long grp = (long)blockIdx.x * WARPS + warp; grp < ngroups; grp += (long)gridDim.x * WARPS) {
-        const long pen = grp * G + g;   // = kx * 2 Ny + ky
+        long pen = grp * G + g;   // = kx * 2 Ny + ky
+        // (G divides the 2 Ny pencils of a plane unless G = 16: the last group may then be ragged)
+        constexpr bool RAGGED = G > 8;
+        bool valid = true;
+        if constexpr (RAGGED) {
+            valid = pen < npencils;
+            if (!valid) pen = npencils - 1;
+        }
         const long kx = pen / ny2;
         const int ky = (int)(pen - kx * ny2), qy = ky <= Ny ? ky : (int)ny2 - ky;
         double2* base = B2 + pen * M;
@@ -60,13 +67,17 @@ k_conv_z_periodic(double2* __restrict__ B2, const double* __restrict__ Gk, const
 #pragma unroll
                 for (int i = 0; i < R; ++i) {
                     const int kz = t + T * i;
-                    const double gk = __ldg(row + (2 * kz <= M ? 2 * kz : 2 * M - 2 * kz));
+                    // Ghat_2Nz[2 kz] = Ghat_2Nz[2 Nz - 2 kz]: entry min(2 kz, 2 Nz - 2 kz) of a natural-order row, entry
+                    // min(kz, Nz - kz) of the E half of an [E | O] row (k_layout_spectrum_oct: E[m] = Ghat[2 m])
+                    const int e = kz <= M - kz ? kz : M - kz;
+                    const double gk = __ldg(row + (NATURAL ? 2 * e : e));
                     vr[i] *= gk; vi[i] *= -gk;
                 }
             }
         }
 #pragma unroll
-        for (int i = 0; i < R; ++i) base[t + T * i] = make_double2(vr[i], -vi[i]);   // FFT(conj Y) = conj(y)
+        for (int i = 0; i < R; ++i)
+            if (!RAGGED || valid) base[t + T * i] = make_double2(vr[i], -vi[i]);   // FFT(conj Y) = conj(y)
     }
 }
 

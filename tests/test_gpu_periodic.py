@@ -89,9 +89,11 @@ def test_periodic_is_rejected_where_it_is_not_defined():
         binding.plan_set_param(p.handle, binding.PARAM_PERIODIC, 0)
 
 
-@pytest.mark.parametrize("N,h", [((16, 8, 512), (0.1, 0.2, 0.01)), ((8, 16, 256), (0.1, 0.1, 0.02))])
+@pytest.mark.parametrize("N,h", [((16, 8, 512), (0.1, 0.2, 0.01)), ((8, 16, 256), (0.1, 0.1, 0.02)), ((8, 8, 1024), (0.1, 0.1, 0.01)),
+                                 ((8, 24, 128), (0.1, 0.1, 0.02)), ((12, 8, 64), (0.1, 0.1, 0.05)), ((20, 12, 16), (0.1, 0.1, 0.1)), ((8, 12, 8), (0.1, 0.1, 0.1))])
 def test_periodic_z_on_nz_point_transforms(N, h):
-    """k_conv_z_periodic (periodic z at Nz = 256, 512: Nz-point transforms instead of the padded 2 Nz) against the
+    """k_conv_z_periodic (periodic z, Nz a power of two: Nz-point transforms instead of the padded 2 Nz; both spectrum
+    row layouts, ragged last lane group at the small sizes) against the
     oracle's literal step 1, full field, and against the doubled-grid kernel (FSP_PARAM_PERIODIC_FAST_Z = 0)."""
     rng = np.random.default_rng(N[2])
     rho = rng.standard_normal(N)
@@ -108,4 +110,8 @@ def test_periodic_z_on_nz_point_transforms(N, h):
                 got[fast] = phi.cpu().numpy()
             assert rel_l2(got[fast], ref) <= L2_TOL, (fast, rel_l2(got[fast], ref))
             assert rel_max(got[fast], ref) <= MAX_TOL, (fast, rel_max(got[fast], ref))
-        assert not np.array_equal(got[0], got[1])   # (two different kernels ran)
+        # two different kernels ran: visible in the rounding where the doubled-grid kernel transforms the padded pencil in
+        # one piece (k_conv_z_f, Nz = 256, 512); the branch-pair kernels of the other sizes compute their even branch
+        # exactly as k_conv_z_periodic does and add an odd branch that is zero to rounding, so the bits may agree there
+        if N[2] in (256, 512):
+            assert not np.array_equal(got[0], got[1])
