@@ -724,6 +724,22 @@ def extras(args, peak):
                                          "frac_of_measured_peak": model / (ms * 1e-3) / 1e9 / peak,
                                          "plan_bytes": plan.bytes}
         del rho, phi, E
+    # periodic z (FSP_PARAM_PERIODIC, R20): the z pass on Nz-point transforms (k_conv_z_periodic)
+    for wname in ("256", args.workload):
+        try:
+            _, builder, kw, wdesc = WORKLOADS[wname]
+            w = getattr(W, builder)(**kw)
+            with binding.Plan(w.N, w.h, binding.HOCKNEY, periodic=(0, 0, 1)) as plan:
+                plan.precompute_green()
+                rho = torch.from_numpy(w.rho).cuda()
+                phi = torch.empty_like(rho)
+                steps = 100 if int(np.prod(w.N)) <= 256 ** 3 else args.steps
+                ms, _ = time_solves(plan, rho, phi, steps, 10)
+                out[f"periodic_z_{wname}_HE"] = {"workload": wdesc + ", z periodic (nearest-image kernel)", "ms_per_solve": ms,
+                                                 "solves_per_s": 1e3 / ms, "steps": steps}
+            del rho, phi
+        except Exception as e:   # an extra line must never fail the bench
+            out[f"periodic_z_{wname}_HE"] = {"error": repr(e)[:200]}
     # fsp_solve allocates nothing and never synchronises, so a caller can capture it into a CUDA graph (a PIC loop
     # captures its whole time step): K solves per replay against the same K plain calls, on the plan's own stream
     for wname in ("64", "256"):
